@@ -1,0 +1,188 @@
+/* adept.h — C ABI of the B200-native AdePT transport step (arXiv 2302.08252 hot path).
+ *
+ * What the library computes.  The paper keeps, per particle type (e-, e+, gamma), "a list of
+ * active particle tracks"; every iteration runs one transport pass per type, and survivors and
+ * secondaries go to next-iteration storage (§2).  Two containers are described: the
+ * sparse single buffer with two integer slot lists (Fig. 1a) and the dense double
+ * buffer (Fig. 1b).  The record layout is switched at compile time between AoS, SoA
+ * and AoSoA-n.  The result of a run is "the energy deposit in the
+ * detector's layers" of a stack of "50 alternating box-shaped layers of absorber and gap material"
+ * (§4).  The four calls create / inject / step / run are named by
+ * BASELINE.json:north_star; what one step computes is DESIGN.md §3 (rules R1-R6, M7-M11, T12-T15,
+ * S16-S32), the simplified analytic physics BASELINE.json prescribes.
+ *
+ * Conventions.
+ *  - Every function returns ADEPT_OK (0) or a negative adept_status; nothing throws across the ABI.
+ *  - "host" pointers are ordinary CPU memory, read or written during the call only (copied, never
+ *    kept).  "device" pointers are CUDA global memory of the current device.
+ *  - The caller owns everything it passes, including the device workspace, which must stay alive
+ *    and untouched (except as noted under "Workspace") until adept_destroy.  The library allocates
+ *    no device memory; it keeps a small pinned host buffer for count read-back.
+ *  - All device work is enqueued on config.cuda_stream (a cudaStream_t, NULL = legacy default
+ *    stream).  Calls that return data synchronise that stream; adept_step(ctx, NULL) does not.
+ *  - A context is not thread-safe.  Units: MeV, mm.  Particle kinds: 0 = e-, 1 = e+, 2 = gamma.
+ *  - Capacity overflow: a full buffer/queue sets a device flag, the step completes without any
+ *    out-of-bounds write (excess tracks are dropped), and the next synchronising call returns
+ *    ADEPT_ECAPACITY; afterwards only adept_reset / adept_destroy are accepted.
+ *
+ * Workspace.  The workspace holds the complete device state of a context (control block, tables,
+ * track buffers, queues, tallies).  A byte copy of it taken while no call is in flight may be
+ * written back later to rewind the context (bench.py restores a pristine copy between timed
+ * steps this way).
+ */
+#ifndef ADEPT_B200_H
+#define ADEPT_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct adept_ctx adept_ctx; /* opaque, host object */
+
+typedef enum {
+  ADEPT_OK = 0,
+  ADEPT_EINVAL = -1,    /* bad argument; nothing was changed */
+  ADEPT_ECAPACITY = -2, /* a track buffer or queue overflowed (see above) */
+  ADEPT_ECUDA = -3,     /* a CUDA call failed; adept_last_error() has the text */
+  ADEPT_ESTATE = -4     /* call not allowed in the context's current state */
+} adept_status;
+
+/* Record layout in device memory ("AoS", "SoA", "AoSoA-n", n = 32 lanes). */
+typedef enum { ADEPT_AOS = 0, ADEPT_SOA = 1, ADEPT_AOSOA32 = 2 } adept_layout;
+/* Track container (PAPER.md:29 / PAPER.md:31). */
+typedef enum { ADEPT_SPARSE_SINGLE = 0, ADEPT_DENSE_DOUBLE = 1 } adept_scheme;
+
+/* Slab calorimeter: layer L = absorber slab 2L then gap slab 2L+1 along +z,
+ * starting at z = 0; transverse box |x|,|y| <= half_xy_mm; outside is vacuum (escape). */
+typedef struct {
+  uint32_t n_layers;         /* 1 .. 2048 */
+  float abs_mm, gap_mm;      /* slab thicknesses, > 0 */
+  float half_xy_mm;          /* > 0 */
+  uint32_t mat_abs, mat_gap; /* material index of each slab type, < n_materials */
+} adept_geometry;
+
+/* fp32 log-grid tables (DESIGN.md rules T12-T14).  data is a HOST array
+ * [n_materials][group 2][qty 3][n_bins+1]: group 0 = gamma {pair, Compton, photoelectric} [1/mm];
+ * group 1 = e+- {bremsstrahlung [1/mm], stopping power [MeV/mm], range [mm]}.  Copied at create. */
+typedef struct {
+  uint32_t n_bins, n_materials;
+  float e_min, e_max;      /* grid end points [MeV] */
+  float ln_e_min, inv_dln; /* fl32(ln e_min), fl32(n_bins / ln(e_max/e_min)) */
+  float e_cut;             /* production = tracking cut [MeV] */
+  const float *data;       /* host */
+} adept_tables;
+
+typedef struct {
+  int32_t layout;             /* adept_layout */
+  int32_t scheme;             /* adept_scheme */
+  uint32_t capacity_per_kind; /* slots per particle kind (dense: per buffer), 1 .. 2^30 */
+  uint32_t batch_primaries;   /* adept_run: 0 = inject everything at once, else batch size */
+  uint64_t seed;              /* primary ids, rule R4 */
+  void *workspace;            /* device, 256-byte aligned, >= adept_workspace_bytes() */
+  size_t workspace_bytes;
+  void *cuda_stream;          /* cudaStream_t */
+  uint32_t instrument;        /* 1 = counting build of the same kernels */
+  uint32_t reserved;
+} adept_config;
+
+typedef struct { uint32_t kind; float pos[3], dir[3], ekin; } adept_primary; /* 32 B */
+
+/* One track, 14 four-byte words.  nial = number of interaction lengths left
+ * ("NumIALeft"); vol = slab index (navigation state); (id_lo,id_hi,step) address the
+ * track's Philox-4x32-10 stream (rule R2). */
+typedef struct {
+  float pos[3], dir[3], ekin, nial[3];
+  uint32_t vol, id_lo, id_hi, step;
+} adept_track; /* 56 B */
+
+typedef struct {
+  uint64_t live[3];        /* tracks alive now, per kind */
+  uint64_t steps[3];       /* track-steps taken so far, per kind (rule S28) */
+  uint64_t secondaries[3]; /* tracks created so far, per kind of the NEW track */
+  uint64_t killed[3];      /* tracks that ended (absorbed, below cut, escaped), per kind */
+  uint64_t escaped_n[3];   /* of which left the calorimeter */
+  uint64_t slots_used[3];  /* dense: high-water live count; sparse: high-water of the slot allocator */
+  uint64_t iterations;     /* iterations in which at least one track was alive */
+  uint32_t overflow;       /* 1 after a capacity overflow */
+  uint32_t reserved;
+} adept_counts;
+
+typedef struct {
+  adept_counts total;
+  double e_injected; /* sum of primary kinetic energies (+ 2 mc^2 per e+), MeV */
+  double e_escaped;  /* energy carried out of the calorimeter, MeV */
+  double *edep_slab;  /* host, caller buffer of 2*n_layers doubles, or NULL */
+  double *edep_layer; /* host, caller buffer of n_layers doubles (slab 2L + slab 2L+1), or NULL */
+} adept_result;
+
+/* Bytes of device workspace a context with these parameters needs (0 on invalid arguments).
+ * Only geometry.n_layers, tables.n_bins/n_materials and config.layout/scheme/capacity/instrument
+ * are read. */
+size_t adept_workspace_bytes(const adept_geometry *, const adept_tables *, const adept_config *);
+
+/* Build a context: validates, copies geometry and tables to the workspace, clears all state. */
+int adept_create(const adept_geometry *, const adept_tables *, const adept_config *, adept_ctx **out);
+
+/* Add n primaries (host array).  batch_primaries == 0: they become live tracks immediately (ids by
+ * rule R4 from a running global index; slab located from pos.z); otherwise they are queued for
+ * adept_run.  EINVAL if a primary is outside the calorimeter or its energy outside [e_cut, e_max]. */
+int adept_inject(adept_ctx *, const adept_primary *primaries, uint64_t n);
+
+/* One iteration: every live track of every kind takes one step (DESIGN.md rules S16-S28).
+ * out == NULL: enqueue only.  out != NULL: synchronise and report the counts after the step. */
+int adept_step(adept_ctx *, adept_counts *out);
+
+/* Iterate until no track is alive (and no primary is pending), or max_iterations (0 = no limit)
+ * iterations were done in this call.  Fills *out (tallies are cumulative since create/reset). */
+int adept_run(adept_ctx *, uint64_t max_iterations, adept_result *out);
+
+/* Fill *out with the current tallies without stepping (synchronises). */
+int adept_get_result(adept_ctx *, adept_result *out);
+
+/* Append n tracks (host array, 56-byte records) to kind's live set.  slots (host, n entries) is
+ * used by the sparse scheme only: slot of each track, all distinct, free and < capacity; NULL =
+ * next free slots.  The queue order is the array order. */
+int adept_load_tracks(adept_ctx *, uint32_t kind, const adept_track *tracks, uint64_t n,
+                      const uint32_t *slots);
+
+/* Copy kind's live tracks to a host array of cap records (buffer order: unspecified, rule S29).
+ * *n receives the live count; ECAPACITY-free: if *n > cap nothing is copied and EINVAL returns. */
+int adept_read_tracks(adept_ctx *, uint32_t kind, adept_track *out, uint64_t cap, uint64_t *n);
+
+/* Instrumented contexts only (config.instrument = 1), all host buffers, any may be NULL:
+ *  field_rw[3][14][2]  u64: per kind, per record word, {reads, writes} done by the step kernel
+ *                      through the layout accessor (Fig. 5);
+ *  lines[3][n_lines]   u32: accesses per 128-byte line of each kind's record storage, where
+ *                      n_lines = adept_instr_lines(ctx) (PAPER.md:131, 135 heatmap, row = cache line);
+ *  slots[3][n_slots]   u32: accesses per track slot, n_slots = adept_instr_slots(ctx). */
+int adept_read_counters(adept_ctx *, uint64_t *field_rw, uint32_t *lines, uint32_t *slots);
+uint64_t adept_instr_lines(const adept_ctx *);
+uint64_t adept_instr_slots(const adept_ctx *);
+
+/* Byte offset of word `field` (0..13: pos xyz, dir xyz, ekin, nial 0-2, vol, id_lo, id_hi, step) of
+ * slot `slot` inside one record buffer of `capacity` slots under `layout` (Fig. 3:
+ * where each field is placed).  Pure host arithmetic; UINT64_MAX on invalid arguments. */
+uint64_t adept_field_offset(int32_t layout, uint32_t capacity, uint32_t slot, uint32_t field);
+
+/* Drop all tracks, pending primaries and tallies; keeps geometry, tables and configuration. */
+int adept_reset(adept_ctx *);
+int adept_destroy(adept_ctx *);
+/* Text of the last error of this context ("" if none).  ctx may be NULL: last create error. */
+const char *adept_last_error(const adept_ctx *);
+
+/* Elementary functions of the step, evaluated on the device for bit-equality tests against the
+ * oracle (DESIGN.md rules R1, R3, M8-M10, T13).  in/out are DEVICE arrays; n = element count.
+ *  fn 0: Philox-4x32-10; in = n x {ctr[4], key[2]} u32, out = n x 4 u32
+ *  fn 1: u01;            in = n u32,  out = n f32
+ *  fn 2: lg;             in = n f32,  out = n f32
+ *  fn 3: ex;             in = n f32,  out = n f32
+ *  fn 4: sincos2pi;      in = n f32,  out = n x {sin, cos} f32 */
+int adept_dev_math(int fn, const void *in, void *out, uint64_t n, void *cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ADEPT_B200_H */

@@ -1,0 +1,186 @@
+// Track record and its compile-time switchable memory layout.
+//
+// The paper separates "the algorithmic view of data from its mapping to device memory" (LLAMA,
+// PAPER.md:25, 35): kernels address a field of a track, a mapping chosen at compile time turns
+// (slot, field) into an address — AoS, SoA or AoSoA-n ("AABBCCAABBCC" for n = 2) —
+// and instrumented mappings count accesses per field (Trace/FieldAccessCount)
+// and per byte/row (Heatmap).  This header is that idea reduced to what the
+// step needs: `Mapping<L>` is pure index arithmetic with no run-time state, `TrackView<L, INSTR>`
+// moves whole records or single words between registers and memory, and `Probe` is the counting
+// hook compiled in only for the instrumented build.
+//
+// Record = 14 four-byte words, word order = adept_track (include/adept.h).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace adept {
+
+enum Field : int {
+  F_PX = 0, F_PY, F_PZ, F_DX, F_DY, F_DZ, F_EKIN, F_N0, F_N1, F_N2, F_VOL, F_IDLO, F_IDHI, F_STEP,
+  kNumFields = 14
+};
+enum LayoutId : int { L_AOS = 0, L_SOA = 1, L_AOSOA32 = 2 };
+
+// A track in registers.
+struct Trk {
+  float px, py, pz, dx, dy, dz, ekin, n0, n1, n2;
+  uint32_t vol, id_lo, id_hi, step;
+};
+
+__device__ __forceinline__ uint32_t trk_word(const Trk &t, int f) {
+  switch (f) {
+    case F_PX: return __float_as_uint(t.px);
+    case F_PY: return __float_as_uint(t.py);
+    case F_PZ: return __float_as_uint(t.pz);
+    case F_DX: return __float_as_uint(t.dx);
+    case F_DY: return __float_as_uint(t.dy);
+    case F_DZ: return __float_as_uint(t.dz);
+    case F_EKIN: return __float_as_uint(t.ekin);
+    case F_N0: return __float_as_uint(t.n0);
+    case F_N1: return __float_as_uint(t.n1);
+    case F_N2: return __float_as_uint(t.n2);
+    case F_VOL: return t.vol;
+    case F_IDLO: return t.id_lo;
+    case F_IDHI: return t.id_hi;
+    default: return t.step;
+  }
+}
+
+__device__ __forceinline__ void trk_set_word(Trk &t, int f, uint32_t w) {
+  switch (f) {
+    case F_PX: t.px = __uint_as_float(w); break;
+    case F_PY: t.py = __uint_as_float(w); break;
+    case F_PZ: t.pz = __uint_as_float(w); break;
+    case F_DX: t.dx = __uint_as_float(w); break;
+    case F_DY: t.dy = __uint_as_float(w); break;
+    case F_DZ: t.dz = __uint_as_float(w); break;
+    case F_EKIN: t.ekin = __uint_as_float(w); break;
+    case F_N0: t.n0 = __uint_as_float(w); break;
+    case F_N1: t.n1 = __uint_as_float(w); break;
+    case F_N2: t.n2 = __uint_as_float(w); break;
+    case F_VOL: t.vol = w; break;
+    case F_IDLO: t.id_lo = w; break;
+    case F_IDHI: t.id_hi = w; break;
+    default: t.step = w; break;
+  }
+}
+
+// ---- mappings: (capacity, slot, field) -> word index inside one record buffer ---------------
+// Capacities are multiples of 32 slots, so every SoA field array and every AoSoA block starts on a
+// 128-byte line.
+template <int L> struct Mapping;
+
+template <> struct Mapping<L_AOS> {  // 14 words padded to 16: one record = 64 B = 2 sectors = 4 x 16 B
+  static constexpr int kStride = 16;
+  __host__ __device__ static constexpr size_t words(size_t cap) { return cap * kStride; }
+  __host__ __device__ static constexpr size_t index(size_t, size_t slot, int f) { return slot * kStride + f; }
+};
+template <> struct Mapping<L_SOA> {  // 14 arrays of `cap` words
+  __host__ __device__ static constexpr size_t words(size_t cap) { return cap * kNumFields; }
+  __host__ __device__ static constexpr size_t index(size_t cap, size_t slot, int f) { return f * cap + slot; }
+};
+template <> struct Mapping<L_AOSOA32> {  // blocks of 32 tracks, field-major inside a block (1792 B)
+  static constexpr int kLanes = 32;
+  __host__ __device__ static constexpr size_t words(size_t cap) { return cap * kNumFields; }
+  __host__ __device__ static constexpr size_t index(size_t, size_t slot, int f) {
+    return (slot / kLanes) * (kLanes * kNumFields) + f * kLanes + (slot % kLanes);
+  }
+};
+
+// ---- access counting (instrumented build only) -----------------------------------------------
+// field_rw: shared-memory counters [14][2] of the CTA (flushed once per kernel);
+// lines / slots: global counters of the kind's record storage (line = 128 B, "row").
+struct ProbeSink {
+  uint32_t *cta_field_rw;  // shared
+  uint32_t *lines;         // global, indexed by (byte offset in the kind's record storage) / 128
+  uint32_t *slots;         // global, indexed by buffer_index * capacity + slot
+};
+
+template <bool INSTR> struct Probe {
+  __device__ __forceinline__ void touch(const ProbeSink &, int, int, size_t, size_t) const {}
+};
+template <> struct Probe<true> {
+  __device__ __forceinline__ void touch(const ProbeSink &s, int field, int is_write, size_t byte_off,
+                                        size_t slot_index) const {
+    atomicAdd(&s.cta_field_rw[field * 2 + is_write], 1u);
+    atomicAdd(&s.lines[byte_off >> 7], 1u);
+    atomicAdd(&s.slots[slot_index], 1u);
+  }
+};
+
+// ---- view of one record buffer ----------------------------------------------------------------
+template <int L, bool INSTR> struct TrackView {
+  uint32_t *base;      // first word of this buffer
+  uint32_t cap;        // slots
+  size_t storage_off;  // byte offset of this buffer inside the kind's record storage (probe only)
+  uint32_t buf_index;  // 0/1 (probe only)
+  ProbeSink sink;
+
+  using Map = Mapping<L>;
+
+  __device__ __forceinline__ void probe(int f, int w, size_t slot) const {
+    Probe<INSTR>().touch(sink, f, w, storage_off + Map::index(cap, slot, f) * 4, size_t(buf_index) * cap + slot);
+  }
+
+  __device__ __forceinline__ uint32_t load_word(uint32_t slot, int f) const {
+    probe(f, 0, slot);
+    return base[Map::index(cap, slot, f)];
+  }
+  __device__ __forceinline__ void store_word(uint32_t slot, int f, uint32_t w) const {
+    probe(f, 1, slot);
+    base[Map::index(cap, slot, f)] = w;
+  }
+
+  // whole record -> registers
+  __device__ __forceinline__ Trk load(uint32_t slot) const {
+    Trk t;
+    if constexpr (L == L_AOS) {
+      const uint4 *r = reinterpret_cast<const uint4 *>(base + size_t(slot) * Map::kStride);
+      const uint4 a = r[0], b = r[1], c = r[2];
+      const uint2 d = *reinterpret_cast<const uint2 *>(r + 3);
+      t.px = __uint_as_float(a.x); t.py = __uint_as_float(a.y); t.pz = __uint_as_float(a.z);
+      t.dx = __uint_as_float(a.w); t.dy = __uint_as_float(b.x); t.dz = __uint_as_float(b.y);
+      t.ekin = __uint_as_float(b.z); t.n0 = __uint_as_float(b.w);
+      t.n1 = __uint_as_float(c.x); t.n2 = __uint_as_float(c.y);
+      t.vol = c.z; t.id_lo = c.w; t.id_hi = d.x; t.step = d.y;
+      if constexpr (INSTR) {
+#pragma unroll
+        for (int f = 0; f < kNumFields; ++f) probe(f, 0, slot);
+      }
+    } else {
+#pragma unroll
+      for (int f = 0; f < kNumFields; ++f) trk_set_word(t, f, load_word(slot, f));
+    }
+    return t;
+  }
+
+  // registers -> whole record
+  __device__ __forceinline__ void store(uint32_t slot, const Trk &t) const {
+    if constexpr (L == L_AOS) {
+      uint4 *r = reinterpret_cast<uint4 *>(base + size_t(slot) * Map::kStride);
+      r[0] = make_uint4(__float_as_uint(t.px), __float_as_uint(t.py), __float_as_uint(t.pz), __float_as_uint(t.dx));
+      r[1] = make_uint4(__float_as_uint(t.dy), __float_as_uint(t.dz), __float_as_uint(t.ekin), __float_as_uint(t.n0));
+      r[2] = make_uint4(__float_as_uint(t.n1), __float_as_uint(t.n2), t.vol, t.id_lo);
+      r[3] = make_uint4(t.id_hi, t.step, 0u, 0u);  // tail padding written so that sectors are whole
+      if constexpr (INSTR) {
+#pragma unroll
+        for (int f = 0; f < kNumFields; ++f) probe(f, 1, slot);
+      }
+    } else {
+#pragma unroll
+      for (int f = 0; f < kNumFields; ++f) store_word(slot, f, trk_word(t, f));
+    }
+  }
+
+  // registers -> only the words that differ from `old` (sparse single buffer: in-place update)
+  __device__ __forceinline__ void store_changed(uint32_t slot, const Trk &t, const Trk &old) const {
+#pragma unroll
+    for (int f = 0; f < kNumFields; ++f) {
+      const uint32_t w = trk_word(t, f);
+      if (w != trk_word(old, f)) store_word(slot, f, w);
+    }
+  }
+};
+
+}  // namespace adept

@@ -1,0 +1,376 @@
+// One transport step of one track (DESIGN.md rules S16-S27, S31).
+//
+// The paper's per-type kernels read a track, ask the physics library for the step
+// length from the numbers of interaction lengths left (Fig. 3, "NumIALeft"), ask the
+// geometry for the distance to the next boundary, move, apply continuous loss and the discrete
+// interaction, and initialise secondaries from the parent's position and navigation state (Fig. 2,
+// PAPER.md:47-60).  The physics itself is BASELINE.json's simplified analytic model; every formula
+// below is the rule of DESIGN.md §3 named in its comment, in that rule's operation order (the order
+// is part of the rule: rule M7 makes results bit-reproducible).
+//
+// Everything lives in registers; the only memory touched is the shared-memory copy of the tables.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "layout.cuh"
+#include "mathfn.cuh"
+#include "rng.cuh"
+
+namespace adept {
+
+enum Kind : int { K_EM = 0, K_EP = 1, K_GAMMA = 2 };
+
+// What the step needs besides the track: tables (shared memory) and geometry (registers).
+struct Env {
+  const float4 *tab;  // [material][group][node] -> {qty0, qty1, qty2, 0}; group 0 = gamma, 1 = e+-
+  uint32_t nodes;     // n_bins + 1
+  float ln_e_min, inv_dln, e_cut;
+  uint32_t n_slabs;   // 2 * n_layers
+  float abs_mm, pitch, half_xy;
+  uint32_t mat_abs, mat_gap;
+};
+
+struct Kid {  // a secondary: position, slab, nial = -1, step = 0 come from the parent (S28, R6)
+  float dx, dy, dz, ekin;
+  uint32_t id_lo, id_hi;
+  int kind;  // -1 = none
+};
+
+struct Outcome {
+  bool alive;    // track goes to the next iteration
+  bool escaped;  // left the calorimeter (S25)
+  Kid kid[2];    // by child ordinal (R5)
+  double dep;    // energy deposited in the pre-step slab
+  double esc_e;  // energy carried out (S25)
+  double dep2;   // S31 guard only: deposit in the post-step slab
+};
+
+constexpr float kInf = __builtin_huge_valf();
+constexpr float kMc2 = 0.51099895f;
+__device__ __forceinline__ float two_mc2() { return 2.0f * kMc2; }
+
+// T13: position on the log grid
+struct Bin {
+  int j;
+  float f;
+};
+__device__ __forceinline__ Bin locate_bin(const Env &g, float lnE) {
+  const float x = (lnE - g.ln_e_min) * g.inv_dln;
+  int j = static_cast<int>(x);
+  const int last = static_cast<int>(g.nodes) - 2;
+  j = j < 0 ? 0 : j;
+  j = j > last ? last : j;
+  Bin b;
+  b.j = j;
+  b.f = x - static_cast<float>(j);
+  return b;
+}
+__device__ __forceinline__ float lerp_node(float f, float lo, float hi) { return fmaf(f, hi - lo, lo); }
+
+// S21 geometry of slab i
+__device__ __forceinline__ float slab_zlo(const Env &g, uint32_t i) {
+  return fmaf(static_cast<float>(i >> 1), g.pitch, (i & 1u) ? g.abs_mm : 0.0f);
+}
+
+enum Face : int { FACE_ZP = 0, FACE_ZM = 1, FACE_XY = 2 };
+
+// S21: distance to the slab faces and the transverse box, and which face is hit first.
+__device__ __forceinline__ float geometry_step(const Trk &t, const Env &g, float z_lo, float z_hi, int &face) {
+  const float H = g.half_xy;
+  const float s_z = (t.dz > 0.0f) ? (z_hi - t.pz) / t.dz : (t.dz < 0.0f) ? (z_lo - t.pz) / t.dz : kInf;
+  const float s_x = (t.dx > 0.0f) ? (H - t.px) / t.dx : (t.dx < 0.0f) ? (-H - t.px) / t.dx : kInf;
+  const float s_y = (t.dy > 0.0f) ? (H - t.py) / t.dy : (t.dy < 0.0f) ? (-H - t.py) / t.dy : kInf;
+  float s_g = s_z;
+  face = (t.dz > 0.0f) ? FACE_ZP : FACE_ZM;
+  if (s_x < s_g) { s_g = s_x; face = FACE_XY; }
+  if (s_y < s_g) { s_g = s_y; face = FACE_XY; }
+  if (!(s_g > 0.0f)) s_g = 0.0f;
+  return s_g;
+}
+
+// S25: snap to the plane and change slab, or escape.  Returns true if the track escaped.
+__device__ __forceinline__ bool cross_boundary(Trk &t, const Env &g, uint32_t vol0, int face, float z_lo,
+                                               float z_hi) {
+  if (face == FACE_ZP) {
+    t.pz = z_hi;
+    if (vol0 + 1u >= g.n_slabs) return true;
+    t.vol = vol0 + 1u;
+    return false;
+  }
+  if (face == FACE_ZM) {
+    t.pz = z_lo;
+    if (vol0 == 0u) return true;
+    t.vol = vol0 - 1u;
+    return false;
+  }
+  return true;
+}
+
+__device__ __forceinline__ void make_kid(Kid &k, int kind, float dx, float dy, float dz, float ekin, uint32_t id_lo,
+                                         uint32_t id_hi) {
+  k.kind = kind; k.dx = dx; k.dy = dy; k.dz = dz; k.ekin = ekin; k.id_lo = id_lo; k.id_hi = id_hi;
+}
+
+// S27: rotate unit vector d by polar (st, ct) and azimuth (sphi, cphi); renormalise.
+__device__ __forceinline__ void rotate_dir(float dx, float dy, float dz, float st, float ct, float sphi, float cphi,
+                                           float &ox, float &oy, float &oz) {
+  const float q2 = fmaf(-dz, dz, 1.0f);
+  float a, b, c;
+  if (q2 > 1e-10f) {
+    const float sp = sqrtf(q2);
+    const float ux = ((dx * dz) * cphi - dy * sphi) / sp;
+    const float uy = ((dy * dz) * cphi + dx * sphi) / sp;
+    const float uz = -(sp * cphi);
+    a = fmaf(st, ux, ct * dx);
+    b = fmaf(st, uy, ct * dy);
+    c = fmaf(st, uz, ct * dz);
+  } else {
+    a = st * cphi;
+    b = st * sphi;
+    c = (dz < 0.0f) ? -ct : ct;
+  }
+  const float nn = sqrtf(fmaf(a, a, fmaf(b, b, c * c)));
+  ox = a / nn;
+  oy = b / nn;
+  oz = c / nn;
+}
+
+__device__ __forceinline__ void outcome_init(Outcome &o) {
+  o.alive = true; o.escaped = false; o.kid[0].kind = -1; o.kid[1].kind = -1;
+  o.dep = 0.0; o.esc_e = 0.0; o.dep2 = 0.0;
+}
+
+// S31: runaway guard
+template <int KIND> __device__ __forceinline__ void runaway_guard(Trk &t, Outcome &o) {
+  if (t.step >= (1u << 20)) {
+    o.dep2 += static_cast<double>(t.ekin);
+    if (KIND == K_EP) o.dep2 += static_cast<double>(two_mc2());
+    o.alive = false;
+  }
+}
+
+// ------------------------------------------------------------------------------ photon -------
+__device__ __forceinline__ void step_gamma(Trk &t, const Env &g, Outcome &o) {
+  outcome_init(o);
+  const Stream rs{t.id_lo, t.id_hi, t.step};
+
+  // S18: re-sample spent interaction lengths (pair, Compton, photoelectric)
+  if (t.n0 <= 0.0f || t.n1 <= 0.0f || t.n2 <= 0.0f) {
+    const uint4 r = rs.call(0);
+    if (t.n0 <= 0.0f) t.n0 = -lg(u01(r.x));
+    if (t.n1 <= 0.0f) t.n1 = -lg(u01(r.y));
+    if (t.n2 <= 0.0f) t.n2 = -lg(u01(r.z));
+  }
+
+  // S19: cross sections at the pre-step energy and material
+  const uint32_t vol0 = t.vol;
+  const uint32_t mat = (vol0 & 1u) ? g.mat_gap : g.mat_abs;
+  const float E0 = t.ekin;
+  const Bin b = locate_bin(g, lg(E0));
+  const float4 *node = g.tab + (mat * 2u + 0u) * g.nodes + b.j;
+  const float4 A = node[0], B = node[1];
+  const float sig0 = lerp_node(b.f, A.x, B.x);
+  const float sig1 = lerp_node(b.f, A.y, B.y);
+  const float sig2 = lerp_node(b.f, A.z, B.z);
+  const float s0 = (sig0 > 0.0f) ? t.n0 / sig0 : kInf;
+  const float s1 = (sig1 > 0.0f) ? t.n1 / sig1 : kInf;
+  const float s2 = (sig2 > 0.0f) ? t.n2 / sig2 : kInf;
+
+  // S21
+  const float z_lo = slab_zlo(g, vol0), z_hi = slab_zlo(g, vol0 + 1u);
+  int face;
+  float s = geometry_step(t, g, z_lo, z_hi, face);
+
+  // S22: strict '<', earlier candidate wins ties
+  int w = -1;
+  if (s0 < s) { s = s0; w = 0; }
+  if (s1 < s) { s = s1; w = 1; }
+  if (s2 < s) { s = s2; w = 2; }
+
+  // S23
+  t.px = fmaf(s, t.dx, t.px);
+  t.py = fmaf(s, t.dy, t.py);
+  t.pz = fmaf(s, t.dz, t.pz);
+  t.n0 = fmaf(-s, sig0, t.n0);
+  t.n1 = fmaf(-s, sig1, t.n1);
+  t.n2 = fmaf(-s, sig2, t.n2);
+  t.step = rs.step + 1u;
+
+  if (w < 0) {  // S25
+    if (cross_boundary(t, g, vol0, face, z_lo, z_hi)) {
+      o.esc_e = static_cast<double>(t.ekin);
+      o.escaped = true;
+      o.alive = false;
+      return;
+    }
+  } else if (w == 0) {  // S26 pair: uniform split of E - 2 mc^2, both along dir; photon dies
+    t.n0 = -1.0f;
+    const uint4 r1 = rs.call(1), r2 = rs.call(2);
+    const float E_av = t.ekin - two_mc2();
+    const float T_minus = u01(r1.x) * E_av;
+    const float T_plus = E_av - T_minus;
+    if (T_minus >= g.e_cut) make_kid(o.kid[0], K_EM, t.dx, t.dy, t.dz, T_minus, r2.x, r2.y);
+    else o.dep += static_cast<double>(T_minus);
+    make_kid(o.kid[1], K_EP, t.dx, t.dy, t.dz, T_plus, r2.z, r2.w);
+    o.alive = false;
+    return;
+  } else if (w == 1) {  // S26 Compton: 1/eps spectrum, exact kinematics
+    t.n1 = -1.0f;
+    const uint4 r1 = rs.call(1);
+    const float E = t.ekin;
+    const float kappa = E / kMc2;
+    const float L = lg(fmaf(2.0f, kappa, 1.0f));
+    const float eps = ex(-(u01(r1.x) * L));
+    const float E1 = eps * E;
+    const float T = E - E1;
+    float ct = 1.0f - (((1.0f / eps) - 1.0f) / kappa);
+    if (ct > 1.0f) ct = 1.0f;
+    if (ct < -1.0f) ct = -1.0f;
+    const float st = sqrtf(fmaf(-ct, ct, 1.0f));
+    float sphi, cphi;
+    sincos2pi(u01(r1.y), sphi, cphi);
+    float nx, ny, nz;
+    rotate_dir(t.dx, t.dy, t.dz, st, ct, sphi, cphi, nx, ny, nz);
+    const float qx = fmaf(E, t.dx, -(E1 * nx));
+    const float qy = fmaf(E, t.dy, -(E1 * ny));
+    const float qz = fmaf(E, t.dz, -(E1 * nz));
+    const float pn = sqrtf(fmaf(qx, qx, fmaf(qy, qy, qz * qz)));
+    if (T >= g.e_cut && pn > 0.0f) {
+      const uint4 r2 = rs.call(2);
+      make_kid(o.kid[0], K_EM, qx / pn, qy / pn, qz / pn, T, r2.x, r2.y);
+    } else {
+      o.dep += static_cast<double>(T);
+    }
+    if (E1 < g.e_cut) {
+      o.dep += static_cast<double>(E1);
+      o.alive = false;
+      return;
+    }
+    t.ekin = E1;
+    t.dx = nx; t.dy = ny; t.dz = nz;
+  } else {  // S26 photoelectric: e- with T = E along dir; photon dies
+    t.n2 = -1.0f;
+    const uint4 r2 = rs.call(2);
+    make_kid(o.kid[0], K_EM, t.dx, t.dy, t.dz, t.ekin, r2.x, r2.y);
+    o.alive = false;
+    return;
+  }
+  runaway_guard<K_GAMMA>(t, o);
+}
+
+// --------------------------------------------------------------------- electron / positron ---
+template <int KIND> __device__ __forceinline__ void step_elec(Trk &t, const Env &g, Outcome &o) {
+  static_assert(KIND == K_EM || KIND == K_EP, "e- or e+");
+  outcome_init(o);
+  const Stream rs{t.id_lo, t.id_hi, t.step};
+  const float e_cut = g.e_cut;
+
+  // S17: a positron below the cut annihilates at rest into two back-to-back photons
+  if (KIND == K_EP && t.ekin < e_cut) {
+    o.dep += static_cast<double>(t.ekin);
+    const uint4 r1 = rs.call(1), r2 = rs.call(2);
+    const float ct = 1.0f - 2.0f * u01(r1.z);
+    const float st = sqrtf(fmaf(-ct, ct, 1.0f));
+    float sphi, cphi;
+    sincos2pi(u01(r1.w), sphi, cphi);
+    const float ax = st * cphi, ay = st * sphi, az = ct;
+    make_kid(o.kid[0], K_GAMMA, ax, ay, az, kMc2, r2.x, r2.y);
+    make_kid(o.kid[1], K_GAMMA, -ax, -ay, -az, kMc2, r2.z, r2.w);
+    o.alive = false;
+    return;
+  }
+
+  // S18: bremsstrahlung is the only discrete process; nial[1], nial[2] are carried unchanged
+  if (t.n0 <= 0.0f) t.n0 = -lg(u01(rs.call(0).x));
+
+  // S19, S20
+  const uint32_t vol0 = t.vol;
+  const uint32_t mat = (vol0 & 1u) ? g.mat_gap : g.mat_abs;
+  const float E0 = t.ekin;
+  const Bin b = locate_bin(g, lg(E0));
+  const float4 *tab = g.tab + (mat * 2u + 1u) * g.nodes;
+  const float4 A = tab[b.j], B = tab[b.j + 1];
+  const float sig0 = lerp_node(b.f, A.x, B.x);
+  const float S0 = lerp_node(b.f, A.y, B.y);
+  const float R = lerp_node(b.f, A.z, B.z);
+  const float s0 = (sig0 > 0.0f) ? t.n0 / sig0 : kInf;
+  float s_e;
+  {
+    const float r_min = 0.1f, f_r = 0.2f;
+    if (R <= r_min) {
+      s_e = R;
+    } else {
+      const float fr = f_r * R;
+      s_e = (fr > r_min) ? fr : r_min;
+    }
+  }
+
+  // S21
+  const float z_lo = slab_zlo(g, vol0), z_hi = slab_zlo(g, vol0 + 1u);
+  int face;
+  float s = geometry_step(t, g, z_lo, z_hi, face);
+
+  // S22: GEOM (-1), ELOSS (3), brems (0)
+  int w = -1;
+  if (s_e < s) { s = s_e; w = 3; }
+  if (s0 < s) { s = s0; w = 0; }
+
+  // S23
+  t.px = fmaf(s, t.dx, t.px);
+  t.py = fmaf(s, t.dy, t.py);
+  t.pz = fmaf(s, t.dz, t.pz);
+  t.n0 = fmaf(-s, sig0, t.n0);
+  t.step = rs.step + 1u;
+
+  // S24: continuous loss by the midpoint rule, deposit in the pre-step slab
+  float E_post;
+  if (w == 3 && s >= R) {
+    E_post = 0.0f;
+  } else {
+    float E_mid = fmaf(-0.5f * s, S0, E0);
+    if (!(E_mid > e_cut)) E_mid = e_cut;
+    const Bin bm = locate_bin(g, lg(E_mid));
+    const float S_mid = lerp_node(bm.f, tab[bm.j].y, tab[bm.j + 1].y);
+    float dE = s * S_mid;
+    if (!(dE < E0)) dE = E0;
+    E_post = E0 - dE;
+  }
+  o.dep += static_cast<double>(E0 - E_post);
+  if (E_post < e_cut) {
+    if (KIND == K_EM) {
+      o.dep += static_cast<double>(E_post);
+      o.alive = false;
+      return;
+    }
+    t.ekin = E_post;  // e+ is kept for S17 at its next step
+    return;
+  }
+  t.ekin = E_post;
+
+  if (w < 0) {  // S25
+    if (cross_boundary(t, g, vol0, face, z_lo, z_hi)) {
+      o.esc_e = static_cast<double>(t.ekin) + ((KIND == K_EP) ? static_cast<double>(two_mc2()) : 0.0);
+      o.escaped = true;
+      o.alive = false;
+      return;
+    }
+  } else if (w == 0) {  // S26 bremsstrahlung: k from the 1/k spectrum on [e_cut, E], photon along dir
+    t.n0 = -1.0f;
+    const uint4 r1 = rs.call(1), r2 = rs.call(2);
+    const float E = t.ekin;
+    float k = e_cut * ex(u01(r1.x) * lg(E / e_cut));
+    if (!(k < E)) k = E;
+    make_kid(o.kid[0], K_GAMMA, t.dx, t.dy, t.dz, k, r2.x, r2.y);
+    const float E_new = E - k;
+    if (E_new < e_cut && KIND == K_EM) {
+      o.dep += static_cast<double>(E_new);
+      o.alive = false;
+      return;
+    }
+    t.ekin = E_new;
+  }
+  runaway_guard<KIND>(t, o);
+}
+
+}  // namespace adept

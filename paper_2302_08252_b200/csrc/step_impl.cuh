@@ -1,0 +1,555 @@
+// The transport-step kernel and its helper kernels, templated on <layout, scheme, instrumented>.
+//
+// One launch = one iteration of all three per-type track buffers ("the tracks of each
+// particle type are processed by a dedicated kernel"; here the three passes share one persistent
+// grid so that an iteration costs one launch, and a tile of 256 tracks always holds one type, so
+// divergence between types never occurs inside a CTA).  SURVEY.md §8(a) rows:
+//   A0/A11  iteration control: counts live on the device; the last CTA to finish ends the
+//           iteration (swap current/next, reset counters, accumulate tallies) — no host round trip;
+//   A1      track load through the layout accessor (layout.cuh);
+//   A2-A8   the physics/geometry step (physics.cuh), tables staged in shared memory by one TMA
+//           bulk copy per CTA;
+//   A9      dense: secondaries and survivors are ranked by one packed block scan (3 x 10-bit
+//           counters, one per destination type; warp shuffles + one shared-memory hop) and the CTA
+//           reserves its output ranges with one atomicAdd per destination type;
+//           sparse: new slots come from a bump allocator and slot-list pushes are warp-aggregated
+//           (warp scan + one atomicAdd per warp and list);
+//   A10     dense: survivors are written to the next array (whole record); sparse: only the words
+//           that changed are written back in place, and the slot is pushed onto the next list;
+//   A12     the instrumented instantiation counts every accessor call.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "device_state.cuh"
+#include "layout.cuh"
+#include "physics.cuh"
+
+namespace adept {
+
+// ---------------------------------------------------------------- small device utilities ------
+__device__ __forceinline__ uint32_t warp_inclusive_scan(uint32_t v, int lane) {
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const uint32_t n = __shfl_up_sync(0xFFFFFFFFu, v, d);
+    if (lane >= d) v += n;
+  }
+  return v;
+}
+
+// Warp-aggregated reservation: every lane asks for `mine` (0..2) consecutive entries of *counter;
+// one atomicAdd per warp.  Must be called by all 32 lanes.  Returns the lane's first entry.
+__device__ __forceinline__ uint32_t warp_reserve(uint32_t *counter, uint32_t mine, int lane) {
+  const uint32_t inc = warp_inclusive_scan(mine, lane);
+  const uint32_t total = __shfl_sync(0xFFFFFFFFu, inc, 31);
+  if (total == 0u) return 0u;
+  uint32_t base = 0u;
+  if (lane == 31) base = atomicAdd(counter, total);
+  base = __shfl_sync(0xFFFFFFFFu, base, 31);
+  return base + inc - mine;
+}
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) v += __shfl_down_sync(0xFFFFFFFFu, v, d);
+  return v;
+}
+
+// One TMA bulk copy global -> shared of `bytes` (multiple of 16), completion on an mbarrier.
+__device__ __forceinline__ void tma_stage(void *smem_dst, const void *gmem_src, uint32_t bytes, uint64_t *mbar,
+                                          int tid) {
+  const uint32_t bar = static_cast<uint32_t>(__cvta_generic_to_shared(mbar));
+  const uint32_t dst = static_cast<uint32_t>(__cvta_generic_to_shared(smem_dst));
+  if (tid == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (tid == 0) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+        "l"(gmem_src), "r"(bytes), "r"(bar)
+        : "memory");
+  }
+}
+__device__ __forceinline__ void tma_wait(uint64_t *mbar) {
+  const uint32_t bar = static_cast<uint32_t>(__cvta_generic_to_shared(mbar));
+  uint32_t done = 0;
+  while (!done) {
+    asm volatile(
+        "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\n selp.u32 %0, 1, 0, p;\n}"
+        : "=r"(done)
+        : "r"(bar)
+        : "memory");
+  }
+}
+
+template <int L, bool INSTR>
+__device__ __forceinline__ TrackView<L, INSTR> make_view(const Params &p, int kind, int buf, uint32_t *cta_probe) {
+  TrackView<L, INSTR> v;
+  v.base = p.kind[kind].rec[buf];
+  v.cap = p.capacity;
+  v.storage_off = size_t(buf) * Mapping<L>::words(p.capacity) * 4;
+  v.buf_index = uint32_t(buf);
+  v.sink.cta_field_rw = cta_probe + kind * (kNumFields * 2);
+  v.sink.lines = p.kind[kind].instr_lines;
+  v.sink.slots = p.kind[kind].instr_slots;
+  return v;
+}
+
+__device__ __forceinline__ Trk kid_track(const Trk &parent, const Kid &k) {
+  Trk c;
+  c.px = parent.px; c.py = parent.py; c.pz = parent.pz;
+  c.dx = k.dx; c.dy = k.dy; c.dz = k.dz;
+  c.ekin = k.ekin;
+  c.n0 = -1.0f; c.n1 = -1.0f; c.n2 = -1.0f;
+  c.vol = parent.vol;
+  c.id_lo = k.id_lo; c.id_hi = k.id_hi;
+  c.step = 0u;
+  return c;
+}
+
+// Per-CTA shared state of the step kernel.
+struct CtaShared {
+  uint64_t mbar;
+  uint32_t warp_tot[2][kBlock / 32];
+  uint32_t base[2][4];
+  uint32_t alive[4];
+  uint32_t escaped[4];
+  uint32_t last_flag;
+  double esc_e;
+  uint32_t probe[3 * kNumFields * 2];
+};
+
+// A9 + A11: the last CTA closes the iteration.
+template <int SCHEME> __device__ void finish_iteration(const Params &p) {
+  Ctl *c = p.ctl;
+  uint32_t live_before = 0, live_after = 0;
+  for (int k = 0; k < 3; ++k) {
+    const uint32_t n = c->n_cur[k];
+    uint32_t nn = __ldcg(&c->n_next[k]);
+    const uint32_t alive = __ldcg(&c->it_alive[k]);
+    const uint32_t esc = __ldcg(&c->it_escaped[k]);
+    live_before += n;
+    c->steps[k] += n;
+    c->killed[k] += n - alive;
+    c->escaped_n[k] += esc;
+    c->secondaries[k] += nn - alive;
+    if (nn > p.capacity) { nn = p.capacity; c->overflow = 1u; }
+    if (SCHEME == S_SPARSE) {
+      uint32_t top = __ldcg(&c->slot_top[k]);
+      if (top > p.capacity) { top = p.capacity; c->slot_top[k] = top; c->overflow = 1u; }
+      if (top > c->slots_used[k]) c->slots_used[k] = top;
+    } else {
+      if (nn > c->slots_used[k]) c->slots_used[k] = nn;
+    }
+    c->n_cur[k] = nn;
+    c->n_next[k] = 0u;
+    c->it_alive[k] = 0u;
+    c->it_escaped[k] = 0u;
+    live_after += nn;
+  }
+  c->parity ^= 1u;
+  if (live_before) c->iterations += 1ull;
+  if (SCHEME == S_SPARSE && live_after == 0u) {  // rule S30: slots are recycled only when the buffer is empty
+    for (int k = 0; k < 3; ++k) c->slot_top[k] = 0u;
+  }
+  c->done_ctas = 0u;
+}
+
+// -------------------------------------------------------------------------- one tile ---------
+// Output counters of a thread, packed 3 x 10 bits (destination kind q at bits 10q..10q+9).
+template <int KIND> __device__ __forceinline__ uint32_t packed_outputs(const Outcome &o) {
+  uint32_t c = o.alive ? (1u << (10 * KIND)) : 0u;
+  if (KIND == K_GAMMA) {  // kid 0 is an e-, kid 1 an e+ (rule R5)
+    c += (o.kid[0].kind >= 0) ? 1u : 0u;
+    c += (o.kid[1].kind >= 0) ? (1u << 10) : 0u;
+  } else {  // kids of e-/e+ are photons
+    c += (o.kid[0].kind >= 0) ? (1u << 20) : 0u;
+    c += (o.kid[1].kind >= 0) ? (1u << 20) : 0u;
+  }
+  return c;
+}
+template <int KIND> __device__ __forceinline__ constexpr int kid_kind(int ordinal) {
+  return KIND == K_GAMMA ? (ordinal == 0 ? K_EM : K_EP) : K_GAMMA;
+}
+
+template <int KIND> __device__ __forceinline__ void do_step(Trk &t, const Env &env, Outcome &o) {
+  if constexpr (KIND == K_GAMMA) step_gamma(t, env, o);
+  else step_elec<KIND>(t, env, o);
+}
+
+// Process tile `tile` (256 consecutive entries) of kind KIND's current set.
+template <int L, int SCHEME, bool INSTR, int KIND>
+__device__ __forceinline__ void process_tile(const Params &p, const Env &env, CtaShared &sh, double *s_edep,
+                                             uint32_t par, uint32_t tile, uint32_t n_kind, int sbuf,
+                                             uint32_t &acc_alive, uint32_t &acc_esc, double &acc_esc_e) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const uint32_t i = tile * kBlock + tid;
+  const bool active = i < n_kind;
+  Ctl *ctl = p.ctl;
+
+  // A1: load
+  uint32_t slot = i;
+  if (SCHEME == S_SPARSE && active) slot = p.kind[KIND].queue[par][i];
+  const TrackView<L, INSTR> cur = make_view<L, INSTR>(p, KIND, (SCHEME == S_DENSE) ? int(par) : 0, sh.probe);
+  Trk t, old;
+  Outcome o;
+  outcome_init(o);
+  o.alive = false;
+  if (active) {
+    t = cur.load(slot);
+    old = t;
+    // A2-A8
+    do_step<KIND>(t, env, o);
+    // A6: scoring into the CTA's histogram (pre-step slab; the S31 guard uses the post-step slab)
+    if (o.dep != 0.0) atomicAdd(&s_edep[old.vol], o.dep);
+    if (o.dep2 != 0.0) atomicAdd(&s_edep[t.vol], o.dep2);
+    acc_esc_e += o.esc_e;
+  }
+
+  // tallies: survivors and escapes of this warp (lane 0 keeps the packed per-kind sums)
+  {
+    const uint32_t m_alive = __ballot_sync(0xFFFFFFFFu, o.alive);
+    const uint32_t m_esc = __ballot_sync(0xFFFFFFFFu, o.escaped);
+    acc_alive += __popc(m_alive);
+    acc_esc += __popc(m_esc);
+  }
+
+  const bool has0 = o.kid[0].kind >= 0, has1 = o.kid[1].kind >= 0;
+  constexpr int Q0 = kid_kind<KIND>(0), Q1 = kid_kind<KIND>(1);
+
+  if (SCHEME == S_DENSE) {
+    // A9: rank every output of the tile per destination kind with one packed scan
+    const uint32_t mine = packed_outputs<KIND>(o);
+    const uint32_t inc = warp_inclusive_scan(mine, lane);
+    if (lane == 31) sh.warp_tot[sbuf][warp] = inc;
+    __syncthreads();
+    uint32_t before = 0, total = 0;
+#pragma unroll
+    for (int w = 0; w < kBlock / 32; ++w) {
+      const uint32_t v = sh.warp_tot[sbuf][w];
+      total += v;
+      if (w < warp) before += v;
+    }
+    if (tid < 3) {
+      const uint32_t want = (total >> (10 * tid)) & 1023u;
+      sh.base[sbuf][tid] = want ? atomicAdd(&ctl->n_next[tid], want) : 0u;
+    }
+    __syncthreads();
+    const uint32_t excl = before + inc - mine;
+    uint32_t off[3];
+#pragma unroll
+    for (int q = 0; q < 3; ++q) off[q] = sh.base[sbuf][q] + ((excl >> (10 * q)) & 1023u);
+    const int nbuf = int(par ^ 1u);
+    bool dropped = false;
+    // A10: survivor, then children in ordinal order
+    if (o.alive) {
+      const uint32_t dst = off[KIND]++;
+      if (dst < p.capacity) make_view<L, INSTR>(p, KIND, nbuf, sh.probe).store(dst, t);
+      else dropped = true;
+    }
+    if (has0) {
+      const uint32_t dst = off[Q0]++;
+      if (dst < p.capacity) make_view<L, INSTR>(p, Q0, nbuf, sh.probe).store(dst, kid_track(t, o.kid[0]));
+      else dropped = true;
+    }
+    if (has1) {
+      const uint32_t dst = off[Q1]++;
+      if (dst < p.capacity) make_view<L, INSTR>(p, Q1, nbuf, sh.probe).store(dst, kid_track(t, o.kid[1]));
+      else dropped = true;
+    }
+    if (dropped) ctl->overflow = 1u;
+  } else {
+    // A10 sparse: in-place update of the words that changed, slot pushed onto the next list
+    const uint32_t qpos = warp_reserve(&ctl->n_next[KIND], o.alive ? 1u : 0u, lane);
+    bool dropped = false;
+    if (o.alive) {
+      cur.store_changed(slot, t, old);
+      if (qpos < p.capacity) p.kind[KIND].queue[par ^ 1u][qpos] = slot;
+      else dropped = true;
+    }
+    // A9 sparse: bump-allocated slots for the children (rule S30), warp-aggregated
+    if (Q0 == Q1) {
+      const uint32_t want = (has0 ? 1u : 0u) + (has1 ? 1u : 0u);
+      uint32_t s_new = warp_reserve(&ctl->slot_top[Q0], want, lane);
+      uint32_t q_new = warp_reserve(&ctl->n_next[Q0], want, lane);
+      const TrackView<L, INSTR> dst = make_view<L, INSTR>(p, Q0, 0, sh.probe);
+      if (has0) {
+        if (s_new < p.capacity && q_new < p.capacity) {
+          dst.store(s_new, kid_track(t, o.kid[0]));
+          p.kind[Q0].queue[par ^ 1u][q_new] = s_new;
+        } else dropped = true;
+        ++s_new; ++q_new;
+      }
+      if (has1) {
+        if (s_new < p.capacity && q_new < p.capacity) {
+          dst.store(s_new, kid_track(t, o.kid[1]));
+          p.kind[Q0].queue[par ^ 1u][q_new] = s_new;
+        } else dropped = true;
+      }
+    } else {
+      const uint32_t s0 = warp_reserve(&ctl->slot_top[Q0], has0 ? 1u : 0u, lane);
+      const uint32_t q0 = warp_reserve(&ctl->n_next[Q0], has0 ? 1u : 0u, lane);
+      const uint32_t s1 = warp_reserve(&ctl->slot_top[Q1], has1 ? 1u : 0u, lane);
+      const uint32_t q1 = warp_reserve(&ctl->n_next[Q1], has1 ? 1u : 0u, lane);
+      if (has0) {
+        if (s0 < p.capacity && q0 < p.capacity) {
+          make_view<L, INSTR>(p, Q0, 0, sh.probe).store(s0, kid_track(t, o.kid[0]));
+          p.kind[Q0].queue[par ^ 1u][q0] = s0;
+        } else dropped = true;
+      }
+      if (has1) {
+        if (s1 < p.capacity && q1 < p.capacity) {
+          make_view<L, INSTR>(p, Q1, 0, sh.probe).store(s1, kid_track(t, o.kid[1]));
+          p.kind[Q1].queue[par ^ 1u][q1] = s1;
+        } else dropped = true;
+      }
+    }
+    if (dropped) ctl->overflow = 1u;
+  }
+}
+
+// ---------------------------------------------------------------------- the step kernel ------
+// Dynamic shared memory: [tables (p.table_bytes)] [edep histogram (n_slabs doubles)].
+template <int L, int SCHEME, bool INSTR>
+__global__ void __launch_bounds__(kBlock) step_kernel(const __grid_constant__ Params p) {
+  extern __shared__ __align__(16) unsigned char dyn_smem[];
+  __shared__ CtaShared sh;
+  float4 *s_tab = reinterpret_cast<float4 *>(dyn_smem);
+  double *s_edep = reinterpret_cast<double *>(dyn_smem + p.table_bytes);
+  const int tid = threadIdx.x;
+  Ctl *ctl = p.ctl;
+
+  // A0: what is alive (written by the previous iteration's last CTA; constant during this launch)
+  const uint32_t par = ctl->parity;
+  const uint32_t n0 = ctl->n_cur[0], n1 = ctl->n_cur[1], n2 = ctl->n_cur[2];
+  const uint32_t t0 = (n0 + kBlock - 1) / kBlock, t1 = (n1 + kBlock - 1) / kBlock, t2 = (n2 + kBlock - 1) / kBlock;
+  const uint32_t tiles = t0 + t1 + t2;
+
+  if (blockIdx.x < tiles) {
+    // A3: tables -> shared memory, one TMA bulk copy; histogram and counters cleared meanwhile
+    tma_stage(s_tab, p.tables, p.table_bytes, &sh.mbar, tid);
+    for (uint32_t s = tid; s < p.n_slabs; s += kBlock) s_edep[s] = 0.0;
+    if (tid < 4) { sh.alive[tid] = 0u; sh.escaped[tid] = 0u; }
+    if (tid == 0) sh.esc_e = 0.0;
+    if (INSTR) for (int s = tid; s < 3 * kNumFields * 2; s += kBlock) sh.probe[s] = 0u;
+    tma_wait(&sh.mbar);
+    __syncthreads();
+
+    Env env;
+    env.tab = s_tab; env.nodes = p.nodes;
+    env.ln_e_min = p.ln_e_min; env.inv_dln = p.inv_dln; env.e_cut = p.e_cut;
+    env.n_slabs = p.n_slabs; env.abs_mm = p.abs_mm; env.pitch = p.pitch; env.half_xy = p.half_xy;
+    env.mat_abs = p.mat_abs; env.mat_gap = p.mat_gap;
+
+    uint32_t alive0 = 0, alive1 = 0, alive2 = 0, esc0 = 0, esc1 = 0, esc2 = 0;
+    double esc_e = 0.0;
+    int sbuf = 0;
+    for (uint32_t tile = blockIdx.x; tile < tiles; tile += gridDim.x, sbuf ^= 1) {
+      if (tile < t0) {
+        process_tile<L, SCHEME, INSTR, K_EM>(p, env, sh, s_edep, par, tile, n0, sbuf, alive0, esc0, esc_e);
+      } else if (tile < t0 + t1) {
+        process_tile<L, SCHEME, INSTR, K_EP>(p, env, sh, s_edep, par, tile - t0, n1, sbuf, alive1, esc1, esc_e);
+      } else {
+        process_tile<L, SCHEME, INSTR, K_GAMMA>(p, env, sh, s_edep, par, tile - t0 - t1, n2, sbuf, alive2, esc2, esc_e);
+      }
+    }
+
+    // flush the CTA's tallies
+    esc_e = warp_sum(esc_e);
+    if ((tid & 31) == 0) {
+      if (alive0) atomicAdd(&sh.alive[0], alive0);
+      if (alive1) atomicAdd(&sh.alive[1], alive1);
+      if (alive2) atomicAdd(&sh.alive[2], alive2);
+      if (esc0) atomicAdd(&sh.escaped[0], esc0);
+      if (esc1) atomicAdd(&sh.escaped[1], esc1);
+      if (esc2) atomicAdd(&sh.escaped[2], esc2);
+      if (esc_e != 0.0) atomicAdd(&sh.esc_e, esc_e);
+    }
+    __syncthreads();
+    for (uint32_t s = tid; s < p.n_slabs; s += kBlock) {
+      const double v = s_edep[s];
+      if (v != 0.0) atomicAdd(&p.edep[s], v);
+    }
+    if (tid < 3) {
+      if (sh.alive[tid]) atomicAdd(&ctl->it_alive[tid], sh.alive[tid]);
+      if (sh.escaped[tid]) atomicAdd(&ctl->it_escaped[tid], sh.escaped[tid]);
+    }
+    if (tid == 0 && sh.esc_e != 0.0) atomicAdd(&ctl->e_escaped, sh.esc_e);
+    if (INSTR) {
+      for (int s = tid; s < 3 * kNumFields * 2; s += kBlock)
+        if (sh.probe[s]) atomicAdd(&p.instr_field_rw[s], static_cast<unsigned long long>(sh.probe[s]));
+    }
+  }
+
+  // A11: the last CTA to arrive ends the iteration
+  __syncthreads();
+  if (tid == 0) {
+    __threadfence();
+    const uint32_t ticket = atomicAdd(&ctl->done_ctas, 1u);
+    if (ticket == gridDim.x - 1) {
+      __threadfence();
+      finish_iteration<SCHEME>(p);
+    }
+  }
+}
+
+// ------------------------------------------------------------- host <-> buffer helper kernels --
+struct StagedPrimary {  // adept_primary + its global index (rule R4)
+  uint32_t kind;
+  float pos[3], dir[3], ekin;
+  unsigned long long gidx;
+};
+struct PackedTrack {  // = adept_track, 56 B
+  float pos[3], dir[3], ekin, nial[3];
+  uint32_t vol, id_lo, id_hi, step;
+};
+
+__device__ __forceinline__ Trk unpack(const PackedTrack &a) {
+  Trk t;
+  t.px = a.pos[0]; t.py = a.pos[1]; t.pz = a.pos[2];
+  t.dx = a.dir[0]; t.dy = a.dir[1]; t.dz = a.dir[2];
+  t.ekin = a.ekin; t.n0 = a.nial[0]; t.n1 = a.nial[1]; t.n2 = a.nial[2];
+  t.vol = a.vol; t.id_lo = a.id_lo; t.id_hi = a.id_hi; t.step = a.step;
+  return t;
+}
+__device__ __forceinline__ PackedTrack pack(const Trk &t) {
+  PackedTrack a;
+  a.pos[0] = t.px; a.pos[1] = t.py; a.pos[2] = t.pz;
+  a.dir[0] = t.dx; a.dir[1] = t.dy; a.dir[2] = t.dz;
+  a.ekin = t.ekin; a.nial[0] = t.n0; a.nial[1] = t.n1; a.nial[2] = t.n2;
+  a.vol = t.vol; a.id_lo = t.id_lo; a.id_hi = t.id_hi; a.step = t.step;
+  return a;
+}
+
+template <int L> __device__ __forceinline__ TrackView<L, false> plain_view(const Params &p, int kind, int buf) {
+  TrackView<L, false> v;
+  v.base = p.kind[kind].rec[buf];
+  v.cap = p.capacity;
+  v.storage_off = 0; v.buf_index = 0;
+  v.sink.cta_field_rw = nullptr; v.sink.lines = nullptr; v.sink.slots = nullptr;
+  return v;
+}
+
+// Where entry `i` of the current set of `kind` lives: dense = array index, sparse = slot list.
+template <int SCHEME>
+__device__ __forceinline__ void place(const Params &p, int kind, uint32_t par, uint32_t entry, uint32_t slot,
+                                      int &buf, uint32_t &where) {
+  if (SCHEME == S_DENSE) { buf = int(par); where = entry; }
+  else { buf = 0; where = slot; p.kind[kind].queue[par][entry] = slot; }
+}
+
+// Primaries -> tracks (rule R4 ids, slab located from z; step 0, nial -1).
+template <int L, int SCHEME>
+__global__ void inject_kernel(const __grid_constant__ Params p, const StagedPrimary *sp, uint32_t n, int kind,
+                              uint32_t par, uint32_t entry_base, uint32_t slot_base, unsigned long long seed) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const StagedPrimary a = sp[i];
+  Trk t;
+  t.px = a.pos[0]; t.py = a.pos[1]; t.pz = a.pos[2];
+  t.dx = a.dir[0]; t.dy = a.dir[1]; t.dz = a.dir[2];
+  t.ekin = a.ekin;
+  t.n0 = -1.0f; t.n1 = -1.0f; t.n2 = -1.0f;
+  int layer = static_cast<int>(a.pos[2] / p.pitch);
+  const int last = static_cast<int>(p.n_slabs / 2u) - 1;
+  if (layer > last) layer = last;
+  const float rel = a.pos[2] - static_cast<float>(layer) * p.pitch;
+  t.vol = 2u * static_cast<uint32_t>(layer) + ((rel >= p.abs_mm) ? 1u : 0u);
+  const uint2 id = primary_id(a.gidx, seed);
+  t.id_lo = id.x; t.id_hi = id.y;
+  t.step = 0u;
+  int buf; uint32_t where;
+  place<SCHEME>(p, kind, par, entry_base + i, slot_base + i, buf, where);
+  plain_view<L>(p, kind, buf).store(where, t);
+}
+
+template <int L, int SCHEME>
+__global__ void load_kernel(const __grid_constant__ Params p, const PackedTrack *src, const uint32_t *slots,
+                            uint32_t n, int kind, uint32_t par, uint32_t entry_base, uint32_t slot_base) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  int buf; uint32_t where;
+  place<SCHEME>(p, kind, par, entry_base + i, slots ? slots[i] : slot_base + i, buf, where);
+  plain_view<L>(p, kind, buf).store(where, unpack(src[i]));
+}
+
+template <int L, int SCHEME>
+__global__ void read_kernel(const __grid_constant__ Params p, PackedTrack *dst, uint32_t first, uint32_t n,
+                            int kind, uint32_t par) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint32_t entry = first + i;
+  if (SCHEME == S_DENSE) dst[i] = pack(plain_view<L>(p, kind, int(par)).load(entry));
+  else dst[i] = pack(plain_view<L>(p, kind, 0).load(p.kind[kind].queue[par][entry]));
+}
+
+// ----------------------------------------------------------------- per-layout entry points ----
+// One table of launchers per layout; adept_api.cu picks the table once at adept_create.  (Layout,
+// scheme and instrumentation are compile-time parameters of every kernel.)
+struct LayoutOps {
+  size_t (*record_words)(size_t capacity);
+  int (*step_ctas_per_sm)(int scheme, int instr, size_t dyn_smem);
+  cudaError_t (*launch_step)(int scheme, int instr, const Params &, unsigned grid, size_t dyn_smem, cudaStream_t);
+  cudaError_t (*launch_inject)(int scheme, const Params &, const void *staged, uint32_t n, int kind, uint32_t par,
+                               uint32_t entry_base, uint32_t slot_base, unsigned long long seed, cudaStream_t);
+  cudaError_t (*launch_load)(int scheme, const Params &, const void *staged, const uint32_t *slots, uint32_t n,
+                             int kind, uint32_t par, uint32_t entry_base, uint32_t slot_base, cudaStream_t);
+  cudaError_t (*launch_read)(int scheme, const Params &, void *staged, uint32_t first, uint32_t n, int kind,
+                             uint32_t par, cudaStream_t);
+};
+
+template <int L> struct OpsImpl {
+  template <typename F> static auto pick(int scheme, int instr, F f) {
+    if (scheme == S_DENSE) return instr ? f(step_kernel<L, S_DENSE, true>) : f(step_kernel<L, S_DENSE, false>);
+    return instr ? f(step_kernel<L, S_SPARSE, true>) : f(step_kernel<L, S_SPARSE, false>);
+  }
+  static size_t record_words(size_t cap) { return Mapping<L>::words(cap); }
+  static int step_ctas_per_sm(int scheme, int instr, size_t dyn) {
+    return pick(scheme, instr, [&](auto *k) {
+      int n = 0;
+      if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, int(dyn)) != cudaSuccess) return -1;
+      if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k, kBlock, dyn) != cudaSuccess) return -1;
+      return n;
+    });
+  }
+  static cudaError_t launch_step(int scheme, int instr, const Params &p, unsigned grid, size_t dyn, cudaStream_t s) {
+    return pick(scheme, instr, [&](auto *k) {
+      k<<<grid, kBlock, dyn, s>>>(p);
+      return cudaGetLastError();
+    });
+  }
+  static cudaError_t launch_inject(int scheme, const Params &p, const void *staged, uint32_t n, int kind,
+                                   uint32_t par, uint32_t eb, uint32_t sb, unsigned long long seed, cudaStream_t s) {
+    const unsigned g = (n + 255) / 256;
+    const StagedPrimary *sp = static_cast<const StagedPrimary *>(staged);
+    if (scheme == S_DENSE) inject_kernel<L, S_DENSE><<<g, 256, 0, s>>>(p, sp, n, kind, par, eb, sb, seed);
+    else inject_kernel<L, S_SPARSE><<<g, 256, 0, s>>>(p, sp, n, kind, par, eb, sb, seed);
+    return cudaGetLastError();
+  }
+  static cudaError_t launch_load(int scheme, const Params &p, const void *staged, const uint32_t *slots, uint32_t n,
+                                 int kind, uint32_t par, uint32_t eb, uint32_t sb, cudaStream_t s) {
+    const unsigned g = (n + 255) / 256;
+    const PackedTrack *src = static_cast<const PackedTrack *>(staged);
+    if (scheme == S_DENSE) load_kernel<L, S_DENSE><<<g, 256, 0, s>>>(p, src, slots, n, kind, par, eb, sb);
+    else load_kernel<L, S_SPARSE><<<g, 256, 0, s>>>(p, src, slots, n, kind, par, eb, sb);
+    return cudaGetLastError();
+  }
+  static cudaError_t launch_read(int scheme, const Params &p, void *staged, uint32_t first, uint32_t n, int kind,
+                                 uint32_t par, cudaStream_t s) {
+    const unsigned g = (n + 255) / 256;
+    PackedTrack *dst = static_cast<PackedTrack *>(staged);
+    if (scheme == S_DENSE) read_kernel<L, S_DENSE><<<g, 256, 0, s>>>(p, dst, first, n, kind, par);
+    else read_kernel<L, S_SPARSE><<<g, 256, 0, s>>>(p, dst, first, n, kind, par);
+    return cudaGetLastError();
+  }
+  static LayoutOps make() {
+    return LayoutOps{record_words, step_ctas_per_sm, launch_step, launch_inject, launch_load, launch_read};
+  }
+};
+
+extern const LayoutOps kOpsAoS, kOpsSoA, kOpsAoSoA32;
+
+}  // namespace adept
