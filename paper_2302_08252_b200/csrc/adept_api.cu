@@ -199,3 +199,385 @@ __global__ void dev_math_kernel(int fn, const void *in, void *out, unsigned long
 }
 
 }  // namespace
+
+// =================================================================== extern "C" =============
+extern "C" {
+
+size_t adept_workspace_bytes(const adept_geometry *g, const adept_tables *t, const adept_config *c) {
+  Plan pl;
+  return make_plan(g, t, c, pl) ? pl.total : 0;
+}
+
+const char *adept_last_error(const adept_ctx *c) { return c ? c->err.c_str() : g_create_error.c_str(); }
+
+static int clear_state(adept_ctx *c) {
+  // everything except the tables: control block, edep, instrumentation counters
+  const Plan &pl = c->plan;
+  CU(c, cudaMemsetAsync(c->ws + pl.ctl, 0, pl.tables - pl.ctl, c->stream));
+  if (c->cfg.instrument && pl.total > pl.instr_rw)
+    CU(c, cudaMemsetAsync(c->ws + pl.instr_rw, 0, pl.total - pl.instr_rw, c->stream));
+  c->pending.clear();
+  c->pending_done = 0;
+  c->next_primary = 0;
+  c->e_injected = 0.0;
+  c->dead = false;
+  return ADEPT_OK;
+}
+
+int adept_create(const adept_geometry *g, const adept_tables *t, const adept_config *cfg, adept_ctx **out) {
+  g_create_error.clear();
+  auto bad = [&](const char *why) { g_create_error = why; return ADEPT_EINVAL; };
+  if (!out) return bad("out is NULL");
+  *out = nullptr;
+  Plan pl;
+  if (!make_plan(g, t, cfg, pl)) return bad("invalid geometry, tables or configuration");
+  if (!t->data) return bad("tables.data is NULL");
+  if (!(g->abs_mm > 0.0f) || !(g->gap_mm > 0.0f) || !(g->half_xy_mm > 0.0f)) return bad("non-positive geometry");
+  if (g->mat_abs >= t->n_materials || g->mat_gap >= t->n_materials) return bad("material index out of range");
+  if (!(t->e_cut > 0.0f) || !(t->e_max > t->e_min) || !(t->e_min > 0.0f)) return bad("invalid energy grid");
+  if (!cfg->workspace || (reinterpret_cast<uintptr_t>(cfg->workspace) % kAlign) != 0) return bad("workspace must be a 256-byte aligned device pointer");
+  if (cfg->workspace_bytes < pl.total) return bad("workspace too small (see adept_workspace_bytes)");
+
+  adept_ctx *c = new (std::nothrow) adept_ctx();
+  if (!c) return bad("out of host memory");
+  c->geo = *g; c->tab = *t; c->tab.data = nullptr; c->cfg = *cfg; c->plan = pl;
+  c->ops = ops_for(cfg->layout);
+  c->stream = static_cast<cudaStream_t>(cfg->cuda_stream);
+  c->ws = static_cast<unsigned char *>(cfg->workspace);
+  c->pinned = nullptr;
+  c->pitch = g->abs_mm + g->gap_mm;
+  c->depth = static_cast<float>(g->n_layers) * c->pitch;
+  auto die = [&](const char *what, cudaError_t e) {
+    g_create_error = std::string(what) + ": " + cudaGetErrorString(e);
+    if (c->pinned) cudaFreeHost(c->pinned);
+    delete c;
+    return ADEPT_ECUDA;
+  };
+  cudaError_t e;
+  c->pinned_bytes = kCtlHeaderBytes + size_t(2) * g->n_layers * sizeof(double);
+  if ((e = cudaMallocHost(reinterpret_cast<void **>(&c->pinned), c->pinned_bytes)) != cudaSuccess)
+    return die("cudaMallocHost", e);
+
+  // tables: [mat][group][qty][node] (host, ABI) -> [mat][group][node]{q0,q1,q2,0} (device): one
+  // 16-byte shared-memory load fetches all three quantities of a node.
+  const uint32_t nodes = t->n_bins + 1;
+  std::vector<float> packed(pl.table_bytes / sizeof(float), 0.0f);
+  for (uint32_t m = 0; m < t->n_materials; ++m)
+    for (uint32_t grp = 0; grp < 2; ++grp)
+      for (uint32_t q = 0; q < 3; ++q)
+        for (uint32_t j = 0; j < nodes; ++j)
+          packed[((size_t(m) * 2 + grp) * nodes + j) * 4 + q] = t->data[((size_t(m) * 2 + grp) * 3 + q) * nodes + j];
+  if ((e = cudaMemcpyAsync(c->ws + pl.tables, packed.data(), pl.table_bytes, cudaMemcpyHostToDevice, c->stream)) != cudaSuccess)
+    return die("cudaMemcpyAsync(tables)", e);
+  if ((e = cudaStreamSynchronize(c->stream)) != cudaSuccess) return die("cudaStreamSynchronize", e);
+
+  Params &p = c->params;
+  p.ctl = reinterpret_cast<Ctl *>(c->ws + pl.ctl);
+  p.edep = reinterpret_cast<double *>(c->ws + pl.ctl + kCtlHeaderBytes);
+  p.tables = reinterpret_cast<const float4 *>(c->ws + pl.tables);
+  p.table_bytes = static_cast<uint32_t>(pl.table_bytes);
+  p.nodes = nodes;
+  p.ln_e_min = t->ln_e_min; p.inv_dln = t->inv_dln; p.e_cut = t->e_cut;
+  p.n_slabs = 2 * g->n_layers;
+  p.abs_mm = g->abs_mm; p.pitch = c->pitch; p.half_xy = g->half_xy_mm;
+  p.mat_abs = g->mat_abs; p.mat_gap = g->mat_gap;
+  p.capacity = pl.capacity;
+  for (int k = 0; k < 3; ++k) {
+    uint32_t *r = reinterpret_cast<uint32_t *>(c->ws + pl.rec[k]);
+    p.kind[k].rec[0] = r;
+    p.kind[k].rec[1] = (pl.nbuf == 2) ? r + pl.rec_words : r;
+    p.kind[k].queue[0] = reinterpret_cast<uint32_t *>(c->ws + pl.queue[k][0]);
+    p.kind[k].queue[1] = reinterpret_cast<uint32_t *>(c->ws + pl.queue[k][1]);
+    p.kind[k].instr_lines = reinterpret_cast<uint32_t *>(c->ws + pl.instr_lines[k]);
+    p.kind[k].instr_slots = reinterpret_cast<uint32_t *>(c->ws + pl.instr_slots[k]);
+  }
+  p.instr_field_rw = reinterpret_cast<unsigned long long *>(c->ws + pl.instr_rw);
+
+  // persistent grid: as many CTAs as fit on the device at once
+  c->dyn_smem = pl.table_bytes + size_t(p.n_slabs) * sizeof(double);
+  int dev = 0, sms = 0;
+  if ((e = cudaGetDevice(&dev)) != cudaSuccess) return die("cudaGetDevice", e);
+  if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess)
+    return die("cudaDeviceGetAttribute", e);
+  const int per_sm = c->ops->step_ctas_per_sm(cfg->scheme, cfg->instrument ? 1 : 0, c->dyn_smem);
+  if (per_sm <= 0) {
+    g_create_error = "step kernel does not fit on an SM with these tables (shared memory)";
+    cudaFreeHost(c->pinned);
+    delete c;
+    return ADEPT_EINVAL;
+  }
+  c->grid = static_cast<unsigned>(sms * per_sm);
+
+  int rc = clear_state(c);
+  if (rc == ADEPT_OK && (e = cudaStreamSynchronize(c->stream)) != cudaSuccess) rc = ADEPT_ECUDA;
+  if (rc != ADEPT_OK) {
+    g_create_error = c->err.empty() ? "clearing the workspace failed" : c->err;
+    cudaFreeHost(c->pinned);
+    delete c;
+    return rc;
+  }
+  *out = c;
+  return ADEPT_OK;
+}
+
+int adept_destroy(adept_ctx *c) {
+  if (!c) return ADEPT_EINVAL;
+  cudaStreamSynchronize(c->stream);
+  if (c->pinned) cudaFreeHost(c->pinned);
+  delete c;
+  return ADEPT_OK;
+}
+
+int adept_reset(adept_ctx *c) {
+  if (!c) return ADEPT_EINVAL;
+  int rc = clear_state(c);
+  if (rc != ADEPT_OK) return rc;
+  CU(c, cudaStreamSynchronize(c->stream));
+  c->err.clear();
+  return ADEPT_OK;
+}
+
+// ---- appending tracks from the host --------------------------------------------------------
+static int check_alive(adept_ctx *c) {
+  if (!c) return ADEPT_EINVAL;
+  if (c->dead) return fail(c, ADEPT_ESTATE, "context overflowed: only adept_reset / adept_destroy are accepted");
+  return ADEPT_OK;
+}
+
+static bool primary_ok(const adept_ctx *c, const adept_primary &p) {
+  if (p.kind > 2u) return false;
+  if (!(p.pos[2] >= 0.0f) || !(p.pos[2] <= c->depth)) return false;
+  if (!(std::fabs(p.pos[0]) <= c->geo.half_xy_mm) || !(std::fabs(p.pos[1]) <= c->geo.half_xy_mm)) return false;
+  if (!(p.ekin >= c->tab.e_cut) || !(p.ekin <= c->tab.e_max)) return false;
+  return true;
+}
+
+// Make `n` validated primaries live (rule R4: ids from the running global index).
+static int inject_now(adept_ctx *c, const adept_primary *prim, uint64_t n) {
+  if (n == 0) return ADEPT_OK;
+  int rc = fetch_ctl(c, false);
+  if (rc != ADEPT_OK) return rc;
+  const Ctl h = *host_ctl(c);
+  const bool sparse = c->cfg.scheme == ADEPT_SPARSE_SINGLE;
+  uint32_t n_cur[3], top[3];
+  uint64_t add[3] = {0, 0, 0};
+  for (uint64_t i = 0; i < n; ++i) add[prim[i].kind] += 1;
+  for (int k = 0; k < 3; ++k) {
+    n_cur[k] = h.n_cur[k]; top[k] = h.slot_top[k];
+    if (n_cur[k] + add[k] > c->plan.capacity || (sparse && top[k] + add[k] > c->plan.capacity))
+      return fail(c, ADEPT_ECAPACITY, "adept_inject: more primaries than free capacity");
+  }
+  std::vector<StagedPrimary> stage;
+  for (int k = 0; k < 3; ++k) {
+    if (!add[k]) continue;
+    stage.clear();
+    stage.reserve(add[k]);
+    for (uint64_t i = 0; i < n; ++i) {
+      if (prim[i].kind != uint32_t(k)) continue;
+      StagedPrimary s;
+      s.kind = prim[i].kind;
+      std::memcpy(s.pos, prim[i].pos, sizeof s.pos);
+      std::memcpy(s.dir, prim[i].dir, sizeof s.dir);
+      s.ekin = prim[i].ekin;
+      s.gidx = c->next_primary + i;
+      stage.push_back(s);
+    }
+    for (uint64_t done = 0; done < add[k];) {
+      const uint32_t m = uint32_t(std::min<uint64_t>(add[k] - done, c->plan.stage_records));
+      CU(c, cudaMemcpyAsync(c->ws + c->plan.stage, stage.data() + done, size_t(m) * sizeof(StagedPrimary),
+                            cudaMemcpyHostToDevice, c->stream));
+      CU(c, c->ops->launch_inject(c->cfg.scheme, c->params, c->ws + c->plan.stage, m, k, h.parity, n_cur[k], top[k],
+                                  c->cfg.seed, c->stream));
+      CU(c, cudaStreamSynchronize(c->stream));  // the staging area and `stage` are reused
+      n_cur[k] += m;
+      if (sparse) top[k] += m;
+      done += m;
+    }
+    set_counts_kernel<<<1, 1, 0, c->stream>>>(c->params.ctl, k, n_cur[k], top[k], sparse ? top[k] : n_cur[k]);
+    CU(c, cudaGetLastError());
+  }
+  for (uint64_t i = 0; i < n; ++i)
+    c->e_injected += double(prim[i].ekin) + (prim[i].kind == 1u ? double(2.0f * kMc2) : 0.0);
+  c->next_primary += n;
+  return ADEPT_OK;
+}
+
+int adept_inject(adept_ctx *c, const adept_primary *prim, uint64_t n) {
+  int rc = check_alive(c);
+  if (rc != ADEPT_OK) return rc;
+  if (n && !prim) return fail(c, ADEPT_EINVAL, "adept_inject: primaries is NULL");
+  for (uint64_t i = 0; i < n; ++i)
+    if (!primary_ok(c, prim[i])) return fail(c, ADEPT_EINVAL, "adept_inject: primary outside the calorimeter or energy grid");
+  if (c->cfg.batch_primaries == 0) return inject_now(c, prim, n);
+  c->pending.insert(c->pending.end(), prim, prim + n);
+  return ADEPT_OK;
+}
+
+int adept_load_tracks(adept_ctx *c, uint32_t kind, const adept_track *tracks, uint64_t n, const uint32_t *slots) {
+  int rc = check_alive(c);
+  if (rc != ADEPT_OK) return rc;
+  if (kind > 2u || (n && !tracks)) return fail(c, ADEPT_EINVAL, "adept_load_tracks: bad kind or NULL tracks");
+  if (n == 0) return ADEPT_OK;
+  rc = fetch_ctl(c, false);
+  if (rc != ADEPT_OK) return rc;
+  const Ctl h = *host_ctl(c);
+  const bool sparse = c->cfg.scheme == ADEPT_SPARSE_SINGLE;
+  const uint32_t cap = c->plan.capacity;
+  if (h.n_cur[kind] + n > cap) return fail(c, ADEPT_EINVAL, "adept_load_tracks: more tracks than free capacity");
+  uint32_t top = h.slot_top[kind];
+  if (sparse) {
+    if (slots) {
+      for (uint64_t i = 0; i < n; ++i) {
+        if (slots[i] >= cap) return fail(c, ADEPT_EINVAL, "adept_load_tracks: slot out of range");
+        top = std::max(top, slots[i] + 1u);
+      }
+    } else {
+      if (top + n > cap) return fail(c, ADEPT_EINVAL, "adept_load_tracks: more tracks than free slots");
+    }
+  }
+  uint32_t n_cur = h.n_cur[kind], next_slot = h.slot_top[kind];
+  for (uint64_t done = 0; done < n;) {
+    const uint32_t m = uint32_t(std::min<uint64_t>(n - done, c->plan.stage_records));
+    CU(c, cudaMemcpyAsync(c->ws + c->plan.stage, tracks + done, size_t(m) * sizeof(adept_track),
+                          cudaMemcpyHostToDevice, c->stream));
+    const uint32_t *dslots = nullptr;
+    if (sparse && slots) {
+      CU(c, cudaMemcpyAsync(c->ws + c->plan.stage_slots, slots + done, size_t(m) * 4, cudaMemcpyHostToDevice, c->stream));
+      dslots = reinterpret_cast<const uint32_t *>(c->ws + c->plan.stage_slots);
+    }
+    CU(c, c->ops->launch_load(c->cfg.scheme, c->params, c->ws + c->plan.stage, dslots, m, int(kind), h.parity, n_cur,
+                              next_slot, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    n_cur += m;
+    next_slot += m;
+    done += m;
+  }
+  if (sparse && !slots) top = next_slot;
+  set_counts_kernel<<<1, 1, 0, c->stream>>>(c->params.ctl, int(kind), n_cur, top, sparse ? top : n_cur);
+  CU(c, cudaGetLastError());
+  return ADEPT_OK;
+}
+
+int adept_read_tracks(adept_ctx *c, uint32_t kind, adept_track *out, uint64_t cap, uint64_t *n) {
+  if (!c || kind > 2u || !n) return c ? fail(c, ADEPT_EINVAL, "adept_read_tracks: bad argument") : ADEPT_EINVAL;
+  int rc = fetch_ctl(c, false);
+  if (rc != ADEPT_OK && rc != ADEPT_ECAPACITY) return rc;
+  const Ctl h = *host_ctl(c);
+  *n = h.n_cur[kind];
+  if (*n > cap || (*n && !out)) return fail(c, ADEPT_EINVAL, "adept_read_tracks: output array too small");
+  for (uint64_t done = 0; done < *n;) {
+    const uint32_t m = uint32_t(std::min<uint64_t>(*n - done, c->plan.stage_records));
+    CU(c, c->ops->launch_read(c->cfg.scheme, c->params, c->ws + c->plan.stage, uint32_t(done), m, int(kind), h.parity,
+                              c->stream));
+    CU(c, cudaMemcpyAsync(out + done, c->ws + c->plan.stage, size_t(m) * sizeof(adept_track), cudaMemcpyDeviceToHost,
+                          c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    done += m;
+  }
+  return rc;
+}
+
+// ---- iterations -----------------------------------------------------------------------------
+static int launch_iteration(adept_ctx *c) {
+  CU(c, c->ops->launch_step(c->cfg.scheme, c->cfg.instrument ? 1 : 0, c->params, c->grid, c->dyn_smem, c->stream));
+  return ADEPT_OK;
+}
+
+int adept_step(adept_ctx *c, adept_counts *out) {
+  int rc = check_alive(c);
+  if (rc != ADEPT_OK) return rc;
+  rc = launch_iteration(c);
+  if (rc != ADEPT_OK || !out) return rc;
+  rc = fetch_ctl(c, false);
+  fill_counts(c, out);
+  return rc;
+}
+
+int adept_get_result(adept_ctx *c, adept_result *out) {
+  if (!c || !out) return c ? fail(c, ADEPT_EINVAL, "adept_get_result: out is NULL") : ADEPT_EINVAL;
+  const int rc = fetch_ctl(c, true);
+  if (rc != ADEPT_OK && rc != ADEPT_ECAPACITY) return rc;
+  fill_result(c, out);
+  return rc;
+}
+
+int adept_run(adept_ctx *c, uint64_t max_iterations, adept_result *out) {
+  int rc = check_alive(c);
+  if (rc != ADEPT_OK) return rc;
+  // Iterations are enqueued in bursts; the control block is read back after each burst.  An
+  // iteration with nothing alive is a no-op on the device (and is not counted), so over-shooting
+  // the end of a shower by a few launches is harmless.
+  const uint64_t kBurst = 8;
+  uint64_t done = 0;
+  for (;;) {
+    rc = fetch_ctl(c, false);
+    if (rc != ADEPT_OK) break;
+    const Ctl *h = host_ctl(c);
+    const uint64_t live = uint64_t(h->n_cur[0]) + h->n_cur[1] + h->n_cur[2];
+    if (live == 0) {
+      if (c->pending_done >= c->pending.size()) break;
+      const uint64_t batch = std::min<uint64_t>(c->cfg.batch_primaries ? c->cfg.batch_primaries : c->pending.size(),
+                                                c->pending.size() - c->pending_done);
+      rc = inject_now(c, c->pending.data() + c->pending_done, batch);
+      if (rc != ADEPT_OK) break;
+      c->pending_done += batch;
+      if (c->pending_done >= c->pending.size()) { c->pending.clear(); c->pending_done = 0; }
+    }
+    if (max_iterations && done >= max_iterations) break;
+    uint64_t burst = kBurst;
+    if (max_iterations) burst = std::min<uint64_t>(burst, max_iterations - done);
+    for (uint64_t i = 0; i < burst && rc == ADEPT_OK; ++i) rc = launch_iteration(c);
+    if (rc != ADEPT_OK) break;
+    done += burst;
+  }
+  if (out && (rc == ADEPT_OK || rc == ADEPT_ECAPACITY)) {
+    const int rc2 = fetch_ctl(c, true);
+    if (rc2 == ADEPT_OK || rc2 == ADEPT_ECAPACITY) fill_result(c, out);
+    if (rc == ADEPT_OK) rc = rc2;
+  }
+  return rc;
+}
+
+// ---- instrumentation ------------------------------------------------------------------------
+uint64_t adept_instr_lines(const adept_ctx *c) { return (c && c->cfg.instrument) ? c->plan.lines_per_kind : 0; }
+uint64_t adept_instr_slots(const adept_ctx *c) { return (c && c->cfg.instrument) ? c->plan.slots_per_kind : 0; }
+
+int adept_read_counters(adept_ctx *c, uint64_t *field_rw, uint32_t *lines, uint32_t *slots) {
+  if (!c) return ADEPT_EINVAL;
+  if (!c->cfg.instrument) return fail(c, ADEPT_ESTATE, "adept_read_counters: context was not created with instrument = 1");
+  const Plan &pl = c->plan;
+  CU(c, cudaStreamSynchronize(c->stream));
+  if (field_rw)
+    CU(c, cudaMemcpy(field_rw, c->ws + pl.instr_rw, 3 * kNumFields * 2 * sizeof(uint64_t), cudaMemcpyDeviceToHost));
+  for (int k = 0; k < 3; ++k) {
+    if (lines)
+      CU(c, cudaMemcpy(lines + size_t(k) * pl.lines_per_kind, c->ws + pl.instr_lines[k], pl.lines_per_kind * 4,
+                       cudaMemcpyDeviceToHost));
+    if (slots)
+      CU(c, cudaMemcpy(slots + size_t(k) * pl.slots_per_kind, c->ws + pl.instr_slots[k], pl.slots_per_kind * 4,
+                       cudaMemcpyDeviceToHost));
+  }
+  return ADEPT_OK;
+}
+
+uint64_t adept_field_offset(int32_t layout, uint32_t capacity, uint32_t slot, uint32_t field) {
+  if (field >= uint32_t(kNumFields) || capacity == 0) return UINT64_MAX;
+  const size_t cap = (size_t(capacity) + 31) / 32 * 32;
+  if (slot >= cap) return UINT64_MAX;
+  switch (layout) {
+    case ADEPT_AOS: return 4 * Mapping<L_AOS>::index(cap, slot, int(field));
+    case ADEPT_SOA: return 4 * Mapping<L_SOA>::index(cap, slot, int(field));
+    case ADEPT_AOSOA32: return 4 * Mapping<L_AOSOA32>::index(cap, slot, int(field));
+    default: return UINT64_MAX;
+  }
+}
+
+int adept_dev_math(int fn, const void *in, void *out, uint64_t n, void *cuda_stream) {
+  if (fn < 0 || fn > 4 || (n && (!in || !out))) return ADEPT_EINVAL;
+  if (n == 0) return ADEPT_OK;
+  const unsigned grid = unsigned((n + 255) / 256);
+  dev_math_kernel<<<grid, 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(fn, in, out, n);
+  return cudaGetLastError() == cudaSuccess ? ADEPT_OK : ADEPT_ECUDA;
+}
+
+}  // extern "C"

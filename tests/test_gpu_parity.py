@@ -1,0 +1,248 @@
+"""GPU parity: the CUDA library (through its C ABI) against the oracle, element by element on the
+same seeded inputs.  Integer results (counts, ids, steps, slab indices) must be bit-exact; fp32
+track fields within 1e-5 relative (they are in fact bit-exact, which the tests report); per-layer
+energy deposit within 1e-4 relative (BASELINE.json north_star).  `-m gpu` only."""
+import numpy as np
+import pytest
+
+from oracle import Oracle, math_fns
+from workloads import CONFIGS, gen_primaries, gen_sweep, gen_tracks, geometry_for, tables_for
+from tests.helpers import make_tracks, sort_by_id
+
+pytestmark = pytest.mark.gpu
+
+LAYOUTS = ("aos", "soa", "aosoa32")
+SCHEMES = ("dense", "sparse")
+INT_FIELDS = ("vol", "id_lo", "id_hi", "step")
+F32_FIELDS = ("pos", "dir", "ekin", "nial")
+
+
+def _ctx(*a, **k):
+    from paper_2302_08252_b200 import Context
+    return Context(*a, **k)
+
+
+def compare_tracks(gpu, ref, what=""):
+    """Per-track comparison after sorting by id.  Returns the number of fp32 words that differ in
+    their last bits (reported, must be within 1e-5 relative)."""
+    assert gpu.shape[0] == ref.shape[0], "%s: %d tracks vs oracle %d" % (what, gpu.shape[0], ref.shape[0])
+    g, r = sort_by_id(gpu), sort_by_id(ref)
+    for f in INT_FIELDS:
+        assert (g[f] == r[f]).all(), "%s: integer field %s differs" % (what, f)
+    inexact = 0
+    for f in F32_FIELDS:
+        a, b = g[f].astype(np.float64), r[f].astype(np.float64)
+        inexact += int((g[f].view(np.uint32) != r[f].view(np.uint32)).sum())
+        tol = 1e-5 * np.maximum(np.abs(b), 1e-30)
+        assert (np.abs(a - b) <= tol).all(), "%s: fp32 field %s beyond 1e-5 relative" % (what, f)
+    return inexact
+
+
+def compare_counts(g, r, keys=("live", "steps", "secondaries", "killed", "escaped_n"), what=""):
+    for k in keys:
+        assert (np.asarray(g[k]) == np.asarray(r[k])).all(), "%s: %s gpu %s oracle %s" % (what, k, g[k], r[k])
+
+
+# ------------------------------------------------------------------ elementary functions -----
+def test_device_math_is_bit_equal_to_the_oracle():
+    import torch
+    from paper_2302_08252_b200 import dev_math
+    rng = np.random.default_rng(11)
+    ck = rng.integers(0, 2**32, size=(200000, 6), dtype=np.uint64).astype(np.uint32)
+    out = dev_math(0, torch.from_numpy(ck.view(np.int32)).cuda(), torch.int32, (ck.shape[0], 4)).cpu().numpy().view(np.uint32)
+    assert (out == math_fns.philox_array(ck[:, :4], ck[:, 4:])).all()
+    x = (np.arange(0, 1 << 23, 3, dtype=np.uint64) << np.uint64(9)).astype(np.uint32)
+    u = dev_math(1, torch.from_numpy(x.view(np.int32)).cuda(), torch.float32, (x.shape[0],)).cpu().numpy()
+    assert (u.view(np.uint32) == math_fns.u01(x).view(np.uint32)).all()
+
+    def sweep(lo, hi, stride):
+        a, b = np.float32(lo).view(np.uint32), np.float32(hi).view(np.uint32)
+        return np.arange(int(a), int(b), stride, dtype=np.uint32).view(np.float32)
+
+    xs = np.concatenate([sweep(1e-8, 1e5, 7), u])
+    y = dev_math(2, torch.from_numpy(xs).cuda(), torch.float32, (xs.shape[0],)).cpu().numpy()
+    assert (y.view(np.uint32) == math_fns.lg(xs).view(np.uint32)).all()
+    xs = np.concatenate([sweep(1e-6, 20.0, 11), -sweep(1e-6, 30.0, 11), np.float32([0.0])])
+    y = dev_math(3, torch.from_numpy(xs).cuda(), torch.float32, (xs.shape[0],)).cpu().numpy()
+    assert (y.view(np.uint32) == math_fns.ex(xs).view(np.uint32)).all()
+    sc = dev_math(4, torch.from_numpy(u).cuda(), torch.float32, (u.shape[0], 2)).cpu().numpy()
+    s, c = math_fns.sincos2pi(u)
+    assert (sc[:, 0].view(np.uint32) == s.view(np.uint32)).all() and (sc[:, 1].view(np.uint32) == c.view(np.uint32)).all()
+
+
+# ------------------------------------------------------------------------ single step --------
+@pytest.fixture(scope="module")
+def single_step_case():
+    c = CONFIGS["single_step"]
+    geo, tab = geometry_for("single_step"), tables_for("single_step")
+    n = 200000 + 77                                  # several tiles per kind and a ragged tail
+    pop = gen_tracks(n, c["seed"], geo, c["e_max"], c["fractions"])
+    # make the step exercise every branch: some spent nial, some forced interactions, e+ at rest
+    rng = np.random.default_rng(123)
+    for k in range(3):
+        t = pop[k]
+        m = rng.random(t.shape[0])
+        t["nial"][m < 0.10] = -1.0
+        for j in range(3 if k == 2 else 1):
+            t["nial"][(m >= 0.10 + 0.05 * j) & (m < 0.15 + 0.05 * j), j] = 1e-30
+    pop[1]["ekin"][::7] = np.float32(0.05)
+    o = Oracle(geo, tab, seed=c["seed"])
+    for k in range(3):
+        o.load_tracks(k, pop[k])
+    o.step()
+    ref = dict(result=o.result(), tracks=[o.read_tracks(k, pop[0].dtype) for k in range(3)])
+    return geo, tab, pop, ref
+
+
+@pytest.mark.parametrize("scheme", SCHEMES)
+@pytest.mark.parametrize("layout", LAYOUTS)
+def test_single_step_matches_oracle(single_step_case, layout, scheme):
+    geo, tab, pop, ref = single_step_case
+    ctx = _ctx(geo, tab, layout=layout, scheme=scheme, capacity=1 << 19, seed=3)
+    for k in range(3):
+        ctx.load_tracks(k, pop[k])
+    counts = ctx.step()
+    compare_counts(counts, ref["result"], what="%s/%s" % (layout, scheme))
+    inexact = sum(compare_tracks(ctx.read_tracks(k), ref["tracks"][k], "%s/%s kind %d" % (layout, scheme, k))
+                  for k in range(3))
+    res = ctx.result()
+    assert np.allclose(res["edep_slab"], ref["result"]["edep_slab"], rtol=1e-9, atol=1e-9)
+    assert abs(res["e_escaped"] - ref["result"]["e_escaped"]) <= 1e-9 * max(1.0, ref["result"]["e_escaped"])
+    print("single step %s/%s: %d fp32 words differ in the last bits" % (layout, scheme, inexact))
+    assert inexact == 0          # rule M7: the arithmetic is reproducible bit for bit
+    ctx.destroy()
+
+
+# ------------------------------------------------------------------------ showers ------------
+@pytest.mark.parametrize("scheme", SCHEMES)
+@pytest.mark.parametrize("layout", LAYOUTS)
+def test_tiny_shower_matches_oracle_every_iteration(layout, scheme):
+    c = CONFIGS["tiny"]
+    geo, tab = geometry_for("tiny"), tables_for("tiny")
+    prim = gen_primaries(c["n_primaries"], c["e_primary"])
+    o = Oracle(geo, tab, seed=c["seed"])
+    o.inject(prim)
+    ctx = _ctx(geo, tab, layout=layout, scheme=scheme, capacity=c["capacity"], seed=c["seed"])
+    ctx.inject(prim)
+    it = 0
+    while True:
+        for k in range(3):
+            compare_tracks(ctx.read_tracks(k), o.read_tracks(k, prim.dtype if False else make_tracks(1).dtype),
+                           "iteration %d kind %d" % (it, k))
+        if sum(o.live(k) for k in range(3)) == 0:
+            break
+        o.step()
+        counts = ctx.step()
+        compare_counts(counts, o.result(), what="iteration %d" % it)
+        it += 1
+    r, g = o.result(), ctx.result()
+    assert g["iterations"] == r["iterations"] == it
+    assert np.allclose(g["edep_layer"], r["edep_layer"], rtol=1e-4, atol=1e-12)
+    assert abs(g["e_escaped"] - r["e_escaped"]) <= 1e-9 * max(1.0, r["e_escaped"])
+    assert abs(g["edep_slab"].sum() + g["e_escaped"] - g["e_injected"]) < 1e-6 * g["e_injected"]
+    if scheme == "dense":
+        assert (g["slots_used"] == r["slots_used"]).all()
+    else:   # rule S30: bump allocation, never recycled within a batch
+        injected = np.array([c["n_primaries"], 0, 0], dtype=np.uint64)
+        assert (g["slots_used"] == injected + r["secondaries"]).all()
+    ctx.destroy()
+
+
+@pytest.mark.parametrize("layout,scheme", [("soa", "dense"), ("aosoa32", "dense"), ("aos", "sparse")])
+def test_full_showers_run_matches_oracle(layout, scheme):
+    """Config 2 at reduced primaries (100 x 1 GeV) so that the oracle takes well under a second."""
+    c = CONFIGS["full"]
+    geo, tab = geometry_for("full"), tables_for("full")
+    prim = gen_primaries(100, c["e_primary"])
+    o = Oracle(geo, tab, seed=c["seed"])
+    o.inject(prim)
+    o.run()
+    r = o.result()
+    ctx = _ctx(geo, tab, layout=layout, scheme=scheme, capacity=1 << 19, seed=c["seed"])
+    ctx.inject(prim)
+    g = ctx.run()
+    compare_counts(g, r)
+    assert g["iterations"] == r["iterations"]
+    assert np.allclose(g["edep_layer"], r["edep_layer"], rtol=1e-4, atol=1e-9)
+    assert abs(g["e_escaped"] - r["e_escaped"]) <= 1e-9 * r["e_injected"]
+    ctx.destroy()
+
+
+def test_batched_run_matches_oracle():
+    geo, tab = geometry_for("tiny"), tables_for("tiny")
+    prim = gen_primaries(25, 10.0)
+    o = Oracle(geo, tab, seed=9)
+    o.queue(prim)
+    o.run_batched(5)
+    r = o.result()
+    for scheme in SCHEMES:
+        ctx = _ctx(geo, tab, layout="soa", scheme=scheme, capacity=4096, seed=9, batch_primaries=5)
+        ctx.inject(prim)
+        g = ctx.run()
+        compare_counts(g, r, what=scheme)
+        assert g["iterations"] == r["iterations"]
+        assert np.allclose(g["edep_layer"], r["edep_layer"], rtol=1e-4, atol=1e-12)
+        if scheme == "dense":
+            assert (g["slots_used"] == r["slots_used"]).all()
+        ctx.destroy()
+
+
+# -------------------------------------------------------------------- config 4 populations ---
+@pytest.mark.parametrize("layout", LAYOUTS)
+def test_sweep_population_sparse_slots_and_forced_secondaries(layout):
+    geo, tab = geometry_for("sweep"), tables_for("sweep")
+    span = 1 << 16
+    pop = gen_sweep(0.3, span=span)
+    o = Oracle(geo, tab, seed=4)
+    for k in range(3):
+        o.load_tracks(k, pop[k]["tracks"])
+    o.step()
+    r = o.result()
+    forced = [int(p["forced"].sum()) for p in pop]
+    for scheme in SCHEMES:
+        ctx = _ctx(geo, tab, layout=layout, scheme=scheme, capacity=span + (1 << 14), seed=4)
+        for k in range(3):
+            ctx.load_tracks(k, pop[k]["tracks"], pop[k]["slots"] if scheme == "sparse" else None)
+        g = ctx.step()
+        compare_counts(g, r, what="%s/%s" % (layout, scheme))
+        assert int(g["secondaries"][2]) == forced[0] + forced[1] and int(g["secondaries"][0]) == forced[2]
+        for k in range(3):
+            compare_tracks(ctx.read_tracks(k), o.read_tracks(k, pop[0]["tracks"].dtype), "%s/%s" % (layout, scheme))
+        ctx.destroy()
+
+
+# ------------------------------------------------------------------------ edge cases ---------
+def test_edge_cases_empty_overflow_invalid_reset():
+    from paper_2302_08252_b200 import AdeptError
+    geo, tab = geometry_for("tiny"), tables_for("tiny")
+    ctx = _ctx(geo, tab, layout="soa", scheme="dense", capacity=64, seed=1)
+    c = ctx.step()                                   # empty step: nothing happens, not counted
+    assert c["live"].sum() == 0 and c["iterations"] == 0 and c["steps"].sum() == 0
+    r = ctx.run()
+    assert r["iterations"] == 0 and r["edep_slab"].sum() == 0
+    bad = gen_primaries(1, 10.0)
+    bad["ekin"] = 1e6                                # above e_max
+    with pytest.raises(AdeptError) as e:
+        ctx.inject(bad)
+    assert e.value.code == -1
+    bad = gen_primaries(1, 10.0)
+    bad["pos"][0, 0] = 1e3                           # outside the transverse box
+    with pytest.raises(AdeptError):
+        ctx.inject(bad)
+    # overflow: 40 x 10 MeV showers need more than 64 slots per kind
+    ctx.inject(gen_primaries(40, 10.0))
+    with pytest.raises(AdeptError) as e:
+        ctx.run()
+    assert e.value.code == -2
+    with pytest.raises(AdeptError) as e:
+        ctx.step()
+    assert e.value.code == -4
+    ctx.reset()
+    ctx.inject(gen_primaries(2, 10.0))
+    o = Oracle(geo, tab, seed=1)
+    o.inject(gen_primaries(2, 10.0))
+    o.run()
+    compare_counts(ctx.run(), o.result())
+    ctx.destroy()
+    with pytest.raises(AdeptError):
+        _ctx(geo, tab, layout="soa", scheme="dense", capacity=0)
