@@ -1,0 +1,325 @@
+#!/usr/bin/env python
+"""bench.py — BASELINE.json's metric on BASELINE.json's workload.
+
+Metric: track-steps/s (and step-kernel HBM GB/s as a fraction of the measured B200 peak) on the
+single-step microbenchmark (BASELINE.json configs[2]): 2^24 tracks, 40 % e- / 10 % e+ / 50 % gamma,
+uniform in the 50-layer Pb/lAr calorimeter, isotropic, log-uniform 100 keV - 10 GeV, exp(1)
+interaction lengths; one adept_step per "step", dense double buffer, per layout.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--layout soa|aos|aosoa32|all] [--impl reference]
+
+One JSON line on stdout (rank 0).  `value` is measured with the tracks resident in HBM: every timed
+step starts from a pristine copy of the workspace (restored outside the timed region, L2 flushed) and
+is timed with CUDA events on the stream the kernel is launched on.  `e2e` is the same step through
+the C ABI with HOST buffers: adept_load_tracks (H2D) + adept_step + adept_read_tracks (D2H) inside
+the timed region.  `cpu_baseline` / `--impl reference` time the oracle (oracle/, single thread) on
+the host cores; that is the only use of oracle/ here.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from workloads import CONFIGS, gen_tracks, geometry_for, tables_for  # noqa: E402
+
+WORKLOAD = "single_step"
+RECORD_BYTES = {"aos": 64, "soa": 56, "aosoa32": 56}     # bytes per record per layout
+
+
+def measured_peak():
+    """HBM GB/s denominator: MEASURED_PEAKS.json (driver-written) else the profiling guide's fallback."""
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons during the timed region (profiling recipe's clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._pump, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, smax, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for l in self.lines:
+            f = [x.strip() for x in l.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        # under load = the upper half of the samples (idle gaps between steps pull the clock down)
+        sm.sort()
+        load = sm[len(sm) // 2:] if sm else []
+        return {"sm_mhz": float(np.median(load)) if load else None,
+                "sm_max_mhz": max(smax) if smax else None, "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def population(n_tracks: int, rank: int):
+    c = CONFIGS[WORKLOAD]
+    return gen_tracks(n_tracks, c["seed"] + 1000 * rank, geometry_for(WORKLOAD), c["e_max"], c["fractions"])
+
+
+def oracle_single_step(pop, sample_tracks: int):
+    """Time the oracle, as it stands, on the first `sample_tracks` tracks of each kind's share."""
+    from oracle import Oracle
+    c = CONFIGS[WORKLOAD]
+    total = sum(p.shape[0] for p in pop)
+    frac = min(1.0, sample_tracks / total)
+    o = Oracle(geometry_for(WORKLOAD), tables_for(WORKLOAD), seed=c["seed"])
+    n = 0
+    for k in range(3):
+        m = int(round(pop[k].shape[0] * frac))
+        o.load_tracks(k, pop[k][:m])
+        n += m
+    t0 = time.perf_counter()
+    o.step()
+    dt = time.perf_counter() - t0
+    r = o.result()
+    o.close()
+    return n, dt, r
+
+
+def run_reference(args, rank: int):
+    """--impl reference: the oracle on the host cores, same metric/config, bounded sample per step."""
+    if rank != 0:
+        return
+    sample = min(args.tracks, 1 << 21)
+    pop = population(sample, 0)
+    for _ in range(args.warmup):
+        oracle_single_step(pop, sample)
+    n_tot, t_tot = 0, 0.0
+    for _ in range(args.steps):
+        n, dt, _ = oracle_single_step(pop, sample)
+        n_tot += n
+        t_tot += dt
+    v = n_tot / t_tot
+    cpu = {"value": v, "unit": "track-steps/s", "cores": 1, "kind": "oracle",
+           "sample": "one adept_step-equivalent oracle iteration over %d tracks of the config-3 population per step" % sample}
+    print(json.dumps({
+        "impl": "reference", "metric": "track-steps/sec", "value": v, "unit": "track-steps/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_tot / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "single-step microbenchmark (BASELINE.json configs[2]), oracle on host, "
+                               "%d-track sample per step" % sample},
+        "cpu_baseline": cpu,
+        "e2e": {"value": v, "unit": "track-steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
+def bench_layout(ctx, torch, pop, steps, warmup, flush, barrier):
+    """Device-resident timing of adept_step: returns per-step ms list and the counts after one step."""
+    for k in range(3):
+        ctx.load_tracks(k, pop[k])
+    torch.cuda.synchronize()
+    pristine = ctx.workspace.clone()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+
+    def one(e0, e1):
+        ctx.workspace.copy_(pristine)          # rewind (include/adept.h "Workspace"), untimed
+        flush.zero_()                          # L2 flush: 256 MiB > 126 MB L2, untimed
+        if e0 is not None:
+            e0.record(ctx.stream)
+        ctx.step(sync=False)
+        if e1 is not None:
+            e1.record(ctx.stream)
+
+    for _ in range(warmup):
+        one(None, None)
+    torch.cuda.synchronize()
+    barrier()
+    t0 = time.perf_counter()
+    for e0, e1 in ev:
+        one(e0, e1)
+    torch.cuda.synchronize()
+    barrier()
+    wall = time.perf_counter() - t0
+    ms = [e0.elapsed_time(e1) for e0, e1 in ev]
+    res = ctx.result()
+    del pristine
+    return ms, res, wall
+
+
+def run_gpu(args, rank: int, world: int, local_rank: int):
+    import torch
+    from paper_2302_08252_b200 import Context
+    from paper_2302_08252_b200.binding import TRACK_DTYPE
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        torch.cuda.set_device(local_rank)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+
+    def max_over_ranks(x: float) -> float:
+        if dist is None:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    geo, tab = geometry_for(WORKLOAD), tables_for(WORKLOAD)
+    n_tracks = args.tracks
+    pop = population(n_tracks, rank)                       # weak scaling: each rank its own 2^24 tracks
+    biggest = max(p.shape[0] for p in pop)
+    capacity = int(biggest * 1.125) + 4096                 # room for the secondaries of one step
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    layouts = ["soa", "aosoa32", "aos"] if args.layout == "all" else [args.layout]
+    main = layouts[0]
+    per_layout, main_res = {}, None
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    for layout in layouts:
+        ctx = Context(geo, tab, layout=layout, scheme="dense", capacity=capacity,
+                      seed=CONFIGS[WORKLOAD]["seed"], device="cuda:%d" % local_rank)
+        ms, res, wall = bench_layout(ctx, torch, pop, args.steps, args.warmup, flush, barrier)
+        total_ms = max_over_ranks(float(np.sum(ms)))
+        n_out = int(res["live"].sum())
+        bytes_per_launch = RECORD_BYTES[layout] * (n_tracks + n_out)
+        per_layout[layout] = {
+            "ms_per_step": total_ms / args.steps, "ms_min": float(np.min(ms)), "ms_median": float(np.median(ms)),
+            "track_steps_per_s": world * n_tracks * args.steps / (total_ms * 1e-3),
+            "algorithmic_bytes_per_launch": bytes_per_launch,
+            "algorithmic_GBps": bytes_per_launch / (float(np.mean(ms)) * 1e-3) / 1e9,
+            "survivors_plus_secondaries": n_out}
+        if layout == main:
+            main_res = res
+            main_ctx_ms = ms
+        ctx.destroy()
+        del ctx
+        torch.cuda.empty_cache()
+    clocks = sampler.stop()
+
+    # ---- e2e: host buffers, H2D + step + D2H inside the timed region (main layout) ----------
+    ctx = Context(geo, tab, layout=main, scheme="dense", capacity=capacity,
+                  seed=CONFIGS[WORKLOAD]["seed"], device="cuda:%d" % local_rank)
+    pinned_in = [torch.from_numpy(p.view(np.uint8).copy()).pin_memory() for p in pop]
+    host_in = [t.numpy().view(TRACK_DTYPE) for t in pinned_in]
+    pinned_out = [torch.empty(capacity * 56, dtype=torch.uint8).pin_memory() for _ in range(3)]
+    host_out = [t.numpy().view(TRACK_DTYPE) for t in pinned_out]
+    e2e_steps = max(1, min(args.steps, 3))
+    e2e_t, d2h = 0.0, 0
+    for it in range(1 + e2e_steps):                        # first pass is a warm-up
+        ctx.reset()
+        torch.cuda.synchronize()
+        barrier()
+        t0 = time.perf_counter()
+        for k in range(3):
+            ctx.load_tracks(k, host_in[k])
+        counts = ctx.step()
+        d2h = 0
+        for k in range(3):
+            d2h += 56 * ctx.read_tracks(k, out=host_out[k])
+        torch.cuda.synchronize()
+        dt = max_over_ranks(time.perf_counter() - t0)
+        if it > 0:
+            e2e_t += dt
+    ctx.destroy()
+    e2e_value = world * n_tracks * e2e_steps / e2e_t
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+    peak, peak_src = measured_peak()
+    m = per_layout[main]
+    out = {
+        "metric": "track-steps/sec", "value": m["track_steps_per_s"], "unit": "track-steps/s", "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": m["ms_per_step"], "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "single-step microbenchmark (BASELINE.json configs[2]): %d tracks per GPU, "
+                               "40/10/50 %% e-/e+/gamma, one adept_step, dense double buffer" % n_tracks,
+                   "layout": main, "scheme": "dense", "tracks_per_gpu": n_tracks, "capacity_per_kind": capacity,
+                   "parallelism": "independent track shards, no collective" if world > 1 else "single GPU",
+                   "l2": "workspace restored from a pristine copy and 256 MiB written between timed steps; "
+                         "inputs (0.94 GB) exceed L2"},
+        "clocks": clocks,
+        "gpu_launches": args.steps,
+        "e2e": {"value": e2e_value, "unit": "track-steps/s", "h2d_bytes_per_step": 56 * n_tracks,
+                "d2h_bytes_per_step": d2h + 256, "steps": e2e_steps,
+                "what": "adept_load_tracks x3 (pinned host) + adept_step + adept_read_tracks x3"},
+        "roofline": {"bound": "hbm", "achieved": m["algorithmic_GBps"], "peak": peak, "unit": "GB/s",
+                     "frac": m["algorithmic_GBps"] / peak, "traffic": None, "peak_source": peak_src,
+                     "kernel": "adept::step_kernel<%s, dense>" % main,
+                     "bytes_per_launch": m["algorithmic_bytes_per_launch"]},
+        "layouts": per_layout,
+    }
+    if world == 1 and not args.no_cpu:
+        n, dt, r = oracle_single_step(pop, n_tracks)
+        out["cpu_baseline"] = {"value": n / dt, "unit": "track-steps/s", "cores": 1, "kind": "oracle",
+                               "sample": "one oracle iteration over all %d tracks of the same population" % n,
+                               "seconds": dt}
+        keys = ("steps", "secondaries", "killed", "escaped_n", "live")
+        out["parity_full_size"] = {"counts_bit_exact": bool(all((main_res[k] == r[k]).all() for k in keys)),
+                                   "edep_rel_err": float(np.max(np.abs(main_res["edep_layer"] - r["edep_layer"])
+                                                                / np.maximum(r["edep_layer"], 1e-30)))}
+    print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--layout", default="all", choices=["soa", "aosoa32", "aos", "all"])
+    ap.add_argument("--tracks", type=int, default=CONFIGS[WORKLOAD]["n_tracks"])
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+    run_gpu(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

@@ -217,13 +217,18 @@ class Context:
         self._check(self._L.adept_load_tracks(self._h, kind, t.ctypes.data, t.shape[0],
                                               s.ctypes.data if s is not None else None))
 
-    def read_tracks(self, kind: int, cap: int | None = None) -> np.ndarray:
-        cap = self.capacity + 32 if cap is None else cap
+    def read_tracks(self, kind: int, cap: int | None = None, out: np.ndarray | None = None):
+        """Without `out`: returns a new array of the live tracks.  With `out` (a TRACK_DTYPE host array,
+        e.g. pinned): fills it in place and returns the number of tracks."""
         n = C.c_uint64(0)
-        # first ask for the count with a zero-capacity call when the caller gave no bound
-        out = np.zeros(cap, dtype=TRACK_DTYPE)
-        self._check(self._L.adept_read_tracks(self._h, kind, out.ctypes.data, cap, C.byref(n)))
-        return out[: n.value].copy()
+        if out is not None:
+            assert out.dtype.itemsize == 56 and out.flags["C_CONTIGUOUS"]
+            self._check(self._L.adept_read_tracks(self._h, kind, out.ctypes.data, out.shape[0], C.byref(n)))
+            return int(n.value)
+        cap = self.capacity + 32 if cap is None else cap
+        buf = np.empty(cap, dtype=TRACK_DTYPE)
+        self._check(self._L.adept_read_tracks(self._h, kind, buf.ctypes.data, cap, C.byref(n)))
+        return buf[: n.value].copy()
 
     def read_counters(self):
         n_lines = int(self._L.adept_instr_lines(self._h))

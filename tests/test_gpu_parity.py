@@ -215,7 +215,7 @@ def test_sweep_population_sparse_slots_and_forced_secondaries(layout):
 def test_edge_cases_empty_overflow_invalid_reset():
     from paper_2302_08252_b200 import AdeptError
     geo, tab = geometry_for("tiny"), tables_for("tiny")
-    ctx = _ctx(geo, tab, layout="soa", scheme="dense", capacity=64, seed=1)
+    ctx = _ctx(geo, tab, layout="soa", scheme="dense", capacity=32, seed=1)
     c = ctx.step()                                   # empty step: nothing happens, not counted
     assert c["live"].sum() == 0 and c["iterations"] == 0 and c["steps"].sum() == 0
     r = ctx.run()
@@ -229,8 +229,8 @@ def test_edge_cases_empty_overflow_invalid_reset():
     bad["pos"][0, 0] = 1e3                           # outside the transverse box
     with pytest.raises(AdeptError):
         ctx.inject(bad)
-    # overflow: 40 x 10 MeV showers need more than 64 slots per kind
-    ctx.inject(gen_primaries(40, 10.0))
+    # overflow: 32 x 10 MeV showers need more than 32 slots per kind
+    ctx.inject(gen_primaries(32, 10.0))
     with pytest.raises(AdeptError) as e:
         ctx.run()
     assert e.value.code == -2
