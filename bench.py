@@ -205,7 +205,7 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
     n_tracks = args.tracks
     pop = population(n_tracks, rank)                       # weak scaling: each rank its own 2^24 tracks
     biggest = max(p.shape[0] for p in pop)
-    capacity = int(biggest * 1.125) + 4096                 # room for the secondaries of one step
+    capacity = int(biggest * 1.25) + 4096                  # one step grows the photon set by ~16 %
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
     layouts = ["soa", "aosoa32", "aos"] if args.layout == "all" else [args.layout]
     main = layouts[0]
