@@ -12,7 +12,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SO = os.path.join(_HERE, "libadept_b200.so")
+_SO = os.environ.get("ADEPT_B200_LIB") or os.path.join(_HERE, "libadept_b200.so")
 
 ADEPT_AOS, ADEPT_SOA, ADEPT_AOSOA32 = 0, 1, 2
 ADEPT_SPARSE_SINGLE, ADEPT_DENSE_DOUBLE = 0, 1

@@ -78,9 +78,15 @@ enum Face : int { FACE_ZP = 0, FACE_ZM = 1, FACE_XY = 2 };
 // S21: distance to the slab faces and the transverse box, and which face is hit first.
 __device__ __forceinline__ float geometry_step(const Trk &t, const Env &g, float z_lo, float z_hi, int &face) {
   const float H = g.half_xy;
-  const float s_z = (t.dz > 0.0f) ? (z_hi - t.pz) / t.dz : (t.dz < 0.0f) ? (z_lo - t.pz) / t.dz : kInf;
-  const float s_x = (t.dx > 0.0f) ? (H - t.px) / t.dx : (t.dx < 0.0f) ? (-H - t.px) / t.dx : kInf;
-  const float s_y = (t.dy > 0.0f) ? (H - t.py) / t.dy : (t.dy < 0.0f) ? (-H - t.py) / t.dy : kInf;
+  // each quotient is the rule's (plane - pos) / dir; the plane is selected first so that a warp
+  // executes one division per axis whatever the signs of its lanes' directions
+  const float n_z = ((t.dz > 0.0f) ? z_hi : z_lo) - t.pz;
+  const float n_x = ((t.dx > 0.0f) ? H : -H) - t.px;
+  const float n_y = ((t.dy > 0.0f) ? H : -H) - t.py;
+  const float q_z = n_z / t.dz, q_x = n_x / t.dx, q_y = n_y / t.dy;
+  const float s_z = (t.dz != 0.0f) ? q_z : kInf;
+  const float s_x = (t.dx != 0.0f) ? q_x : kInf;
+  const float s_y = (t.dy != 0.0f) ? q_y : kInf;
   float s_g = s_z;
   face = (t.dz > 0.0f) ? FACE_ZP : FACE_ZM;
   if (s_x < s_g) { s_g = s_x; face = FACE_XY; }
@@ -173,9 +179,10 @@ __device__ __forceinline__ void step_gamma(Trk &t, const Env &g, Outcome &o) {
   const float sig0 = lerp_node(b.f, A.x, B.x);
   const float sig1 = lerp_node(b.f, A.y, B.y);
   const float sig2 = lerp_node(b.f, A.z, B.z);
-  const float s0 = (sig0 > 0.0f) ? t.n0 / sig0 : kInf;
-  const float s1 = (sig1 > 0.0f) ? t.n1 / sig1 : kInf;
-  const float s2 = (sig2 > 0.0f) ? t.n2 / sig2 : kInf;
+  const float q0 = t.n0 / sig0, q1 = t.n1 / sig1, q2 = t.n2 / sig2;  // selected below: no divergent branch
+  const float s0 = (sig0 > 0.0f) ? q0 : kInf;
+  const float s1 = (sig1 > 0.0f) ? q1 : kInf;
+  const float s2 = (sig2 > 0.0f) ? q2 : kInf;
 
   // S21
   const float z_lo = slab_zlo(g, vol0), z_hi = slab_zlo(g, vol0 + 1u);
@@ -204,57 +211,56 @@ __device__ __forceinline__ void step_gamma(Trk &t, const Env &g, Outcome &o) {
       o.alive = false;
       return;
     }
-  } else if (w == 0) {  // S26 pair: uniform split of E - 2 mc^2, both along dir; photon dies
-    t.n0 = -1.0f;
+  } else {
+    // S26.  The draws of call 1 and the child ids of call 2 are evaluated once for whatever
+    // interaction the lanes of a warp take (a block that ends up unused costs nothing extra: the
+    // other lanes need it anyway, and an unread draw changes no result).
     const uint4 r1 = rs.call(1), r2 = rs.call(2);
-    const float E_av = t.ekin - two_mc2();
-    const float T_minus = u01(r1.x) * E_av;
-    const float T_plus = E_av - T_minus;
-    if (T_minus >= g.e_cut) make_kid(o.kid[0], K_EM, t.dx, t.dy, t.dz, T_minus, r2.x, r2.y);
-    else o.dep += static_cast<double>(T_minus);
-    make_kid(o.kid[1], K_EP, t.dx, t.dy, t.dz, T_plus, r2.z, r2.w);
-    o.alive = false;
-    return;
-  } else if (w == 1) {  // S26 Compton: 1/eps spectrum, exact kinematics
-    t.n1 = -1.0f;
-    const uint4 r1 = rs.call(1);
-    const float E = t.ekin;
-    const float kappa = E / kMc2;
-    const float L = lg(fmaf(2.0f, kappa, 1.0f));
-    const float eps = ex(-(u01(r1.x) * L));
-    const float E1 = eps * E;
-    const float T = E - E1;
-    float ct = 1.0f - (((1.0f / eps) - 1.0f) / kappa);
-    if (ct > 1.0f) ct = 1.0f;
-    if (ct < -1.0f) ct = -1.0f;
-    const float st = sqrtf(fmaf(-ct, ct, 1.0f));
-    float sphi, cphi;
-    sincos2pi(u01(r1.y), sphi, cphi);
-    float nx, ny, nz;
-    rotate_dir(t.dx, t.dy, t.dz, st, ct, sphi, cphi, nx, ny, nz);
-    const float qx = fmaf(E, t.dx, -(E1 * nx));
-    const float qy = fmaf(E, t.dy, -(E1 * ny));
-    const float qz = fmaf(E, t.dz, -(E1 * nz));
-    const float pn = sqrtf(fmaf(qx, qx, fmaf(qy, qy, qz * qz)));
-    if (T >= g.e_cut && pn > 0.0f) {
-      const uint4 r2 = rs.call(2);
-      make_kid(o.kid[0], K_EM, qx / pn, qy / pn, qz / pn, T, r2.x, r2.y);
-    } else {
-      o.dep += static_cast<double>(T);
-    }
-    if (E1 < g.e_cut) {
-      o.dep += static_cast<double>(E1);
+    if (w == 0) {  // pair: uniform split of E - 2 mc^2, both along dir; photon dies
+      t.n0 = -1.0f;
+      const float E_av = t.ekin - two_mc2();
+      const float T_minus = u01(r1.x) * E_av;
+      const float T_plus = E_av - T_minus;
+      if (T_minus >= g.e_cut) make_kid(o.kid[0], K_EM, t.dx, t.dy, t.dz, T_minus, r2.x, r2.y);
+      else o.dep += static_cast<double>(T_minus);
+      make_kid(o.kid[1], K_EP, t.dx, t.dy, t.dz, T_plus, r2.z, r2.w);
+      o.alive = false;
+      return;
+    } else if (w == 1) {  // Compton: 1/eps spectrum, exact kinematics
+      t.n1 = -1.0f;
+      const float E = t.ekin;
+      const float kappa = E / kMc2;
+      const float L = lg(fmaf(2.0f, kappa, 1.0f));
+      const float eps = ex(-(u01(r1.x) * L));
+      const float E1 = eps * E;
+      const float T = E - E1;
+      float ct = 1.0f - (((1.0f / eps) - 1.0f) / kappa);
+      if (ct > 1.0f) ct = 1.0f;
+      if (ct < -1.0f) ct = -1.0f;
+      const float st = sqrtf(fmaf(-ct, ct, 1.0f));
+      float sphi, cphi;
+      sincos2pi(u01(r1.y), sphi, cphi);
+      float nx, ny, nz;
+      rotate_dir(t.dx, t.dy, t.dz, st, ct, sphi, cphi, nx, ny, nz);
+      const float qx = fmaf(E, t.dx, -(E1 * nx));
+      const float qy = fmaf(E, t.dy, -(E1 * ny));
+      const float qz = fmaf(E, t.dz, -(E1 * nz));
+      const float pn = sqrtf(fmaf(qx, qx, fmaf(qy, qy, qz * qz)));
+      if (T >= g.e_cut && pn > 0.0f) make_kid(o.kid[0], K_EM, qx / pn, qy / pn, qz / pn, T, r2.x, r2.y);
+      else o.dep += static_cast<double>(T);
+      if (E1 < g.e_cut) {
+        o.dep += static_cast<double>(E1);
+        o.alive = false;
+        return;
+      }
+      t.ekin = E1;
+      t.dx = nx; t.dy = ny; t.dz = nz;
+    } else {  // photoelectric: e- with T = E along dir; photon dies
+      t.n2 = -1.0f;
+      make_kid(o.kid[0], K_EM, t.dx, t.dy, t.dz, t.ekin, r2.x, r2.y);
       o.alive = false;
       return;
     }
-    t.ekin = E1;
-    t.dx = nx; t.dy = ny; t.dz = nz;
-  } else {  // S26 photoelectric: e- with T = E along dir; photon dies
-    t.n2 = -1.0f;
-    const uint4 r2 = rs.call(2);
-    make_kid(o.kid[0], K_EM, t.dx, t.dy, t.dz, t.ekin, r2.x, r2.y);
-    o.alive = false;
-    return;
   }
   runaway_guard<K_GAMMA>(t, o);
 }
@@ -266,111 +272,110 @@ template <int KIND> __device__ __forceinline__ void step_elec(Trk &t, const Env 
   const Stream rs{t.id_lo, t.id_hi, t.step};
   const float e_cut = g.e_cut;
 
-  // S17: a positron below the cut annihilates at rest into two back-to-back photons
-  if (KIND == K_EP && t.ekin < e_cut) {
-    o.dep += static_cast<double>(t.ekin);
-    const uint4 r1 = rs.call(1), r2 = rs.call(2);
-    const float ct = 1.0f - 2.0f * u01(r1.z);
-    const float st = sqrtf(fmaf(-ct, ct, 1.0f));
-    float sphi, cphi;
-    sincos2pi(u01(r1.w), sphi, cphi);
-    const float ax = st * cphi, ay = st * sphi, az = ct;
-    make_kid(o.kid[0], K_GAMMA, ax, ay, az, kMc2, r2.x, r2.y);
-    make_kid(o.kid[1], K_GAMMA, -ax, -ay, -az, kMc2, r2.z, r2.w);
-    o.alive = false;
-    return;
-  }
-
-  // S18: bremsstrahlung is the only discrete process; nial[1], nial[2] are carried unchanged
-  if (t.n0 <= 0.0f) t.n0 = -lg(u01(rs.call(0).x));
-
-  // S19, S20
-  const uint32_t vol0 = t.vol;
-  const uint32_t mat = (vol0 & 1u) ? g.mat_gap : g.mat_abs;
-  const float E0 = t.ekin;
-  const Bin b = locate_bin(g, lg(E0));
-  const float4 *tab = g.tab + (mat * 2u + 1u) * g.nodes;
-  const float4 A = tab[b.j], B = tab[b.j + 1];
-  const float sig0 = lerp_node(b.f, A.x, B.x);
-  const float S0 = lerp_node(b.f, A.y, B.y);
-  const float R = lerp_node(b.f, A.z, B.z);
-  const float s0 = (sig0 > 0.0f) ? t.n0 / sig0 : kInf;
-  float s_e;
-  {
-    const float r_min = 0.1f, f_r = 0.2f;
-    if (R <= r_min) {
-      s_e = R;
-    } else {
-      const float fr = f_r * R;
-      s_e = (fr > r_min) ? fr : r_min;
-    }
-  }
-
-  // S21
-  const float z_lo = slab_zlo(g, vol0), z_hi = slab_zlo(g, vol0 + 1u);
-  int face;
-  float s = geometry_step(t, g, z_lo, z_hi, face);
-
-  // S22: GEOM (-1), ELOSS (3), brems (0)
+  // S17: a positron below the cut annihilates at rest (handled with the other draws of call 1/2
+  // below, so that a warp evaluates those Philox blocks once)
+  const bool annih = (KIND == K_EP) && (t.ekin < e_cut);
+  bool done = annih;  // nothing more to do in S18-S25
   int w = -1;
-  if (s_e < s) { s = s_e; w = 3; }
-  if (s0 < s) { s = s0; w = 0; }
+  uint32_t vol0 = t.vol;
+  if (!annih) {
+    // S18: bremsstrahlung is the only discrete process; nial[1], nial[2] are carried unchanged
+    if (t.n0 <= 0.0f) t.n0 = -lg(u01(rs.call(0).x));
 
-  // S23
-  t.px = fmaf(s, t.dx, t.px);
-  t.py = fmaf(s, t.dy, t.py);
-  t.pz = fmaf(s, t.dz, t.pz);
-  t.n0 = fmaf(-s, sig0, t.n0);
-  t.step = rs.step + 1u;
-
-  // S24: continuous loss by the midpoint rule, deposit in the pre-step slab
-  float E_post;
-  if (w == 3 && s >= R) {
-    E_post = 0.0f;
-  } else {
-    float E_mid = fmaf(-0.5f * s, S0, E0);
-    if (!(E_mid > e_cut)) E_mid = e_cut;
-    const Bin bm = locate_bin(g, lg(E_mid));
-    const float S_mid = lerp_node(bm.f, tab[bm.j].y, tab[bm.j + 1].y);
-    float dE = s * S_mid;
-    if (!(dE < E0)) dE = E0;
-    E_post = E0 - dE;
-  }
-  o.dep += static_cast<double>(E0 - E_post);
-  if (E_post < e_cut) {
-    if (KIND == K_EM) {
-      o.dep += static_cast<double>(E_post);
-      o.alive = false;
-      return;
+    // S19, S20
+    const uint32_t mat = (vol0 & 1u) ? g.mat_gap : g.mat_abs;
+    const float E0 = t.ekin;
+    const Bin b = locate_bin(g, lg(E0));
+    const float4 *tab = g.tab + (mat * 2u + 1u) * g.nodes;
+    const float4 A = tab[b.j], B = tab[b.j + 1];
+    const float sig0 = lerp_node(b.f, A.x, B.x);
+    const float S0 = lerp_node(b.f, A.y, B.y);
+    const float R = lerp_node(b.f, A.z, B.z);
+    const float q0 = t.n0 / sig0;
+    const float s0 = (sig0 > 0.0f) ? q0 : kInf;
+    float s_e;
+    {
+      const float r_min = 0.1f, f_r = 0.2f;
+      const float fr = f_r * R;
+      s_e = (R <= r_min) ? R : ((fr > r_min) ? fr : r_min);
     }
-    t.ekin = E_post;  // e+ is kept for S17 at its next step
-    return;
-  }
-  t.ekin = E_post;
 
-  if (w < 0) {  // S25
-    if (cross_boundary(t, g, vol0, face, z_lo, z_hi)) {
-      o.esc_e = static_cast<double>(t.ekin) + ((KIND == K_EP) ? static_cast<double>(two_mc2()) : 0.0);
-      o.escaped = true;
-      o.alive = false;
-      return;
+    // S21
+    const float z_lo = slab_zlo(g, vol0), z_hi = slab_zlo(g, vol0 + 1u);
+    int face;
+    float s = geometry_step(t, g, z_lo, z_hi, face);
+
+    // S22: GEOM (-1), ELOSS (3), brems (0)
+    if (s_e < s) { s = s_e; w = 3; }
+    if (s0 < s) { s = s0; w = 0; }
+
+    // S23
+    t.px = fmaf(s, t.dx, t.px);
+    t.py = fmaf(s, t.dy, t.py);
+    t.pz = fmaf(s, t.dz, t.pz);
+    t.n0 = fmaf(-s, sig0, t.n0);
+    t.step = rs.step + 1u;
+
+    // S24: continuous loss by the midpoint rule, deposit in the pre-step slab
+    float E_post;
+    {
+      float E_mid = fmaf(-0.5f * s, S0, E0);
+      if (!(E_mid > e_cut)) E_mid = e_cut;
+      const Bin bm = locate_bin(g, lg(E_mid));
+      const float S_mid = lerp_node(bm.f, tab[bm.j].y, tab[bm.j + 1].y);
+      float dE = s * S_mid;
+      if (!(dE < E0)) dE = E0;
+      E_post = E0 - dE;
+      if (w == 3 && s >= R) E_post = 0.0f;  // the track stops
     }
-  } else if (w == 0) {  // S26 bremsstrahlung: k from the 1/k spectrum on [e_cut, E], photon along dir
-    t.n0 = -1.0f;
+    o.dep += static_cast<double>(E0 - E_post);
+    t.ekin = E_post;
+    if (E_post < e_cut) {
+      done = true;
+      if (KIND == K_EM) {
+        o.dep += static_cast<double>(E_post);
+        o.alive = false;
+      }  // e+ is kept for S17 at its next step
+    } else if (w < 0) {  // S25
+      if (cross_boundary(t, g, vol0, face, z_lo, z_hi)) {
+        o.esc_e = static_cast<double>(t.ekin) + ((KIND == K_EP) ? static_cast<double>(two_mc2()) : 0.0);
+        o.escaped = true;
+        o.alive = false;
+        done = true;
+      }
+    }
+  }
+
+  const bool brems = !done && w == 0;
+  if (annih || brems) {
     const uint4 r1 = rs.call(1), r2 = rs.call(2);
-    const float E = t.ekin;
-    float k = e_cut * ex(u01(r1.x) * lg(E / e_cut));
-    if (!(k < E)) k = E;
-    make_kid(o.kid[0], K_GAMMA, t.dx, t.dy, t.dz, k, r2.x, r2.y);
-    const float E_new = E - k;
-    if (E_new < e_cut && KIND == K_EM) {
-      o.dep += static_cast<double>(E_new);
+    if (KIND == K_EP && annih) {  // S17: two back-to-back photons of energy mc^2, isotropic
+      o.dep += static_cast<double>(t.ekin);
+      const float ct = 1.0f - 2.0f * u01(r1.z);
+      const float st = sqrtf(fmaf(-ct, ct, 1.0f));
+      float sphi, cphi;
+      sincos2pi(u01(r1.w), sphi, cphi);
+      const float ax = st * cphi, ay = st * sphi, az = ct;
+      make_kid(o.kid[0], K_GAMMA, ax, ay, az, kMc2, r2.x, r2.y);
+      make_kid(o.kid[1], K_GAMMA, -ax, -ay, -az, kMc2, r2.z, r2.w);
       o.alive = false;
-      return;
+    } else {  // S26 bremsstrahlung: k from the 1/k spectrum on [e_cut, E], photon along dir
+      t.n0 = -1.0f;
+      const float E = t.ekin;
+      float k = e_cut * ex(u01(r1.x) * lg(E / e_cut));
+      if (!(k < E)) k = E;
+      make_kid(o.kid[0], K_GAMMA, t.dx, t.dy, t.dz, k, r2.x, r2.y);
+      const float E_new = E - k;
+      if (E_new < e_cut && KIND == K_EM) {
+        o.dep += static_cast<double>(E_new);
+        o.alive = false;
+        done = true;
+      } else {
+        t.ekin = E_new;
+      }
     }
-    t.ekin = E_new;
   }
-  runaway_guard<KIND>(t, o);
+  if (!done) runaway_guard<KIND>(t, o);
 }
 
 }  // namespace adept

@@ -313,8 +313,11 @@ __device__ __forceinline__ void process_tile(const Params &p, const Env &env, Ct
 
 // ---------------------------------------------------------------------- the step kernel ------
 // Dynamic shared memory: [tables (p.table_bytes)] [edep histogram (n_slabs doubles)].
+#ifndef ADEPT_STEP_MIN_CTAS
+#define ADEPT_STEP_MIN_CTAS 4
+#endif
 template <int L, int SCHEME, bool INSTR>
-__global__ void __launch_bounds__(kBlock) step_kernel(const __grid_constant__ Params p) {
+__global__ void __launch_bounds__(kBlock, ADEPT_STEP_MIN_CTAS) step_kernel(const __grid_constant__ Params p) {
   extern __shared__ __align__(16) unsigned char dyn_smem[];
   __shared__ CtaShared sh;
   float4 *s_tab = reinterpret_cast<float4 *>(dyn_smem);
