@@ -294,7 +294,7 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
   p.instr_field_rw = reinterpret_cast<unsigned long long *>(c->ws + pl.instr_rw);
 
   // persistent grid: as many CTAs as fit on the device at once
-  c->dyn_smem = pl.table_bytes + size_t(p.n_slabs) * sizeof(double);
+  c->dyn_smem = pl.table_bytes + size_t(p.n_slabs) * sizeof(double) + kQueueBytes;
   int dev = 0, sms = 0;
   if ((e = cudaGetDevice(&dev)) != cudaSuccess) return die("cudaGetDevice", e);
   if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess)

@@ -15,6 +15,12 @@ namespace adept {
 enum SchemeId : int { S_SPARSE = 0, S_DENSE = 1 };
 
 constexpr int kBlock = 256;  // threads per CTA of the step kernel = tracks per tile
+// Shared-memory queue of tracks parked between the two halves of the step: 14 record words + the
+// pending interaction + the slot (sparse scheme), field-major.  At most kBlock - 1 left over from
+// earlier tiles plus kBlock from the current one.
+constexpr int kQueueCap = 2 * kBlock;
+constexpr int kQueueWords = 16;
+constexpr size_t kQueueBytes = size_t(kQueueCap) * kQueueWords * 4;
 
 struct Ctl {
   // dense: tracks in the current / next array.  sparse: length of the current / next slot list.

@@ -37,13 +37,30 @@ struct Kid {  // a secondary: position, slab, nial = -1, step = 0 come from the 
   int kind;  // -1 = none
 };
 
-struct Outcome {
-  bool alive;    // track goes to the next iteration
+// The step is split in two so that a warp never drags idle lanes through an interaction:
+//   move_*      rules S17(test)-S25: everything up to and including the boundary crossing.  Most
+//               tracks end their step here.  A track whose step ends in a discrete interaction
+//               (or an e+ that must annihilate) is only *marked* (MoveOut::pending).
+//   interact_*  rule S26 (and the S17 annihilation): run later by the kernel on a dense batch of
+//               marked tracks, so that the Philox blocks of calls 1 and 2 and the sampling code are
+//               executed by full warps.
+// Both halves together are exactly the rule sequence; the split changes no operation and no operand.
+enum Pending : int { P_NONE = -1, P_PROC0 = 0, P_PROC1 = 1, P_PROC2 = 2, P_ANNIH = 4 };
+
+struct MoveOut {
+  bool alive;    // track goes to the next iteration (meaningless while pending)
   bool escaped;  // left the calorimeter (S25)
-  Kid kid[2];    // by child ordinal (R5)
+  int pending;   // Pending: interaction still to be done
   double dep;    // energy deposited in the pre-step slab
   double esc_e;  // energy carried out (S25)
   double dep2;   // S31 guard only: deposit in the post-step slab
+};
+
+struct InteractOut {
+  bool alive;
+  Kid kid[2];   // by child ordinal (R5)
+  double dep;   // deposited in the track's slab (interactions do not change slab)
+  double dep2;  // S31 guard
 };
 
 constexpr float kInf = __builtin_huge_valf();
@@ -142,13 +159,15 @@ __device__ __forceinline__ void rotate_dir(float dx, float dy, float dz, float s
   oz = c / nn;
 }
 
-__device__ __forceinline__ void outcome_init(Outcome &o) {
-  o.alive = true; o.escaped = false; o.kid[0].kind = -1; o.kid[1].kind = -1;
-  o.dep = 0.0; o.esc_e = 0.0; o.dep2 = 0.0;
+__device__ __forceinline__ void move_out_init(MoveOut &o) {
+  o.alive = true; o.escaped = false; o.pending = P_NONE; o.dep = 0.0; o.esc_e = 0.0; o.dep2 = 0.0;
+}
+__device__ __forceinline__ void interact_out_init(InteractOut &o) {
+  o.alive = true; o.kid[0].kind = -1; o.kid[1].kind = -1; o.dep = 0.0; o.dep2 = 0.0;
 }
 
 // S31: runaway guard
-template <int KIND> __device__ __forceinline__ void runaway_guard(Trk &t, Outcome &o) {
+template <int KIND, typename Out> __device__ __forceinline__ void runaway_guard(Trk &t, Out &o) {
   if (t.step >= (1u << 20)) {
     o.dep2 += static_cast<double>(t.ekin);
     if (KIND == K_EP) o.dep2 += static_cast<double>(two_mc2());
@@ -157,8 +176,8 @@ template <int KIND> __device__ __forceinline__ void runaway_guard(Trk &t, Outcom
 }
 
 // ------------------------------------------------------------------------------ photon -------
-__device__ __forceinline__ void step_gamma(Trk &t, const Env &g, Outcome &o) {
-  outcome_init(o);
+__device__ __forceinline__ void move_gamma(Trk &t, const Env &g, MoveOut &o) {
+  move_out_init(o);
   const Stream rs{t.id_lo, t.id_hi, t.step};
 
   // S18: re-sample spent interaction lengths (pair, Compton, photoelectric)
@@ -172,8 +191,7 @@ __device__ __forceinline__ void step_gamma(Trk &t, const Env &g, Outcome &o) {
   // S19: cross sections at the pre-step energy and material
   const uint32_t vol0 = t.vol;
   const uint32_t mat = (vol0 & 1u) ? g.mat_gap : g.mat_abs;
-  const float E0 = t.ekin;
-  const Bin b = locate_bin(g, lg(E0));
+  const Bin b = locate_bin(g, lg(t.ekin));
   const float4 *node = g.tab + (mat * 2u + 0u) * g.nodes + b.j;
   const float4 A = node[0], B = node[1];
   const float sig0 = lerp_node(b.f, A.x, B.x);
@@ -204,178 +222,194 @@ __device__ __forceinline__ void step_gamma(Trk &t, const Env &g, Outcome &o) {
   t.n2 = fmaf(-s, sig2, t.n2);
   t.step = rs.step + 1u;
 
-  if (w < 0) {  // S25
-    if (cross_boundary(t, g, vol0, face, z_lo, z_hi)) {
-      o.esc_e = static_cast<double>(t.ekin);
-      o.escaped = true;
-      o.alive = false;
-      return;
-    }
-  } else {
-    // S26.  The draws of call 1 and the child ids of call 2 are evaluated once for whatever
-    // interaction the lanes of a warp take (a block that ends up unused costs nothing extra: the
-    // other lanes need it anyway, and an unread draw changes no result).
-    const uint4 r1 = rs.call(1), r2 = rs.call(2);
-    if (w == 0) {  // pair: uniform split of E - 2 mc^2, both along dir; photon dies
-      t.n0 = -1.0f;
-      const float E_av = t.ekin - two_mc2();
-      const float T_minus = u01(r1.x) * E_av;
-      const float T_plus = E_av - T_minus;
-      if (T_minus >= g.e_cut) make_kid(o.kid[0], K_EM, t.dx, t.dy, t.dz, T_minus, r2.x, r2.y);
-      else o.dep += static_cast<double>(T_minus);
-      make_kid(o.kid[1], K_EP, t.dx, t.dy, t.dz, T_plus, r2.z, r2.w);
-      o.alive = false;
-      return;
-    } else if (w == 1) {  // Compton: 1/eps spectrum, exact kinematics
-      t.n1 = -1.0f;
-      const float E = t.ekin;
-      const float kappa = E / kMc2;
-      const float L = lg(fmaf(2.0f, kappa, 1.0f));
-      const float eps = ex(-(u01(r1.x) * L));
-      const float E1 = eps * E;
-      const float T = E - E1;
-      float ct = 1.0f - (((1.0f / eps) - 1.0f) / kappa);
-      if (ct > 1.0f) ct = 1.0f;
-      if (ct < -1.0f) ct = -1.0f;
-      const float st = sqrtf(fmaf(-ct, ct, 1.0f));
-      float sphi, cphi;
-      sincos2pi(u01(r1.y), sphi, cphi);
-      float nx, ny, nz;
-      rotate_dir(t.dx, t.dy, t.dz, st, ct, sphi, cphi, nx, ny, nz);
-      const float qx = fmaf(E, t.dx, -(E1 * nx));
-      const float qy = fmaf(E, t.dy, -(E1 * ny));
-      const float qz = fmaf(E, t.dz, -(E1 * nz));
-      const float pn = sqrtf(fmaf(qx, qx, fmaf(qy, qy, qz * qz)));
-      if (T >= g.e_cut && pn > 0.0f) make_kid(o.kid[0], K_EM, qx / pn, qy / pn, qz / pn, T, r2.x, r2.y);
-      else o.dep += static_cast<double>(T);
-      if (E1 < g.e_cut) {
-        o.dep += static_cast<double>(E1);
-        o.alive = false;
-        return;
-      }
-      t.ekin = E1;
-      t.dx = nx; t.dy = ny; t.dz = nz;
-    } else {  // photoelectric: e- with T = E along dir; photon dies
-      t.n2 = -1.0f;
-      make_kid(o.kid[0], K_EM, t.dx, t.dy, t.dz, t.ekin, r2.x, r2.y);
-      o.alive = false;
-      return;
-    }
+  if (w >= 0) {  // S26 follows in interact_gamma
+    o.pending = w;
+    return;
+  }
+  // S25
+  if (cross_boundary(t, g, vol0, face, z_lo, z_hi)) {
+    o.esc_e = static_cast<double>(t.ekin);
+    o.escaped = true;
+    o.alive = false;
+    return;
   }
   runaway_guard<K_GAMMA>(t, o);
 }
 
+// S26 for a photon whose step (already taken: t.step is the post-increment value) ended in process w.
+__device__ __forceinline__ void interact_gamma(Trk &t, int w, const Env &g, InteractOut &o) {
+  interact_out_init(o);
+  const Stream rs{t.id_lo, t.id_hi, t.step - 1u};  // draws are addressed by the pre-increment step (R2)
+  const uint4 r1 = rs.call(1), r2 = rs.call(2);
+  if (w == 0) {  // pair: uniform split of E - 2 mc^2, both along dir; photon dies
+    const float E_av = t.ekin - two_mc2();
+    const float T_minus = u01(r1.x) * E_av;
+    const float T_plus = E_av - T_minus;
+    if (T_minus >= g.e_cut) make_kid(o.kid[0], K_EM, t.dx, t.dy, t.dz, T_minus, r2.x, r2.y);
+    else o.dep += static_cast<double>(T_minus);
+    make_kid(o.kid[1], K_EP, t.dx, t.dy, t.dz, T_plus, r2.z, r2.w);
+    o.alive = false;
+    return;
+  }
+  if (w == 2) {  // photoelectric: e- with T = E along dir; photon dies
+    make_kid(o.kid[0], K_EM, t.dx, t.dy, t.dz, t.ekin, r2.x, r2.y);
+    o.alive = false;
+    return;
+  }
+  // Compton: 1/eps spectrum on [1/(1+2 kappa), 1], exact kinematics
+  t.n1 = -1.0f;
+  const float E = t.ekin;
+  const float kappa = E / kMc2;
+  const float L = lg(fmaf(2.0f, kappa, 1.0f));
+  const float eps = ex(-(u01(r1.x) * L));
+  const float E1 = eps * E;
+  const float T = E - E1;
+  float ct = 1.0f - (((1.0f / eps) - 1.0f) / kappa);
+  if (ct > 1.0f) ct = 1.0f;
+  if (ct < -1.0f) ct = -1.0f;
+  const float st = sqrtf(fmaf(-ct, ct, 1.0f));
+  float sphi, cphi;
+  sincos2pi(u01(r1.y), sphi, cphi);
+  float nx, ny, nz;
+  rotate_dir(t.dx, t.dy, t.dz, st, ct, sphi, cphi, nx, ny, nz);
+  const float qx = fmaf(E, t.dx, -(E1 * nx));
+  const float qy = fmaf(E, t.dy, -(E1 * ny));
+  const float qz = fmaf(E, t.dz, -(E1 * nz));
+  const float pn = sqrtf(fmaf(qx, qx, fmaf(qy, qy, qz * qz)));
+  if (T >= g.e_cut && pn > 0.0f) make_kid(o.kid[0], K_EM, qx / pn, qy / pn, qz / pn, T, r2.x, r2.y);
+  else o.dep += static_cast<double>(T);
+  if (E1 < g.e_cut) {
+    o.dep += static_cast<double>(E1);
+    o.alive = false;
+    return;
+  }
+  t.ekin = E1;
+  t.dx = nx; t.dy = ny; t.dz = nz;
+  runaway_guard<K_GAMMA>(t, o);
+}
+
 // --------------------------------------------------------------------- electron / positron ---
-template <int KIND> __device__ __forceinline__ void step_elec(Trk &t, const Env &g, Outcome &o) {
+template <int KIND> __device__ __forceinline__ void move_elec(Trk &t, const Env &g, MoveOut &o) {
   static_assert(KIND == K_EM || KIND == K_EP, "e- or e+");
-  outcome_init(o);
+  move_out_init(o);
   const Stream rs{t.id_lo, t.id_hi, t.step};
   const float e_cut = g.e_cut;
 
-  // S17: a positron below the cut annihilates at rest (handled with the other draws of call 1/2
-  // below, so that a warp evaluates those Philox blocks once)
-  const bool annih = (KIND == K_EP) && (t.ekin < e_cut);
-  bool done = annih;  // nothing more to do in S18-S25
+  // S17: a positron below the cut annihilates at rest, first (done in interact_elec; the track is
+  // untouched here, in particular its step counter)
+  if (KIND == K_EP && t.ekin < e_cut) {
+    o.pending = P_ANNIH;
+    return;
+  }
+
+  // S18: bremsstrahlung is the only discrete process; nial[1], nial[2] are carried unchanged
+  if (t.n0 <= 0.0f) t.n0 = -lg(u01(rs.call(0).x));
+
+  // S19, S20
+  const uint32_t vol0 = t.vol;
+  const uint32_t mat = (vol0 & 1u) ? g.mat_gap : g.mat_abs;
+  const float E0 = t.ekin;
+  const Bin b = locate_bin(g, lg(E0));
+  const float4 *tab = g.tab + (mat * 2u + 1u) * g.nodes;
+  const float4 A = tab[b.j], B = tab[b.j + 1];
+  const float sig0 = lerp_node(b.f, A.x, B.x);
+  const float S0 = lerp_node(b.f, A.y, B.y);
+  const float R = lerp_node(b.f, A.z, B.z);
+  const float q0 = t.n0 / sig0;
+  const float s0 = (sig0 > 0.0f) ? q0 : kInf;
+  float s_e;
+  {
+    const float r_min = 0.1f, f_r = 0.2f;
+    const float fr = f_r * R;
+    s_e = (R <= r_min) ? R : ((fr > r_min) ? fr : r_min);
+  }
+
+  // S21
+  const float z_lo = slab_zlo(g, vol0), z_hi = slab_zlo(g, vol0 + 1u);
+  int face;
+  float s = geometry_step(t, g, z_lo, z_hi, face);
+
+  // S22: GEOM (-1), ELOSS (3), brems (0)
   int w = -1;
-  uint32_t vol0 = t.vol;
-  if (!annih) {
-    // S18: bremsstrahlung is the only discrete process; nial[1], nial[2] are carried unchanged
-    if (t.n0 <= 0.0f) t.n0 = -lg(u01(rs.call(0).x));
+  if (s_e < s) { s = s_e; w = 3; }
+  if (s0 < s) { s = s0; w = 0; }
 
-    // S19, S20
-    const uint32_t mat = (vol0 & 1u) ? g.mat_gap : g.mat_abs;
-    const float E0 = t.ekin;
-    const Bin b = locate_bin(g, lg(E0));
-    const float4 *tab = g.tab + (mat * 2u + 1u) * g.nodes;
-    const float4 A = tab[b.j], B = tab[b.j + 1];
-    const float sig0 = lerp_node(b.f, A.x, B.x);
-    const float S0 = lerp_node(b.f, A.y, B.y);
-    const float R = lerp_node(b.f, A.z, B.z);
-    const float q0 = t.n0 / sig0;
-    const float s0 = (sig0 > 0.0f) ? q0 : kInf;
-    float s_e;
-    {
-      const float r_min = 0.1f, f_r = 0.2f;
-      const float fr = f_r * R;
-      s_e = (R <= r_min) ? R : ((fr > r_min) ? fr : r_min);
-    }
+  // S23
+  t.px = fmaf(s, t.dx, t.px);
+  t.py = fmaf(s, t.dy, t.py);
+  t.pz = fmaf(s, t.dz, t.pz);
+  t.n0 = fmaf(-s, sig0, t.n0);
+  t.step = rs.step + 1u;
 
-    // S21
-    const float z_lo = slab_zlo(g, vol0), z_hi = slab_zlo(g, vol0 + 1u);
-    int face;
-    float s = geometry_step(t, g, z_lo, z_hi, face);
-
-    // S22: GEOM (-1), ELOSS (3), brems (0)
-    if (s_e < s) { s = s_e; w = 3; }
-    if (s0 < s) { s = s0; w = 0; }
-
-    // S23
-    t.px = fmaf(s, t.dx, t.px);
-    t.py = fmaf(s, t.dy, t.py);
-    t.pz = fmaf(s, t.dz, t.pz);
-    t.n0 = fmaf(-s, sig0, t.n0);
-    t.step = rs.step + 1u;
-
-    // S24: continuous loss by the midpoint rule, deposit in the pre-step slab
-    float E_post;
-    {
-      float E_mid = fmaf(-0.5f * s, S0, E0);
-      if (!(E_mid > e_cut)) E_mid = e_cut;
-      const Bin bm = locate_bin(g, lg(E_mid));
-      const float S_mid = lerp_node(bm.f, tab[bm.j].y, tab[bm.j + 1].y);
-      float dE = s * S_mid;
-      if (!(dE < E0)) dE = E0;
-      E_post = E0 - dE;
-      if (w == 3 && s >= R) E_post = 0.0f;  // the track stops
-    }
-    o.dep += static_cast<double>(E0 - E_post);
-    t.ekin = E_post;
-    if (E_post < e_cut) {
-      done = true;
-      if (KIND == K_EM) {
-        o.dep += static_cast<double>(E_post);
-        o.alive = false;
-      }  // e+ is kept for S17 at its next step
-    } else if (w < 0) {  // S25
-      if (cross_boundary(t, g, vol0, face, z_lo, z_hi)) {
-        o.esc_e = static_cast<double>(t.ekin) + ((KIND == K_EP) ? static_cast<double>(two_mc2()) : 0.0);
-        o.escaped = true;
-        o.alive = false;
-        done = true;
-      }
-    }
+  // S24: continuous loss by the midpoint rule, deposit in the pre-step slab
+  float E_post;
+  {
+    float E_mid = fmaf(-0.5f * s, S0, E0);
+    if (!(E_mid > e_cut)) E_mid = e_cut;
+    const Bin bm = locate_bin(g, lg(E_mid));
+    const float S_mid = lerp_node(bm.f, tab[bm.j].y, tab[bm.j + 1].y);
+    float dE = s * S_mid;
+    if (!(dE < E0)) dE = E0;
+    E_post = E0 - dE;
+    if (w == 3 && s >= R) E_post = 0.0f;  // the track stops
   }
-
-  const bool brems = !done && w == 0;
-  if (annih || brems) {
-    const uint4 r1 = rs.call(1), r2 = rs.call(2);
-    if (KIND == K_EP && annih) {  // S17: two back-to-back photons of energy mc^2, isotropic
-      o.dep += static_cast<double>(t.ekin);
-      const float ct = 1.0f - 2.0f * u01(r1.z);
-      const float st = sqrtf(fmaf(-ct, ct, 1.0f));
-      float sphi, cphi;
-      sincos2pi(u01(r1.w), sphi, cphi);
-      const float ax = st * cphi, ay = st * sphi, az = ct;
-      make_kid(o.kid[0], K_GAMMA, ax, ay, az, kMc2, r2.x, r2.y);
-      make_kid(o.kid[1], K_GAMMA, -ax, -ay, -az, kMc2, r2.z, r2.w);
+  o.dep += static_cast<double>(E0 - E_post);
+  t.ekin = E_post;
+  if (E_post < e_cut) {
+    if (KIND == K_EM) {
+      o.dep += static_cast<double>(E_post);
       o.alive = false;
-    } else {  // S26 bremsstrahlung: k from the 1/k spectrum on [e_cut, E], photon along dir
-      t.n0 = -1.0f;
-      const float E = t.ekin;
-      float k = e_cut * ex(u01(r1.x) * lg(E / e_cut));
-      if (!(k < E)) k = E;
-      make_kid(o.kid[0], K_GAMMA, t.dx, t.dy, t.dz, k, r2.x, r2.y);
-      const float E_new = E - k;
-      if (E_new < e_cut && KIND == K_EM) {
-        o.dep += static_cast<double>(E_new);
-        o.alive = false;
-        done = true;
-      } else {
-        t.ekin = E_new;
-      }
+    }  // e+ is kept for S17 at its next step
+    return;
+  }
+  if (w == 0) {  // S26 follows in interact_elec
+    o.pending = P_PROC0;
+    return;
+  }
+  if (w < 0) {  // S25
+    if (cross_boundary(t, g, vol0, face, z_lo, z_hi)) {
+      o.esc_e = static_cast<double>(t.ekin) + ((KIND == K_EP) ? static_cast<double>(two_mc2()) : 0.0);
+      o.escaped = true;
+      o.alive = false;
+      return;
     }
   }
-  if (!done) runaway_guard<KIND>(t, o);
+  runaway_guard<KIND>(t, o);
+}
+
+// S17 annihilation (pending == P_ANNIH: track untouched) or S26 bremsstrahlung (step already taken).
+template <int KIND> __device__ __forceinline__ void interact_elec(Trk &t, int pending, const Env &g, InteractOut &o) {
+  interact_out_init(o);
+  const bool annih = (KIND == K_EP) && (pending == P_ANNIH);
+  const Stream rs{t.id_lo, t.id_hi, annih ? t.step : t.step - 1u};
+  const uint4 r1 = rs.call(1), r2 = rs.call(2);
+  if (annih) {  // two back-to-back photons of energy mc^2, isotropic
+    o.dep += static_cast<double>(t.ekin);
+    const float ct = 1.0f - 2.0f * u01(r1.z);
+    const float st = sqrtf(fmaf(-ct, ct, 1.0f));
+    float sphi, cphi;
+    sincos2pi(u01(r1.w), sphi, cphi);
+    const float ax = st * cphi, ay = st * sphi, az = ct;
+    make_kid(o.kid[0], K_GAMMA, ax, ay, az, kMc2, r2.x, r2.y);
+    make_kid(o.kid[1], K_GAMMA, -ax, -ay, -az, kMc2, r2.z, r2.w);
+    o.alive = false;
+    return;
+  }
+  // bremsstrahlung: k from the 1/k spectrum on [e_cut, E], photon along dir
+  const float e_cut = g.e_cut;
+  t.n0 = -1.0f;
+  const float E = t.ekin;
+  float k = e_cut * ex(u01(r1.x) * lg(E / e_cut));
+  if (!(k < E)) k = E;
+  make_kid(o.kid[0], K_GAMMA, t.dx, t.dy, t.dz, k, r2.x, r2.y);
+  const float E_new = E - k;
+  if (E_new < e_cut && KIND == K_EM) {
+    o.dep += static_cast<double>(E_new);
+    o.alive = false;
+    return;
+  }
+  t.ekin = E_new;
+  runaway_guard<KIND>(t, o);
 }
 
 }  // namespace adept

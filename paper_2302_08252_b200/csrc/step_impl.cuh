@@ -9,6 +9,11 @@
 //   A1      track load through the layout accessor (layout.cuh);
 //   A2-A8   the physics/geometry step (physics.cuh), tables staged in shared memory by one TMA
 //           bulk copy per CTA;
+//           The step is split (physics.cuh): every track takes the "move" half; tracks whose step ends
+//           in a discrete interaction are parked in a shared-memory queue and the "interact" half
+//           runs on dense batches of 256 parked tracks, so that the Philox blocks and the sampling
+//           code of rule S26 are executed by full warps instead of a few lanes per warp (the paper's
+//           "diverging code paths");
 //   A9      dense: secondaries and survivors are ranked by one packed block scan (3 x 10-bit
 //           counters, one per destination type; warp shuffles + one shared-memory hop) and the CTA
 //           reserves its output ranges with one atomicAdd per destination type;
@@ -117,7 +122,7 @@ struct CtaShared {
   uint32_t base[2][4];
   uint32_t alive[4];
   uint32_t escaped[4];
-  uint32_t last_flag;
+  uint32_t q_count;  // parked tracks waiting for their interaction
   double esc_e;
   uint32_t probe[3 * kNumFields * 2];
 };
@@ -158,74 +163,156 @@ template <int SCHEME> __device__ void finish_iteration(const Params &p) {
   c->done_ctas = 0u;
 }
 
-// -------------------------------------------------------------------------- one tile ---------
-// Output counters of a thread, packed 3 x 10 bits (destination kind q at bits 10q..10q+9).
-template <int KIND> __device__ __forceinline__ uint32_t packed_outputs(const Outcome &o) {
-  uint32_t c = o.alive ? (1u << (10 * KIND)) : 0u;
-  if (KIND == K_GAMMA) {  // kid 0 is an e-, kid 1 an e+ (rule R5)
-    c += (o.kid[0].kind >= 0) ? 1u : 0u;
-    c += (o.kid[1].kind >= 0) ? (1u << 10) : 0u;
-  } else {  // kids of e-/e+ are photons
-    c += (o.kid[0].kind >= 0) ? (1u << 20) : 0u;
-    c += (o.kid[1].kind >= 0) ? (1u << 20) : 0u;
-  }
-  return c;
-}
+// ------------------------------------------------------------------- tile = 256 tracks --------
 template <int KIND> __device__ __forceinline__ constexpr int kid_kind(int ordinal) {
-  return KIND == K_GAMMA ? (ordinal == 0 ? K_EM : K_EP) : K_GAMMA;
+  return KIND == K_GAMMA ? (ordinal == 0 ? K_EM : K_EP) : K_GAMMA;  // rule R5
 }
 
-template <int KIND> __device__ __forceinline__ void do_step(Trk &t, const Env &env, Outcome &o) {
-  if constexpr (KIND == K_GAMMA) step_gamma(t, env, o);
-  else step_elec<KIND>(t, env, o);
-}
+// What a CTA carries through its tiles.
+struct CtaRefs {
+  CtaShared *sh;
+  double *edep;     // shared histogram, n_slabs
+  uint32_t *queue;  // shared, [kQueueWords][kQueueCap]
+};
 
-// Process tile `tile` (256 consecutive entries) of kind KIND's current set.
+struct Tally {  // per-thread running sums of one kind (warp-uniform except esc_e)
+  uint32_t alive, escaped;
+};
+
+// First half of the step for tile `tile` of kind KIND's current set (rows A1-A7, A10 for the
+// tracks whose step ends without an interaction).  Returns the number of parked tracks, read by
+// every thread between two block barriers (so the value is the same for the whole CTA).
 template <int L, int SCHEME, bool INSTR, int KIND>
-__device__ __forceinline__ void process_tile(const Params &p, const Env &env, CtaShared &sh, double *s_edep,
-                                             uint32_t par, uint32_t tile, uint32_t n_kind, int sbuf,
-                                             uint32_t &acc_alive, uint32_t &acc_esc, double &acc_esc_e) {
+__device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, const CtaRefs &c, uint32_t par,
+                                          uint32_t tile, uint32_t n_kind, int sbuf, Tally &tally, double &esc_e) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const uint32_t lt_mask = (1u << lane) - 1u;
   const uint32_t i = tile * kBlock + tid;
   const bool active = i < n_kind;
   Ctl *ctl = p.ctl;
+  CtaShared &sh = *c.sh;
 
   // A1: load
   uint32_t slot = i;
   if (SCHEME == S_SPARSE && active) slot = p.kind[KIND].queue[par][i];
   const TrackView<L, INSTR> cur = make_view<L, INSTR>(p, KIND, (SCHEME == S_DENSE) ? int(par) : 0, sh.probe);
   Trk t, old;
-  Outcome o;
-  outcome_init(o);
+  MoveOut o;
+  move_out_init(o);
   o.alive = false;
   if (active) {
     t = cur.load(slot);
     old = t;
-    // A2-A8
-    do_step<KIND>(t, env, o);
+    if constexpr (KIND == K_GAMMA) move_gamma(t, env, o);
+    else move_elec<KIND>(t, env, o);
     // A6: scoring into the CTA's histogram (pre-step slab; the S31 guard uses the post-step slab)
-    if (o.dep != 0.0) atomicAdd(&s_edep[old.vol], o.dep);
-    if (o.dep2 != 0.0) atomicAdd(&s_edep[t.vol], o.dep2);
-    acc_esc_e += o.esc_e;
+    if (o.dep != 0.0) atomicAdd(&c.edep[old.vol], o.dep);
+    if (o.dep2 != 0.0) atomicAdd(&c.edep[t.vol], o.dep2);
+    esc_e += o.esc_e;
+  }
+  const bool parked = active && o.pending != P_NONE;
+  const bool survives = active && !parked && o.alive;
+  const uint32_t m_surv = __ballot_sync(0xFFFFFFFFu, survives);
+  const uint32_t m_esc = __ballot_sync(0xFFFFFFFFu, o.escaped);
+  const uint32_t m_park = __ballot_sync(0xFFFFFFFFu, parked);
+  tally.alive += __popc(m_surv);
+  tally.escaped += __popc(m_esc);
+
+  // park the tracks that still owe an interaction (one shared-memory atomic per warp)
+  if (m_park) {
+    uint32_t qbase = 0;
+    if (lane == 0) qbase = atomicAdd(&sh.q_count, uint32_t(__popc(m_park)));
+    qbase = __shfl_sync(0xFFFFFFFFu, qbase, 0);
+    if (parked) {
+      const uint32_t q = qbase + __popc(m_park & lt_mask);
+#pragma unroll
+      for (int f = 0; f < kNumFields; ++f) c.queue[f * kQueueCap + q] = trk_word(t, f);
+      c.queue[14 * kQueueCap + q] = uint32_t(o.pending);
+      c.queue[15 * kQueueCap + q] = slot;
+    }
   }
 
-  // tallies: survivors and escapes of this warp (lane 0 keeps the packed per-kind sums)
-  {
-    const uint32_t m_alive = __ballot_sync(0xFFFFFFFFu, o.alive);
-    const uint32_t m_esc = __ballot_sync(0xFFFFFFFFu, o.escaped);
-    acc_alive += __popc(m_alive);
-    acc_esc += __popc(m_esc);
+  if (SCHEME == S_DENSE) {
+    // A9/A10: survivors of the tile go to one contiguous range of the next array
+    const uint32_t rank_in_warp = __popc(m_surv & lt_mask);
+    if (lane == 0) sh.warp_tot[sbuf][warp] = __popc(m_surv);
+    __syncthreads();
+    uint32_t before = 0, total = 0;
+#pragma unroll
+    for (int w = 0; w < kBlock / 32; ++w) {
+      const uint32_t v = sh.warp_tot[sbuf][w];
+      total += v;
+      if (w < warp) before += v;
+    }
+    if (tid == 0) sh.base[sbuf][KIND] = total ? atomicAdd(&ctl->n_next[KIND], total) : 0u;
+    const uint32_t queued = sh.q_count;
+    __syncthreads();
+    if (survives) {
+      const uint32_t dst = sh.base[sbuf][KIND] + before + rank_in_warp;
+      if (dst < p.capacity) make_view<L, INSTR>(p, KIND, int(par ^ 1u), sh.probe).store(dst, t);
+      else ctl->overflow = 1u;
+    }
+    return queued;
+  } else {
+    // A10 sparse: in-place update of the words that changed (parked tracks too: the interaction
+    // later writes only what it changes), slot pushed onto the next list
+    if (survives || parked) cur.store_changed(slot, t, old);
+    const uint32_t qpos = warp_reserve(&ctl->n_next[KIND], survives ? 1u : 0u, lane);
+    if (survives) {
+      if (qpos < p.capacity) p.kind[KIND].queue[par ^ 1u][qpos] = slot;
+      else ctl->overflow = 1u;
+    }
+    __syncthreads();
+    const uint32_t queued = sh.q_count;
+    __syncthreads();
+    return queued;
   }
+}
+
+// Second half of the step on a dense batch of up to 256 parked tracks taken from the top of the
+// queue (rows A8, A9, A10).  `queued` is sh.q_count as read by every thread after a barrier.
+template <int L, int SCHEME, bool INSTR, int KIND>
+__device__ __forceinline__ void interact_batch(const Params &p, const Env &env, const CtaRefs &c, uint32_t par,
+                                               uint32_t queued, int sbuf, Tally &tally) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  Ctl *ctl = p.ctl;
+  CtaShared &sh = *c.sh;
+  const uint32_t batch = queued < uint32_t(kBlock) ? queued : uint32_t(kBlock);
+  const uint32_t first = queued - batch;
+  __syncthreads();  // every thread has read q_count
+  if (tid == 0) sh.q_count = first;
+
+  const bool have = uint32_t(tid) < batch;
+  Trk t, before_interaction;
+  InteractOut o;
+  interact_out_init(o);
+  o.alive = false;
+  uint32_t slot = 0;
+  if (have) {
+    const uint32_t q = first + tid;
+#pragma unroll
+    for (int f = 0; f < kNumFields; ++f) trk_set_word(t, f, c.queue[f * kQueueCap + q]);
+    const int pending = int(c.queue[14 * kQueueCap + q]);
+    slot = c.queue[15 * kQueueCap + q];
+    before_interaction = t;
+    if constexpr (KIND == K_GAMMA) interact_gamma(t, pending, env, o);
+    else interact_elec<KIND>(t, pending, env, o);
+    if (o.dep != 0.0) atomicAdd(&c.edep[t.vol], o.dep);
+    if (o.dep2 != 0.0) atomicAdd(&c.edep[t.vol], o.dep2);
+  }
+  tally.alive += __popc(__ballot_sync(0xFFFFFFFFu, o.alive));
 
   const bool has0 = o.kid[0].kind >= 0, has1 = o.kid[1].kind >= 0;
   constexpr int Q0 = kid_kind<KIND>(0), Q1 = kid_kind<KIND>(1);
 
   if (SCHEME == S_DENSE) {
-    // A9: rank every output of the tile per destination kind with one packed scan
-    const uint32_t mine = packed_outputs<KIND>(o);
+    // A9: rank every output of the batch per destination kind with one packed scan (3 x 10 bits)
+    uint32_t mine = o.alive ? (1u << (10 * KIND)) : 0u;
+    mine += has0 ? (1u << (10 * Q0)) : 0u;
+    mine += has1 ? (1u << (10 * Q1)) : 0u;
     const uint32_t inc = warp_inclusive_scan(mine, lane);
     if (lane == 31) sh.warp_tot[sbuf][warp] = inc;
-    __syncthreads();
+    __syncthreads();  // also: all queue entries of the batch have been read
     uint32_t before = 0, total = 0;
 #pragma unroll
     for (int w = 0; w < kBlock / 32; ++w) {
@@ -262,11 +349,12 @@ __device__ __forceinline__ void process_tile(const Params &p, const Env &env, Ct
     }
     if (dropped) ctl->overflow = 1u;
   } else {
-    // A10 sparse: in-place update of the words that changed, slot pushed onto the next list
-    const uint32_t qpos = warp_reserve(&ctl->n_next[KIND], o.alive ? 1u : 0u, lane);
+    __syncthreads();  // all queue entries of the batch have been read; q_count update is visible
     bool dropped = false;
+    // A10 sparse: the words the interaction changed, slot pushed onto the next list
+    const uint32_t qpos = warp_reserve(&ctl->n_next[KIND], o.alive ? 1u : 0u, lane);
     if (o.alive) {
-      cur.store_changed(slot, t, old);
+      make_view<L, INSTR>(p, KIND, 0, sh.probe).store_changed(slot, t, before_interaction);
       if (qpos < p.capacity) p.kind[KIND].queue[par ^ 1u][qpos] = slot;
       else dropped = true;
     }
@@ -311,8 +399,33 @@ __device__ __forceinline__ void process_tile(const Params &p, const Env &env, Ct
   }
 }
 
+// All tiles of one kind that belong to this CTA, then the left-over parked tracks.
+template <int L, int SCHEME, bool INSTR, int KIND>
+__device__ __forceinline__ void run_kind(const Params &p, const Env &env, const CtaRefs &c, uint32_t par,
+                                         uint32_t first_global_tile, uint32_t n_tiles, uint32_t n_kind, int &sbuf,
+                                         Tally &tally, double &esc_e) {
+  // global tile index g = first_global_tile + tile must be congruent to blockIdx.x modulo gridDim.x
+  const uint32_t grid = gridDim.x;
+  const uint32_t shift = (blockIdx.x + grid - first_global_tile % grid) % grid;
+  for (uint32_t tile = shift; tile < n_tiles; tile += grid) {
+    const uint32_t queued = move_tile<L, SCHEME, INSTR, KIND>(p, env, c, par, tile, n_kind, sbuf, tally, esc_e);
+    sbuf ^= 1;
+    if (queued >= uint32_t(kBlock)) {
+      interact_batch<L, SCHEME, INSTR, KIND>(p, env, c, par, queued, sbuf, tally);
+      sbuf ^= 1;
+    }
+  }
+  for (;;) {
+    __syncthreads();
+    const uint32_t queued = c.sh->q_count;
+    if (queued == 0u) break;
+    interact_batch<L, SCHEME, INSTR, KIND>(p, env, c, par, queued, sbuf, tally);
+    sbuf ^= 1;
+  }
+}
+
 // ---------------------------------------------------------------------- the step kernel ------
-// Dynamic shared memory: [tables (p.table_bytes)] [edep histogram (n_slabs doubles)].
+// Dynamic shared memory: [tables (p.table_bytes)] [edep histogram (n_slabs doubles)] [queue].
 #ifndef ADEPT_STEP_MIN_CTAS
 #define ADEPT_STEP_MIN_CTAS 4
 #endif
@@ -321,9 +434,12 @@ __global__ void __launch_bounds__(kBlock, ADEPT_STEP_MIN_CTAS) step_kernel(const
   extern __shared__ __align__(16) unsigned char dyn_smem[];
   __shared__ CtaShared sh;
   float4 *s_tab = reinterpret_cast<float4 *>(dyn_smem);
-  double *s_edep = reinterpret_cast<double *>(dyn_smem + p.table_bytes);
   const int tid = threadIdx.x;
   Ctl *ctl = p.ctl;
+  CtaRefs c;
+  c.sh = &sh;
+  c.edep = reinterpret_cast<double *>(dyn_smem + p.table_bytes);
+  c.queue = reinterpret_cast<uint32_t *>(dyn_smem + p.table_bytes + size_t(p.n_slabs) * sizeof(double));
 
   // A0: what is alive (written by the previous iteration's last CTA; constant during this launch)
   const uint32_t par = ctl->parity;
@@ -334,9 +450,9 @@ __global__ void __launch_bounds__(kBlock, ADEPT_STEP_MIN_CTAS) step_kernel(const
   if (blockIdx.x < tiles) {
     // A3: tables -> shared memory, one TMA bulk copy; histogram and counters cleared meanwhile
     tma_stage(s_tab, p.tables, p.table_bytes, &sh.mbar, tid);
-    for (uint32_t s = tid; s < p.n_slabs; s += kBlock) s_edep[s] = 0.0;
+    for (uint32_t s = tid; s < p.n_slabs; s += kBlock) c.edep[s] = 0.0;
     if (tid < 4) { sh.alive[tid] = 0u; sh.escaped[tid] = 0u; }
-    if (tid == 0) sh.esc_e = 0.0;
+    if (tid == 0) { sh.esc_e = 0.0; sh.q_count = 0u; }
     if (INSTR) for (int s = tid; s < 3 * kNumFields * 2; s += kBlock) sh.probe[s] = 0u;
     tma_wait(&sh.mbar);
     __syncthreads();
@@ -347,33 +463,27 @@ __global__ void __launch_bounds__(kBlock, ADEPT_STEP_MIN_CTAS) step_kernel(const
     env.n_slabs = p.n_slabs; env.abs_mm = p.abs_mm; env.pitch = p.pitch; env.half_xy = p.half_xy;
     env.mat_abs = p.mat_abs; env.mat_gap = p.mat_gap;
 
-    uint32_t alive0 = 0, alive1 = 0, alive2 = 0, esc0 = 0, esc1 = 0, esc2 = 0;
+    Tally ta0{0u, 0u}, ta1{0u, 0u}, ta2{0u, 0u};
     double esc_e = 0.0;
     int sbuf = 0;
-    for (uint32_t tile = blockIdx.x; tile < tiles; tile += gridDim.x, sbuf ^= 1) {
-      if (tile < t0) {
-        process_tile<L, SCHEME, INSTR, K_EM>(p, env, sh, s_edep, par, tile, n0, sbuf, alive0, esc0, esc_e);
-      } else if (tile < t0 + t1) {
-        process_tile<L, SCHEME, INSTR, K_EP>(p, env, sh, s_edep, par, tile - t0, n1, sbuf, alive1, esc1, esc_e);
-      } else {
-        process_tile<L, SCHEME, INSTR, K_GAMMA>(p, env, sh, s_edep, par, tile - t0 - t1, n2, sbuf, alive2, esc2, esc_e);
-      }
-    }
+    run_kind<L, SCHEME, INSTR, K_EM>(p, env, c, par, 0u, t0, n0, sbuf, ta0, esc_e);
+    run_kind<L, SCHEME, INSTR, K_EP>(p, env, c, par, t0, t1, n1, sbuf, ta1, esc_e);
+    run_kind<L, SCHEME, INSTR, K_GAMMA>(p, env, c, par, t0 + t1, t2, n2, sbuf, ta2, esc_e);
 
     // flush the CTA's tallies
     esc_e = warp_sum(esc_e);
     if ((tid & 31) == 0) {
-      if (alive0) atomicAdd(&sh.alive[0], alive0);
-      if (alive1) atomicAdd(&sh.alive[1], alive1);
-      if (alive2) atomicAdd(&sh.alive[2], alive2);
-      if (esc0) atomicAdd(&sh.escaped[0], esc0);
-      if (esc1) atomicAdd(&sh.escaped[1], esc1);
-      if (esc2) atomicAdd(&sh.escaped[2], esc2);
+      if (ta0.alive) atomicAdd(&sh.alive[0], ta0.alive);
+      if (ta1.alive) atomicAdd(&sh.alive[1], ta1.alive);
+      if (ta2.alive) atomicAdd(&sh.alive[2], ta2.alive);
+      if (ta0.escaped) atomicAdd(&sh.escaped[0], ta0.escaped);
+      if (ta1.escaped) atomicAdd(&sh.escaped[1], ta1.escaped);
+      if (ta2.escaped) atomicAdd(&sh.escaped[2], ta2.escaped);
       if (esc_e != 0.0) atomicAdd(&sh.esc_e, esc_e);
     }
     __syncthreads();
     for (uint32_t s = tid; s < p.n_slabs; s += kBlock) {
-      const double v = s_edep[s];
+      const double v = c.edep[s];
       if (v != 0.0) atomicAdd(&p.edep[s], v);
     }
     if (tid < 3) {
