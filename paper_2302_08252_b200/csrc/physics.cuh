@@ -100,7 +100,9 @@ __device__ __forceinline__ float geometry_step(const Trk &t, const Env &g, float
   const float n_z = ((t.dz > 0.0f) ? z_hi : z_lo) - t.pz;
   const float n_x = ((t.dx > 0.0f) ? H : -H) - t.px;
   const float n_y = ((t.dy > 0.0f) ? H : -H) - t.py;
-  const float q_z = n_z / t.dz, q_x = n_x / t.dx, q_y = n_y / t.dy;
+  const float q_z = n_z / ((t.dz != 0.0f) ? t.dz : 1.0f);
+  const float q_x = n_x / ((t.dx != 0.0f) ? t.dx : 1.0f);
+  const float q_y = n_y / ((t.dy != 0.0f) ? t.dy : 1.0f);
   const float s_z = (t.dz != 0.0f) ? q_z : kInf;
   const float s_x = (t.dx != 0.0f) ? q_x : kInf;
   const float s_y = (t.dy != 0.0f) ? q_y : kInf;
@@ -197,7 +199,12 @@ __device__ __forceinline__ void move_gamma(Trk &t, const Env &g, MoveOut &o) {
   const float sig0 = lerp_node(b.f, A.x, B.x);
   const float sig1 = lerp_node(b.f, A.y, B.y);
   const float sig2 = lerp_node(b.f, A.z, B.z);
-  const float q0 = t.n0 / sig0, q1 = t.n1 / sig1, q2 = t.n2 / sig2;  // selected below: no divergent branch
+  // s_j = nial_j / Sigma_j where Sigma_j > 0, else +inf.  The divisor is selected first (1 where the
+  // quotient is not used): no divergent branch, and no division by zero, which would send the lane
+  // through the slow path of the IEEE division (Sigma_pair is exactly 0 below ~3.4 MeV).
+  const float q0 = t.n0 / ((sig0 > 0.0f) ? sig0 : 1.0f);
+  const float q1 = t.n1 / ((sig1 > 0.0f) ? sig1 : 1.0f);
+  const float q2 = t.n2 / ((sig2 > 0.0f) ? sig2 : 1.0f);
   const float s0 = (sig0 > 0.0f) ? q0 : kInf;
   const float s1 = (sig1 > 0.0f) ? q1 : kInf;
   const float s2 = (sig2 > 0.0f) ? q2 : kInf;
@@ -315,7 +322,7 @@ template <int KIND> __device__ __forceinline__ void move_elec(Trk &t, const Env 
   const float sig0 = lerp_node(b.f, A.x, B.x);
   const float S0 = lerp_node(b.f, A.y, B.y);
   const float R = lerp_node(b.f, A.z, B.z);
-  const float q0 = t.n0 / sig0;
+  const float q0 = t.n0 / ((sig0 > 0.0f) ? sig0 : 1.0f);  // divisor selected first, see move_gamma
   const float s0 = (sig0 > 0.0f) ? q0 : kInf;
   float s_e;
   {
