@@ -258,15 +258,16 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
   if ((e = cudaMallocHost(reinterpret_cast<void **>(&c->pinned), c->pinned_bytes)) != cudaSuccess)
     return die("cudaMallocHost", e);
 
-  // tables: [mat][group][qty][node] (host, ABI) -> [mat][group][node]{q0,q1,q2,0} (device): one
-  // 16-byte shared-memory load fetches all three quantities of a node.
+  // tables: [mat][group][qty][node] (host, ABI) -> [group][mat][node]{q0,q1,q2,0} (device): a CTA
+  // stages only the group of the particle kind it is stepping, and one 16-byte shared-memory load
+  // fetches all three quantities of a node.
   const uint32_t nodes = t->n_bins + 1;
   std::vector<float> packed(pl.table_bytes / sizeof(float), 0.0f);
   for (uint32_t m = 0; m < t->n_materials; ++m)
     for (uint32_t grp = 0; grp < 2; ++grp)
       for (uint32_t q = 0; q < 3; ++q)
         for (uint32_t j = 0; j < nodes; ++j)
-          packed[((size_t(m) * 2 + grp) * nodes + j) * 4 + q] = t->data[((size_t(m) * 2 + grp) * 3 + q) * nodes + j];
+          packed[((size_t(grp) * t->n_materials + m) * nodes + j) * 4 + q] = t->data[((size_t(m) * 2 + grp) * 3 + q) * nodes + j];
   if ((e = cudaMemcpyAsync(c->ws + pl.tables, packed.data(), pl.table_bytes, cudaMemcpyHostToDevice, c->stream)) != cudaSuccess)
     return die("cudaMemcpyAsync(tables)", e);
   if ((e = cudaStreamSynchronize(c->stream)) != cudaSuccess) return die("cudaStreamSynchronize", e);
@@ -275,7 +276,7 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
   p.ctl = reinterpret_cast<Ctl *>(c->ws + pl.ctl);
   p.edep = reinterpret_cast<double *>(c->ws + pl.ctl + kCtlHeaderBytes);
   p.tables = reinterpret_cast<const float4 *>(c->ws + pl.tables);
-  p.table_bytes = static_cast<uint32_t>(pl.table_bytes);
+  p.table_bytes = static_cast<uint32_t>(pl.table_bytes / 2);  // per particle group
   p.nodes = nodes;
   p.ln_e_min = t->ln_e_min; p.inv_dln = t->inv_dln; p.e_cut = t->e_cut;
   p.n_slabs = 2 * g->n_layers;
@@ -294,7 +295,7 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
   p.instr_field_rw = reinterpret_cast<unsigned long long *>(c->ws + pl.instr_rw);
 
   // persistent grid: as many CTAs as fit on the device at once
-  c->dyn_smem = pl.table_bytes + size_t(p.n_slabs) * sizeof(double) + kQueueBytes;
+  c->dyn_smem = pl.table_bytes / 2 + size_t(p.n_slabs) * sizeof(double) + queue_bytes(cfg->scheme) + in_buf_bytes(cfg->scheme, c->ops->record_words(kBlock));
   int dev = 0, sms = 0;
   if ((e = cudaGetDevice(&dev)) != cudaSuccess) return die("cudaGetDevice", e);
   if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess)

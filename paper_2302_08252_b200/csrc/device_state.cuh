@@ -16,11 +16,15 @@ enum SchemeId : int { S_SPARSE = 0, S_DENSE = 1 };
 
 constexpr int kBlock = 256;  // threads per CTA of the step kernel = tracks per tile
 // Shared-memory queue of tracks parked between the two halves of the step: 14 record words + the
-// pending interaction + the slot (sparse scheme), field-major.  At most kBlock - 1 left over from
-// earlier tiles plus kBlock from the current one.
+// pending interaction (+ the slot, sparse scheme only), field-major.  At most kBlock - 1 left over
+// from earlier tiles plus kBlock from the current one.
 constexpr int kQueueCap = 2 * kBlock;
-constexpr int kQueueWords = 16;
-constexpr size_t kQueueBytes = size_t(kQueueCap) * kQueueWords * 4;
+__host__ __device__ constexpr int queue_words(int scheme) { return scheme == S_DENSE ? 15 : 16; }
+__host__ __device__ constexpr size_t queue_bytes(int scheme) { return size_t(kQueueCap) * queue_words(scheme) * 4; }
+// Dense scheme: one tile staged in shared memory by TMA (record_words(kBlock) words of the layout).
+__host__ __device__ constexpr size_t in_buf_bytes(int scheme, size_t tile_words) {
+  return scheme == S_DENSE ? tile_words * 4 : 0;
+}
 
 struct Ctl {
   // dense: tracks in the current / next array.  sparse: length of the current / next slot list.
@@ -52,8 +56,8 @@ struct KindStorage {
 struct Params {
   Ctl *ctl;
   double *edep;              // [n_slabs], right after the control header
-  const float4 *tables;      // [material][group][node] {q0, q1, q2, 0}
-  uint32_t table_bytes;      // multiple of 16
+  const float4 *tables;      // [group][material][node] {q0, q1, q2, 0}; group 0 = gamma, 1 = e+-
+  uint32_t table_bytes;      // bytes of ONE group, multiple of 16
   uint32_t nodes;            // n_bins + 1
   float ln_e_min, inv_dln, e_cut;
   uint32_t n_slabs;

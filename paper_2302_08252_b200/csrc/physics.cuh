@@ -23,7 +23,7 @@ enum Kind : int { K_EM = 0, K_EP = 1, K_GAMMA = 2 };
 
 // What the step needs besides the track: tables (shared memory) and geometry (registers).
 struct Env {
-  const float4 *tab;  // [material][group][node] -> {qty0, qty1, qty2, 0}; group 0 = gamma, 1 = e+-
+  const float4 *tab;  // the particle group's tables: [material][node] -> {qty0, qty1, qty2, 0}
   uint32_t nodes;     // n_bins + 1
   float ln_e_min, inv_dln, e_cut;
   uint32_t n_slabs;   // 2 * n_layers
@@ -194,7 +194,7 @@ __device__ __forceinline__ void move_gamma(Trk &t, const Env &g, MoveOut &o) {
   const uint32_t vol0 = t.vol;
   const uint32_t mat = (vol0 & 1u) ? g.mat_gap : g.mat_abs;
   const Bin b = locate_bin(g, lg(t.ekin));
-  const float4 *node = g.tab + (mat * 2u + 0u) * g.nodes + b.j;
+  const float4 *node = g.tab + mat * g.nodes + b.j;
   const float4 A = node[0], B = node[1];
   const float sig0 = lerp_node(b.f, A.x, B.x);
   const float sig1 = lerp_node(b.f, A.y, B.y);
@@ -317,7 +317,7 @@ template <int KIND> __device__ __forceinline__ void move_elec(Trk &t, const Env 
   const uint32_t mat = (vol0 & 1u) ? g.mat_gap : g.mat_abs;
   const float E0 = t.ekin;
   const Bin b = locate_bin(g, lg(E0));
-  const float4 *tab = g.tab + (mat * 2u + 1u) * g.nodes;
+  const float4 *tab = g.tab + mat * g.nodes;
   const float4 A = tab[b.j], B = tab[b.j + 1];
   const float sig0 = lerp_node(b.f, A.x, B.x);
   const float S0 = lerp_node(b.f, A.y, B.y);

@@ -60,34 +60,71 @@ __device__ __forceinline__ double warp_sum(double v) {
   return v;
 }
 
-// One TMA bulk copy global -> shared of `bytes` (multiple of 16), completion on an mbarrier.
-__device__ __forceinline__ void tma_stage(void *smem_dst, const void *gmem_src, uint32_t bytes, uint64_t *mbar,
-                                          int tid) {
-  const uint32_t bar = static_cast<uint32_t>(__cvta_generic_to_shared(mbar));
-  const uint32_t dst = static_cast<uint32_t>(__cvta_generic_to_shared(smem_dst));
-  if (tid == 0) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar));
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  }
-  __syncthreads();
-  if (tid == 0) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-    asm volatile(
-        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
-        "l"(gmem_src), "r"(bytes), "r"(bar)
-        : "memory");
-  }
+// ---- asynchronous tile prefetch (dense scheme) ---------------------------------------------------
+// A tile of 256 consecutive slots is contiguous in global memory per layout (AoS: one 16 KB run;
+// AoSoA-32: eight 1792-byte blocks back to back; SoA: one 1 KB run per field), so the next tile is
+// fetched into shared memory by TMA bulk copies while the current one is being stepped: the global
+// load latency leaves the critical path and no load instruction or address arithmetic is issued.
+__device__ __forceinline__ void mbar_init(uint64_t *mbar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(static_cast<uint32_t>(__cvta_generic_to_shared(mbar))),
+               "r"(count));
 }
-__device__ __forceinline__ void tma_wait(uint64_t *mbar) {
+__device__ __forceinline__ void mbar_wait(uint64_t *mbar, uint32_t parity) {
   const uint32_t bar = static_cast<uint32_t>(__cvta_generic_to_shared(mbar));
   uint32_t done = 0;
   while (!done) {
     asm volatile(
-        "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\n selp.u32 %0, 1, 0, p;\n}"
+        "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
         : "=r"(done)
-        : "r"(bar)
+        : "r"(bar), "r"(parity)
         : "memory");
   }
+}
+__device__ __forceinline__ void bulk_g2s(void *smem_dst, const void *gmem_src, uint32_t bytes, uint64_t *mbar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   static_cast<uint32_t>(__cvta_generic_to_shared(smem_dst))),
+               "l"(gmem_src), "r"(bytes), "r"(static_cast<uint32_t>(__cvta_generic_to_shared(mbar)))
+               : "memory");
+}
+
+// Called by ONE thread, after a barrier that follows every thread's last read of `in_buf`.
+template <int L>
+__device__ __forceinline__ void prefetch_tile(const uint32_t *rec, uint32_t cap, uint32_t tile, uint32_t n_kind,
+                                              uint32_t *in_buf, uint64_t *mbar) {
+  const uint32_t first = tile * kBlock;
+  const uint32_t n = (n_kind - first < uint32_t(kBlock)) ? n_kind - first : uint32_t(kBlock);
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic reads of in_buf before async writes
+  const uint32_t bar = static_cast<uint32_t>(__cvta_generic_to_shared(mbar));
+  if (L == L_SOA) {
+    const uint32_t bytes = ((n + 3u) / 4u) * 16u;  // slots are padded to a multiple of 32: stays inside the array
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes * kNumFields) : "memory");
+#pragma unroll
+    for (int f = 0; f < kNumFields; ++f) bulk_g2s(in_buf + f * kBlock, rec + size_t(f) * cap + first, bytes, mbar);
+  } else {
+    const uint32_t bytes = (L == L_AOS) ? n * 64u : ((n + 31u) / 32u) * (32u * kNumFields * 4u);
+    const uint32_t *src = rec + ((L == L_AOS) ? size_t(first) * 16 : size_t(first / 32u) * (32 * kNumFields));
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+    bulk_g2s(in_buf, src, bytes, mbar);
+  }
+}
+
+// The thread's record out of the staged tile (same mapping as in global memory, capacity = kBlock).
+template <int L> __device__ __forceinline__ Trk staged_load(const uint32_t *in_buf, int tid) {
+  Trk t;
+  if constexpr (L == L_AOS) {
+    const uint4 *r = reinterpret_cast<const uint4 *>(in_buf + tid * 16);
+    const uint4 a = r[0], b = r[1], c = r[2];
+    const uint2 d = *reinterpret_cast<const uint2 *>(r + 3);
+    t.px = __uint_as_float(a.x); t.py = __uint_as_float(a.y); t.pz = __uint_as_float(a.z);
+    t.dx = __uint_as_float(a.w); t.dy = __uint_as_float(b.x); t.dz = __uint_as_float(b.y);
+    t.ekin = __uint_as_float(b.z); t.n0 = __uint_as_float(b.w);
+    t.n1 = __uint_as_float(c.x); t.n2 = __uint_as_float(c.y);
+    t.vol = c.z; t.id_lo = c.w; t.id_hi = d.x; t.step = d.y;
+  } else {
+#pragma unroll
+    for (int f = 0; f < kNumFields; ++f) trk_set_word(t, f, in_buf[Mapping<L>::index(kBlock, tid, f)]);
+  }
+  return t;
 }
 
 template <int L, bool INSTR>
@@ -118,6 +155,7 @@ __device__ __forceinline__ Trk kid_track(const Trk &parent, const Kid &k) {
 // Per-CTA shared state of the step kernel.
 struct CtaShared {
   uint64_t mbar;
+  uint64_t mbar_in;  // completion of the staged tile
   uint32_t warp_tot[2][kBlock / 32];
   uint32_t base[2][4];
   uint32_t alive[4];
@@ -173,6 +211,7 @@ struct CtaRefs {
   CtaShared *sh;
   double *edep;     // shared histogram, n_slabs
   uint32_t *queue;  // shared, [kQueueWords][kQueueCap]
+  uint32_t *in_buf; // shared, one staged tile (dense scheme)
 };
 
 struct Tally {  // per-thread running sums of one kind (warp-uniform except esc_e)
@@ -184,7 +223,8 @@ struct Tally {  // per-thread running sums of one kind (warp-uniform except esc_
 // every thread between two block barriers (so the value is the same for the whole CTA).
 template <int L, int SCHEME, bool INSTR, int KIND>
 __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, const CtaRefs &c, uint32_t par,
-                                          uint32_t tile, uint32_t n_kind, int sbuf, Tally &tally, double &esc_e) {
+                                          uint32_t tile, uint32_t next_tile, uint32_t n_kind, int sbuf,
+                                          uint32_t &in_phase, Tally &tally, double &esc_e) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t lt_mask = (1u << lane) - 1u;
   const uint32_t i = tile * kBlock + tid;
@@ -200,8 +240,20 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
   MoveOut o;
   move_out_init(o);
   o.alive = false;
+  if (SCHEME == S_DENSE) {  // the tile was staged in shared memory by prefetch_tile
+    mbar_wait(&sh.mbar_in, in_phase);
+    in_phase ^= 1u;
+  }
   if (active) {
-    t = cur.load(slot);
+    if (SCHEME == S_DENSE) {
+      t = staged_load<L>(c.in_buf, tid);
+      if (INSTR) {
+#pragma unroll
+        for (int f = 0; f < kNumFields; ++f) cur.probe(f, 0, slot);
+      }
+    } else {
+      t = cur.load(slot);
+    }
     old = t;
     if constexpr (KIND == K_GAMMA) move_gamma(t, env, o);
     else move_elec<KIND>(t, env, o);
@@ -228,7 +280,7 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
 #pragma unroll
       for (int f = 0; f < kNumFields; ++f) c.queue[f * kQueueCap + q] = trk_word(t, f);
       c.queue[14 * kQueueCap + q] = uint32_t(o.pending);
-      c.queue[15 * kQueueCap + q] = slot;
+      if (SCHEME == S_SPARSE) c.queue[15 * kQueueCap + q] = slot;
     }
   }
 
@@ -237,6 +289,8 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
     const uint32_t rank_in_warp = __popc(m_surv & lt_mask);
     if (lane == 0) sh.warp_tot[sbuf][warp] = __popc(m_surv);
     __syncthreads();
+    if (tid == 0 && next_tile != 0xFFFFFFFFu)  // every thread has taken its record out of in_buf
+      prefetch_tile<L>(p.kind[KIND].rec[par], p.capacity, next_tile, n_kind, c.in_buf, &sh.mbar_in);
     uint32_t before = 0, total = 0;
 #pragma unroll
     for (int w = 0; w < kBlock / 32; ++w) {
@@ -293,7 +347,7 @@ __device__ __forceinline__ void interact_batch(const Params &p, const Env &env, 
 #pragma unroll
     for (int f = 0; f < kNumFields; ++f) trk_set_word(t, f, c.queue[f * kQueueCap + q]);
     const int pending = int(c.queue[14 * kQueueCap + q]);
-    slot = c.queue[15 * kQueueCap + q];
+    if (SCHEME == S_SPARSE) slot = c.queue[15 * kQueueCap + q];
     before_interaction = t;
     if constexpr (KIND == K_GAMMA) interact_gamma(t, pending, env, o);
     else interact_elec<KIND>(t, pending, env, o);
@@ -403,12 +457,34 @@ __device__ __forceinline__ void interact_batch(const Params &p, const Env &env, 
 template <int L, int SCHEME, bool INSTR, int KIND>
 __device__ __forceinline__ void run_kind(const Params &p, const Env &env, const CtaRefs &c, uint32_t par,
                                          uint32_t first_global_tile, uint32_t n_tiles, uint32_t n_kind, int &sbuf,
-                                         Tally &tally, double &esc_e) {
+                                         uint32_t &in_phase, uint32_t &tab_phase, int &staged_group, Tally &tally,
+                                         double &esc_e) {
+  // A3: the cross-section tables of this kind's particle group -> shared memory, one TMA bulk copy
+  // (e- and e+ share a group).  The previous group's last reader has passed a barrier.
+  constexpr int group = (KIND == K_GAMMA) ? 0 : 1;
+  if (n_tiles != 0u && staged_group != group) {
+    if (threadIdx.x == 0) {
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(
+                       static_cast<uint32_t>(__cvta_generic_to_shared(&c.sh->mbar))),
+                   "r"(p.table_bytes)
+                   : "memory");
+      bulk_g2s(const_cast<float4 *>(env.tab), reinterpret_cast<const unsigned char *>(p.tables) + size_t(group) * p.table_bytes,
+               p.table_bytes, &c.sh->mbar);
+    }
+    mbar_wait(&c.sh->mbar, tab_phase);
+    tab_phase ^= 1u;
+    staged_group = group;
+  }
   // global tile index g = first_global_tile + tile must be congruent to blockIdx.x modulo gridDim.x
   const uint32_t grid = gridDim.x;
   const uint32_t shift = (blockIdx.x + grid - first_global_tile % grid) % grid;
+  if (SCHEME == S_DENSE && shift < n_tiles && threadIdx.x == 0)  // in_buf is free: its last reader passed a barrier
+    prefetch_tile<L>(p.kind[KIND].rec[par], p.capacity, shift, n_kind, c.in_buf, &c.sh->mbar_in);
   for (uint32_t tile = shift; tile < n_tiles; tile += grid) {
-    const uint32_t queued = move_tile<L, SCHEME, INSTR, KIND>(p, env, c, par, tile, n_kind, sbuf, tally, esc_e);
+    const uint32_t next_tile = (tile + grid < n_tiles) ? tile + grid : 0xFFFFFFFFu;
+    const uint32_t queued =
+        move_tile<L, SCHEME, INSTR, KIND>(p, env, c, par, tile, next_tile, n_kind, sbuf, in_phase, tally, esc_e);
     sbuf ^= 1;
     if (queued >= uint32_t(kBlock)) {
       interact_batch<L, SCHEME, INSTR, KIND>(p, env, c, par, queued, sbuf, tally);
@@ -425,7 +501,8 @@ __device__ __forceinline__ void run_kind(const Params &p, const Env &env, const 
 }
 
 // ---------------------------------------------------------------------- the step kernel ------
-// Dynamic shared memory: [tables (p.table_bytes)] [edep histogram (n_slabs doubles)] [queue].
+// Dynamic shared memory: [tables (p.table_bytes)] [staged tile (kInBufBytes)] [edep histogram
+// (n_slabs doubles)] [queue].
 #ifndef ADEPT_STEP_MIN_CTAS
 #define ADEPT_STEP_MIN_CTAS 4
 #endif
@@ -438,8 +515,10 @@ __global__ void __launch_bounds__(kBlock, ADEPT_STEP_MIN_CTAS) step_kernel(const
   Ctl *ctl = p.ctl;
   CtaRefs c;
   c.sh = &sh;
-  c.edep = reinterpret_cast<double *>(dyn_smem + p.table_bytes);
-  c.queue = reinterpret_cast<uint32_t *>(dyn_smem + p.table_bytes + size_t(p.n_slabs) * sizeof(double));
+  c.in_buf = reinterpret_cast<uint32_t *>(dyn_smem + p.table_bytes);
+  constexpr size_t kInBuf = in_buf_bytes(SCHEME, Mapping<L>::words(kBlock));
+  c.edep = reinterpret_cast<double *>(dyn_smem + p.table_bytes + kInBuf);
+  c.queue = reinterpret_cast<uint32_t *>(dyn_smem + p.table_bytes + kInBuf + size_t(p.n_slabs) * sizeof(double));
 
   // A0: what is alive (written by the previous iteration's last CTA; constant during this launch)
   const uint32_t par = ctl->parity;
@@ -448,13 +527,17 @@ __global__ void __launch_bounds__(kBlock, ADEPT_STEP_MIN_CTAS) step_kernel(const
   const uint32_t tiles = t0 + t1 + t2;
 
   if (blockIdx.x < tiles) {
-    // A3: tables -> shared memory, one TMA bulk copy; histogram and counters cleared meanwhile
-    tma_stage(s_tab, p.tables, p.table_bytes, &sh.mbar, tid);
+    // A3: barriers of the two asynchronous copies (tables of a particle group, staged tile);
+    // histogram and counters cleared
+    if (tid == 0) {
+      mbar_init(&sh.mbar, 1u);
+      mbar_init(&sh.mbar_in, 1u);
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
     for (uint32_t s = tid; s < p.n_slabs; s += kBlock) c.edep[s] = 0.0;
     if (tid < 4) { sh.alive[tid] = 0u; sh.escaped[tid] = 0u; }
     if (tid == 0) { sh.esc_e = 0.0; sh.q_count = 0u; }
     if (INSTR) for (int s = tid; s < 3 * kNumFields * 2; s += kBlock) sh.probe[s] = 0u;
-    tma_wait(&sh.mbar);
     __syncthreads();
 
     Env env;
@@ -466,9 +549,11 @@ __global__ void __launch_bounds__(kBlock, ADEPT_STEP_MIN_CTAS) step_kernel(const
     Tally ta0{0u, 0u}, ta1{0u, 0u}, ta2{0u, 0u};
     double esc_e = 0.0;
     int sbuf = 0;
-    run_kind<L, SCHEME, INSTR, K_EM>(p, env, c, par, 0u, t0, n0, sbuf, ta0, esc_e);
-    run_kind<L, SCHEME, INSTR, K_EP>(p, env, c, par, t0, t1, n1, sbuf, ta1, esc_e);
-    run_kind<L, SCHEME, INSTR, K_GAMMA>(p, env, c, par, t0 + t1, t2, n2, sbuf, ta2, esc_e);
+    uint32_t in_phase = 0u, tab_phase = 0u;
+    int staged_group = -1;
+    run_kind<L, SCHEME, INSTR, K_EM>(p, env, c, par, 0u, t0, n0, sbuf, in_phase, tab_phase, staged_group, ta0, esc_e);
+    run_kind<L, SCHEME, INSTR, K_EP>(p, env, c, par, t0, t1, n1, sbuf, in_phase, tab_phase, staged_group, ta1, esc_e);
+    run_kind<L, SCHEME, INSTR, K_GAMMA>(p, env, c, par, t0 + t1, t2, n2, sbuf, in_phase, tab_phase, staged_group, ta2, esc_e);
 
     // flush the CTA's tallies
     esc_e = warp_sum(esc_e);
