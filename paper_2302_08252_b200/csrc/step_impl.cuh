@@ -157,6 +157,8 @@ struct CtaShared {
   uint64_t mbar;
   uint64_t mbar_in;  // completion of the staged tile
   uint32_t warp_tot[2][kBlock / 32];
+  uint32_t tile_acc[2];  // move_tile: survivors so far (low 16 bits) | warps arrived (high bits)
+  uint32_t q_snapshot;   // q_count as seen by the last warp to arrive
   uint32_t base[2][4];
   uint32_t alive[4];
   uint32_t escaped[4];
@@ -285,24 +287,31 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
   }
 
   if (SCHEME == S_DENSE) {
-    // A9/A10: survivors of the tile go to one contiguous range of the next array
+    // A9/A10: survivors of the tile go to one contiguous range of the next array.  Warps rank
+    // themselves in arrival order with one shared-memory atomic; the last warp to arrive knows the
+    // tile's total, starts the prefetch of the next tile (every warp has taken its records out of
+    // in_buf by then) and reserves the range with one global atomic.  One block barrier per tile.
     const uint32_t rank_in_warp = __popc(m_surv & lt_mask);
-    if (lane == 0) sh.warp_tot[sbuf][warp] = __popc(m_surv);
-    __syncthreads();
-    if (tid == 0 && next_tile != 0xFFFFFFFFu)  // every thread has taken its record out of in_buf
-      prefetch_tile<L>(p.kind[KIND].rec[par], p.capacity, next_tile, n_kind, c.in_buf, &sh.mbar_in);
-    uint32_t before = 0, total = 0;
-#pragma unroll
-    for (int w = 0; w < kBlock / 32; ++w) {
-      const uint32_t v = sh.warp_tot[sbuf][w];
-      total += v;
-      if (w < warp) before += v;
+    uint32_t warp_base = 0;
+    if (lane == 0) {
+      __threadfence_block();  // this warp's queue pushes and in_buf reads come before its arrival
+      const uint32_t mine = uint32_t(__popc(m_surv));
+      const uint32_t old = atomicAdd(&sh.tile_acc[sbuf], mine | (1u << 16));
+      warp_base = old & 0xFFFFu;
+      if ((old >> 16) == uint32_t(kBlock / 32 - 1)) {  // last to arrive
+        const uint32_t total = warp_base + mine;
+        sh.tile_acc[sbuf] = 0u;  // next used two tiles from now, behind a barrier
+        sh.q_snapshot = sh.q_count;
+        if (next_tile != 0xFFFFFFFFu)
+          prefetch_tile<L>(p.kind[KIND].rec[par], p.capacity, next_tile, n_kind, c.in_buf, &sh.mbar_in);
+        sh.base[sbuf][KIND] = total ? atomicAdd(&ctl->n_next[KIND], total) : 0u;
+      }
     }
-    if (tid == 0) sh.base[sbuf][KIND] = total ? atomicAdd(&ctl->n_next[KIND], total) : 0u;
-    const uint32_t queued = sh.q_count;
+    warp_base = __shfl_sync(0xFFFFFFFFu, warp_base, 0);
     __syncthreads();
+    const uint32_t queued = sh.q_snapshot;
     if (survives) {
-      const uint32_t dst = sh.base[sbuf][KIND] + before + rank_in_warp;
+      const uint32_t dst = sh.base[sbuf][KIND] + warp_base + rank_in_warp;
       if (dst < p.capacity) make_view<L, INSTR>(p, KIND, int(par ^ 1u), sh.probe).store(dst, t);
       else ctl->overflow = 1u;
     }
@@ -536,7 +545,7 @@ __global__ void __launch_bounds__(kBlock, ADEPT_STEP_MIN_CTAS) step_kernel(const
     }
     for (uint32_t s = tid; s < p.n_slabs; s += kBlock) c.edep[s] = 0.0;
     if (tid < 4) { sh.alive[tid] = 0u; sh.escaped[tid] = 0u; }
-    if (tid == 0) { sh.esc_e = 0.0; sh.q_count = 0u; }
+    if (tid == 0) { sh.esc_e = 0.0; sh.q_count = 0u; sh.tile_acc[0] = 0u; sh.tile_acc[1] = 0u; }
     if (INSTR) for (int s = tid; s < 3 * kNumFields * 2; s += kBlock) sh.probe[s] = 0u;
     __syncthreads();
 
