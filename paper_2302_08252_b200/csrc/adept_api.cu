@@ -65,7 +65,7 @@ static bool make_plan(const adept_geometry *g, const adept_tables *t, const adep
   pl.table_bytes = size_t(t->n_materials) * 2 * (t->n_bins + 1) * sizeof(float4);
   pl.stage_records = std::min<uint32_t>(pl.capacity, kStageRecords);
   size_t off = 0;
-  pl.ctl = off; off = align_up(off + kCtlHeaderBytes + size_t(2) * g->n_layers * sizeof(double));
+  pl.ctl = off; off = align_up(off + kCtlHeaderBytes + (size_t(2) * g->n_layers + 1) * sizeof(unsigned long long));
   pl.tables = off; off = align_up(off + pl.table_bytes);
   pl.stage = off; off = align_up(off + size_t(pl.stage_records) * kStageRecordBytes);
   pl.stage_slots = off; off = align_up(off + size_t(pl.stage_records) * 4);
@@ -105,7 +105,7 @@ struct adept_ctx {
   unsigned grid;
   size_t dyn_smem;
   unsigned char *ws;
-  unsigned char *pinned;  // kCtlHeaderBytes + edep
+  unsigned char *pinned;  // kCtlHeaderBytes + tallies
   size_t pinned_bytes;
   std::vector<adept_primary> pending;
   size_t pending_done;
@@ -164,11 +164,15 @@ void fill_result(const adept_ctx *c, adept_result *out) {
   const Ctl *h = reinterpret_cast<const Ctl *>(c->pinned);
   fill_counts(c, &out->total);
   out->e_injected = c->e_injected;
-  out->e_escaped = h->e_escaped;
-  const double *edep = reinterpret_cast<const double *>(c->pinned + kCtlHeaderBytes);
-  if (out->edep_slab) std::memcpy(out->edep_slab, edep, size_t(2) * c->geo.n_layers * sizeof(double));
+  // tallies are 64-bit fixed point on the device (device_state.cuh): per slab, then the escaped energy
+  const unsigned long long *fx = reinterpret_cast<const unsigned long long *>(c->pinned + kCtlHeaderBytes);
+  const uint32_t n_slabs = 2 * c->geo.n_layers;
+  out->e_escaped = double(fx[n_slabs]) * kTallyUnit;
+  if (out->edep_slab)
+    for (uint32_t s = 0; s < n_slabs; ++s) out->edep_slab[s] = double(fx[s]) * kTallyUnit;
   if (out->edep_layer)
-    for (uint32_t l = 0; l < c->geo.n_layers; ++l) out->edep_layer[l] = edep[2 * l] + edep[2 * l + 1];
+    for (uint32_t l = 0; l < c->geo.n_layers; ++l)
+      out->edep_layer[l] = double(fx[2 * l]) * kTallyUnit + double(fx[2 * l + 1]) * kTallyUnit;
 }
 
 // write n_cur / slot_top / slots_used of one kind after a host-driven append
@@ -211,7 +215,7 @@ size_t adept_workspace_bytes(const adept_geometry *g, const adept_tables *t, con
 const char *adept_last_error(const adept_ctx *c) { return c ? c->err.c_str() : g_create_error.c_str(); }
 
 static int clear_state(adept_ctx *c) {
-  // everything except the tables: control block, edep, instrumentation counters
+  // everything except the tables: control block, tallies, instrumentation counters
   const Plan &pl = c->plan;
   CU(c, cudaMemsetAsync(c->ws + pl.ctl, 0, pl.tables - pl.ctl, c->stream));
   if (c->cfg.instrument && pl.total > pl.instr_rw)
@@ -254,7 +258,7 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
     return ADEPT_ECUDA;
   };
   cudaError_t e;
-  c->pinned_bytes = kCtlHeaderBytes + size_t(2) * g->n_layers * sizeof(double);
+  c->pinned_bytes = kCtlHeaderBytes + (size_t(2) * g->n_layers + 1) * sizeof(unsigned long long);
   if ((e = cudaMallocHost(reinterpret_cast<void **>(&c->pinned), c->pinned_bytes)) != cudaSuccess)
     return die("cudaMallocHost", e);
 
@@ -274,7 +278,7 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
 
   Params &p = c->params;
   p.ctl = reinterpret_cast<Ctl *>(c->ws + pl.ctl);
-  p.edep = reinterpret_cast<double *>(c->ws + pl.ctl + kCtlHeaderBytes);
+  p.tally = reinterpret_cast<unsigned long long *>(c->ws + pl.ctl + kCtlHeaderBytes);
   p.tables = reinterpret_cast<const float4 *>(c->ws + pl.tables);
   p.table_bytes = static_cast<uint32_t>(pl.table_bytes / 2);  // per particle group
   p.nodes = nodes;
@@ -295,7 +299,7 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
   p.instr_field_rw = reinterpret_cast<unsigned long long *>(c->ws + pl.instr_rw);
 
   // persistent grid: as many CTAs as fit on the device at once
-  c->dyn_smem = pl.table_bytes / 2 + size_t(p.n_slabs) * sizeof(double) + queue_bytes(cfg->scheme) + in_buf_bytes(cfg->scheme, c->ops->record_words(kBlock));
+  c->dyn_smem = step_smem_bytes(cfg->scheme, pl.table_bytes / 2, p.n_slabs, c->ops->record_words(kGroup));
   int dev = 0, sms = 0;
   if ((e = cudaGetDevice(&dev)) != cudaSuccess) return die("cudaGetDevice", e);
   if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess)

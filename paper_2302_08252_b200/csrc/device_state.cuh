@@ -14,17 +14,41 @@ namespace adept {
 
 enum SchemeId : int { S_SPARSE = 0, S_DENSE = 1 };
 
-constexpr int kBlock = 256;  // threads per CTA of the step kernel = tracks per tile
-// Shared-memory queue of tracks parked between the two halves of the step: 14 record words + the
-// pending interaction (+ the slot, sparse scheme only), field-major.  At most kBlock - 1 left over
-// from earlier tiles plus kBlock from the current one.
-constexpr int kQueueCap = 2 * kBlock;
+constexpr int kBlock = 256;  // threads per CTA of the step kernel
+// A CTA is split into groups of kGroup threads.  A group steps one tile of kGroup tracks at a time
+// and synchronises only with itself (a named barrier), so that while one group waits -- for its
+// tile's output range (a global atomic) or for a straggling warp -- the other groups of the SM keep
+// the schedulers busy.  The groups of a CTA share the staged tables and the tally bins.
+#ifndef ADEPT_GROUP
+#define ADEPT_GROUP 128
+#endif
+constexpr int kGroup = ADEPT_GROUP;
+constexpr int kGroupsPerCta = kBlock / kGroup;
+constexpr int kWarpsPerGroup = kGroup / 32;
+static_assert(kGroup == 64 || kGroup == 128, "a group is 2 or 4 warps (arrival word: 3 x 9-bit counts + 3-bit ticket)");
+// Shared-memory queue (one per group) of tracks parked between the two halves of the step: 14
+// record words + the pending interaction (+ the slot, sparse scheme only), field-major.  At most
+// kGroup - 1 left over from earlier tiles plus kGroup from the current one.
+constexpr int kQueueCap = 2 * kGroup;
 __host__ __device__ constexpr int queue_words(int scheme) { return scheme == S_DENSE ? 15 : 16; }
 __host__ __device__ constexpr size_t queue_bytes(int scheme) { return size_t(kQueueCap) * queue_words(scheme) * 4; }
-// Dense scheme: one tile staged in shared memory by TMA (record_words(kBlock) words of the layout).
+// Dense scheme: one tile staged in shared memory by TMA (record_words(kGroup) words of the layout).
 __host__ __device__ constexpr size_t in_buf_bytes(int scheme, size_t tile_words) {
   return scheme == S_DENSE ? tile_words * 4 : 0;
 }
+// Tally bins of a CTA: per slab (+ one bin for the energy carried out of the calorimeter) a 64-bit
+// fixed-point sum kept as two 32-bit limbs, [lo limbs][hi limbs].
+__host__ __device__ constexpr size_t bins_bytes(uint32_t n_slabs) { return ((size_t(n_slabs) + 1) * 8 + 15) / 16 * 16; }
+// Dynamic shared memory of the step kernel: [tables of one particle group][bins][per group: staged tile, queue]
+__host__ __device__ constexpr size_t step_smem_bytes(int scheme, size_t table_bytes, uint32_t n_slabs, size_t tile_words) {
+  return table_bytes + bins_bytes(n_slabs) + size_t(kGroupsPerCta) * (in_buf_bytes(scheme, tile_words) + queue_bytes(scheme));
+}
+
+// Energy tallies (rule M7: sums of fp32 terms) are accumulated in 64-bit fixed point, unit
+// 2^-32 MeV: every term is rounded to the unit once (absolute error <= 2^-33 MeV = 1.2e-10 MeV),
+// after which the additions are exact and therefore independent of the order in which threads,
+// warps and CTAs arrive.  Range 2^32 MeV (4.3e3 TeV) per slab.
+constexpr double kTallyUnit = 1.0 / 4294967296.0;
 
 struct Ctl {
   // dense: tracks in the current / next array.  sparse: length of the current / next slot list.
@@ -39,9 +63,9 @@ struct Ctl {
   uint32_t it_escaped[4];  // this iteration: parents that left the calorimeter, per kind
   unsigned long long steps[3], secondaries[3], killed[3], escaped_n[3], slots_used[3];
   unsigned long long iterations;
-  double e_escaped;
-  unsigned long long pad1[2];
-  // double edep[n_slabs] follows at byte kCtlHeaderBytes
+  unsigned long long pad1[3];
+  // unsigned long long tally[n_slabs + 1] follows at byte kCtlHeaderBytes: fixed-point energy
+  // deposit per slab, then the energy carried out of the calorimeter
 };
 constexpr size_t kCtlHeaderBytes = 256;
 static_assert(sizeof(Ctl) <= kCtlHeaderBytes, "control block header");
@@ -55,7 +79,7 @@ struct KindStorage {
 
 struct Params {
   Ctl *ctl;
-  double *edep;              // [n_slabs], right after the control header
+  unsigned long long *tally; // [n_slabs + 1] fixed point, right after the control header
   const float4 *tables;      // [group][material][node] {q0, q1, q2, 0}; group 0 = gamma, 1 = e+-
   uint32_t table_bytes;      // bytes of ONE group, multiple of 16
   uint32_t nodes;            // n_bins + 1

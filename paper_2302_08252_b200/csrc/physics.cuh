@@ -47,20 +47,24 @@ struct Kid {  // a secondary: position, slab, nial = -1, step = 0 come from the 
 // Both halves together are exactly the rule sequence; the split changes no operation and no operand.
 enum Pending : int { P_NONE = -1, P_PROC0 = 0, P_PROC1 = 1, P_PROC2 = 2, P_ANNIH = 4 };
 
+// Energy tallies are sums of fp32 terms (rule M7); a step hands its terms over one by one:
+// at most two deposits in the step's slab, and the track's whole energy when it escapes (S25) or
+// trips the runaway guard (S31) -- the kernel adds them to its accumulators (step_impl.cuh).
 struct MoveOut {
   bool alive;    // track goes to the next iteration (meaningless while pending)
-  bool escaped;  // left the calorimeter (S25)
+  bool escaped;  // left the calorimeter (S25): ekin (+ 2 mc^2 for e+) is carried out
+  bool guard;    // S31: ekin (+ 2 mc^2 for e+) is deposited in the post-step slab
   int pending;   // Pending: interaction still to be done
-  double dep;    // energy deposited in the pre-step slab
-  double esc_e;  // energy carried out (S25)
-  double dep2;   // S31 guard only: deposit in the post-step slab
+  float dep;     // energy deposited in the pre-step slab (0 = none)
+  float dep_b;   // second term into the same slab (0 = none)
 };
 
 struct InteractOut {
   bool alive;
+  bool guard;   // S31
   Kid kid[2];   // by child ordinal (R5)
-  double dep;   // deposited in the track's slab (interactions do not change slab)
-  double dep2;  // S31 guard
+  float dep;    // deposited in the track's slab (interactions do not change slab)
+  float dep_b;  // second term into the same slab
 };
 
 constexpr float kInf = __builtin_huge_valf();
@@ -92,6 +96,18 @@ __device__ __forceinline__ float slab_zlo(const Env &g, uint32_t i) {
 
 enum Face : int { FACE_ZP = 0, FACE_ZM = 1, FACE_XY = 2 };
 
+// The rule's `valid ? n / d : +inf`.  The divisor is selected first (1 where the quotient is not
+// used), so that no lane divides by zero: a zero divisor sends the whole warp through the slow path
+// of the IEEE division (Sigma_pair is exactly 0 below ~3.4 MeV, i.e. for a third of the photons).
+// The empty asm keeps the compiler from undoing the selection (it otherwise proves the quotient
+// unused on those lanes and divides by the raw value).
+__device__ __forceinline__ float quotient_or_inf(float n, float d, bool valid) {
+  float dd = valid ? d : 1.0f;
+  asm("" : "+f"(dd));
+  const float q = n / dd;
+  return valid ? q : kInf;
+}
+
 // S21: distance to the slab faces and the transverse box, and which face is hit first.
 __device__ __forceinline__ float geometry_step(const Trk &t, const Env &g, float z_lo, float z_hi, int &face) {
   const float H = g.half_xy;
@@ -100,12 +116,9 @@ __device__ __forceinline__ float geometry_step(const Trk &t, const Env &g, float
   const float n_z = ((t.dz > 0.0f) ? z_hi : z_lo) - t.pz;
   const float n_x = ((t.dx > 0.0f) ? H : -H) - t.px;
   const float n_y = ((t.dy > 0.0f) ? H : -H) - t.py;
-  const float q_z = n_z / ((t.dz != 0.0f) ? t.dz : 1.0f);
-  const float q_x = n_x / ((t.dx != 0.0f) ? t.dx : 1.0f);
-  const float q_y = n_y / ((t.dy != 0.0f) ? t.dy : 1.0f);
-  const float s_z = (t.dz != 0.0f) ? q_z : kInf;
-  const float s_x = (t.dx != 0.0f) ? q_x : kInf;
-  const float s_y = (t.dy != 0.0f) ? q_y : kInf;
+  const float s_z = quotient_or_inf(n_z, t.dz, t.dz != 0.0f);
+  const float s_x = quotient_or_inf(n_x, t.dx, t.dx != 0.0f);
+  const float s_y = quotient_or_inf(n_y, t.dy, t.dy != 0.0f);
   float s_g = s_z;
   face = (t.dz > 0.0f) ? FACE_ZP : FACE_ZM;
   if (s_x < s_g) { s_g = s_x; face = FACE_XY; }
@@ -114,22 +127,16 @@ __device__ __forceinline__ float geometry_step(const Trk &t, const Env &g, float
   return s_g;
 }
 
-// S25: snap to the plane and change slab, or escape.  Returns true if the track escaped.
+// S25: snap to the plane and change slab, or escape.  Returns true if the track escaped.  Written
+// with selects: the faces of a warp's lanes differ, a branch per face would serialise them.
 __device__ __forceinline__ bool cross_boundary(Trk &t, const Env &g, uint32_t vol0, int face, float z_lo,
                                                float z_hi) {
-  if (face == FACE_ZP) {
-    t.pz = z_hi;
-    if (vol0 + 1u >= g.n_slabs) return true;
-    t.vol = vol0 + 1u;
-    return false;
-  }
-  if (face == FACE_ZM) {
-    t.pz = z_lo;
-    if (vol0 == 0u) return true;
-    t.vol = vol0 - 1u;
-    return false;
-  }
-  return true;
+  const bool zp = face == FACE_ZP, zm = face == FACE_ZM;
+  const uint32_t vol_new = zp ? vol0 + 1u : vol0 - 1u;  // vol0 - 1 wraps for slab 0: caught by the range test
+  const bool out = (face == FACE_XY) || (vol_new >= g.n_slabs);
+  t.pz = zp ? z_hi : (zm ? z_lo : t.pz);
+  t.vol = out ? vol0 : vol_new;
+  return out;
 }
 
 __device__ __forceinline__ void make_kid(Kid &k, int kind, float dx, float dy, float dz, float ekin, uint32_t id_lo,
@@ -162,17 +169,16 @@ __device__ __forceinline__ void rotate_dir(float dx, float dy, float dz, float s
 }
 
 __device__ __forceinline__ void move_out_init(MoveOut &o) {
-  o.alive = true; o.escaped = false; o.pending = P_NONE; o.dep = 0.0; o.esc_e = 0.0; o.dep2 = 0.0;
+  o.alive = true; o.escaped = false; o.guard = false; o.pending = P_NONE; o.dep = 0.0f; o.dep_b = 0.0f;
 }
 __device__ __forceinline__ void interact_out_init(InteractOut &o) {
-  o.alive = true; o.kid[0].kind = -1; o.kid[1].kind = -1; o.dep = 0.0; o.dep2 = 0.0;
+  o.alive = true; o.guard = false; o.kid[0].kind = -1; o.kid[1].kind = -1; o.dep = 0.0f; o.dep_b = 0.0f;
 }
 
 // S31: runaway guard
 template <int KIND, typename Out> __device__ __forceinline__ void runaway_guard(Trk &t, Out &o) {
   if (t.step >= (1u << 20)) {
-    o.dep2 += static_cast<double>(t.ekin);
-    if (KIND == K_EP) o.dep2 += static_cast<double>(two_mc2());
+    o.guard = true;
     o.alive = false;
   }
 }
@@ -199,15 +205,10 @@ __device__ __forceinline__ void move_gamma(Trk &t, const Env &g, MoveOut &o) {
   const float sig0 = lerp_node(b.f, A.x, B.x);
   const float sig1 = lerp_node(b.f, A.y, B.y);
   const float sig2 = lerp_node(b.f, A.z, B.z);
-  // s_j = nial_j / Sigma_j where Sigma_j > 0, else +inf.  The divisor is selected first (1 where the
-  // quotient is not used): no divergent branch, and no division by zero, which would send the lane
-  // through the slow path of the IEEE division (Sigma_pair is exactly 0 below ~3.4 MeV).
-  const float q0 = t.n0 / ((sig0 > 0.0f) ? sig0 : 1.0f);
-  const float q1 = t.n1 / ((sig1 > 0.0f) ? sig1 : 1.0f);
-  const float q2 = t.n2 / ((sig2 > 0.0f) ? sig2 : 1.0f);
-  const float s0 = (sig0 > 0.0f) ? q0 : kInf;
-  const float s1 = (sig1 > 0.0f) ? q1 : kInf;
-  const float s2 = (sig2 > 0.0f) ? q2 : kInf;
+  // s_j = nial_j / Sigma_j where Sigma_j > 0, else +inf
+  const float s0 = quotient_or_inf(t.n0, sig0, sig0 > 0.0f);
+  const float s1 = quotient_or_inf(t.n1, sig1, sig1 > 0.0f);
+  const float s2 = quotient_or_inf(t.n2, sig2, sig2 > 0.0f);
 
   // S21
   const float z_lo = slab_zlo(g, vol0), z_hi = slab_zlo(g, vol0 + 1u);
@@ -235,7 +236,6 @@ __device__ __forceinline__ void move_gamma(Trk &t, const Env &g, MoveOut &o) {
   }
   // S25
   if (cross_boundary(t, g, vol0, face, z_lo, z_hi)) {
-    o.esc_e = static_cast<double>(t.ekin);
     o.escaped = true;
     o.alive = false;
     return;
@@ -253,7 +253,7 @@ __device__ __forceinline__ void interact_gamma(Trk &t, int w, const Env &g, Inte
     const float T_minus = u01(r1.x) * E_av;
     const float T_plus = E_av - T_minus;
     if (T_minus >= g.e_cut) make_kid(o.kid[0], K_EM, t.dx, t.dy, t.dz, T_minus, r2.x, r2.y);
-    else o.dep += static_cast<double>(T_minus);
+    else o.dep = T_minus;
     make_kid(o.kid[1], K_EP, t.dx, t.dy, t.dz, T_plus, r2.z, r2.w);
     o.alive = false;
     return;
@@ -284,9 +284,9 @@ __device__ __forceinline__ void interact_gamma(Trk &t, int w, const Env &g, Inte
   const float qz = fmaf(E, t.dz, -(E1 * nz));
   const float pn = sqrtf(fmaf(qx, qx, fmaf(qy, qy, qz * qz)));
   if (T >= g.e_cut && pn > 0.0f) make_kid(o.kid[0], K_EM, qx / pn, qy / pn, qz / pn, T, r2.x, r2.y);
-  else o.dep += static_cast<double>(T);
+  else o.dep = T;
   if (E1 < g.e_cut) {
-    o.dep += static_cast<double>(E1);
+    o.dep_b = E1;
     o.alive = false;
     return;
   }
@@ -322,8 +322,7 @@ template <int KIND> __device__ __forceinline__ void move_elec(Trk &t, const Env 
   const float sig0 = lerp_node(b.f, A.x, B.x);
   const float S0 = lerp_node(b.f, A.y, B.y);
   const float R = lerp_node(b.f, A.z, B.z);
-  const float q0 = t.n0 / ((sig0 > 0.0f) ? sig0 : 1.0f);  // divisor selected first, see move_gamma
-  const float s0 = (sig0 > 0.0f) ? q0 : kInf;
+  const float s0 = quotient_or_inf(t.n0, sig0, sig0 > 0.0f);
   float s_e;
   {
     const float r_min = 0.1f, f_r = 0.2f;
@@ -360,11 +359,11 @@ template <int KIND> __device__ __forceinline__ void move_elec(Trk &t, const Env 
     E_post = E0 - dE;
     if (w == 3 && s >= R) E_post = 0.0f;  // the track stops
   }
-  o.dep += static_cast<double>(E0 - E_post);
+  o.dep = E0 - E_post;
   t.ekin = E_post;
   if (E_post < e_cut) {
     if (KIND == K_EM) {
-      o.dep += static_cast<double>(E_post);
+      o.dep_b = E_post;
       o.alive = false;
     }  // e+ is kept for S17 at its next step
     return;
@@ -375,7 +374,6 @@ template <int KIND> __device__ __forceinline__ void move_elec(Trk &t, const Env 
   }
   if (w < 0) {  // S25
     if (cross_boundary(t, g, vol0, face, z_lo, z_hi)) {
-      o.esc_e = static_cast<double>(t.ekin) + ((KIND == K_EP) ? static_cast<double>(two_mc2()) : 0.0);
       o.escaped = true;
       o.alive = false;
       return;
@@ -391,7 +389,7 @@ template <int KIND> __device__ __forceinline__ void interact_elec(Trk &t, int pe
   const Stream rs{t.id_lo, t.id_hi, annih ? t.step : t.step - 1u};
   const uint4 r1 = rs.call(1), r2 = rs.call(2);
   if (annih) {  // two back-to-back photons of energy mc^2, isotropic
-    o.dep += static_cast<double>(t.ekin);
+    o.dep = t.ekin;
     const float ct = 1.0f - 2.0f * u01(r1.z);
     const float st = sqrtf(fmaf(-ct, ct, 1.0f));
     float sphi, cphi;
@@ -411,7 +409,7 @@ template <int KIND> __device__ __forceinline__ void interact_elec(Trk &t, int pe
   make_kid(o.kid[0], K_GAMMA, t.dx, t.dy, t.dz, k, r2.x, r2.y);
   const float E_new = E - k;
   if (E_new < e_cut && KIND == K_EM) {
-    o.dep += static_cast<double>(E_new);
+    o.dep = E_new;
     o.alive = false;
     return;
   }

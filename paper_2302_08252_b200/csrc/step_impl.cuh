@@ -2,23 +2,25 @@
 //
 // One launch = one iteration of all three per-type track buffers ("the tracks of each
 // particle type are processed by a dedicated kernel"; here the three passes share one persistent
-// grid so that an iteration costs one launch, and a tile of 256 tracks always holds one type, so
-// divergence between types never occurs inside a CTA).  SURVEY.md §8(a) rows:
+// grid so that an iteration costs one launch, and a tile always holds one type, so divergence
+// between types never occurs inside a warp).  SURVEY.md §8(a) rows:
 //   A0/A11  iteration control: counts live on the device; the last CTA to finish ends the
-//           iteration (swap current/next, reset counters, accumulate tallies) — no host round trip;
-//   A1      track load through the layout accessor (layout.cuh);
+//           iteration (swap current/next, reset counters) -- no host round trip;
+//   A1      track load through the layout accessor (layout.cuh); dense scheme: the next tile is
+//           fetched into shared memory by TMA while the current one is stepped;
 //   A2-A8   the physics/geometry step (physics.cuh), tables staged in shared memory by one TMA
-//           bulk copy per CTA;
+//           bulk copy per CTA and particle group.
 //           The step is split (physics.cuh): every track takes the "move" half; tracks whose step ends
 //           in a discrete interaction are parked in a shared-memory queue and the "interact" half
-//           runs on dense batches of 256 parked tracks, so that the Philox blocks and the sampling
+//           runs on dense batches of parked tracks, so that the Philox blocks and the sampling
 //           code of rule S26 are executed by full warps instead of a few lanes per warp (the paper's
 //           "diverging code paths");
-//   A9      dense: secondaries and survivors are ranked by one packed block scan (3 x 10-bit
-//           counters, one per destination type; warp shuffles + one shared-memory hop) and the CTA
-//           reserves its output ranges with one atomicAdd per destination type;
-//           sparse: new slots come from a bump allocator and slot-list pushes are warp-aggregated
-//           (warp scan + one atomicAdd per warp and list);
+//   A6      energy deposits go to per-CTA shared-memory bins in 64-bit fixed point (two native 32-bit
+//           atomics; a 64-bit or fp64 shared-memory add would be a compare-and-swap loop);
+//   A9      the warps of a group rank their outputs in arrival order with ONE shared-memory atomic
+//           per warp on a packed word (3 x 9-bit counts + ticket); the last warp to arrive reserves
+//           the group's output ranges with one global atomicAdd per destination type (dense: next
+//           arrays; sparse: bump-allocated slots and the next slot lists);
 //   A10     dense: survivors are written to the next array (whole record); sparse: only the words
 //           that changed are written back in place, and the slot is pushed onto the next list;
 //   A12     the instrumented instantiation counts every accessor call.
@@ -33,38 +35,30 @@
 namespace adept {
 
 // ---------------------------------------------------------------- small device utilities ------
-__device__ __forceinline__ uint32_t warp_inclusive_scan(uint32_t v, int lane) {
-#pragma unroll
-  for (int d = 1; d < 32; d <<= 1) {
-    const uint32_t n = __shfl_up_sync(0xFFFFFFFFu, v, d);
-    if (lane >= d) v += n;
-  }
-  return v;
+// Barrier of one group of kGroup threads (named barrier 1 + group; barrier 0 is __syncthreads).
+__device__ __forceinline__ void group_sync(int group) {
+  asm volatile("bar.sync %0, %1;" ::"r"(group + 1), "n"(kGroup) : "memory");
 }
 
-// Warp-aggregated reservation: every lane asks for `mine` (0..2) consecutive entries of *counter;
-// one atomicAdd per warp.  Must be called by all 32 lanes.  Returns the lane's first entry.
-__device__ __forceinline__ uint32_t warp_reserve(uint32_t *counter, uint32_t mine, int lane) {
-  const uint32_t inc = warp_inclusive_scan(mine, lane);
-  const uint32_t total = __shfl_sync(0xFFFFFFFFu, inc, 31);
-  if (total == 0u) return 0u;
-  uint32_t base = 0u;
-  if (lane == 31) base = atomicAdd(counter, total);
-  base = __shfl_sync(0xFFFFFFFFu, base, 31);
-  return base + inc - mine;
-}
-
-__device__ __forceinline__ double warp_sum(double v) {
-#pragma unroll
-  for (int d = 16; d > 0; d >>= 1) v += __shfl_down_sync(0xFFFFFFFFu, v, d);
-  return v;
+// ---- tally bins (row A6) -------------------------------------------------------------------------
+struct Bins {
+  uint32_t *lo, *hi;  // shared, n_slabs + 1 entries each
+};
+// bins[bin] += x, x >= 0 an fp32 term in MeV, in 64-bit fixed point of unit 2^-32 MeV (device_state.cuh).
+__device__ __forceinline__ void bin_add(const Bins &b, uint32_t bin, float x) {
+  const unsigned long long f = __float2ull_rn(x * 4294967296.0f);
+  const uint32_t l = static_cast<uint32_t>(f), h = static_cast<uint32_t>(f >> 32);
+  const uint32_t old = atomicAdd(&b.lo[bin], l);
+  const uint32_t up = h + ((old + l < old) ? 1u : 0u);  // carry out of the low limb
+  if (up) atomicAdd(&b.hi[bin], up);
 }
 
 // ---- asynchronous tile prefetch (dense scheme) ---------------------------------------------------
-// A tile of 256 consecutive slots is contiguous in global memory per layout (AoS: one 16 KB run;
-// AoSoA-32: eight 1792-byte blocks back to back; SoA: one 1 KB run per field), so the next tile is
-// fetched into shared memory by TMA bulk copies while the current one is being stepped: the global
-// load latency leaves the critical path and no load instruction or address arithmetic is issued.
+// A tile of kGroup consecutive slots is contiguous in global memory per layout (AoS: one run of
+// 64-byte records; AoSoA-32: 1792-byte blocks back to back; SoA: one run per field), so the next
+// tile is fetched into shared memory by TMA bulk copies while the current one is being stepped:
+// the global load latency leaves the critical path and no load instruction or address arithmetic
+// is issued.
 __device__ __forceinline__ void mbar_init(uint64_t *mbar, uint32_t count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(static_cast<uint32_t>(__cvta_generic_to_shared(mbar))),
                "r"(count));
@@ -86,20 +80,29 @@ __device__ __forceinline__ void bulk_g2s(void *smem_dst, const void *gmem_src, u
                "l"(gmem_src), "r"(bytes), "r"(static_cast<uint32_t>(__cvta_generic_to_shared(mbar)))
                : "memory");
 }
+// shared-memory counter += 1 with release/acquire ordering at CTA scope; returns the old value
+__device__ __forceinline__ uint32_t arrive_acq_rel(uint32_t *counter) {
+  uint32_t old;
+  asm volatile("atom.acq_rel.cta.shared::cta.add.u32 %0, [%1], 1;"
+               : "=r"(old)
+               : "r"(static_cast<uint32_t>(__cvta_generic_to_shared(counter)))
+               : "memory");
+  return old;
+}
 
-// Called by ONE thread, after a barrier that follows every thread's last read of `in_buf`.
+// Called by ONE thread, after every warp of the group has taken its records out of `in_buf`.
 template <int L>
 __device__ __forceinline__ void prefetch_tile(const uint32_t *rec, uint32_t cap, uint32_t tile, uint32_t n_kind,
                                               uint32_t *in_buf, uint64_t *mbar) {
-  const uint32_t first = tile * kBlock;
-  const uint32_t n = (n_kind - first < uint32_t(kBlock)) ? n_kind - first : uint32_t(kBlock);
+  const uint32_t first = tile * kGroup;
+  const uint32_t n = (n_kind - first < uint32_t(kGroup)) ? n_kind - first : uint32_t(kGroup);
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic reads of in_buf before async writes
   const uint32_t bar = static_cast<uint32_t>(__cvta_generic_to_shared(mbar));
   if (L == L_SOA) {
     const uint32_t bytes = ((n + 3u) / 4u) * 16u;  // slots are padded to a multiple of 32: stays inside the array
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes * kNumFields) : "memory");
 #pragma unroll
-    for (int f = 0; f < kNumFields; ++f) bulk_g2s(in_buf + f * kBlock, rec + size_t(f) * cap + first, bytes, mbar);
+    for (int f = 0; f < kNumFields; ++f) bulk_g2s(in_buf + f * kGroup, rec + size_t(f) * cap + first, bytes, mbar);
   } else {
     const uint32_t bytes = (L == L_AOS) ? n * 64u : ((n + 31u) / 32u) * (32u * kNumFields * 4u);
     const uint32_t *src = rec + ((L == L_AOS) ? size_t(first) * 16 : size_t(first / 32u) * (32 * kNumFields));
@@ -108,11 +111,11 @@ __device__ __forceinline__ void prefetch_tile(const uint32_t *rec, uint32_t cap,
   }
 }
 
-// The thread's record out of the staged tile (same mapping as in global memory, capacity = kBlock).
-template <int L> __device__ __forceinline__ Trk staged_load(const uint32_t *in_buf, int tid) {
+// The thread's record out of the staged tile (same mapping as in global memory, capacity = kGroup).
+template <int L> __device__ __forceinline__ Trk staged_load(const uint32_t *in_buf, int gtid) {
   Trk t;
   if constexpr (L == L_AOS) {
-    const uint4 *r = reinterpret_cast<const uint4 *>(in_buf + tid * 16);
+    const uint4 *r = reinterpret_cast<const uint4 *>(in_buf + gtid * 16);
     const uint4 a = r[0], b = r[1], c = r[2];
     const uint2 d = *reinterpret_cast<const uint2 *>(r + 3);
     t.px = __uint_as_float(a.x); t.py = __uint_as_float(a.y); t.pz = __uint_as_float(a.z);
@@ -122,7 +125,7 @@ template <int L> __device__ __forceinline__ Trk staged_load(const uint32_t *in_b
     t.vol = c.z; t.id_lo = c.w; t.id_hi = d.x; t.step = d.y;
   } else {
 #pragma unroll
-    for (int f = 0; f < kNumFields; ++f) trk_set_word(t, f, in_buf[Mapping<L>::index(kBlock, tid, f)]);
+    for (int f = 0; f < kNumFields; ++f) trk_set_word(t, f, in_buf[Mapping<L>::index(kGroup, gtid, f)]);
   }
   return t;
 }
@@ -152,19 +155,32 @@ __device__ __forceinline__ Trk kid_track(const Trk &parent, const Kid &k) {
   return c;
 }
 
-// Per-CTA shared state of the step kernel.
+// ---- arrival word (row A9) -----------------------------------------------------------------------
+// Three 9-bit counts (bits 0-8, 9-17, 18-26) and a ticket (bits 27-29).  Every warp of a group adds
+// its counts and one ticket with a single shared-memory atomic; what the atomic returns are the
+// counts of the warps that arrived before it = the warp's ranks.  The warp that draws the last ticket
+// knows the group's totals.
+constexpr uint32_t kCountMask = 511u;
+constexpr uint32_t kTicket = 1u << 27;
+__device__ __forceinline__ uint32_t count_of(uint32_t word, int field) { return (word >> (9 * field)) & kCountMask; }
+__device__ __forceinline__ bool last_ticket(uint32_t old) { return (old >> 27) == uint32_t(kWarpsPerGroup - 1); }
+
+// Per-group shared state.
+struct GroupShared {
+  uint64_t mbar_in;      // completion of the staged tile
+  uint32_t loaded;       // warps that have taken their records out of the staged tile (monotonic)
+  uint32_t acc[2];       // arrival words, alternating between consecutive tiles / batches
+  uint32_t qtot[2];      // parked tracks after the tile
+  uint32_t base[2][4];   // first output entry per destination kind (dense: next array; sparse: next slot list)
+  uint32_t sbase[2][4];  // sparse: first new slot per destination kind
+};
+// Per-CTA shared state.
 struct CtaShared {
-  uint64_t mbar;
-  uint64_t mbar_in;  // completion of the staged tile
-  uint32_t warp_tot[2][kBlock / 32];
-  uint32_t tile_acc[2];  // move_tile: survivors so far (low 16 bits) | warps arrived (high bits)
-  uint32_t q_snapshot;   // q_count as seen by the last warp to arrive
-  uint32_t base[2][4];
+  uint64_t mbar;  // completion of the staged tables
   uint32_t alive[4];
   uint32_t escaped[4];
-  uint32_t q_count;  // parked tracks waiting for their interaction
-  double esc_e;
   uint32_t probe[3 * kNumFields * 2];
+  GroupShared grp[kGroupsPerCta];
 };
 
 // A9 + A11: the last CTA closes the iteration.
@@ -203,52 +219,68 @@ template <int SCHEME> __device__ void finish_iteration(const Params &p) {
   c->done_ctas = 0u;
 }
 
-// ------------------------------------------------------------------- tile = 256 tracks --------
+// ------------------------------------------------------------------- tile = kGroup tracks -----
 template <int KIND> __device__ __forceinline__ constexpr int kid_kind(int ordinal) {
   return KIND == K_GAMMA ? (ordinal == 0 ? K_EM : K_EP) : K_GAMMA;  // rule R5
 }
 
-// What a CTA carries through its tiles.
-struct CtaRefs {
-  CtaShared *sh;
-  double *edep;     // shared histogram, n_slabs
-  uint32_t *queue;  // shared, [kQueueWords][kQueueCap]
-  uint32_t *in_buf; // shared, one staged tile (dense scheme)
+// What a group carries through its tiles.
+struct GroupRefs {
+  CtaShared *cta;
+  GroupShared *g;
+  Bins bins;         // shared, CTA-wide
+  uint32_t *queue;   // shared, [queue_words][kQueueCap]
+  uint32_t *in_buf;  // shared, one staged tile (dense scheme)
+  int group, gtid;   // group index inside the CTA, thread index inside the group
 };
 
-struct Tally {  // per-thread running sums of one kind (warp-uniform except esc_e)
+struct Tally {  // per-warp running sums of one kind (warp-uniform)
   uint32_t alive, escaped;
 };
 
+// S25 / S31 energy of a track that leaves the simulation
+template <int KIND> __device__ __forceinline__ void bin_add_track_energy(const Bins &b, uint32_t bin, float ekin) {
+  bin_add(b, bin, ekin);
+  if (KIND == K_EP) bin_add(b, bin, two_mc2());
+}
+
 // First half of the step for tile `tile` of kind KIND's current set (rows A1-A7, A10 for the
-// tracks whose step ends without an interaction).  Returns the number of parked tracks, read by
-// every thread between two block barriers (so the value is the same for the whole CTA).
+// tracks whose step ends without an interaction).  `queued` = parked tracks of the group before
+// the tile; returns the number after it (the same value in every thread of the group).
 template <int L, int SCHEME, bool INSTR, int KIND>
-__device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, const CtaRefs &c, uint32_t par,
-                                          uint32_t tile, uint32_t next_tile, uint32_t n_kind, int sbuf,
-                                          uint32_t &in_phase, Tally &tally, double &esc_e) {
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+__device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, const GroupRefs &c, uint32_t par,
+                                              uint32_t tile, uint32_t next_tile, uint32_t n_kind, int sbuf,
+                                              uint32_t &in_phase, uint32_t queued, Tally &tally) {
+  const int gtid = c.gtid, lane = gtid & 31;
   const uint32_t lt_mask = (1u << lane) - 1u;
-  const uint32_t i = tile * kBlock + tid;
+  const uint32_t i = tile * kGroup + gtid;
   const bool active = i < n_kind;
   Ctl *ctl = p.ctl;
-  CtaShared &sh = *c.sh;
+  GroupShared &g = *c.g;
 
   // A1: load
   uint32_t slot = i;
   if (SCHEME == S_SPARSE && active) slot = p.kind[KIND].queue[par][i];
-  const TrackView<L, INSTR> cur = make_view<L, INSTR>(p, KIND, (SCHEME == S_DENSE) ? int(par) : 0, sh.probe);
+  const TrackView<L, INSTR> cur = make_view<L, INSTR>(p, KIND, (SCHEME == S_DENSE) ? int(par) : 0, c.cta->probe);
   Trk t, old;
   MoveOut o;
   move_out_init(o);
   o.alive = false;
   if (SCHEME == S_DENSE) {  // the tile was staged in shared memory by prefetch_tile
-    mbar_wait(&sh.mbar_in, in_phase);
+    mbar_wait(&g.mbar_in, in_phase);
     in_phase ^= 1u;
+    if (active) t = staged_load<L>(c.in_buf, gtid);
+    // the warp has its records in registers; the last warp to get there refills the staging buffer
+    // with the group's next tile, which then loads while this one is stepped
+    __syncwarp();
+    if (lane == 0) {
+      const uint32_t arrived = arrive_acq_rel(&g.loaded);
+      if ((arrived % uint32_t(kWarpsPerGroup)) == uint32_t(kWarpsPerGroup - 1) && next_tile != 0xFFFFFFFFu)
+        prefetch_tile<L>(p.kind[KIND].rec[par], p.capacity, next_tile, n_kind, c.in_buf, &g.mbar_in);
+    }
   }
   if (active) {
     if (SCHEME == S_DENSE) {
-      t = staged_load<L>(c.in_buf, tid);
       if (INSTR) {
 #pragma unroll
         for (int f = 0; f < kNumFields; ++f) cur.probe(f, 0, slot);
@@ -259,10 +291,11 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
     old = t;
     if constexpr (KIND == K_GAMMA) move_gamma(t, env, o);
     else move_elec<KIND>(t, env, o);
-    // A6: scoring into the CTA's histogram (pre-step slab; the S31 guard uses the post-step slab)
-    if (o.dep != 0.0) atomicAdd(&c.edep[old.vol], o.dep);
-    if (o.dep2 != 0.0) atomicAdd(&c.edep[t.vol], o.dep2);
-    esc_e += o.esc_e;
+    // A6: scoring into the CTA's bins (pre-step slab; the S31 guard uses the post-step slab)
+    if (o.dep != 0.0f) bin_add(c.bins, old.vol, o.dep);
+    if (o.dep_b != 0.0f) bin_add(c.bins, old.vol, o.dep_b);
+    if (o.escaped) bin_add_track_energy<KIND>(c.bins, env.n_slabs, t.ekin);
+    if (o.guard) bin_add_track_energy<KIND>(c.bins, t.vol, t.ekin);
   }
   const bool parked = active && o.pending != P_NONE;
   const bool survives = active && !parked && o.alive;
@@ -272,87 +305,66 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
   tally.alive += __popc(m_surv);
   tally.escaped += __popc(m_esc);
 
-  // park the tracks that still owe an interaction (one shared-memory atomic per warp)
-  if (m_park) {
-    uint32_t qbase = 0;
-    if (lane == 0) qbase = atomicAdd(&sh.q_count, uint32_t(__popc(m_park)));
-    qbase = __shfl_sync(0xFFFFFFFFu, qbase, 0);
-    if (parked) {
-      const uint32_t q = qbase + __popc(m_park & lt_mask);
-#pragma unroll
-      for (int f = 0; f < kNumFields; ++f) c.queue[f * kQueueCap + q] = trk_word(t, f);
-      c.queue[14 * kQueueCap + q] = uint32_t(o.pending);
-      if (SCHEME == S_SPARSE) c.queue[15 * kQueueCap + q] = slot;
+  // A9: rank survivors and parked tracks of the warp inside the group; last warp reserves the range
+  uint32_t word = 0;
+  if (lane == 0) {
+    const uint32_t mine = uint32_t(__popc(m_surv)) | (uint32_t(__popc(m_park)) << 9) | kTicket;
+    word = atomicAdd(&g.acc[sbuf], mine);
+    if (last_ticket(word)) {
+      const uint32_t total = word + mine;
+      g.acc[sbuf] = 0u;  // next used two tiles from now, behind a group barrier
+      g.qtot[sbuf] = queued + count_of(total, 1);
+      const uint32_t n_out = count_of(total, 0);
+      g.base[sbuf][0] = n_out ? atomicAdd(&ctl->n_next[KIND], n_out) : 0u;
     }
   }
+  word = __shfl_sync(0xFFFFFFFFu, word, 0);
 
-  if (SCHEME == S_DENSE) {
-    // A9/A10: survivors of the tile go to one contiguous range of the next array.  Warps rank
-    // themselves in arrival order with one shared-memory atomic; the last warp to arrive knows the
-    // tile's total, starts the prefetch of the next tile (every warp has taken its records out of
-    // in_buf by then) and reserves the range with one global atomic.  One block barrier per tile.
-    const uint32_t rank_in_warp = __popc(m_surv & lt_mask);
-    uint32_t warp_base = 0;
-    if (lane == 0) {
-      __threadfence_block();  // this warp's queue pushes and in_buf reads come before its arrival
-      const uint32_t mine = uint32_t(__popc(m_surv));
-      const uint32_t old = atomicAdd(&sh.tile_acc[sbuf], mine | (1u << 16));
-      warp_base = old & 0xFFFFu;
-      if ((old >> 16) == uint32_t(kBlock / 32 - 1)) {  // last to arrive
-        const uint32_t total = warp_base + mine;
-        sh.tile_acc[sbuf] = 0u;  // next used two tiles from now, behind a barrier
-        sh.q_snapshot = sh.q_count;
-        if (next_tile != 0xFFFFFFFFu)
-          prefetch_tile<L>(p.kind[KIND].rec[par], p.capacity, next_tile, n_kind, c.in_buf, &sh.mbar_in);
-        sh.base[sbuf][KIND] = total ? atomicAdd(&ctl->n_next[KIND], total) : 0u;
-      }
-    }
-    warp_base = __shfl_sync(0xFFFFFFFFu, warp_base, 0);
-    __syncthreads();
-    const uint32_t queued = sh.q_snapshot;
-    if (survives) {
-      const uint32_t dst = sh.base[sbuf][KIND] + warp_base + rank_in_warp;
-      if (dst < p.capacity) make_view<L, INSTR>(p, KIND, int(par ^ 1u), sh.probe).store(dst, t);
-      else ctl->overflow = 1u;
-    }
-    return queued;
-  } else {
-    // A10 sparse: in-place update of the words that changed (parked tracks too: the interaction
-    // later writes only what it changes), slot pushed onto the next list
-    if (survives || parked) cur.store_changed(slot, t, old);
-    const uint32_t qpos = warp_reserve(&ctl->n_next[KIND], survives ? 1u : 0u, lane);
-    if (survives) {
-      if (qpos < p.capacity) p.kind[KIND].queue[par ^ 1u][qpos] = slot;
-      else ctl->overflow = 1u;
-    }
-    __syncthreads();
-    const uint32_t queued = sh.q_count;
-    __syncthreads();
-    return queued;
+  // park the tracks that still owe an interaction
+  if (parked) {
+    const uint32_t q = queued + count_of(word, 1) + __popc(m_park & lt_mask);
+#pragma unroll
+    for (int f = 0; f < kNumFields; ++f) c.queue[f * kQueueCap + q] = trk_word(t, f);
+    c.queue[14 * kQueueCap + q] = uint32_t(o.pending);
+    if (SCHEME == S_SPARSE) c.queue[15 * kQueueCap + q] = slot;
   }
+  // A10 sparse: in-place update of the words that changed (parked tracks too: the interaction
+  // later writes only what it changes)
+  if (SCHEME == S_SPARSE && (survives || parked)) cur.store_changed(slot, t, old);
+
+  group_sync(c.group);
+  if (survives) {
+    const uint32_t dst = g.base[sbuf][0] + count_of(word, 0) + __popc(m_surv & lt_mask);
+    if (dst < p.capacity) {
+      if (SCHEME == S_DENSE) make_view<L, INSTR>(p, KIND, int(par ^ 1u), c.cta->probe).store(dst, t);  // A10
+      else p.kind[KIND].queue[par ^ 1u][dst] = slot;  // slot pushed onto the next list
+    } else {
+      ctl->overflow = 1u;
+    }
+  }
+  return g.qtot[sbuf];
 }
 
-// Second half of the step on a dense batch of up to 256 parked tracks taken from the top of the
-// queue (rows A8, A9, A10).  `queued` is sh.q_count as read by every thread after a barrier.
+// Second half of the step on a dense batch of up to kGroup parked tracks taken from the top of the
+// group's queue (rows A8, A9, A10).  Returns the number of tracks left in the queue.
 template <int L, int SCHEME, bool INSTR, int KIND>
-__device__ __forceinline__ void interact_batch(const Params &p, const Env &env, const CtaRefs &c, uint32_t par,
-                                               uint32_t queued, int sbuf, Tally &tally) {
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+__device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &env, const GroupRefs &c, uint32_t par,
+                                                   uint32_t queued, int sbuf, Tally &tally) {
+  const int gtid = c.gtid, lane = gtid & 31;
+  const uint32_t lt_mask = (1u << lane) - 1u;
   Ctl *ctl = p.ctl;
-  CtaShared &sh = *c.sh;
-  const uint32_t batch = queued < uint32_t(kBlock) ? queued : uint32_t(kBlock);
+  GroupShared &g = *c.g;
+  const uint32_t batch = queued < uint32_t(kGroup) ? queued : uint32_t(kGroup);
   const uint32_t first = queued - batch;
-  __syncthreads();  // every thread has read q_count
-  if (tid == 0) sh.q_count = first;
 
-  const bool have = uint32_t(tid) < batch;
+  const bool have = uint32_t(gtid) < batch;
   Trk t, before_interaction;
   InteractOut o;
   interact_out_init(o);
   o.alive = false;
   uint32_t slot = 0;
   if (have) {
-    const uint32_t q = first + tid;
+    const uint32_t q = first + gtid;
 #pragma unroll
     for (int f = 0; f < kNumFields; ++f) trk_set_word(t, f, c.queue[f * kQueueCap + q]);
     const int pending = int(c.queue[14 * kQueueCap + q]);
@@ -360,158 +372,136 @@ __device__ __forceinline__ void interact_batch(const Params &p, const Env &env, 
     before_interaction = t;
     if constexpr (KIND == K_GAMMA) interact_gamma(t, pending, env, o);
     else interact_elec<KIND>(t, pending, env, o);
-    if (o.dep != 0.0) atomicAdd(&c.edep[t.vol], o.dep);
-    if (o.dep2 != 0.0) atomicAdd(&c.edep[t.vol], o.dep2);
+    if (o.dep != 0.0f) bin_add(c.bins, t.vol, o.dep);
+    if (o.dep_b != 0.0f) bin_add(c.bins, t.vol, o.dep_b);
+    if (o.guard) bin_add_track_energy<KIND>(c.bins, t.vol, t.ekin);
   }
-  tally.alive += __popc(__ballot_sync(0xFFFFFFFFu, o.alive));
+  constexpr int Q0 = kid_kind<KIND>(0), Q1 = kid_kind<KIND>(1);  // never KIND itself
+  const uint32_t m_alive = __ballot_sync(0xFFFFFFFFu, o.alive);
+  const uint32_t m_k0 = __ballot_sync(0xFFFFFFFFu, o.kid[0].kind >= 0);
+  const uint32_t m_k1 = __ballot_sync(0xFFFFFFFFu, o.kid[1].kind >= 0);
+  tally.alive += __popc(m_alive);
 
-  const bool has0 = o.kid[0].kind >= 0, has1 = o.kid[1].kind >= 0;
-  constexpr int Q0 = kid_kind<KIND>(0), Q1 = kid_kind<KIND>(1);
+  // A9: one arrival per warp with its output counts per destination kind
+  uint32_t word = 0;
+  if (lane == 0) {
+    const uint32_t mine = (uint32_t(__popc(m_alive)) << (9 * KIND)) + (uint32_t(__popc(m_k0)) << (9 * Q0)) +
+                          (uint32_t(__popc(m_k1)) << (9 * Q1)) + kTicket;
+    word = atomicAdd(&g.acc[sbuf], mine);
+    if (last_ticket(word)) {
+      const uint32_t total = word + mine;
+      g.acc[sbuf] = 0u;
+#pragma unroll
+      for (int q = 0; q < 3; ++q) {
+        const uint32_t want = count_of(total, q);
+        g.base[sbuf][q] = want ? atomicAdd(&ctl->n_next[q], want) : 0u;
+        // sparse: children get bump-allocated, never recycled slots (rule S30)
+        if (SCHEME == S_SPARSE && q != KIND) g.sbase[sbuf][q] = want ? atomicAdd(&ctl->slot_top[q], want) : 0u;
+      }
+    }
+  }
+  word = __shfl_sync(0xFFFFFFFFu, word, 0);
+  group_sync(c.group);  // also: all queue entries of the batch have been read
 
+  // position of this thread's outputs among its warp's: survivor; child 0; child 1 (after the warp's
+  // children 0 when both go to the same kind)
+  const uint32_t r_alive = count_of(word, KIND) + __popc(m_alive & lt_mask);
+  const uint32_t r_k0 = count_of(word, Q0) + __popc(m_k0 & lt_mask);
+  const uint32_t r_k1 = count_of(word, Q1) + ((Q0 == Q1) ? uint32_t(__popc(m_k0)) : 0u) + __popc(m_k1 & lt_mask);
+  const int nbuf = int(par ^ 1u);
+  bool dropped = false;
   if (SCHEME == S_DENSE) {
-    // A9: rank every output of the batch per destination kind with one packed scan (3 x 10 bits)
-    uint32_t mine = o.alive ? (1u << (10 * KIND)) : 0u;
-    mine += has0 ? (1u << (10 * Q0)) : 0u;
-    mine += has1 ? (1u << (10 * Q1)) : 0u;
-    const uint32_t inc = warp_inclusive_scan(mine, lane);
-    if (lane == 31) sh.warp_tot[sbuf][warp] = inc;
-    __syncthreads();  // also: all queue entries of the batch have been read
-    uint32_t before = 0, total = 0;
-#pragma unroll
-    for (int w = 0; w < kBlock / 32; ++w) {
-      const uint32_t v = sh.warp_tot[sbuf][w];
-      total += v;
-      if (w < warp) before += v;
-    }
-    if (tid < 3) {
-      const uint32_t want = (total >> (10 * tid)) & 1023u;
-      sh.base[sbuf][tid] = want ? atomicAdd(&ctl->n_next[tid], want) : 0u;
-    }
-    __syncthreads();
-    const uint32_t excl = before + inc - mine;
-    uint32_t off[3];
-#pragma unroll
-    for (int q = 0; q < 3; ++q) off[q] = sh.base[sbuf][q] + ((excl >> (10 * q)) & 1023u);
-    const int nbuf = int(par ^ 1u);
-    bool dropped = false;
-    // A10: survivor, then children in ordinal order
+    // A10: whole records into the next arrays
     if (o.alive) {
-      const uint32_t dst = off[KIND]++;
-      if (dst < p.capacity) make_view<L, INSTR>(p, KIND, nbuf, sh.probe).store(dst, t);
+      const uint32_t dst = g.base[sbuf][KIND] + r_alive;
+      if (dst < p.capacity) make_view<L, INSTR>(p, KIND, nbuf, c.cta->probe).store(dst, t);
       else dropped = true;
     }
-    if (has0) {
-      const uint32_t dst = off[Q0]++;
-      if (dst < p.capacity) make_view<L, INSTR>(p, Q0, nbuf, sh.probe).store(dst, kid_track(t, o.kid[0]));
+    if (o.kid[0].kind >= 0) {
+      const uint32_t dst = g.base[sbuf][Q0] + r_k0;
+      if (dst < p.capacity) make_view<L, INSTR>(p, Q0, nbuf, c.cta->probe).store(dst, kid_track(t, o.kid[0]));
       else dropped = true;
     }
-    if (has1) {
-      const uint32_t dst = off[Q1]++;
-      if (dst < p.capacity) make_view<L, INSTR>(p, Q1, nbuf, sh.probe).store(dst, kid_track(t, o.kid[1]));
+    if (o.kid[1].kind >= 0) {
+      const uint32_t dst = g.base[sbuf][Q1] + r_k1;
+      if (dst < p.capacity) make_view<L, INSTR>(p, Q1, nbuf, c.cta->probe).store(dst, kid_track(t, o.kid[1]));
       else dropped = true;
     }
-    if (dropped) ctl->overflow = 1u;
   } else {
-    __syncthreads();  // all queue entries of the batch have been read; q_count update is visible
-    bool dropped = false;
     // A10 sparse: the words the interaction changed, slot pushed onto the next list
-    const uint32_t qpos = warp_reserve(&ctl->n_next[KIND], o.alive ? 1u : 0u, lane);
     if (o.alive) {
-      make_view<L, INSTR>(p, KIND, 0, sh.probe).store_changed(slot, t, before_interaction);
-      if (qpos < p.capacity) p.kind[KIND].queue[par ^ 1u][qpos] = slot;
+      make_view<L, INSTR>(p, KIND, 0, c.cta->probe).store_changed(slot, t, before_interaction);
+      const uint32_t qpos = g.base[sbuf][KIND] + r_alive;
+      if (qpos < p.capacity) p.kind[KIND].queue[nbuf][qpos] = slot;
       else dropped = true;
     }
-    // A9 sparse: bump-allocated slots for the children (rule S30), warp-aggregated
-    if (Q0 == Q1) {
-      const uint32_t want = (has0 ? 1u : 0u) + (has1 ? 1u : 0u);
-      uint32_t s_new = warp_reserve(&ctl->slot_top[Q0], want, lane);
-      uint32_t q_new = warp_reserve(&ctl->n_next[Q0], want, lane);
-      const TrackView<L, INSTR> dst = make_view<L, INSTR>(p, Q0, 0, sh.probe);
-      if (has0) {
-        if (s_new < p.capacity && q_new < p.capacity) {
-          dst.store(s_new, kid_track(t, o.kid[0]));
-          p.kind[Q0].queue[par ^ 1u][q_new] = s_new;
-        } else dropped = true;
-        ++s_new; ++q_new;
-      }
-      if (has1) {
-        if (s_new < p.capacity && q_new < p.capacity) {
-          dst.store(s_new, kid_track(t, o.kid[1]));
-          p.kind[Q0].queue[par ^ 1u][q_new] = s_new;
-        } else dropped = true;
-      }
-    } else {
-      const uint32_t s0 = warp_reserve(&ctl->slot_top[Q0], has0 ? 1u : 0u, lane);
-      const uint32_t q0 = warp_reserve(&ctl->n_next[Q0], has0 ? 1u : 0u, lane);
-      const uint32_t s1 = warp_reserve(&ctl->slot_top[Q1], has1 ? 1u : 0u, lane);
-      const uint32_t q1 = warp_reserve(&ctl->n_next[Q1], has1 ? 1u : 0u, lane);
-      if (has0) {
-        if (s0 < p.capacity && q0 < p.capacity) {
-          make_view<L, INSTR>(p, Q0, 0, sh.probe).store(s0, kid_track(t, o.kid[0]));
-          p.kind[Q0].queue[par ^ 1u][q0] = s0;
-        } else dropped = true;
-      }
-      if (has1) {
-        if (s1 < p.capacity && q1 < p.capacity) {
-          make_view<L, INSTR>(p, Q1, 0, sh.probe).store(s1, kid_track(t, o.kid[1]));
-          p.kind[Q1].queue[par ^ 1u][q1] = s1;
-        } else dropped = true;
-      }
+    if (o.kid[0].kind >= 0) {
+      const uint32_t s_new = g.sbase[sbuf][Q0] + r_k0, qpos = g.base[sbuf][Q0] + r_k0;
+      if (s_new < p.capacity && qpos < p.capacity) {
+        make_view<L, INSTR>(p, Q0, 0, c.cta->probe).store(s_new, kid_track(t, o.kid[0]));
+        p.kind[Q0].queue[nbuf][qpos] = s_new;
+      } else dropped = true;
     }
-    if (dropped) ctl->overflow = 1u;
+    if (o.kid[1].kind >= 0) {
+      const uint32_t s_new = g.sbase[sbuf][Q1] + r_k1, qpos = g.base[sbuf][Q1] + r_k1;
+      if (s_new < p.capacity && qpos < p.capacity) {
+        make_view<L, INSTR>(p, Q1, 0, c.cta->probe).store(s_new, kid_track(t, o.kid[1]));
+        p.kind[Q1].queue[nbuf][qpos] = s_new;
+      } else dropped = true;
+    }
   }
+  if (dropped) ctl->overflow = 1u;
+  return first;
 }
 
-// All tiles of one kind that belong to this CTA, then the left-over parked tracks.
+// All tiles of one kind that belong to this group, then the left-over parked tracks.
+// `first_global_tile` = tiles of the kinds before this one; n_tiles, n_kind are launch-uniform.
 template <int L, int SCHEME, bool INSTR, int KIND>
-__device__ __forceinline__ void run_kind(const Params &p, const Env &env, const CtaRefs &c, uint32_t par,
+__device__ __forceinline__ void run_kind(const Params &p, const Env &env, const GroupRefs &c, uint32_t par,
                                          uint32_t first_global_tile, uint32_t n_tiles, uint32_t n_kind, int &sbuf,
-                                         uint32_t &in_phase, uint32_t &tab_phase, int &staged_group, Tally &tally,
-                                         double &esc_e) {
+                                         uint32_t &in_phase, uint32_t &tab_phase, int &staged_group, Tally &tally) {
   // A3: the cross-section tables of this kind's particle group -> shared memory, one TMA bulk copy
-  // (e- and e+ share a group).  The previous group's last reader has passed a barrier.
+  // (e- and e+ share a group).  CTA-wide: every group is done with the previous tables.
   constexpr int group = (KIND == K_GAMMA) ? 0 : 1;
   if (n_tiles != 0u && staged_group != group) {
+    __syncthreads();
     if (threadIdx.x == 0) {
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
       asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(
-                       static_cast<uint32_t>(__cvta_generic_to_shared(&c.sh->mbar))),
+                       static_cast<uint32_t>(__cvta_generic_to_shared(&c.cta->mbar))),
                    "r"(p.table_bytes)
                    : "memory");
       bulk_g2s(const_cast<float4 *>(env.tab), reinterpret_cast<const unsigned char *>(p.tables) + size_t(group) * p.table_bytes,
-               p.table_bytes, &c.sh->mbar);
+               p.table_bytes, &c.cta->mbar);
     }
-    mbar_wait(&c.sh->mbar, tab_phase);
+    mbar_wait(&c.cta->mbar, tab_phase);
     tab_phase ^= 1u;
     staged_group = group;
   }
-  // global tile index g = first_global_tile + tile must be congruent to blockIdx.x modulo gridDim.x
-  const uint32_t grid = gridDim.x;
-  const uint32_t shift = (blockIdx.x + grid - first_global_tile % grid) % grid;
-  if (SCHEME == S_DENSE && shift < n_tiles && threadIdx.x == 0)  // in_buf is free: its last reader passed a barrier
-    prefetch_tile<L>(p.kind[KIND].rec[par], p.capacity, shift, n_kind, c.in_buf, &c.sh->mbar_in);
-  for (uint32_t tile = shift; tile < n_tiles; tile += grid) {
-    const uint32_t next_tile = (tile + grid < n_tiles) ? tile + grid : 0xFFFFFFFFu;
-    const uint32_t queued =
-        move_tile<L, SCHEME, INSTR, KIND>(p, env, c, par, tile, next_tile, n_kind, sbuf, in_phase, tally, esc_e);
+  // tiles are dealt round-robin over all groups of the grid, continuing across the kinds
+  const uint32_t n_groups = gridDim.x * kGroupsPerCta;
+  const uint32_t me = blockIdx.x * kGroupsPerCta + c.group;
+  const uint32_t shift = (me + n_groups - first_global_tile % n_groups) % n_groups;
+  if (SCHEME == S_DENSE && shift < n_tiles && c.gtid == 0)  // the staging buffer is free: its last reader passed a barrier
+    prefetch_tile<L>(p.kind[KIND].rec[par], p.capacity, shift, n_kind, c.in_buf, &c.g->mbar_in);
+  uint32_t queued = 0u;
+  for (uint32_t tile = shift; tile < n_tiles; tile += n_groups) {
+    const uint32_t next_tile = (tile + n_groups < n_tiles) ? tile + n_groups : 0xFFFFFFFFu;
+    queued = move_tile<L, SCHEME, INSTR, KIND>(p, env, c, par, tile, next_tile, n_kind, sbuf, in_phase, queued, tally);
     sbuf ^= 1;
-    if (queued >= uint32_t(kBlock)) {
-      interact_batch<L, SCHEME, INSTR, KIND>(p, env, c, par, queued, sbuf, tally);
+    if (queued >= uint32_t(kGroup)) {
+      queued = interact_batch<L, SCHEME, INSTR, KIND>(p, env, c, par, queued, sbuf, tally);
       sbuf ^= 1;
     }
   }
-  for (;;) {
-    __syncthreads();
-    const uint32_t queued = c.sh->q_count;
-    if (queued == 0u) break;
-    interact_batch<L, SCHEME, INSTR, KIND>(p, env, c, par, queued, sbuf, tally);
+  while (queued != 0u) {
+    queued = interact_batch<L, SCHEME, INSTR, KIND>(p, env, c, par, queued, sbuf, tally);
     sbuf ^= 1;
   }
 }
 
 // ---------------------------------------------------------------------- the step kernel ------
-// Dynamic shared memory: [tables (p.table_bytes)] [staged tile (kInBufBytes)] [edep histogram
-// (n_slabs doubles)] [queue].
+// Dynamic shared memory: step_smem_bytes() in device_state.cuh.
 #ifndef ADEPT_STEP_MIN_CTAS
 #define ADEPT_STEP_MIN_CTAS 4
 #endif
@@ -522,30 +512,37 @@ __global__ void __launch_bounds__(kBlock, ADEPT_STEP_MIN_CTAS) step_kernel(const
   float4 *s_tab = reinterpret_cast<float4 *>(dyn_smem);
   const int tid = threadIdx.x;
   Ctl *ctl = p.ctl;
-  CtaRefs c;
-  c.sh = &sh;
-  c.in_buf = reinterpret_cast<uint32_t *>(dyn_smem + p.table_bytes);
-  constexpr size_t kInBuf = in_buf_bytes(SCHEME, Mapping<L>::words(kBlock));
-  c.edep = reinterpret_cast<double *>(dyn_smem + p.table_bytes + kInBuf);
-  c.queue = reinterpret_cast<uint32_t *>(dyn_smem + p.table_bytes + kInBuf + size_t(p.n_slabs) * sizeof(double));
+  constexpr size_t kInBuf = in_buf_bytes(SCHEME, Mapping<L>::words(kGroup));
+  constexpr size_t kPerGroup = kInBuf + queue_bytes(SCHEME);
+  GroupRefs c;
+  c.cta = &sh;
+  c.group = tid / kGroup;
+  c.gtid = tid % kGroup;
+  c.g = &sh.grp[c.group];
+  c.bins.lo = reinterpret_cast<uint32_t *>(dyn_smem + p.table_bytes);
+  c.bins.hi = c.bins.lo + (p.n_slabs + 1u);
+  unsigned char *mine = dyn_smem + p.table_bytes + bins_bytes(p.n_slabs) + size_t(c.group) * kPerGroup;
+  c.in_buf = reinterpret_cast<uint32_t *>(mine);
+  c.queue = reinterpret_cast<uint32_t *>(mine + kInBuf);
 
   // A0: what is alive (written by the previous iteration's last CTA; constant during this launch)
   const uint32_t par = ctl->parity;
   const uint32_t n0 = ctl->n_cur[0], n1 = ctl->n_cur[1], n2 = ctl->n_cur[2];
-  const uint32_t t0 = (n0 + kBlock - 1) / kBlock, t1 = (n1 + kBlock - 1) / kBlock, t2 = (n2 + kBlock - 1) / kBlock;
+  const uint32_t t0 = (n0 + kGroup - 1) / kGroup, t1 = (n1 + kGroup - 1) / kGroup, t2 = (n2 + kGroup - 1) / kGroup;
   const uint32_t tiles = t0 + t1 + t2;
 
-  if (blockIdx.x < tiles) {
-    // A3: barriers of the two asynchronous copies (tables of a particle group, staged tile);
-    // histogram and counters cleared
+  if (blockIdx.x * kGroupsPerCta < tiles) {  // CTA-uniform: at least one group of this CTA has a tile
+    // barriers of the asynchronous copies (tables of a particle group, staged tiles); bins and
+    // counters cleared
     if (tid == 0) {
       mbar_init(&sh.mbar, 1u);
-      mbar_init(&sh.mbar_in, 1u);
+#pragma unroll
+      for (int gI = 0; gI < kGroupsPerCta; ++gI) mbar_init(&sh.grp[gI].mbar_in, 1u);
       asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    for (uint32_t s = tid; s < p.n_slabs; s += kBlock) c.edep[s] = 0.0;
+    for (uint32_t s = tid; s < 2u * (p.n_slabs + 1u); s += kBlock) c.bins.lo[s] = 0u;
     if (tid < 4) { sh.alive[tid] = 0u; sh.escaped[tid] = 0u; }
-    if (tid == 0) { sh.esc_e = 0.0; sh.q_count = 0u; sh.tile_acc[0] = 0u; sh.tile_acc[1] = 0u; }
+    if (tid < kGroupsPerCta) { sh.grp[tid].loaded = 0u; sh.grp[tid].acc[0] = 0u; sh.grp[tid].acc[1] = 0u; }
     if (INSTR) for (int s = tid; s < 3 * kNumFields * 2; s += kBlock) sh.probe[s] = 0u;
     __syncthreads();
 
@@ -556,16 +553,14 @@ __global__ void __launch_bounds__(kBlock, ADEPT_STEP_MIN_CTAS) step_kernel(const
     env.mat_abs = p.mat_abs; env.mat_gap = p.mat_gap;
 
     Tally ta0{0u, 0u}, ta1{0u, 0u}, ta2{0u, 0u};
-    double esc_e = 0.0;
     int sbuf = 0;
     uint32_t in_phase = 0u, tab_phase = 0u;
     int staged_group = -1;
-    run_kind<L, SCHEME, INSTR, K_EM>(p, env, c, par, 0u, t0, n0, sbuf, in_phase, tab_phase, staged_group, ta0, esc_e);
-    run_kind<L, SCHEME, INSTR, K_EP>(p, env, c, par, t0, t1, n1, sbuf, in_phase, tab_phase, staged_group, ta1, esc_e);
-    run_kind<L, SCHEME, INSTR, K_GAMMA>(p, env, c, par, t0 + t1, t2, n2, sbuf, in_phase, tab_phase, staged_group, ta2, esc_e);
+    run_kind<L, SCHEME, INSTR, K_EM>(p, env, c, par, 0u, t0, n0, sbuf, in_phase, tab_phase, staged_group, ta0);
+    run_kind<L, SCHEME, INSTR, K_EP>(p, env, c, par, t0, t1, n1, sbuf, in_phase, tab_phase, staged_group, ta1);
+    run_kind<L, SCHEME, INSTR, K_GAMMA>(p, env, c, par, t0 + t1, t2, n2, sbuf, in_phase, tab_phase, staged_group, ta2);
 
     // flush the CTA's tallies
-    esc_e = warp_sum(esc_e);
     if ((tid & 31) == 0) {
       if (ta0.alive) atomicAdd(&sh.alive[0], ta0.alive);
       if (ta1.alive) atomicAdd(&sh.alive[1], ta1.alive);
@@ -573,18 +568,16 @@ __global__ void __launch_bounds__(kBlock, ADEPT_STEP_MIN_CTAS) step_kernel(const
       if (ta0.escaped) atomicAdd(&sh.escaped[0], ta0.escaped);
       if (ta1.escaped) atomicAdd(&sh.escaped[1], ta1.escaped);
       if (ta2.escaped) atomicAdd(&sh.escaped[2], ta2.escaped);
-      if (esc_e != 0.0) atomicAdd(&sh.esc_e, esc_e);
     }
     __syncthreads();
-    for (uint32_t s = tid; s < p.n_slabs; s += kBlock) {
-      const double v = c.edep[s];
-      if (v != 0.0) atomicAdd(&p.edep[s], v);
+    for (uint32_t s = tid; s <= p.n_slabs; s += kBlock) {
+      const unsigned long long v = (static_cast<unsigned long long>(c.bins.hi[s]) << 32) + c.bins.lo[s];
+      if (v != 0ull) atomicAdd(&p.tally[s], v);
     }
     if (tid < 3) {
       if (sh.alive[tid]) atomicAdd(&ctl->it_alive[tid], sh.alive[tid]);
       if (sh.escaped[tid]) atomicAdd(&ctl->it_escaped[tid], sh.escaped[tid]);
     }
-    if (tid == 0 && sh.esc_e != 0.0) atomicAdd(&ctl->e_escaped, sh.esc_e);
     if (INSTR) {
       for (int s = tid; s < 3 * kNumFields * 2; s += kBlock)
         if (sh.probe[s]) atomicAdd(&p.instr_field_rw[s], static_cast<unsigned long long>(sh.probe[s]));
