@@ -179,7 +179,8 @@ const char *adept_last_error(const adept_ctx *);
  *  fn 1: u01;            in = n u32,  out = n f32
  *  fn 2: lg;             in = n f32,  out = n f32
  *  fn 3: ex;             in = n f32,  out = n f32
- *  fn 4: sincos2pi;      in = n f32,  out = n x {sin, cos} f32 */
+ *  fn 4: sincos2pi;      in = n f32,  out = n x {sin, cos} f32
+ *  fn 5: in-range division (rule M11, csrc/mathfn.cuh); in = n x {a, b} f32, out = n f32 = a / b */
 int adept_dev_math(int fn, const void *in, void *out, uint64_t n, void *cuda_stream);
 
 #ifdef __cplusplus

@@ -194,10 +194,15 @@ __global__ void dev_math_kernel(int fn, const void *in, void *out, unsigned long
     case 1: static_cast<float *>(out)[i] = u01(static_cast<const uint32_t *>(in)[i]); break;
     case 2: static_cast<float *>(out)[i] = lg(static_cast<const float *>(in)[i]); break;
     case 3: static_cast<float *>(out)[i] = ex(static_cast<const float *>(in)[i]); break;
-    default: {
+    case 4: {
       float s, c;
       sincos2pi(static_cast<const float *>(in)[i], s, c);
       static_cast<float2 *>(out)[i] = make_float2(s, c);
+      break;
+    }
+    default: {
+      const float2 ab = static_cast<const float2 *>(in)[i];
+      static_cast<float *>(out)[i] = div_rn_inrange(ab.x, ab.y);
     }
   }
 }
@@ -578,7 +583,7 @@ uint64_t adept_field_offset(int32_t layout, uint32_t capacity, uint32_t slot, ui
 }
 
 int adept_dev_math(int fn, const void *in, void *out, uint64_t n, void *cuda_stream) {
-  if (fn < 0 || fn > 4 || (n && (!in || !out))) return ADEPT_EINVAL;
+  if (fn < 0 || fn > 5 || (n && (!in || !out))) return ADEPT_EINVAL;
   if (n == 0) return ADEPT_OK;
   const unsigned grid = unsigned((n + 255) / 256);
   dev_math_kernel<<<grid, 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(fn, in, out, n);

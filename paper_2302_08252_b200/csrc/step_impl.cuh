@@ -234,10 +234,6 @@ struct GroupRefs {
   int group, gtid;   // group index inside the CTA, thread index inside the group
 };
 
-struct Tally {  // per-warp running sums of one kind (warp-uniform)
-  uint32_t alive, escaped;
-};
-
 // S25 / S31 energy of a track that leaves the simulation
 template <int KIND> __device__ __forceinline__ void bin_add_track_energy(const Bins &b, uint32_t bin, float ekin) {
   bin_add(b, bin, ekin);
@@ -250,7 +246,7 @@ template <int KIND> __device__ __forceinline__ void bin_add_track_energy(const B
 template <int L, int SCHEME, bool INSTR, int KIND>
 __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, const GroupRefs &c, uint32_t par,
                                               uint32_t tile, uint32_t next_tile, uint32_t n_kind, int sbuf,
-                                              uint32_t &in_phase, uint32_t queued, Tally &tally) {
+                                              uint32_t &in_phase, uint32_t queued) {
   const int gtid = c.gtid, lane = gtid & 31;
   const uint32_t lt_mask = (1u << lane) - 1u;
   const uint32_t i = tile * kGroup + gtid;
@@ -302,20 +298,21 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
   const uint32_t m_surv = __ballot_sync(0xFFFFFFFFu, survives);
   const uint32_t m_esc = __ballot_sync(0xFFFFFFFFu, o.escaped);
   const uint32_t m_park = __ballot_sync(0xFFFFFFFFu, parked);
-  tally.alive += __popc(m_surv);
-  tally.escaped += __popc(m_esc);
 
-  // A9: rank survivors and parked tracks of the warp inside the group; last warp reserves the range
+  // A9: rank survivors and parked tracks of the warp inside the group (the third count, escapes, is
+  // only totalled); last warp reserves the range and books the tile's counts
   uint32_t word = 0;
   if (lane == 0) {
-    const uint32_t mine = uint32_t(__popc(m_surv)) | (uint32_t(__popc(m_park)) << 9) | kTicket;
+    const uint32_t mine = uint32_t(__popc(m_surv)) | (uint32_t(__popc(m_park)) << 9) | (uint32_t(__popc(m_esc)) << 18) | kTicket;
     word = atomicAdd(&g.acc[sbuf], mine);
     if (last_ticket(word)) {
       const uint32_t total = word + mine;
       g.acc[sbuf] = 0u;  // next used two tiles from now, behind a group barrier
       g.qtot[sbuf] = queued + count_of(total, 1);
-      const uint32_t n_out = count_of(total, 0);
+      const uint32_t n_out = count_of(total, 0), n_esc = count_of(total, 2);
       g.base[sbuf][0] = n_out ? atomicAdd(&ctl->n_next[KIND], n_out) : 0u;
+      if (n_out) atomicAdd(&c.cta->alive[KIND], n_out);
+      if (n_esc) atomicAdd(&c.cta->escaped[KIND], n_esc);
     }
   }
   word = __shfl_sync(0xFFFFFFFFu, word, 0);
@@ -349,7 +346,7 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
 // group's queue (rows A8, A9, A10).  Returns the number of tracks left in the queue.
 template <int L, int SCHEME, bool INSTR, int KIND>
 __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &env, const GroupRefs &c, uint32_t par,
-                                                   uint32_t queued, int sbuf, Tally &tally) {
+                                                   uint32_t queued, int sbuf) {
   const int gtid = c.gtid, lane = gtid & 31;
   const uint32_t lt_mask = (1u << lane) - 1u;
   Ctl *ctl = p.ctl;
@@ -380,7 +377,6 @@ __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &e
   const uint32_t m_alive = __ballot_sync(0xFFFFFFFFu, o.alive);
   const uint32_t m_k0 = __ballot_sync(0xFFFFFFFFu, o.kid[0].kind >= 0);
   const uint32_t m_k1 = __ballot_sync(0xFFFFFFFFu, o.kid[1].kind >= 0);
-  tally.alive += __popc(m_alive);
 
   // A9: one arrival per warp with its output counts per destination kind
   uint32_t word = 0;
@@ -391,6 +387,7 @@ __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &e
     if (last_ticket(word)) {
       const uint32_t total = word + mine;
       g.acc[sbuf] = 0u;
+      if (count_of(total, KIND)) atomicAdd(&c.cta->alive[KIND], count_of(total, KIND));  // parents that survive
 #pragma unroll
       for (int q = 0; q < 3; ++q) {
         const uint32_t want = count_of(total, q);
@@ -459,7 +456,7 @@ __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &e
 template <int L, int SCHEME, bool INSTR, int KIND>
 __device__ __forceinline__ void run_kind(const Params &p, const Env &env, const GroupRefs &c, uint32_t par,
                                          uint32_t first_global_tile, uint32_t n_tiles, uint32_t n_kind, int &sbuf,
-                                         uint32_t &in_phase, uint32_t &tab_phase, int &staged_group, Tally &tally) {
+                                         uint32_t &in_phase, uint32_t &tab_phase, int &staged_group) {
   // A3: the cross-section tables of this kind's particle group -> shared memory, one TMA bulk copy
   // (e- and e+ share a group).  CTA-wide: every group is done with the previous tables.
   constexpr int group = (KIND == K_GAMMA) ? 0 : 1;
@@ -487,15 +484,15 @@ __device__ __forceinline__ void run_kind(const Params &p, const Env &env, const 
   uint32_t queued = 0u;
   for (uint32_t tile = shift; tile < n_tiles; tile += n_groups) {
     const uint32_t next_tile = (tile + n_groups < n_tiles) ? tile + n_groups : 0xFFFFFFFFu;
-    queued = move_tile<L, SCHEME, INSTR, KIND>(p, env, c, par, tile, next_tile, n_kind, sbuf, in_phase, queued, tally);
+    queued = move_tile<L, SCHEME, INSTR, KIND>(p, env, c, par, tile, next_tile, n_kind, sbuf, in_phase, queued);
     sbuf ^= 1;
     if (queued >= uint32_t(kGroup)) {
-      queued = interact_batch<L, SCHEME, INSTR, KIND>(p, env, c, par, queued, sbuf, tally);
+      queued = interact_batch<L, SCHEME, INSTR, KIND>(p, env, c, par, queued, sbuf);
       sbuf ^= 1;
     }
   }
   while (queued != 0u) {
-    queued = interact_batch<L, SCHEME, INSTR, KIND>(p, env, c, par, queued, sbuf, tally);
+    queued = interact_batch<L, SCHEME, INSTR, KIND>(p, env, c, par, queued, sbuf);
     sbuf ^= 1;
   }
 }
@@ -552,23 +549,14 @@ __global__ void __launch_bounds__(kBlock, ADEPT_STEP_MIN_CTAS) step_kernel(const
     env.n_slabs = p.n_slabs; env.abs_mm = p.abs_mm; env.pitch = p.pitch; env.half_xy = p.half_xy;
     env.mat_abs = p.mat_abs; env.mat_gap = p.mat_gap;
 
-    Tally ta0{0u, 0u}, ta1{0u, 0u}, ta2{0u, 0u};
     int sbuf = 0;
     uint32_t in_phase = 0u, tab_phase = 0u;
     int staged_group = -1;
-    run_kind<L, SCHEME, INSTR, K_EM>(p, env, c, par, 0u, t0, n0, sbuf, in_phase, tab_phase, staged_group, ta0);
-    run_kind<L, SCHEME, INSTR, K_EP>(p, env, c, par, t0, t1, n1, sbuf, in_phase, tab_phase, staged_group, ta1);
-    run_kind<L, SCHEME, INSTR, K_GAMMA>(p, env, c, par, t0 + t1, t2, n2, sbuf, in_phase, tab_phase, staged_group, ta2);
+    run_kind<L, SCHEME, INSTR, K_EM>(p, env, c, par, 0u, t0, n0, sbuf, in_phase, tab_phase, staged_group);
+    run_kind<L, SCHEME, INSTR, K_EP>(p, env, c, par, t0, t1, n1, sbuf, in_phase, tab_phase, staged_group);
+    run_kind<L, SCHEME, INSTR, K_GAMMA>(p, env, c, par, t0 + t1, t2, n2, sbuf, in_phase, tab_phase, staged_group);
 
     // flush the CTA's tallies
-    if ((tid & 31) == 0) {
-      if (ta0.alive) atomicAdd(&sh.alive[0], ta0.alive);
-      if (ta1.alive) atomicAdd(&sh.alive[1], ta1.alive);
-      if (ta2.alive) atomicAdd(&sh.alive[2], ta2.alive);
-      if (ta0.escaped) atomicAdd(&sh.escaped[0], ta0.escaped);
-      if (ta1.escaped) atomicAdd(&sh.escaped[1], ta1.escaped);
-      if (ta2.escaped) atomicAdd(&sh.escaped[2], ta2.escaped);
-    }
     __syncthreads();
     for (uint32_t s = tid; s <= p.n_slabs; s += kBlock) {
       const unsigned long long v = (static_cast<unsigned long long>(c.bins.hi[s]) << 32) + c.bins.lo[s];

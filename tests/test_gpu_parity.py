@@ -70,6 +70,30 @@ def test_device_math_is_bit_equal_to_the_oracle():
     assert (sc[:, 0].view(np.uint32) == s.view(np.uint32)).all() and (sc[:, 1].view(np.uint32) == c.view(np.uint32)).all()
 
 
+def test_inrange_division_is_the_ieee_quotient():
+    """csrc/mathfn.cuh div_rn_inrange (the division inside lg, rule M8) against numpy's correctly
+    rounded fp32 division, bit for bit, over its whole admitted operand range and on lg's operands."""
+    import torch
+    from paper_2302_08252_b200 import dev_math
+    rng = np.random.default_rng(5)
+    n = 4_000_000
+    mant = lambda: (rng.integers(0, 1 << 23, n, dtype=np.uint64).astype(np.uint32) | np.uint32(0x3F800000)).view(np.float32)
+    sign = lambda: np.where(rng.random(n) < 0.5, np.float32(-1), np.float32(1))
+    a = np.ldexp(mant(), rng.integers(-100, 40, n)).astype(np.float32) * sign()
+    b = np.ldexp(mant(), rng.integers(-60, 20, n)).astype(np.float32) * sign()
+    m = (rng.integers(0, 1 << 23, n, dtype=np.uint64).astype(np.uint32) | np.uint32(0x3F800000)).view(np.float32)
+    m = np.where(m > np.float32(1.41421354), m * np.float32(0.5), m)
+    a = np.concatenate([a, m - np.float32(1), np.float32([0.0, 0.0, 1.0, -1.0])])
+    b = np.concatenate([b, m + np.float32(1), np.float32([2.0, -3.0, 3.0, 3.0])])
+    ab = np.stack([a, b], axis=1).astype(np.float32)
+    q = dev_math(5, torch.from_numpy(ab).cuda(), torch.float32, (ab.shape[0],)).cpu().numpy()
+    with np.errstate(all="ignore"):
+        ref = (a / b).astype(np.float32)
+    nz = ref != 0
+    assert (q[nz].view(np.uint32) == ref[nz].view(np.uint32)).all()
+    assert (q[~nz] == 0).all()
+
+
 # ------------------------------------------------------------------------ single step --------
 @pytest.fixture(scope="module")
 def single_step_case():
