@@ -207,9 +207,8 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
     biggest = max(p.shape[0] for p in pop)
     capacity = int(biggest * 1.25) + 4096                  # one step grows the photon set by ~16 %
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-    layouts = ["soa", "aosoa32", "aos"] if args.layout == "all" else [args.layout]
-    main = layouts[0]
-    per_layout, main_res = {}, None
+    layouts = ["aosoa32", "soa", "aos"] if args.layout == "all" else [args.layout]
+    per_layout, results = {}, {}
     sampler = ClockSampler(local_rank)
     sampler.start()
     for layout in layouts:
@@ -225,13 +224,14 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
             "algorithmic_bytes_per_launch": bytes_per_launch,
             "algorithmic_GBps": bytes_per_launch / (float(np.mean(ms)) * 1e-3) / 1e9,
             "survivors_plus_secondaries": n_out}
-        if layout == main:
-            main_res = res
-            main_ctx_ms = ms
+        results[layout] = res
         ctx.destroy()
         del ctx
         torch.cuda.empty_cache()
     clocks = sampler.stop()
+    # headline = the fastest layout of this run (north_star: "the best layout and buffer scheme")
+    main = min(per_layout, key=lambda l: per_layout[l]["ms_per_step"])
+    main_res = results[main]
 
     # ---- e2e: host buffers, H2D + step + D2H inside the timed region (main layout) ----------
     ctx = Context(geo, tab, layout=main, scheme="dense", capacity=capacity,

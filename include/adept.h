@@ -131,6 +131,13 @@ int adept_create(const adept_geometry *, const adept_tables *, const adept_confi
  * adept_run.  EINVAL if a primary is outside the calorimeter or its energy outside [e_cut, e_max]. */
 int adept_inject(adept_ctx *, const adept_primary *primaries, uint64_t n);
 
+/* Rule R4: primary ids (hence random streams) derive from a running global primary index that
+ * starts at 0 at create/reset.  A caller that simulates only the slice [lo, hi) of a longer primary
+ * list (one rank of a multi-GPU run; events are independent) sets the index to lo
+ * before injecting, so that every primary keeps the id it has in the unsliced run and the per-rank
+ * tallies add up to the single-GPU result.  ESTATE while queued primaries (batch mode) are pending. */
+int adept_set_primary_index(adept_ctx *, uint64_t next_index);
+
 /* One iteration: every live track of every kind takes one step (DESIGN.md rules S16-S28).
  * out == NULL: enqueue only.  out != NULL: synchronise and report the counts after the step. */
 int adept_step(adept_ctx *, adept_counts *out);

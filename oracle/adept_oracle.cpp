@@ -740,6 +740,13 @@ void orc_get_result(const orc_ctx *c, Result *out, double *edep_slab) {
   if (edep_slab) std::memcpy(edep_slab, o.edep.data(), o.edep.size() * sizeof(double));
 }
 
+// Rule R4: ids of primaries come from a running global index; a caller that simulates only a
+// slice [lo, hi) of a larger primary list sets the index to lo first, so that every primary keeps
+// the id (hence the random stream) it has in the unsliced run (sharding by event).
+void orc_set_primary_index(orc_ctx *c, uint64_t next_index) {
+  reinterpret_cast<Oracle *>(c)->next_primary = next_index;
+}
+
 void orc_reset_tallies(orc_ctx *c) {
   Oracle &o = *reinterpret_cast<Oracle *>(c);
   const uint64_t live[3] = {o.cur[0].size(), o.cur[1].size(), o.cur[2].size()};

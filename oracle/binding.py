@@ -75,6 +75,7 @@ def lib():
         L.orc_run_batched.argtypes = [vp, u64]
         L.orc_get_result.argtypes = [vp, C.POINTER(_Result), vp]
         L.orc_reset_tallies.argtypes = [vp]
+        L.orc_set_primary_index.argtypes = [vp, u64]
         L.orc_set_trace.argtypes = [vp, C.c_int]
         L.orc_trace_size.restype = u64
         L.orc_trace_size.argtypes = [vp]
@@ -198,6 +199,10 @@ class Oracle:
         assert p.dtype.itemsize == 32
         if self._L.orc_inject(self._h, _ptr(p), p.shape[0]) != 0:
             raise ValueError("orc_inject: invalid primary")
+
+    def set_primary_index(self, next_index: int):
+        """Rule R4: global index of the next injected primary (event sharding)."""
+        self._L.orc_set_primary_index(self._h, next_index)
 
     def queue(self, primaries: np.ndarray):
         p = np.ascontiguousarray(primaries)

@@ -78,6 +78,7 @@ def lib():
         L.adept_workspace_bytes.argtypes = [C.POINTER(_Geometry), C.POINTER(_Tables), C.POINTER(_Config)]
         L.adept_create.argtypes = [C.POINTER(_Geometry), C.POINTER(_Tables), C.POINTER(_Config), C.POINTER(vp)]
         L.adept_inject.argtypes = [vp, vp, u64]
+        L.adept_set_primary_index.argtypes = [vp, u64]
         L.adept_step.argtypes = [vp, C.POINTER(_Counts)]
         L.adept_run.argtypes = [vp, u64, C.POINTER(_Result)]
         L.adept_get_result.argtypes = [vp, C.POINTER(_Result)]
@@ -181,6 +182,9 @@ class Context:
         p = np.ascontiguousarray(primaries)
         assert p.dtype.itemsize == 32
         self._check(self._L.adept_inject(self._h, p.ctypes.data, p.shape[0]))
+
+    def set_primary_index(self, next_index: int):
+        self._check(self._L.adept_set_primary_index(self._h, next_index))
 
     def step(self, sync: bool = True):
         if not sync:

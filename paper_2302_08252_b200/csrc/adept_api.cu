@@ -338,6 +338,14 @@ int adept_destroy(adept_ctx *c) {
   return ADEPT_OK;
 }
 
+int adept_set_primary_index(adept_ctx *c, uint64_t next_index) {
+  if (!c) return ADEPT_EINVAL;
+  if (c->pending_done < c->pending.size())
+    return fail(c, ADEPT_ESTATE, "adept_set_primary_index: primaries are still queued for adept_run");
+  c->next_primary = next_index;
+  return ADEPT_OK;
+}
+
 int adept_reset(adept_ctx *c) {
   if (!c) return ADEPT_EINVAL;
   int rc = clear_state(c);
@@ -517,7 +525,10 @@ int adept_run(adept_ctx *c, uint64_t max_iterations, adept_result *out) {
   // Iterations are enqueued in bursts; the control block is read back after each burst.  An
   // iteration with nothing alive is a no-op on the device (and is not counted), so over-shooting
   // the end of a shower by a few launches is harmless.
-  const uint64_t kBurst = 8;
+#ifndef ADEPT_RUN_BURST
+#define ADEPT_RUN_BURST 8
+#endif
+  const uint64_t kBurst = ADEPT_RUN_BURST;
   uint64_t done = 0;
   for (;;) {
     rc = fetch_ctl(c, false);

@@ -270,3 +270,88 @@ def test_edge_cases_empty_overflow_invalid_reset():
     ctx.destroy()
     with pytest.raises(AdeptError):
         _ctx(geo, tab, layout="soa", scheme="dense", capacity=0)
+
+
+# ------------------------------------------------------------- event sharding ---
+def test_sliced_runs_add_up_to_the_unsliced_run():
+    """adept_set_primary_index: two contexts that each take a slice of the primary list (what two
+    ranks of a multi-GPU run do, here one after the other on one device) add up to the single run."""
+    geo, tab = geometry_for("tiny"), tables_for("tiny")
+    prim = gen_primaries(13, 10.0)
+    o = Oracle(geo, tab, seed=21)
+    o.inject(prim)
+    o.run()
+    r = o.result()
+    parts = []
+    for lo, hi in ((0, 7), (7, 13)):
+        ctx = _ctx(geo, tab, layout="aosoa32", scheme="dense", capacity=4096, seed=21)
+        ctx.set_primary_index(lo)
+        ctx.inject(prim[lo:hi])
+        parts.append(ctx.run())
+        ctx.destroy()
+    for k in ("steps", "secondaries", "killed", "escaped_n"):
+        assert (parts[0][k] + parts[1][k] == r[k]).all(), k
+    assert max(p["iterations"] for p in parts) == r["iterations"]
+    assert np.allclose(parts[0]["edep_layer"] + parts[1]["edep_layer"], r["edep_layer"], rtol=1e-9, atol=1e-12)
+
+
+# ----------------------------------------------------- instrumented build (SURVEY §8(a) A12) ---
+@pytest.mark.parametrize("layout", LAYOUTS)
+def test_instrumented_dense_counts_follow_the_access_rules(layout):
+    """PAPER.md:115/123 per-field counts, PAPER.md:131/135 per-row heatmap, PAPER.md:137 per-slot use.
+    Dense double buffer: a step reads all 14 words of every live track once and writes all 14 words
+    of every track that enters the next arrays (survivor or secondary)."""
+    c = CONFIGS["single_step"]
+    geo, tab = geometry_for("single_step"), tables_for("single_step")
+    pop = gen_tracks(6000 + 13, c["seed"], geo, c["e_max"], c["fractions"])
+    for k in range(3):
+        pop[k]["nial"][::5] = 1e-30                    # plenty of interactions and secondaries
+    cap = 8192
+    ctx = _ctx(geo, tab, layout=layout, scheme="dense", capacity=cap, seed=3, instrument=True)
+    n_in = [p.shape[0] for p in pop]
+    for k in range(3):
+        ctx.load_tracks(k, pop[k])
+    counts = ctx.step()
+    cnt = ctx.read_counters()
+    rw, lines, slots = cnt["field_rw"], cnt["lines"], cnt["slots"]
+    assert counts["secondaries"].sum() > 100
+    for k in range(3):
+        assert (rw[k, :, 0] == n_in[k]).all()
+        assert (rw[k, :, 1] == counts["live"][k]).all()
+        assert int(lines[k].sum()) == int(rw[k].sum()) == int(slots[k].sum())
+        cur, nxt = slots[k][:cap], slots[k][cap:]       # parity 0 is current before the step
+        assert (cur[:n_in[k]] == 14).all() and (cur[n_in[k]:] == 0).all()
+        assert (nxt[:counts["live"][k]] == 14).all() and (nxt[counts["live"][k]:] == 0).all()
+        # heatmap rows: every 128-byte line of the used part of the current buffer was touched
+        from paper_2302_08252_b200 import LAYOUTS as LAY, field_offset
+        touched = {field_offset(LAY[layout], cap, s, f) // 128 for s in (0, n_in[k] - 1) for f in range(14)}
+        assert all(lines[k][t] > 0 for t in touched)
+    ctx.destroy()
+
+
+def test_instrumented_sparse_writes_only_what_changed():
+    """Sparse single buffer: 14 reads per step; in-place write-back of changed words only -- ids are
+    written for new tracks only, and no field is written more often than twice per live track
+    (once by each half of the step) plus once per secondary."""
+    c = CONFIGS["single_step"]
+    geo, tab = geometry_for("single_step"), tables_for("single_step")
+    pop = gen_tracks(5000, c["seed"], geo, c["e_max"], c["fractions"])
+    for k in range(3):
+        pop[k]["nial"][::4] = 1e-30
+    ctx = _ctx(geo, tab, layout="soa", scheme="sparse", capacity=16384, seed=3, instrument=True)
+    n_in = [p.shape[0] for p in pop]
+    for k in range(3):
+        ctx.load_tracks(k, pop[k])
+    counts = ctx.step()
+    rw = ctx.read_counters()["field_rw"]
+    ID_LO, ID_HI, STEP, EKIN = 11, 12, 13, 6
+    for k in range(3):
+        assert (rw[k, :, 0] == n_in[k]).all()
+        born = int(counts["secondaries"][k])
+        assert rw[k, ID_LO, 1] == born and rw[k, ID_HI, 1] == born
+        survivors = int(counts["live"][k]) - born
+        assert rw[k, STEP, 1] >= survivors + born          # every survivor's step counter changed
+        assert (rw[k, :, 1] <= 2 * n_in[k] + born).all()
+    assert rw[2, EKIN, 1] < rw[2, STEP, 1]                  # photons rarely change energy (PAPER.md:133)
+    assert rw[0, EKIN, 1] >= int(counts["live"][0]) - int(counts["secondaries"][0])   # electrons always do
+    ctx.destroy()
