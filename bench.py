@@ -301,6 +301,140 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
         dist.destroy_process_group()
 
 
+def run_showers(args, name: str):
+    """--workload tiny|full|heavy (BASELINE.json configs[0], [1], [4]): inject + adept_run to
+    completion; a "step" is one whole run.  These runs are launch-latency bound for most of their
+    iterations, so no roofline fraction is claimed for them."""
+    import torch
+    from paper_2302_08252_b200 import Context
+    from workloads import gen_primaries
+    c = CONFIGS[name]
+    geo, tab = geometry_for(name), tables_for(name)
+    prim = gen_primaries(c["n_primaries"], c["e_primary"])
+    layout = "aosoa32" if args.layout == "all" else args.layout
+    ctx = Context(geo, tab, layout=layout, scheme=args.scheme, capacity=c["capacity"], seed=c["seed"],
+                  batch_primaries=args.batch)
+    sampler = ClockSampler(0)
+    sampler.start()
+    times, res = [], None
+    for it in range(args.warmup + args.steps):
+        ctx.reset()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        ctx.inject(prim)                      # host primaries -> device (H2D inside the timed region)
+        res = ctx.run()                       # returns the tallies (D2H inside the timed region)
+        dt = time.perf_counter() - t0
+        if it >= args.warmup:
+            times.append(dt)
+    clocks = sampler.stop()
+    ctx.destroy()
+    steps = int(res["steps"].sum())
+    t = float(np.mean(times))
+    out = {"metric": "track-steps/sec", "value": steps / t, "unit": "track-steps/s", "n_gpus": 1,
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t, "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+           "config": {"workload": "%s showers (BASELINE.json): %d x %g MeV e-, %d layers, adept_inject + adept_run "
+                                  "to completion, wall clock around the two calls" % (name, c["n_primaries"], c["e_primary"], c["n_layers"]),
+                      "layout": layout, "scheme": args.scheme, "capacity_per_kind": c["capacity"],
+                      "batch_primaries": args.batch},
+           "clocks": clocks, "gpu_launches": int(res["iterations"]),
+           "showers_per_s": c["n_primaries"] / t, "track_steps": steps, "iterations": int(res["iterations"]),
+           "secondaries": [int(x) for x in res["secondaries"]], "slots_used": [int(x) for x in res["slots_used"]],
+           "edep_layer_MeV": [float(x) for x in res["edep_layer"]],
+           "energy_balance_rel": float((res["edep_slab"].sum() + res["e_escaped"]) / res["e_injected"] - 1.0),
+           "e2e": {"value": steps / t, "unit": "track-steps/s", "h2d_bytes_per_step": 32 * c["n_primaries"],
+                   "d2h_bytes_per_step": 256 + 8 * (2 * c["n_layers"] + 1),
+                   "what": "same measurement: the timed region is the public API with host buffers"},
+           "roofline": None}
+    if not args.no_cpu and name != "heavy":
+        from oracle import Oracle
+        o = Oracle(geo, tab, seed=c["seed"])
+        o.inject(prim)
+        t0 = time.perf_counter()
+        o.run()
+        dt = time.perf_counter() - t0
+        r = o.result()
+        out["cpu_baseline"] = {"value": int(r["steps"].sum()) / dt, "unit": "track-steps/s", "cores": 1,
+                               "kind": "oracle", "sample": "the whole %s workload" % name, "seconds": dt}
+        keys = ("steps", "secondaries", "killed", "escaped_n")
+        out["parity_full_size"] = {
+            "counts_bit_exact": bool(all((res[k] == r[k]).all() for k in keys) and res["iterations"] == r["iterations"]),
+            "edep_layer_rel_err": float(np.max(np.abs(res["edep_layer"] - r["edep_layer"]) / np.maximum(r["edep_layer"], 1e-30)))}
+    print(json.dumps(out))
+
+
+def run_sweep(args):
+    """--workload sweep (BASELINE.json configs[3]): 4 Mi slots per kind, occupancy 10..90 %, both
+    schemes x three layouts.  Per cell: time of one adept_step (CUDA events, state restored and L2
+    flushed between repetitions; slot allocation / compaction is fused into the step kernel, so it is
+    part of this time), and from an instrumented context of the same population the per-field
+    read/write counts and the slots / 128-byte lines touched."""
+    import torch
+    from paper_2302_08252_b200 import Context, FIELD_NAMES
+    from workloads import gen_sweep
+    c = CONFIGS["sweep"]
+    geo, tab = geometry_for("sweep"), tables_for("sweep")
+    span, cap = c["span"], c["span"] + c["reserve"]
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    layouts = ["aos", "soa", "aosoa32"] if args.layout == "all" else [args.layout]
+    cells = []
+    for occ in c["occupancies"]:
+        pop = gen_sweep(occ)
+        n_live = sum(p["tracks"].shape[0] for p in pop)
+        for scheme in ("dense", "sparse"):
+            for layout in layouts:
+                cell = {"occupancy": occ, "scheme": scheme, "layout": layout, "tracks": n_live}
+                for instrument in (False, True):
+                    ctx = Context(geo, tab, layout=layout, scheme=scheme, capacity=cap, seed=c["seed"],
+                                  instrument=instrument)
+                    for k in range(3):
+                        ctx.load_tracks(k, pop[k]["tracks"], pop[k]["slots"] if scheme == "sparse" else None)
+                    torch.cuda.synchronize()
+                    if not instrument:
+                        pristine = ctx.workspace.clone()
+                        ms = []
+                        for it in range(args.warmup + args.steps):
+                            ctx.workspace.copy_(pristine)
+                            flush.zero_()
+                            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                            e0.record(ctx.stream)
+                            ctx.step(sync=False)
+                            e1.record(ctx.stream)
+                            torch.cuda.synchronize()
+                            if it >= args.warmup:
+                                ms.append(e0.elapsed_time(e1))
+                        res = ctx.result()
+                        del pristine
+                        cell.update(ms_per_step=float(np.mean(ms)), ms_min=float(np.min(ms)),
+                                    track_steps_per_s=n_live / (float(np.mean(ms)) * 1e-3),
+                                    secondaries=[int(x) for x in res["secondaries"]],
+                                    slots_used=[int(x) for x in res["slots_used"]])
+                    else:
+                        ctx.step()
+                        cnt = ctx.read_counters()
+                        rw = cnt["field_rw"].sum(axis=0)                    # over kinds -> [14][2]
+                        cell.update(field_reads={n: int(v) for n, v in zip(FIELD_NAMES, rw[:, 0])},
+                                    field_writes={n: int(v) for n, v in zip(FIELD_NAMES, rw[:, 1])},
+                                    lines_touched=int((cnt["lines"] > 0).sum()),
+                                    slots_touched=int((cnt["slots"] > 0).sum()),
+                                    bytes_touched_per_track_step=128.0 * float((cnt["lines"] > 0).sum()) / n_live)
+                    ctx.destroy()
+                    del ctx
+                    torch.cuda.empty_cache()
+                cells.append(cell)
+                sys.stderr.write("%s\n" % json.dumps({k: cell[k] for k in ("occupancy", "scheme", "layout", "ms_per_step",
+                                                                            "bytes_touched_per_track_step")}))
+    best = max(cells, key=lambda x: x["track_steps_per_s"])
+    print(json.dumps({"metric": "track-steps/sec", "value": best["track_steps_per_s"], "unit": "track-steps/s",
+                      "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": best["ms_per_step"],
+                      "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+                      "data": "synthetic",
+                      "config": {"workload": "buffer-scheme sweep (BASELINE.json configs[3]): %d slots per kind, "
+                                             "5 %% of live tracks spawn one secondary; value = best cell" % span,
+                                 "layout": best["layout"], "scheme": best["scheme"], "occupancy": best["occupancy"]},
+                      "gpu_launches": args.steps, "roofline": None, "cells": cells}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -310,6 +444,10 @@ def main():
     ap.add_argument("--layout", default="all", choices=["soa", "aosoa32", "aos", "all"])
     ap.add_argument("--tracks", type=int, default=CONFIGS[WORKLOAD]["n_tracks"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--workload", default="single_step", choices=["single_step", "tiny", "full", "heavy", "sweep"],
+                    help="single_step = the headline (BASELINE.json configs[2]); the others are reported beside it")
+    ap.add_argument("--scheme", default="dense", choices=["dense", "sparse"], help="shower workloads only")
+    ap.add_argument("--batch", type=int, default=0, help="shower workloads: batch_primaries (0 = all at once)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
     rank = int(os.environ.get("RANK", "0"))
@@ -317,6 +455,14 @@ def main():
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
         run_reference(args, rank)
+        return
+    if args.workload in ("tiny", "full", "heavy"):
+        if rank == 0:
+            run_showers(args, args.workload)
+        return
+    if args.workload == "sweep":
+        if rank == 0:
+            run_sweep(args)
         return
     run_gpu(args, rank, world, local_rank)
 
