@@ -34,7 +34,10 @@ if ROOT not in sys.path:
 from workloads import CONFIGS, gen_tracks, geometry_for, tables_for  # noqa: E402
 
 WORKLOAD = "single_step"
-RECORD_BYTES = {"aos": 64, "soa": 56, "aosoa32": 56}     # DESIGN.md §5: bytes per record per layout
+RECORD_BYTES = {"aos": 64, "soa": 56, "aosoa32": 56}     # DESIGN.md §6: bytes per record per layout
+# dram__bytes_read.sum + dram__bytes_write.sum of one step_kernel launch on this workload, from the
+# `ncu --set full` captures summarised in profiles/r1_step_kernel.md (r1e: AoSoA-32, r1d: SoA)
+NCU_TRAFFIC_BYTES = {"aosoa32": 947.1e6 + 1053.5e6, "soa": 957.0e6 + 1067.9e6, "aos": None}
 
 
 def measured_peak():
@@ -282,7 +285,10 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
                 "d2h_bytes_per_step": d2h + 256, "steps": e2e_steps,
                 "what": "adept_load_tracks x3 (pinned host) + adept_step + adept_read_tracks x3"},
         "roofline": {"bound": "hbm", "achieved": m["algorithmic_GBps"], "peak": peak, "unit": "GB/s",
-                     "frac": m["algorithmic_GBps"] / peak, "traffic": None, "peak_source": peak_src,
+                     "frac": m["algorithmic_GBps"] / peak,
+                     "traffic": NCU_TRAFFIC_BYTES[main] if n_tracks == CONFIGS[WORKLOAD]["n_tracks"] else None,
+                     "traffic_source": "profiles/r1_step_kernel.md (ncu --set full, bytes per launch)",
+                     "peak_source": peak_src,
                      "kernel": "adept::step_kernel<%s, dense>" % main,
                      "bytes_per_launch": m["algorithmic_bytes_per_launch"]},
         "layouts": per_layout,
