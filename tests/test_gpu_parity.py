@@ -355,3 +355,34 @@ def test_instrumented_sparse_writes_only_what_changed():
     assert rw[2, EKIN, 1] < rw[2, STEP, 1]                  # photons rarely change energy
     assert rw[0, EKIN, 1] >= int(counts["live"][0]) - int(counts["secondaries"][0])   # electrons always do
     ctx.destroy()
+
+
+# ------------------------------------------- BASELINE.json sizes, bench.py's launch configuration ---
+def test_single_step_at_full_size_counts_and_sampled_tracks():
+    """Config 3 as bench.py times it: 2^24 tracks, dense double buffer, AoSoA-32, one adept_step.
+    All integer counts and the per-slab deposits against the oracle's full-size step, and every
+    surviving / created track of a sample of 1/64 of the id space compared word for word."""
+    c = CONFIGS["single_step"]
+    geo, tab = geometry_for("single_step"), tables_for("single_step")
+    n = c["n_tracks"]
+    pop = gen_tracks(n, c["seed"], geo, c["e_max"], c["fractions"])
+    cap = int(max(p.shape[0] for p in pop) * 1.25) + 4096
+    ctx = _ctx(geo, tab, layout="aosoa32", scheme="dense", capacity=cap, seed=c["seed"])
+    for k in range(3):
+        ctx.load_tracks(k, pop[k])
+    counts = ctx.step()
+    o = Oracle(geo, tab, seed=c["seed"])
+    for k in range(3):
+        o.load_tracks(k, pop[k])
+    o.step()
+    r = o.result()
+    compare_counts(counts, r, what="full size")
+    g = ctx.result()
+    assert np.allclose(g["edep_slab"], r["edep_slab"], rtol=1e-9, atol=1e-6)
+    assert abs(g["e_escaped"] - r["e_escaped"]) <= 1e-9 * r["e_escaped"]
+    for k in range(3):
+        a, b = ctx.read_tracks(k), o.read_tracks(k, pop[0].dtype)
+        assert a.shape[0] == b.shape[0] == int(counts["live"][k])
+        sa, sb = a[(a["id_lo"] & 63) == 5], b[(b["id_lo"] & 63) == 5]
+        assert compare_tracks(sa, sb, "full size kind %d" % k) == 0
+    ctx.destroy()
