@@ -50,8 +50,9 @@ typedef enum {
   ADEPT_ESTATE = -4     /* call not allowed in the context's current state */
 } adept_status;
 
-/* Record layout in device memory ("AoS", "SoA", "AoSoA-n", n = 32 lanes). */
-typedef enum { ADEPT_AOS = 0, ADEPT_SOA = 1, ADEPT_AOSOA32 = 2 } adept_layout;
+/* Record layout in device memory ("AoS", "SoA", "AoSoA-n" with n = 32 or 64
+ * lanes; AoSoA64 on the dense double buffer was the paper's fastest variant). */
+typedef enum { ADEPT_AOS = 0, ADEPT_SOA = 1, ADEPT_AOSOA32 = 2, ADEPT_AOSOA64 = 3 } adept_layout;
 /* Track container (PAPER.md:29 / PAPER.md:31). */
 typedef enum { ADEPT_SPARSE_SINGLE = 0, ADEPT_DENSE_DOUBLE = 1 } adept_scheme;
 

@@ -34,7 +34,7 @@ struct Plan {  // carve-up of the workspace
   size_t rec[3], queue[3][2];
   size_t instr_rw, instr_lines[3], instr_slots[3];
   size_t total;
-  uint32_t capacity;       // rounded up to a multiple of 32
+  uint32_t capacity;       // rounded up to a multiple of 128 (one tile)
   uint32_t stage_records;
   size_t table_bytes;
   size_t rec_words;        // words of ONE record buffer
@@ -47,6 +47,7 @@ static const LayoutOps *ops_for(int layout) {
     case ADEPT_AOS: return &kOpsAoS;
     case ADEPT_SOA: return &kOpsSoA;
     case ADEPT_AOSOA32: return &kOpsAoSoA32;
+    case ADEPT_AOSOA64: return &kOpsAoSoA64;
     default: return nullptr;
   }
 }
@@ -59,7 +60,7 @@ static bool make_plan(const adept_geometry *g, const adept_tables *t, const adep
   if (g->n_layers == 0 || g->n_layers > 2048) return false;
   if (t->n_bins == 0 || t->n_bins > 4096 || t->n_materials == 0 || t->n_materials > 8) return false;
   if (c->capacity_per_kind == 0 || c->capacity_per_kind > (1u << 30)) return false;
-  pl.capacity = (c->capacity_per_kind + 31u) / 32u * 32u;
+  pl.capacity = (c->capacity_per_kind + 127u) / 128u * 128u;
   pl.nbuf = (c->scheme == ADEPT_DENSE_DOUBLE) ? 2 : 1;
   pl.rec_words = ops->record_words(pl.capacity);
   pl.table_bytes = size_t(t->n_materials) * 2 * (t->n_bins + 1) * sizeof(float4);
@@ -583,12 +584,13 @@ int adept_read_counters(adept_ctx *c, uint64_t *field_rw, uint32_t *lines, uint3
 
 uint64_t adept_field_offset(int32_t layout, uint32_t capacity, uint32_t slot, uint32_t field) {
   if (field >= uint32_t(kNumFields) || capacity == 0) return UINT64_MAX;
-  const size_t cap = (size_t(capacity) + 31) / 32 * 32;
+  const size_t cap = (size_t(capacity) + 127) / 128 * 128;
   if (slot >= cap) return UINT64_MAX;
   switch (layout) {
     case ADEPT_AOS: return 4 * Mapping<L_AOS>::index(cap, slot, int(field));
     case ADEPT_SOA: return 4 * Mapping<L_SOA>::index(cap, slot, int(field));
     case ADEPT_AOSOA32: return 4 * Mapping<L_AOSOA32>::index(cap, slot, int(field));
+    case ADEPT_AOSOA64: return 4 * Mapping<L_AOSOA64>::index(cap, slot, int(field));
     default: return UINT64_MAX;
   }
 }

@@ -87,7 +87,7 @@ struct Params {
   uint32_t n_slabs;
   float abs_mm, pitch, half_xy;
   uint32_t mat_abs, mat_gap;
-  uint32_t capacity;         // slots per kind (multiple of 32)
+  uint32_t capacity;         // slots per kind (multiple of 128)
   KindStorage kind[3];
   unsigned long long *instr_field_rw;  // [3][14][2], instrumented build
 };

@@ -20,7 +20,7 @@ enum Field : int {
   F_PX = 0, F_PY, F_PZ, F_DX, F_DY, F_DZ, F_EKIN, F_N0, F_N1, F_N2, F_VOL, F_IDLO, F_IDHI, F_STEP,
   kNumFields = 14
 };
-enum LayoutId : int { L_AOS = 0, L_SOA = 1, L_AOSOA32 = 2 };
+enum LayoutId : int { L_AOS = 0, L_SOA = 1, L_AOSOA32 = 2, L_AOSOA64 = 3 };
 
 // A track in registers.
 struct Trk {
@@ -67,8 +67,8 @@ __device__ __forceinline__ void trk_set_word(Trk &t, int f, uint32_t w) {
 }
 
 // ---- mappings: (capacity, slot, field) -> word index inside one record buffer ---------------
-// Capacities are multiples of 32 slots, so every SoA field array and every AoSoA block starts on a
-// 128-byte line.
+// Capacities are multiples of 128 slots (one tile), so every SoA field array and every AoSoA block
+// starts on a 128-byte line.
 template <int L> struct Mapping;
 
 template <> struct Mapping<L_AOS> {  // 14 words padded to 16: one record = 64 B = 2 sectors = 4 x 16 B
@@ -80,13 +80,15 @@ template <> struct Mapping<L_SOA> {  // 14 arrays of `cap` words
   __host__ __device__ static constexpr size_t words(size_t cap) { return cap * kNumFields; }
   __host__ __device__ static constexpr size_t index(size_t cap, size_t slot, int f) { return f * cap + slot; }
 };
-template <> struct Mapping<L_AOSOA32> {  // blocks of 32 tracks, field-major inside a block (1792 B)
-  static constexpr int kLanes = 32;
+template <int N> struct AoSoAMapping {  // blocks of N tracks, field-major inside a block (N * 56 B)
+  static constexpr int kLanes = N;
   __host__ __device__ static constexpr size_t words(size_t cap) { return cap * kNumFields; }
   __host__ __device__ static constexpr size_t index(size_t, size_t slot, int f) {
     return (slot / kLanes) * (kLanes * kNumFields) + f * kLanes + (slot % kLanes);
   }
 };
+template <> struct Mapping<L_AOSOA32> : AoSoAMapping<32> {};  // "AoSoA-n"
+template <> struct Mapping<L_AOSOA64> : AoSoAMapping<64> {};  // the paper's fastest
 
 // ---- access counting (instrumented build only) -----------------------------------------------
 // field_rw: shared-memory counters [14][2] of the CTA (flushed once per kernel);

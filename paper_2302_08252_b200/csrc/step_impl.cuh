@@ -98,14 +98,22 @@ __device__ __forceinline__ void prefetch_tile(const uint32_t *rec, uint32_t cap,
   const uint32_t n = (n_kind - first < uint32_t(kGroup)) ? n_kind - first : uint32_t(kGroup);
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic reads of in_buf before async writes
   const uint32_t bar = static_cast<uint32_t>(__cvta_generic_to_shared(mbar));
-  if (L == L_SOA) {
-    const uint32_t bytes = ((n + 3u) / 4u) * 16u;  // slots are padded to a multiple of 32: stays inside the array
+  if constexpr (L == L_SOA) {
+    const uint32_t bytes = ((n + 3u) / 4u) * 16u;  // slots are padded to a multiple of 128: stays inside the array
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes * kNumFields) : "memory");
 #pragma unroll
     for (int f = 0; f < kNumFields; ++f) bulk_g2s(in_buf + f * kGroup, rec + size_t(f) * cap + first, bytes, mbar);
   } else {
-    const uint32_t bytes = (L == L_AOS) ? n * 64u : ((n + 31u) / 32u) * (32u * kNumFields * 4u);
-    const uint32_t *src = rec + ((L == L_AOS) ? size_t(first) * 16 : size_t(first / 32u) * (32 * kNumFields));
+    uint32_t bytes;
+    const uint32_t *src;
+    if constexpr (L == L_AOS) {
+      bytes = n * 64u;
+      src = rec + size_t(first) * 16;
+    } else {  // AoSoA-n: whole blocks
+      constexpr uint32_t kL = Mapping<L>::kLanes;
+      bytes = ((n + kL - 1u) / kL) * (kL * kNumFields * 4u);
+      src = rec + size_t(first / kL) * (kL * kNumFields);
+    }
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
     bulk_g2s(in_buf, src, bytes, mbar);
   }
@@ -738,6 +746,6 @@ template <int L> struct OpsImpl {
   }
 };
 
-extern const LayoutOps kOpsAoS, kOpsSoA, kOpsAoSoA32;
+extern const LayoutOps kOpsAoS, kOpsSoA, kOpsAoSoA32, kOpsAoSoA64;
 
 }  // namespace adept

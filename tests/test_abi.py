@@ -51,8 +51,8 @@ def test_workspace_bytes_is_host_arithmetic(L):
     size = lambda **k: lib.adept_workspace_bytes(*[C.byref(x) for x in _args(L, **k)])
     base = size()
     assert base > 3 * 2 * 4096 * 56                                  # three kinds, two dense arrays
-    assert size(capacity=8192) > base and size(capacity=4097) == size(capacity=4128)   # rounded to 32 slots
-    assert size(layout=0) > size(layout=1) == size(layout=2)         # AoS records are padded to 64 B
+    assert size(capacity=8192) > base and size(capacity=4097) == size(capacity=4224)   # rounded to 128 slots (one tile)
+    assert size(layout=0) > size(layout=1) == size(layout=2) == size(layout=3)   # AoS records are padded to 64 B
     assert size(scheme=0) < base                                     # one slot array + two slot lists
     assert size(instrument=1) > base
     for bad in (dict(layout=7), dict(scheme=5), dict(capacity=0), dict(n_layers=0), dict(n_bins=0)):
@@ -66,11 +66,12 @@ def test_field_offset_follows_the_three_mappings(L):
             assert L.field_offset(L.ADEPT_AOS, cap, slot, f) == 4 * (slot * 16 + f)       # 64-byte records
             assert L.field_offset(L.ADEPT_SOA, cap, slot, f) == 4 * (f * cap + slot)       # 14 arrays
             assert L.field_offset(L.ADEPT_AOSOA32, cap, slot, f) == 4 * ((slot // 32) * 448 + f * 32 + slot % 32)
+            assert L.field_offset(L.ADEPT_AOSOA64, cap, slot, f) == 4 * ((slot // 64) * 896 + f * 64 + slot % 64)
     assert L.field_offset(L.ADEPT_SOA, cap, 0, 14) == 2**64 - 1 and L.field_offset(9, cap, 0, 0) == 2**64 - 1
     # every (slot, field) has its own word in every layout
-    for lay, words in ((L.ADEPT_AOS, 16), (L.ADEPT_SOA, 14), (L.ADEPT_AOSOA32, 14)):
-        offs = {L.field_offset(lay, 64, s, f) for s in range(64) for f in range(14)}
-        assert len(offs) == 64 * 14 and max(offs) < 64 * words * 4
+    for lay, words in ((L.ADEPT_AOS, 16), (L.ADEPT_SOA, 14), (L.ADEPT_AOSOA32, 14), (L.ADEPT_AOSOA64, 14)):
+        offs = {L.field_offset(lay, 128, s, f) for s in range(128) for f in range(14)}
+        assert len(offs) == 128 * 14 and max(offs) < 128 * words * 4
 
 
 def test_create_rejects_bad_arguments_before_touching_the_device(L):

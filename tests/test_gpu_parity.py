@@ -11,7 +11,7 @@ from tests.helpers import make_tracks, sort_by_id
 
 pytestmark = pytest.mark.gpu
 
-LAYOUTS = ("aos", "soa", "aosoa32")
+LAYOUTS = ("aos", "soa", "aosoa32", "aosoa64")
 SCHEMES = ("dense", "sparse")
 INT_FIELDS = ("vol", "id_lo", "id_hi", "step")
 F32_FIELDS = ("pos", "dir", "ekin", "nial")
@@ -172,7 +172,7 @@ def test_tiny_shower_matches_oracle_every_iteration(layout, scheme):
     ctx.destroy()
 
 
-@pytest.mark.parametrize("layout,scheme", [("soa", "dense"), ("aosoa32", "dense"), ("aos", "sparse")])
+@pytest.mark.parametrize("layout,scheme", [("soa", "dense"), ("aosoa32", "dense"), ("aosoa64", "dense"), ("aos", "sparse")])
 def test_full_showers_run_matches_oracle(layout, scheme):
     """Config 2 at reduced primaries (100 x 1 GeV) so that the oracle takes well under a second."""
     c = CONFIGS["full"]
@@ -239,7 +239,7 @@ def test_sweep_population_sparse_slots_and_forced_secondaries(layout):
 def test_edge_cases_empty_overflow_invalid_reset():
     from paper_2302_08252_b200 import AdeptError
     geo, tab = geometry_for("tiny"), tables_for("tiny")
-    ctx = _ctx(geo, tab, layout="soa", scheme="dense", capacity=32, seed=1)
+    ctx = _ctx(geo, tab, layout="soa", scheme="dense", capacity=128, seed=1)
     c = ctx.step()                                   # empty step: nothing happens, not counted
     assert c["live"].sum() == 0 and c["iterations"] == 0 and c["steps"].sum() == 0
     r = ctx.run()
@@ -253,8 +253,8 @@ def test_edge_cases_empty_overflow_invalid_reset():
     bad["pos"][0, 0] = 1e3                           # outside the transverse box
     with pytest.raises(AdeptError):
         ctx.inject(bad)
-    # overflow: 32 x 10 MeV showers need more than 32 slots per kind
-    ctx.inject(gen_primaries(32, 10.0))
+    # overflow: 128 x 10 MeV showers need more than 128 slots per kind
+    ctx.inject(gen_primaries(128, 10.0))
     with pytest.raises(AdeptError) as e:
         ctx.run()
     assert e.value.code == -2
