@@ -10,6 +10,8 @@
 #include <cstddef>
 #include <cstdint>
 
+#include <cuda.h>  // CUtensorMap
+
 namespace adept {
 
 enum SchemeId : int { S_SPARSE = 0, S_DENSE = 1 };
@@ -40,8 +42,12 @@ __host__ __device__ constexpr size_t in_buf_bytes(int scheme, size_t tile_words)
 // fixed-point sum kept as two 32-bit limbs, [lo limbs][hi limbs].
 __host__ __device__ constexpr size_t bins_bytes(uint32_t n_slabs) { return ((size_t(n_slabs) + 1) * 8 + 15) / 16 * 16; }
 // Dynamic shared memory of the step kernel: [tables of one particle group][bins][per group: staged tile, queue]
+// (the per-group part starts on a 128-byte boundary: what a tiled TMA copy needs of its destination)
+__host__ __device__ constexpr size_t units_offset(size_t table_bytes, uint32_t n_slabs) {
+  return (table_bytes + bins_bytes(n_slabs) + 127) / 128 * 128;
+}
 __host__ __device__ constexpr size_t step_smem_bytes(int scheme, size_t table_bytes, uint32_t n_slabs, size_t tile_words) {
-  return table_bytes + bins_bytes(n_slabs) + size_t(kGroupsPerCta) * (in_buf_bytes(scheme, tile_words) + queue_bytes(scheme));
+  return units_offset(table_bytes, n_slabs) + size_t(kGroupsPerCta) * (in_buf_bytes(scheme, tile_words) + queue_bytes(scheme));
 }
 
 // Energy tallies (rule M7: sums of fp32 terms) are accumulated in 64-bit fixed point, unit
@@ -90,6 +96,8 @@ struct Params {
   uint32_t capacity;         // slots per kind (multiple of 128)
   KindStorage kind[3];
   unsigned long long *instr_field_rw;  // [3][14][2], instrumented build
+  // SoA layout, dense scheme: tensor maps of the record buffers, [kind][parity] (see prefetch_tile)
+  alignas(64) CUtensorMap soa_tile[3][2];
 };
 
 }  // namespace adept

@@ -92,17 +92,26 @@ __device__ __forceinline__ uint32_t arrive_acq_rel(uint32_t *counter) {
 
 // Called by ONE thread, after every warp of the group has taken its records out of `in_buf`.
 template <int L>
-__device__ __forceinline__ void prefetch_tile(const uint32_t *rec, uint32_t cap, uint32_t tile, uint32_t n_kind,
+__device__ __forceinline__ void prefetch_tile(const Params &p, int kind, uint32_t par, uint32_t tile, uint32_t n_kind,
                                               uint32_t *in_buf, uint64_t *mbar) {
+  const uint32_t *rec = p.kind[kind].rec[par];
   const uint32_t first = tile * kGroup;
   const uint32_t n = (n_kind - first < uint32_t(kGroup)) ? n_kind - first : uint32_t(kGroup);
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic reads of in_buf before async writes
   const uint32_t bar = static_cast<uint32_t>(__cvta_generic_to_shared(mbar));
   if constexpr (L == L_SOA) {
-    const uint32_t bytes = ((n + 3u) / 4u) * 16u;  // slots are padded to a multiple of 128: stays inside the array
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes * kNumFields) : "memory");
-#pragma unroll
-    for (int f = 0; f < kNumFields; ++f) bulk_g2s(in_buf + f * kGroup, rec + size_t(f) * cap + first, bytes, mbar);
+    // The SoA buffer is a 2-D tensor [14 fields][capacity slots]; a tile is the box [14][kGroup] of
+    // it: ONE tiled TMA copy through the tensor map of this kind's buffer (encoded at adept_create),
+    // landing field-major in shared memory -- the SoA mapping with capacity kGroup.  Slots are padded
+    // to whole tiles, so the box of a ragged last tile stays inside the tensor.
+    (void)rec; (void)n;
+    constexpr uint32_t bytes = uint32_t(kGroup) * kNumFields * 4u;
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(
+            static_cast<uint32_t>(__cvta_generic_to_shared(in_buf))),
+        "l"(reinterpret_cast<uint64_t>(&p.soa_tile[kind][par])), "r"(first), "r"(0u), "r"(bar)
+        : "memory");
   } else {
     uint32_t bytes;
     const uint32_t *src;
@@ -280,7 +289,7 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
     if (lane == 0) {
       const uint32_t arrived = arrive_acq_rel(&g.loaded);
       if ((arrived % uint32_t(kWarpsPerGroup)) == uint32_t(kWarpsPerGroup - 1) && next_tile != 0xFFFFFFFFu)
-        prefetch_tile<L>(p.kind[KIND].rec[par], p.capacity, next_tile, n_kind, c.in_buf, &g.mbar_in);
+        prefetch_tile<L>(p, KIND, par, next_tile, n_kind, c.in_buf, &g.mbar_in);
     }
   }
   if (active) {
@@ -488,7 +497,7 @@ __device__ __forceinline__ void run_kind(const Params &p, const Env &env, const 
   const uint32_t me = blockIdx.x * kGroupsPerCta + c.group;
   const uint32_t shift = (me + n_groups - first_global_tile % n_groups) % n_groups;
   if (SCHEME == S_DENSE && shift < n_tiles && c.gtid == 0)  // the staging buffer is free: its last reader passed a barrier
-    prefetch_tile<L>(p.kind[KIND].rec[par], p.capacity, shift, n_kind, c.in_buf, &c.g->mbar_in);
+    prefetch_tile<L>(p, KIND, par, shift, n_kind, c.in_buf, &c.g->mbar_in);
   uint32_t queued = 0u;
   for (uint32_t tile = shift; tile < n_tiles; tile += n_groups) {
     const uint32_t next_tile = (tile + n_groups < n_tiles) ? tile + n_groups : 0xFFFFFFFFu;
@@ -512,7 +521,7 @@ __device__ __forceinline__ void run_kind(const Params &p, const Env &env, const 
 #endif
 template <int L, int SCHEME, bool INSTR>
 __global__ void __launch_bounds__(kBlock, ADEPT_STEP_MIN_CTAS) step_kernel(const __grid_constant__ Params p) {
-  extern __shared__ __align__(16) unsigned char dyn_smem[];
+  extern __shared__ __align__(128) unsigned char dyn_smem[];
   __shared__ CtaShared sh;
   float4 *s_tab = reinterpret_cast<float4 *>(dyn_smem);
   const int tid = threadIdx.x;
@@ -526,7 +535,7 @@ __global__ void __launch_bounds__(kBlock, ADEPT_STEP_MIN_CTAS) step_kernel(const
   c.g = &sh.grp[c.group];
   c.bins.lo = reinterpret_cast<uint32_t *>(dyn_smem + p.table_bytes);
   c.bins.hi = c.bins.lo + (p.n_slabs + 1u);
-  unsigned char *mine = dyn_smem + p.table_bytes + bins_bytes(p.n_slabs) + size_t(c.group) * kPerGroup;
+  unsigned char *mine = dyn_smem + units_offset(p.table_bytes, p.n_slabs) + size_t(c.group) * kPerGroup;
   c.in_buf = reinterpret_cast<uint32_t *>(mine);
   c.queue = reinterpret_cast<uint32_t *>(mine + kInBuf);
 
