@@ -79,7 +79,8 @@ typedef struct {
 typedef struct {
   int32_t layout;             /* adept_layout */
   int32_t scheme;             /* adept_scheme */
-  uint32_t capacity_per_kind; /* slots per particle kind (dense: per buffer), 1 .. 2^30 */
+  uint32_t capacity_per_kind; /* slots per particle kind (dense: per buffer), 1 .. 2^30; rounded up to a
+                               * multiple of 128 (one tile) */
   uint32_t batch_primaries;   /* adept_run: 0 = inject everything at once, else batch size */
   uint64_t seed;              /* primary ids, rule R4 */
   void *workspace;            /* device, 256-byte aligned, >= adept_workspace_bytes() */
@@ -111,6 +112,9 @@ typedef struct {
   uint32_t reserved;
 } adept_counts;
 
+/* Energies are accumulated on the device in 64-bit fixed point of unit 2^-32 MeV (every fp32 term
+ * rounded to the unit once, then exact, order-independent integer sums; range 2^32 MeV per slab) and
+ * converted to double here (DESIGN.md §3 reading 33). */
 typedef struct {
   adept_counts total;
   double e_injected; /* sum of primary kinetic energies (+ 2 mc^2 per e+), MeV */
