@@ -386,3 +386,40 @@ def test_single_step_at_full_size_counts_and_sampled_tracks():
         sa, sb = a[(a["id_lo"] & 63) == 5], b[(b["id_lo"] & 63) == 5]
         assert compare_tracks(sa, sb, "full size kind %d" % k) == 0
     ctx.destroy()
+
+
+# ------------------------------------------------------------------ ragged and empty inputs ---
+@pytest.mark.parametrize("scheme", SCHEMES)
+@pytest.mark.parametrize("layout", LAYOUTS)
+def test_ragged_tile_sizes_and_empty_kinds(layout, scheme):
+    """Populations around the tile (128) and warp (32) boundaries, kinds with no track at all, every
+    track forced to interact (the parked queue runs full): two steps each, compared per track."""
+    c = CONFIGS["single_step"]
+    geo, tab = geometry_for("single_step"), tables_for("single_step")
+    rng = np.random.default_rng(77)
+    cases = [(1, 0, 0), (0, 1, 0), (0, 0, 1), (31, 33, 32), (127, 129, 128), (255, 0, 257), (0, 385, 1), (640, 3, 1000)]
+    for ci, sizes in enumerate(cases):
+        n = sum(sizes)
+        fr = tuple(s / n for s in sizes)
+        pop = gen_tracks(n, 100 + ci, geo, c["e_max"], fr)
+        assert tuple(p.shape[0] for p in pop) == sizes, (sizes, [p.shape[0] for p in pop])
+        for k in range(3):
+            if ci % 2 == 1 and pop[k].shape[0]:
+                pop[k]["nial"][:, :] = np.float32(1e-30)          # every track interacts this step
+            if k == 1 and pop[k].shape[0]:
+                pop[k]["ekin"][rng.random(pop[k].shape[0]) < 0.3] = np.float32(0.05)   # e+ at rest
+        o = Oracle(geo, tab, seed=5)
+        ctx = _ctx(geo, tab, layout=layout, scheme=scheme, capacity=4096, seed=5)
+        for k in range(3):
+            if pop[k].shape[0]:
+                o.load_tracks(k, pop[k])
+                ctx.load_tracks(k, pop[k])
+        for it in range(2):
+            o.step()
+            counts = ctx.step()
+            compare_counts(counts, o.result(), what="%s/%s case %d step %d" % (layout, scheme, ci, it))
+            for k in range(3):
+                assert compare_tracks(ctx.read_tracks(k), o.read_tracks(k, pop[0].dtype), "case %d kind %d" % (ci, k)) == 0
+        g, r = ctx.result(), o.result()
+        assert np.allclose(g["edep_slab"], r["edep_slab"], rtol=1e-9, atol=1e-7)
+        ctx.destroy()
