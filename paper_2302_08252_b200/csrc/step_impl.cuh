@@ -474,6 +474,14 @@ template <int L, int SCHEME, bool INSTR, int KIND>
 __device__ __forceinline__ void run_kind(const Params &p, const Env &env, const GroupRefs &c, uint32_t par,
                                          uint32_t first_global_tile, uint32_t n_tiles, uint32_t n_kind, int &sbuf,
                                          uint32_t &in_phase, uint32_t &tab_phase, int &staged_group) {
+  // tiles are dealt round-robin over all groups of the grid, continuing across the kinds
+  const uint32_t n_groups = gridDim.x * kGroupsPerCta;
+  const uint32_t me = blockIdx.x * kGroupsPerCta + c.group;
+  const uint32_t shift = (me + n_groups - first_global_tile % n_groups) % n_groups;
+  // the group's first tile of this kind is requested before the tables are: the two copies overlap
+  // (small populations -- the head and tail of a shower -- are latency-bound, one tile per group)
+  if (SCHEME == S_DENSE && shift < n_tiles && c.gtid == 0)  // the staging buffer is free: its last reader passed a barrier
+    prefetch_tile<L>(p, KIND, par, shift, n_kind, c.in_buf, &c.g->mbar_in);
   // A3: the cross-section tables of this kind's particle group -> shared memory, one TMA bulk copy
   // (e- and e+ share a group).  CTA-wide: every group is done with the previous tables.
   constexpr int group = (KIND == K_GAMMA) ? 0 : 1;
@@ -492,12 +500,6 @@ __device__ __forceinline__ void run_kind(const Params &p, const Env &env, const 
     tab_phase ^= 1u;
     staged_group = group;
   }
-  // tiles are dealt round-robin over all groups of the grid, continuing across the kinds
-  const uint32_t n_groups = gridDim.x * kGroupsPerCta;
-  const uint32_t me = blockIdx.x * kGroupsPerCta + c.group;
-  const uint32_t shift = (me + n_groups - first_global_tile % n_groups) % n_groups;
-  if (SCHEME == S_DENSE && shift < n_tiles && c.gtid == 0)  // the staging buffer is free: its last reader passed a barrier
-    prefetch_tile<L>(p, KIND, par, shift, n_kind, c.in_buf, &c.g->mbar_in);
   uint32_t queued = 0u;
   for (uint32_t tile = shift; tile < n_tiles; tile += n_groups) {
     const uint32_t next_tile = (tile + n_groups < n_tiles) ? tile + n_groups : 0xFFFFFFFFu;
