@@ -36,8 +36,8 @@ from workloads import CONFIGS, gen_tracks, geometry_for, tables_for  # noqa: E40
 WORKLOAD = "single_step"
 RECORD_BYTES = {"aos": 64, "soa": 56, "aosoa32": 56, "aosoa64": 56}     # bytes per record per layout
 # dram__bytes_read.sum + dram__bytes_write.sum of one step_kernel launch on this workload, from the
-# `ncu --set full` captures summarised in profiles/r1_step_kernel.md (r1e: AoSoA-32)
-NCU_TRAFFIC_BYTES = {"aosoa32": 947.1e6 + 1053.5e6, "soa": None, "aos": None,
+# `ncu --set full` captures summarised in profiles/r1_step_kernel.md (r1f: AoSoA-32)
+NCU_TRAFFIC_BYTES = {"aosoa32": 942.4e6 + 1044.4e6, "soa": None, "aos": None,
                      "aosoa64": None}
 
 
@@ -290,7 +290,7 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
                      "traffic": NCU_TRAFFIC_BYTES[main] if n_tracks == CONFIGS[WORKLOAD]["n_tracks"] else None,
                      "traffic_source": "profiles/r1_step_kernel.md (ncu --set full, bytes per launch)",
                      "peak_source": peak_src,
-                     "kernel": "adept::step_kernel<%s, dense>" % main,
+                     "kernel": "adept::step_kernel<%s, dense, 1024 threads>" % main,
                      "bytes_per_launch": m["algorithmic_bytes_per_launch"]},
         "layouts": per_layout,
     }

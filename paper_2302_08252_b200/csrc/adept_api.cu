@@ -105,8 +105,8 @@ struct adept_ctx {
   const LayoutOps *ops;
   Params params;
   cudaStream_t stream;
-  unsigned grid;
-  size_t dyn_smem;
+  struct Shape { int threads; unsigned grid; size_t dyn_smem; } small, large;  // CTA shapes of the step kernel
+  uint64_t live_hint;     // live tracks as last seen by the host: picks the shape
   unsigned char *ws;
   unsigned char *pinned;  // kCtlHeaderBytes + tallies
   size_t pinned_bytes;
@@ -141,6 +141,7 @@ int fetch_ctl(adept_ctx *c, bool with_edep) {
   const size_t n = with_edep ? c->pinned_bytes : kCtlHeaderBytes;
   CU(c, cudaMemcpyAsync(c->pinned, c->ws + c->plan.ctl, n, cudaMemcpyDeviceToHost, c->stream));
   CU(c, cudaStreamSynchronize(c->stream));
+  c->live_hint = uint64_t(host_ctl(c)->n_cur[0]) + host_ctl(c)->n_cur[1] + host_ctl(c)->n_cur[2];
   if (host_ctl(c)->overflow) {
     c->dead = true;
     return fail(c, ADEPT_ECAPACITY, "track buffer capacity exceeded");
@@ -232,6 +233,7 @@ static int clear_state(adept_ctx *c) {
   c->pending_done = 0;
   c->next_primary = 0;
   c->e_injected = 0.0;
+  c->live_hint = 0;
   c->dead = false;
   return ADEPT_OK;
 }
@@ -329,20 +331,30 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
       }
   }
 
-  // persistent grid: as many CTAs as fit on the device at once
-  c->dyn_smem = step_smem_bytes(cfg->scheme, pl.table_bytes / 2, p.n_slabs, c->ops->record_words(kGroup));
+  // persistent grids: as many CTAs as fit on the device at once, for both CTA shapes of the step
+  // kernel (device_state.cuh); the large shape is optional (huge tables may not leave room for it)
   int dev = 0, sms = 0;
   if ((e = cudaGetDevice(&dev)) != cudaSuccess) return die("cudaGetDevice", e);
   if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess)
     return die("cudaDeviceGetAttribute", e);
-  const int per_sm = c->ops->step_ctas_per_sm(cfg->scheme, cfg->instrument ? 1 : 0, c->dyn_smem);
+  const int instr = cfg->instrument ? 1 : 0;
+  const size_t tile_words = c->ops->record_words(kGroup);
+  c->small.threads = kBlockSmall;
+  c->small.dyn_smem = step_smem_bytes(cfg->scheme, pl.table_bytes / 2, p.n_slabs, tile_words, kBlockSmall);
+  const int per_sm = c->ops->step_ctas_per_sm(cfg->scheme, instr, kBlockSmall, c->small.dyn_smem);
   if (per_sm <= 0) {
     g_create_error = "step kernel does not fit on an SM with these tables (shared memory)";
     cudaFreeHost(c->pinned);
     delete c;
     return ADEPT_EINVAL;
   }
-  c->grid = static_cast<unsigned>(sms * per_sm);
+  c->small.grid = static_cast<unsigned>(sms * per_sm);
+  c->large.threads = kBlockLarge;
+  c->large.dyn_smem = step_smem_bytes(cfg->scheme, pl.table_bytes / 2, p.n_slabs, tile_words, kBlockLarge);
+  const int per_sm_large = c->ops->step_ctas_per_sm(cfg->scheme, instr, kBlockLarge, c->large.dyn_smem);
+  cudaGetLastError();  // a failed attribute query of the optional shape is not an error of the context
+  c->large.grid = per_sm_large > 0 ? static_cast<unsigned>(sms * per_sm_large) : 0u;
+  c->live_hint = 0;
 
   int rc = clear_state(c);
   if (rc == ADEPT_OK && (e = cudaStreamSynchronize(c->stream)) != cudaSuccess) rc = ADEPT_ECUDA;
@@ -443,6 +455,7 @@ static int inject_now(adept_ctx *c, const adept_primary *prim, uint64_t n) {
   for (uint64_t i = 0; i < n; ++i)
     c->e_injected += double(prim[i].ekin) + (prim[i].kind == 1u ? double(2.0f * kMc2) : 0.0);
   c->next_primary += n;
+  c->live_hint += n;
   return ADEPT_OK;
 }
 
@@ -497,6 +510,7 @@ int adept_load_tracks(adept_ctx *c, uint32_t kind, const adept_track *tracks, ui
     done += m;
   }
   if (sparse && !slots) top = next_slot;
+  c->live_hint += n;
   set_counts_kernel<<<1, 1, 0, c->stream>>>(c->params.ctl, int(kind), n_cur, top, sparse ? top : n_cur);
   CU(c, cudaGetLastError());
   return ADEPT_OK;
@@ -522,8 +536,13 @@ int adept_read_tracks(adept_ctx *c, uint32_t kind, adept_track *out, uint64_t ca
 }
 
 // ---- iterations -----------------------------------------------------------------------------
+#ifndef ADEPT_LARGE_SHAPE_MIN_TRACKS
+#define ADEPT_LARGE_SHAPE_MIN_TRACKS (1u << 22)
+#endif
 static int launch_iteration(adept_ctx *c) {
-  CU(c, c->ops->launch_step(c->cfg.scheme, c->cfg.instrument ? 1 : 0, c->params, c->grid, c->dyn_smem, c->stream));
+  const adept_ctx::Shape &sh = (c->large.grid != 0u && c->live_hint >= ADEPT_LARGE_SHAPE_MIN_TRACKS) ? c->large : c->small;
+  CU(c, c->ops->launch_step(c->cfg.scheme, c->cfg.instrument ? 1 : 0, c->params, sh.threads, sh.grid, sh.dyn_smem,
+                            c->stream));
   return ADEPT_OK;
 }
 

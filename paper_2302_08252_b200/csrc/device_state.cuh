@@ -16,7 +16,11 @@ namespace adept {
 
 enum SchemeId : int { S_SPARSE = 0, S_DENSE = 1 };
 
-constexpr int kBlock = 256;  // threads per CTA of the step kernel
+// The step kernel is built for two CTA shapes: 256 threads (2 groups, 4 CTAs/SM) for small
+// populations -- a shower's head and tail, where CTAs must start and finish quickly -- and 1024
+// threads (8 groups, 1 CTA/SM) for large ones, where one staged copy of the tables, one set of tally
+// bins and one end-of-iteration ticket per SM are worth 3-4 % (adept_api.cu picks per launch).
+constexpr int kBlockSmall = 256, kBlockLarge = 1024;
 // A CTA is split into groups of kGroup threads.  A group steps one tile of kGroup tracks at a time
 // and synchronises only with itself (a named barrier), so that while one group waits -- for its
 // tile's output range (a global atomic) or for a straggling warp -- the other groups of the SM keep
@@ -25,7 +29,7 @@ constexpr int kBlock = 256;  // threads per CTA of the step kernel
 #define ADEPT_GROUP 128
 #endif
 constexpr int kGroup = ADEPT_GROUP;
-constexpr int kGroupsPerCta = kBlock / kGroup;
+constexpr int kMaxGroupsPerCta = kBlockLarge / kGroup;
 constexpr int kWarpsPerGroup = kGroup / 32;
 static_assert(kGroup == 64 || kGroup == 128, "a group is 2 or 4 warps (arrival word: 3 x 9-bit counts + 3-bit ticket)");
 // Shared-memory queue (one per group) of tracks parked between the two halves of the step: 14
@@ -46,8 +50,9 @@ __host__ __device__ constexpr size_t bins_bytes(uint32_t n_slabs) { return ((siz
 __host__ __device__ constexpr size_t units_offset(size_t table_bytes, uint32_t n_slabs) {
   return (table_bytes + bins_bytes(n_slabs) + 127) / 128 * 128;
 }
-__host__ __device__ constexpr size_t step_smem_bytes(int scheme, size_t table_bytes, uint32_t n_slabs, size_t tile_words) {
-  return units_offset(table_bytes, n_slabs) + size_t(kGroupsPerCta) * (in_buf_bytes(scheme, tile_words) + queue_bytes(scheme));
+__host__ __device__ constexpr size_t step_smem_bytes(int scheme, size_t table_bytes, uint32_t n_slabs, size_t tile_words,
+                                                     int threads) {
+  return units_offset(table_bytes, n_slabs) + size_t(threads / kGroup) * (in_buf_bytes(scheme, tile_words) + queue_bytes(scheme));
 }
 
 // Energy tallies (rule M7: sums of fp32 terms) are accumulated in 64-bit fixed point, unit

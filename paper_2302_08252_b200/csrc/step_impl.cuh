@@ -197,7 +197,7 @@ struct CtaShared {
   uint32_t alive[4];
   uint32_t escaped[4];
   uint32_t probe[3 * kNumFields * 2];
-  GroupShared grp[kGroupsPerCta];
+  GroupShared grp[kMaxGroupsPerCta];
 };
 
 // A9 + A11: the last CTA closes the iteration.
@@ -475,8 +475,9 @@ __device__ __forceinline__ void run_kind(const Params &p, const Env &env, const 
                                          uint32_t first_global_tile, uint32_t n_tiles, uint32_t n_kind, int &sbuf,
                                          uint32_t &in_phase, uint32_t &tab_phase, int &staged_group) {
   // tiles are dealt round-robin over all groups of the grid, continuing across the kinds
-  const uint32_t n_groups = gridDim.x * kGroupsPerCta;
-  const uint32_t me = blockIdx.x * kGroupsPerCta + c.group;
+  const uint32_t groups_per_cta = blockDim.x / kGroup;
+  const uint32_t n_groups = gridDim.x * groups_per_cta;
+  const uint32_t me = blockIdx.x * groups_per_cta + c.group;
   const uint32_t shift = (me + n_groups - first_global_tile % n_groups) % n_groups;
   // the group's first tile of this kind is requested before the tables are: the two copies overlap
   // (small populations -- the head and tail of a shower -- are latency-bound, one tile per group)
@@ -521,8 +522,10 @@ __device__ __forceinline__ void run_kind(const Params &p, const Env &env, const 
 #ifndef ADEPT_STEP_MIN_CTAS
 #define ADEPT_STEP_MIN_CTAS 4
 #endif
-template <int L, int SCHEME, bool INSTR>
-__global__ void __launch_bounds__(kBlock, ADEPT_STEP_MIN_CTAS) step_kernel(const __grid_constant__ Params p) {
+template <int L, int SCHEME, bool INSTR, int THREADS>
+__global__ void __launch_bounds__(THREADS, (THREADS == kBlockSmall) ? ADEPT_STEP_MIN_CTAS : 1) step_kernel(const __grid_constant__ Params p) {
+  constexpr int kBlock = THREADS;
+  constexpr int kGroupsPerCta = THREADS / kGroup;
   extern __shared__ __align__(128) unsigned char dyn_smem[];
   __shared__ CtaShared sh;
   float4 *s_tab = reinterpret_cast<float4 *>(dyn_smem);
@@ -698,8 +701,9 @@ __global__ void read_kernel(const __grid_constant__ Params p, PackedTrack *dst, 
 // scheme and instrumentation are compile-time parameters of every kernel.)
 struct LayoutOps {
   size_t (*record_words)(size_t capacity);
-  int (*step_ctas_per_sm)(int scheme, int instr, size_t dyn_smem);
-  cudaError_t (*launch_step)(int scheme, int instr, const Params &, unsigned grid, size_t dyn_smem, cudaStream_t);
+  int (*step_ctas_per_sm)(int scheme, int instr, int threads, size_t dyn_smem);
+  cudaError_t (*launch_step)(int scheme, int instr, const Params &, int threads, unsigned grid, size_t dyn_smem,
+                             cudaStream_t);
   cudaError_t (*launch_inject)(int scheme, const Params &, const void *staged, uint32_t n, int kind, uint32_t par,
                                uint32_t entry_base, uint32_t slot_base, unsigned long long seed, cudaStream_t);
   cudaError_t (*launch_load)(int scheme, const Params &, const void *staged, const uint32_t *slots, uint32_t n,
@@ -709,22 +713,26 @@ struct LayoutOps {
 };
 
 template <int L> struct OpsImpl {
-  template <typename F> static auto pick(int scheme, int instr, F f) {
-    if (scheme == S_DENSE) return instr ? f(step_kernel<L, S_DENSE, true>) : f(step_kernel<L, S_DENSE, false>);
-    return instr ? f(step_kernel<L, S_SPARSE, true>) : f(step_kernel<L, S_SPARSE, false>);
+  template <int T, typename F> static auto pick_t(int scheme, int instr, F f) {
+    if (scheme == S_DENSE) return instr ? f(step_kernel<L, S_DENSE, true, T>) : f(step_kernel<L, S_DENSE, false, T>);
+    return instr ? f(step_kernel<L, S_SPARSE, true, T>) : f(step_kernel<L, S_SPARSE, false, T>);
+  }
+  template <typename F> static auto pick(int scheme, int instr, int threads, F f) {
+    return threads == kBlockLarge ? pick_t<kBlockLarge>(scheme, instr, f) : pick_t<kBlockSmall>(scheme, instr, f);
   }
   static size_t record_words(size_t cap) { return Mapping<L>::words(cap); }
-  static int step_ctas_per_sm(int scheme, int instr, size_t dyn) {
-    return pick(scheme, instr, [&](auto *k) {
+  static int step_ctas_per_sm(int scheme, int instr, int threads, size_t dyn) {
+    return pick(scheme, instr, threads, [&](auto *k) {
       int n = 0;
       if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, int(dyn)) != cudaSuccess) return -1;
-      if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k, kBlock, dyn) != cudaSuccess) return -1;
+      if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k, threads, dyn) != cudaSuccess) return -1;
       return n;
     });
   }
-  static cudaError_t launch_step(int scheme, int instr, const Params &p, unsigned grid, size_t dyn, cudaStream_t s) {
-    return pick(scheme, instr, [&](auto *k) {
-      k<<<grid, kBlock, dyn, s>>>(p);
+  static cudaError_t launch_step(int scheme, int instr, const Params &p, int threads, unsigned grid, size_t dyn,
+                                 cudaStream_t s) {
+    return pick(scheme, instr, threads, [&](auto *k) {
+      k<<<grid, threads, dyn, s>>>(p);
       return cudaGetLastError();
     });
   }
