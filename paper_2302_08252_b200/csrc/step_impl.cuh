@@ -1,4 +1,5 @@
-// The transport-step kernel and its helper kernels, templated on <layout, scheme, instrumented>.
+// The transport-step kernel and its helper kernels, templated on <layout, scheme, instrumented, CTA
+// size (256 threads for small populations, 1024 for large ones: device_state.cuh)>.
 //
 // One launch = one iteration of all three per-type track buffers ("the tracks of each
 // particle type are processed by a dedicated kernel"; here the three passes share one persistent
@@ -518,7 +519,8 @@ __device__ __forceinline__ void run_kind(const Params &p, const Env &env, const 
 }
 
 // ---------------------------------------------------------------------- the step kernel ------
-// Dynamic shared memory: step_smem_bytes() in device_state.cuh.
+// Dynamic shared memory: step_smem_bytes() in device_state.cuh.  THREADS = kBlockSmall (4 CTAs/SM)
+// or kBlockLarge (one CTA per SM); the code is the same, the number of groups per CTA differs.
 #ifndef ADEPT_STEP_MIN_CTAS
 #define ADEPT_STEP_MIN_CTAS 4
 #endif
