@@ -358,16 +358,21 @@ def test_instrumented_sparse_writes_only_what_changed():
 
 
 # ------------------------------------------- BASELINE.json sizes, bench.py's launch configuration ---
-def test_single_step_at_full_size_counts_and_sampled_tracks():
-    """Config 3 as bench.py times it: 2^24 tracks, dense double buffer, AoSoA-32, one adept_step.
-    All integer counts and the per-slab deposits against the oracle's full-size step, and every
-    surviving / created track of a sample of 1/64 of the id space compared word for word."""
+@pytest.mark.parametrize("layout,scheme,n", [("aosoa32", "dense", 1 << 24), ("soa", "dense", 1 << 23),
+                                             ("aos", "sparse", 1 << 23)])
+def test_single_step_at_full_size_counts_and_sampled_tracks(layout, scheme, n):
+    """Config 3 as bench.py times it: 2^24 tracks, dense double buffer, AoSoA-32, one adept_step --
+    and 2^23 tracks in two more variants; all above the population at which the library switches to
+    its 1024-thread CTAs.  All integer counts and the per-slab deposits against the oracle's
+    full-size step, and every surviving / created track of a sample of 1/64 of the id space
+    compared word for word."""
     c = CONFIGS["single_step"]
     geo, tab = geometry_for("single_step"), tables_for("single_step")
-    n = c["n_tracks"]
     pop = gen_tracks(n, c["seed"], geo, c["e_max"], c["fractions"])
     cap = int(max(p.shape[0] for p in pop) * 1.25) + 4096
-    ctx = _ctx(geo, tab, layout="aosoa32", scheme="dense", capacity=cap, seed=c["seed"])
+    if scheme == "sparse":
+        cap = int(max(p.shape[0] for p in pop) * 1.6) + 4096      # slots of new tracks come on top of the old
+    ctx = _ctx(geo, tab, layout=layout, scheme=scheme, capacity=cap, seed=c["seed"])
     for k in range(3):
         ctx.load_tracks(k, pop[k])
     counts = ctx.step()
