@@ -127,16 +127,18 @@ __device__ __forceinline__ float geometry_step(const Trk &t, const Env &g, float
   return s_g;
 }
 
-// S25: snap to the plane and change slab, or escape.  Returns true if the track escaped.  Written
-// with selects: the faces of a warp's lanes differ, a branch per face would serialise them.
-__device__ __forceinline__ bool cross_boundary(Trk &t, const Env &g, uint32_t vol0, int face, float z_lo,
+// S25, applied where `doit` holds: snap to the plane and change slab, or escape.  Returns true if the
+// track escaped.  Written with selects throughout: the faces (and whether the step ends on a face
+// at all) differ between the lanes of a warp, a branch per case would serialise them.
+__device__ __forceinline__ bool cross_boundary(bool doit, Trk &t, const Env &g, uint32_t vol0, int face, float z_lo,
                                                float z_hi) {
   const bool zp = face == FACE_ZP, zm = face == FACE_ZM;
   const uint32_t vol_new = zp ? vol0 + 1u : vol0 - 1u;  // vol0 - 1 wraps for slab 0: caught by the range test
   const bool out = (face == FACE_XY) || (vol_new >= g.n_slabs);
-  t.pz = zp ? z_hi : (zm ? z_lo : t.pz);
-  t.vol = out ? vol0 : vol_new;
-  return out;
+  const float pz_new = zp ? z_hi : (zm ? z_lo : t.pz);
+  t.pz = doit ? pz_new : t.pz;
+  t.vol = (doit && !out) ? vol_new : vol0;
+  return doit && out;
 }
 
 __device__ __forceinline__ void make_kid(Kid &k, int kind, float dx, float dy, float dz, float ekin, uint32_t id_lo,
@@ -230,17 +232,12 @@ __device__ __forceinline__ void move_gamma(Trk &t, const Env &g, MoveOut &o) {
   t.n2 = fmaf(-s, sig2, t.n2);
   t.step = rs.step + 1u;
 
-  if (w >= 0) {  // S26 follows in interact_gamma
-    o.pending = w;
-    return;
-  }
-  // S25
-  if (cross_boundary(t, g, vol0, face, z_lo, z_hi)) {
-    o.escaped = true;
-    o.alive = false;
-    return;
-  }
-  runaway_guard<K_GAMMA>(t, o);
+  // what the step ends in, as flags (no early exits: the outcomes of a warp's lanes differ)
+  const bool geom = w < 0;
+  o.pending = geom ? int(P_NONE) : w;                              // S26 follows in interact_gamma
+  o.escaped = cross_boundary(geom, t, g, vol0, face, z_lo, z_hi);  // S25
+  o.guard = geom && !o.escaped && t.step >= (1u << 20);            // S31
+  o.alive = !(o.escaped || o.guard);
 }
 
 // S26 for a photon whose step (already taken: t.step is the post-increment value) ended in process w.
@@ -361,25 +358,15 @@ template <int KIND> __device__ __forceinline__ void move_elec(Trk &t, const Env 
   }
   o.dep = E0 - E_post;
   t.ekin = E_post;
-  if (E_post < e_cut) {
-    if (KIND == K_EM) {
-      o.dep_b = E_post;
-      o.alive = false;
-    }  // e+ is kept for S17 at its next step
-    return;
-  }
-  if (w == 0) {  // S26 follows in interact_elec
-    o.pending = P_PROC0;
-    return;
-  }
-  if (w < 0) {  // S25
-    if (cross_boundary(t, g, vol0, face, z_lo, z_hi)) {
-      o.escaped = true;
-      o.alive = false;
-      return;
-    }
-  }
-  runaway_guard<KIND>(t, o);
+  // what the step ends in, as flags (no early exits: the outcomes of a warp's lanes differ)
+  const bool below = E_post < e_cut;            // S24: e- deposits the rest and dies; e+ is kept for S17
+  const bool brems = !below && w == 0;          // S26 follows in interact_elec
+  const bool geom = !below && w < 0;
+  o.dep_b = (below && KIND == K_EM) ? E_post : 0.0f;
+  o.pending = brems ? int(P_PROC0) : int(P_NONE);
+  o.escaped = cross_boundary(geom, t, g, vol0, face, z_lo, z_hi);  // S25
+  o.guard = !below && !brems && !o.escaped && t.step >= (1u << 20);  // S31
+  o.alive = !((below && KIND == K_EM) || o.escaped || o.guard);
 }
 
 // S17 annihilation (pending == P_ANNIH: track untouched) or S26 bremsstrahlung (step already taken).
