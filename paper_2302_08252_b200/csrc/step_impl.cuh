@@ -305,11 +305,14 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
     old = t;
     if constexpr (KIND == K_GAMMA) move_gamma(t, env, o);
     else move_elec<KIND>(t, env, o);
-    // A6: scoring into the CTA's bins (pre-step slab; the S31 guard uses the post-step slab)
-    if (o.dep != 0.0f) bin_add(c.bins, old.vol, o.dep);
-    if (o.dep_b != 0.0f) bin_add(c.bins, old.vol, o.dep_b);
-    if (o.escaped) bin_add_track_energy<KIND>(c.bins, env.n_slabs, t.ekin);
-    if (o.guard) bin_add_track_energy<KIND>(c.bins, t.vol, t.ekin);
+    // A6: scoring into the CTA's bins (pre-step slab; the S31 guard uses the post-step slab).  A
+    // photon deposits nothing in this half; the rare terms share one branch.
+    if (KIND != K_GAMMA && o.dep != 0.0f) bin_add(c.bins, old.vol, o.dep);
+    if ((KIND != K_GAMMA && o.dep_b != 0.0f) || o.escaped || o.guard) {
+      if (KIND != K_GAMMA && o.dep_b != 0.0f) bin_add(c.bins, old.vol, o.dep_b);
+      if (o.escaped) bin_add_track_energy<KIND>(c.bins, env.n_slabs, t.ekin);
+      if (o.guard) bin_add_track_energy<KIND>(c.bins, t.vol, t.ekin);
+    }
   }
   const bool parked = active && o.pending != P_NONE;
   const bool survives = active && !parked && o.alive;
