@@ -32,11 +32,13 @@ constexpr int kGroup = ADEPT_GROUP;
 constexpr int kMaxGroupsPerCta = kBlockLarge / kGroup;
 constexpr int kWarpsPerGroup = kGroup / 32;
 static_assert(kGroup == 64 || kGroup == 128, "a group is 2 or 4 warps (arrival word: 3 x 9-bit counts + 3-bit ticket)");
-// Shared-memory queue (one per group) of tracks parked between the two halves of the step: 14
-// record words + the pending interaction (+ the slot, sparse scheme only), field-major.  At most
-// kGroup - 1 left over from earlier tiles plus kGroup from the current one.
+// Shared-memory queue (one per group) of tracks parked between the two halves of the step, entry-
+// major.  At most kGroup - 1 left over from earlier tiles plus kGroup from the current one.
 constexpr int kQueueCap = 2 * kGroup;
-__host__ __device__ constexpr int queue_words(int scheme) { return scheme == S_DENSE ? 15 : 16; }
+// An entry is the 14 record words, the pending interaction packed into the three top bits of the step
+// word (steps stay below 2^21, rule S31), and for the sparse scheme the slot (+ one pad word): 56 or
+// 64 bytes, written and read as 64-bit words (7 or 8 shared-memory instructions, conflict-free).
+__host__ __device__ constexpr int queue_words(int scheme) { return scheme == S_DENSE ? 14 : 16; }
 __host__ __device__ constexpr size_t queue_bytes(int scheme) { return size_t(kQueueCap) * queue_words(scheme) * 4; }
 // Dense scheme: one tile staged in shared memory by TMA (record_words(kGroup) words of the layout).
 __host__ __device__ constexpr size_t in_buf_bytes(int scheme, size_t tile_words) {

@@ -173,6 +173,32 @@ __device__ __forceinline__ Trk kid_track(const Trk &parent, const Kid &k) {
   return c;
 }
 
+// ---- parked tracks (the queue between the two halves of the step) ----------------------------------
+// Entry q = 7 (sparse: 8) 64-bit words; the pending interaction rides in the top bits of the step word.
+template <int SCHEME>
+__device__ __forceinline__ void park_store(uint32_t *queue, uint32_t q, const Trk &t, int pending, uint32_t slot) {
+  uint2 *e = reinterpret_cast<uint2 *>(queue + size_t(q) * queue_words(SCHEME));
+#pragma unroll
+  for (int f = 0; f < 12; f += 2) e[f / 2] = make_uint2(trk_word(t, f), trk_word(t, f + 1));
+  e[6] = make_uint2(t.id_hi, t.step | (uint32_t(pending) << 29));
+  if (SCHEME == S_SPARSE) e[7] = make_uint2(slot, 0u);
+}
+template <int SCHEME>
+__device__ __forceinline__ void park_load(const uint32_t *queue, uint32_t q, Trk &t, int &pending, uint32_t &slot) {
+  const uint2 *e = reinterpret_cast<const uint2 *>(queue + size_t(q) * queue_words(SCHEME));
+#pragma unroll
+  for (int f = 0; f < 12; f += 2) {
+    const uint2 w = e[f / 2];
+    trk_set_word(t, f, w.x);
+    trk_set_word(t, f + 1, w.y);
+  }
+  const uint2 w = e[6];
+  t.id_hi = w.x;
+  t.step = w.y & 0x1FFFFFFFu;
+  pending = int(w.y >> 29);
+  if (SCHEME == S_SPARSE) slot = e[7].x;
+}
+
 // ---- arrival word (row A9) -----------------------------------------------------------------------
 // Three 9-bit counts (bits 0-8, 9-17, 18-26) and a ticket (bits 27-29).  Every warp of a group adds
 // its counts and one ticket with a single shared-memory atomic; what the atomic returns are the
@@ -247,7 +273,7 @@ struct GroupRefs {
   CtaShared *cta;
   GroupShared *g;
   Bins bins;         // shared, CTA-wide
-  uint32_t *queue;   // shared, [queue_words][kQueueCap]
+  uint32_t *queue;   // shared, [kQueueCap][queue_words]
   uint32_t *in_buf;  // shared, one staged tile (dense scheme)
   int group, gtid;   // group index inside the CTA, thread index inside the group
 };
@@ -341,10 +367,7 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
   // park the tracks that still owe an interaction
   if (parked) {
     const uint32_t q = queued + count_of(word, 1) + __popc(m_park & lt_mask);
-#pragma unroll
-    for (int f = 0; f < kNumFields; ++f) c.queue[f * kQueueCap + q] = trk_word(t, f);
-    c.queue[14 * kQueueCap + q] = uint32_t(o.pending);
-    if (SCHEME == S_SPARSE) c.queue[15 * kQueueCap + q] = slot;
+    park_store<SCHEME>(c.queue, q, t, o.pending, slot);
   }
   // A10 sparse: in-place update of the words that changed (parked tracks too: the interaction
   // later writes only what it changes)
@@ -383,10 +406,8 @@ __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &e
   uint32_t slot = 0;
   if (have) {
     const uint32_t q = first + gtid;
-#pragma unroll
-    for (int f = 0; f < kNumFields; ++f) trk_set_word(t, f, c.queue[f * kQueueCap + q]);
-    const int pending = int(c.queue[14 * kQueueCap + q]);
-    if (SCHEME == S_SPARSE) slot = c.queue[15 * kQueueCap + q];
+    int pending;
+    park_load<SCHEME>(c.queue, q, t, pending, slot);
     before_interaction = t;
     if constexpr (KIND == K_GAMMA) interact_gamma(t, pending, env, o);
     else interact_elec<KIND>(t, pending, env, o);
