@@ -353,7 +353,7 @@ def run_showers(args, name: str):
                    "d2h_bytes_per_step": 256 + 8 * (2 * c["n_layers"] + 1),
                    "what": "same measurement: the timed region is the public API with host buffers"},
            "roofline": None}
-    if not args.no_cpu and name != "heavy":
+    if not args.no_cpu:                                    # heavy: the oracle needs ~80 s (use --no-cpu to skip)
         from oracle import Oracle
         o = Oracle(geo, tab, seed=c["seed"])
         o.inject(prim)
