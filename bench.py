@@ -119,8 +119,16 @@ def oracle_single_step(pop, sample_tracks: int):
     o.step()
     dt = time.perf_counter() - t0
     r = o.result()
+    r["sample"] = [sample_of(o.read_tracks(k, pop[0].dtype)) for k in range(3)]
     o.close()
     return n, dt, r
+
+
+def sample_of(tracks):
+    """1/64 of the tracks by id, in id order: what the full-size parity check compares word for word."""
+    t = tracks[(tracks["id_lo"] & 63) == 5]
+    key = t["id_hi"].astype(np.uint64) << np.uint64(32) | t["id_lo"].astype(np.uint64)
+    return t[np.argsort(key, kind="stable")]
 
 
 def run_reference(args, rank: int):
@@ -178,6 +186,7 @@ def bench_layout(ctx, torch, pop, steps, warmup, flush, barrier):
     wall = time.perf_counter() - t0
     ms = [e0.elapsed_time(e1) for e0, e1 in ev]
     res = ctx.result()
+    res["sample"] = [sample_of(ctx.read_tracks(k)) for k in range(3)]
     del pristine
     return ms, res, wall
 
@@ -317,7 +326,21 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
                                "sample": "one oracle iteration over all %d tracks of the same population" % n,
                                "seconds": dt}
         keys = ("steps", "secondaries", "killed", "escaped_n", "live")
+        # discrete-branch disagreements (north_star: to be reported): a track that took another branch
+        # on the GPU has another fate -- it is missing, extra, or of another kind in the output sample
+        n_cmp = n_missing = n_diff = 0
+        for a, b in zip(main_res["sample"], r["sample"]):
+            ka = a["id_hi"].astype(np.uint64) << np.uint64(32) | a["id_lo"].astype(np.uint64)
+            kb = b["id_hi"].astype(np.uint64) << np.uint64(32) | b["id_lo"].astype(np.uint64)
+            common = np.intersect1d(ka, kb)
+            n_missing += int(ka.shape[0] + kb.shape[0] - 2 * common.shape[0])
+            aa, bb = a[np.isin(ka, common)], b[np.isin(kb, common)]
+            n_cmp += int(common.shape[0])
+            n_diff += int((aa.view(np.uint8).reshape(-1, 56) != bb.view(np.uint8).reshape(-1, 56)).any(axis=1).sum())
         out["parity_full_size"] = {"counts_bit_exact": bool(all((main_res[k] == r[k]).all() for k in keys)),
+                                   "tracks_compared": n_cmp, "tracks_with_another_fate": n_missing,
+                                   "tracks_with_any_word_differing": n_diff,
+                                   "branch_disagreement_rate": (n_missing / max(1, n_cmp)),
                                    "edep_rel_err": float(np.max(np.abs(main_res["edep_layer"] - r["edep_layer"])
                                                                 / np.maximum(r["edep_layer"], 1e-30)))}
     print(json.dumps(out))
