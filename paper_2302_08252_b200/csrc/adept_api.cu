@@ -307,10 +307,11 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
     p.kind[k].instr_slots = reinterpret_cast<uint32_t *>(c->ws + pl.instr_slots[k]);
   }
   p.instr_field_rw = reinterpret_cast<unsigned long long *>(c->ws + pl.instr_rw);
-  std::memset(p.soa_tile, 0, sizeof p.soa_tile);
-  if (cfg->layout == ADEPT_SOA && cfg->scheme == ADEPT_DENSE_DOUBLE) {
-    // Tensor maps of the six SoA record buffers, seen as [14 fields][capacity] u32 tensors with a
-    // box of [14][kGroup]: one tiled TMA copy stages a tile (csrc/step_impl.cuh prefetch_tile).
+  std::memset(p.tile_map, 0, sizeof p.tile_map);
+  if ((cfg->layout == ADEPT_SOA || cfg->layout == ADEPT_AOS) && cfg->scheme == ADEPT_DENSE_DOUBLE) {
+    // Tensor maps of the six record buffers: one tiled TMA copy stages a tile (csrc/step_impl.cuh
+    // prefetch_tile).  SoA: a [14 fields][capacity] u32 tensor with a box of [14][kGroup].  AoS: a
+    // [capacity][16 words] tensor with a box of [kGroup][16], copied with the 64-byte swizzle.
     // The encoder is a driver entry point; it is fetched through the runtime so that the library
     // does not link libcuda.
     void *fn = nullptr;
@@ -318,14 +319,16 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
     if ((e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres)) != cudaSuccess || !fn)
       return die("cudaGetDriverEntryPoint(cuTensorMapEncodeTiled)", e == cudaSuccess ? cudaErrorUnknown : e);
     auto encode = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(fn);
-    const cuuint64_t dims[2] = {pl.capacity, cuuint64_t(kNumFields)};
-    const cuuint64_t strides[1] = {cuuint64_t(pl.capacity) * 4};  // bytes between fields
-    const cuuint32_t box[2] = {cuuint32_t(kGroup), cuuint32_t(kNumFields)};
+    const bool soa = cfg->layout == ADEPT_SOA;
+    const cuuint64_t dims[2] = {soa ? cuuint64_t(pl.capacity) : 16u, soa ? cuuint64_t(kNumFields) : cuuint64_t(pl.capacity)};
+    const cuuint64_t strides[1] = {soa ? cuuint64_t(pl.capacity) * 4 : 64u};  // bytes between rows
+    const cuuint32_t box[2] = {soa ? cuuint32_t(kGroup) : 16u, soa ? cuuint32_t(kNumFields) : cuuint32_t(kGroup)};
     const cuuint32_t elem_strides[2] = {1, 1};
     for (int k = 0; k < 3; ++k)
       for (int b = 0; b < 2; ++b) {
-        const CUresult r = encode(&p.soa_tile[k][b], CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, p.kind[k].rec[b], dims, strides,
-                                  box, elem_strides, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+        const CUresult r = encode(&p.tile_map[k][b], CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, p.kind[k].rec[b], dims, strides,
+                                  box, elem_strides, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                  soa ? CU_TENSOR_MAP_SWIZZLE_NONE : CU_TENSOR_MAP_SWIZZLE_64B,
                                   CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) return die("cuTensorMapEncodeTiled", cudaErrorInvalidValue);
       }

@@ -103,8 +103,9 @@ struct Params {
   uint32_t capacity;         // slots per kind (multiple of 128)
   KindStorage kind[3];
   unsigned long long *instr_field_rw;  // [3][14][2], instrumented build
-  // SoA layout, dense scheme: tensor maps of the record buffers, [kind][parity] (see prefetch_tile)
-  alignas(64) CUtensorMap soa_tile[3][2];
+  // SoA and AoS layouts, dense scheme: tensor maps of the record buffers, [kind][parity] (see
+  // prefetch_tile in step_impl.cuh)
+  alignas(64) CUtensorMap tile_map[3][2];
 };
 
 }  // namespace adept

@@ -111,19 +111,25 @@ __device__ __forceinline__ void prefetch_tile(const Params &p, int kind, uint32_
     asm volatile(
         "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(
             static_cast<uint32_t>(__cvta_generic_to_shared(in_buf))),
-        "l"(reinterpret_cast<uint64_t>(&p.soa_tile[kind][par])), "r"(first), "r"(0u), "r"(bar)
+        "l"(reinterpret_cast<uint64_t>(&p.tile_map[kind][par])), "r"(first), "r"(0u), "r"(bar)
         : "memory");
-  } else {
-    uint32_t bytes;
-    const uint32_t *src;
-    if constexpr (L == L_AOS) {
-      bytes = n * 64u;
-      src = rec + size_t(first) * 16;
-    } else {  // AoSoA-n: whole blocks
-      constexpr uint32_t kL = Mapping<L>::kLanes;
-      bytes = ((n + kL - 1u) / kL) * (kL * kNumFields * 4u);
-      src = rec + size_t(first / kL) * (kL * kNumFields);
-    }
+  } else if constexpr (L == L_AOS) {
+    // The AoS buffer is a 2-D tensor [capacity][16 words]; a tile is the box [kGroup][16], copied
+    // with the 64-byte swizzle: the 16-byte chunk c of row r lands at chunk c ^ ((address >> 7) & 3),
+    // so that the threads of a quarter warp, which each read one chunk of their own 64-byte record,
+    // hit different banks (a linear copy makes those loads 4-way bank conflicts).
+    (void)rec; (void)n;
+    constexpr uint32_t bytes = uint32_t(kGroup) * 64u;
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(
+            static_cast<uint32_t>(__cvta_generic_to_shared(in_buf))),
+        "l"(reinterpret_cast<uint64_t>(&p.tile_map[kind][par])), "r"(0u), "r"(first), "r"(bar)
+        : "memory");
+  } else {  // AoSoA-n: whole blocks, one contiguous run
+    constexpr uint32_t kL = Mapping<L>::kLanes;
+    const uint32_t bytes = ((n + kL - 1u) / kL) * (kL * kNumFields * 4u);
+    const uint32_t *src = rec + size_t(first / kL) * (kL * kNumFields);
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
     bulk_g2s(in_buf, src, bytes, mbar);
   }
@@ -133,9 +139,16 @@ __device__ __forceinline__ void prefetch_tile(const Params &p, int kind, uint32_
 template <int L> __device__ __forceinline__ Trk staged_load(const uint32_t *in_buf, int gtid) {
   Trk t;
   if constexpr (L == L_AOS) {
-    const uint4 *r = reinterpret_cast<const uint4 *>(in_buf + gtid * 16);
-    const uint4 a = r[0], b = r[1], c = r[2];
-    const uint2 d = *reinterpret_cast<const uint2 *>(r + 3);
+    // undo the copy's 64-byte swizzle (prefetch_tile): chunk c of this thread's record is at chunk
+    // c ^ s of its row, s = bits 7-8 of the row's shared-memory address
+    const uint32_t row = static_cast<uint32_t>(__cvta_generic_to_shared(in_buf)) + uint32_t(gtid) * 64u;
+    const uint32_t sw = ((row >> 7) & 3u) << 4;
+    uint4 a, b, c;
+    uint2 d;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(a.x), "=r"(a.y), "=r"(a.z), "=r"(a.w) : "r"(row + (0u ^ sw)));
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(b.x), "=r"(b.y), "=r"(b.z), "=r"(b.w) : "r"(row + (16u ^ sw)));
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(c.x), "=r"(c.y), "=r"(c.z), "=r"(c.w) : "r"(row + (32u ^ sw)));
+    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(d.x), "=r"(d.y) : "r"(row + (48u ^ sw)));
     t.px = __uint_as_float(a.x); t.py = __uint_as_float(a.y); t.pz = __uint_as_float(a.z);
     t.dx = __uint_as_float(a.w); t.dy = __uint_as_float(b.x); t.dz = __uint_as_float(b.y);
     t.ekin = __uint_as_float(b.z); t.n0 = __uint_as_float(b.w);
