@@ -6,7 +6,7 @@ single-step microbenchmark (BASELINE.json configs[2]): 2^24 tracks, 40 % e- / 10
 uniform in the 50-layer Pb/lAr calorimeter, isotropic, log-uniform 100 keV - 10 GeV, exp(1)
 interaction lengths; one adept_step per "step", dense double buffer, per layout.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--layout soa|aos|aosoa32|aosoa64|all] [--impl reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--layout soa|aos|aosoa32|aosoa64|soa16|all] [--impl reference]
 
 One JSON line on stdout (rank 0).  `value` is measured with the tracks resident in HBM: every timed
 step starts from a pristine copy of the workspace (restored outside the timed region, L2 flushed) and
@@ -34,11 +34,11 @@ if ROOT not in sys.path:
 from workloads import CONFIGS, gen_tracks, geometry_for, tables_for  # noqa: E402
 
 WORKLOAD = "single_step"
-RECORD_BYTES = {"aos": 64, "soa": 56, "aosoa32": 56, "aosoa64": 56}     # bytes per record per layout
+RECORD_BYTES = {"aos": 64, "soa": 56, "aosoa32": 56, "aosoa64": 56, "soa16": 56}     # bytes per record per layout
 # dram__bytes_read.sum + dram__bytes_write.sum of one step_kernel launch on this workload, from the
 # `ncu --set full` captures summarised in profiles/r1_step_kernel.md (r1g: AoSoA-32)
 NCU_TRAFFIC_BYTES = {"aosoa32": 942.4e6 + 1043.9e6, "soa": None, "aos": None,
-                     "aosoa64": None}
+                     "aosoa64": None, "soa16": None}
 
 
 def measured_peak():
@@ -220,7 +220,7 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
     biggest = max(p.shape[0] for p in pop)
     capacity = int(biggest * 1.25) + 4096                  # one step grows the photon set by ~16 %
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-    layouts = ["aosoa32", "aosoa64", "soa", "aos"] if args.layout == "all" else [args.layout]
+    layouts = ["aosoa32", "aosoa64", "soa16", "soa", "aos"] if args.layout == "all" else [args.layout]
     per_layout, results = {}, {}
     sampler = ClockSampler(local_rank)
     sampler.start()
@@ -423,7 +423,7 @@ def run_sweep(args):
     geo, tab = geometry_for("sweep"), tables_for("sweep")
     span, cap = c["span"], c["span"] + c["reserve"]
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
-    layouts = ["aos", "soa", "aosoa32", "aosoa64"] if args.layout == "all" else [args.layout]
+    layouts = ["aos", "soa", "aosoa32", "aosoa64", "soa16"] if args.layout == "all" else [args.layout]
     cells = []
     for occ in c["occupancies"]:
         pop = gen_sweep(occ)
@@ -488,7 +488,7 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--layout", default="all", choices=["soa", "aosoa32", "aosoa64", "aos", "all"])
+    ap.add_argument("--layout", default="all", choices=["soa", "aosoa32", "aosoa64", "soa16", "aos", "all"])
     ap.add_argument("--tracks", type=int, default=CONFIGS[WORKLOAD]["n_tracks"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--workload", default="single_step", choices=["single_step", "tiny", "full", "heavy", "sweep"],

@@ -50,6 +50,7 @@ static const LayoutOps *ops_for(int layout) {
     case ADEPT_SOA: return &kOpsSoA;
     case ADEPT_AOSOA32: return &kOpsAoSoA32;
     case ADEPT_AOSOA64: return &kOpsAoSoA64;
+    case ADEPT_SOA16: return &kOpsSoA16;
     default: return nullptr;
   }
 }
@@ -638,6 +639,7 @@ uint64_t adept_field_offset(int32_t layout, uint32_t capacity, uint32_t slot, ui
     case ADEPT_SOA: return 4 * Mapping<L_SOA>::index(cap, slot, int(field));
     case ADEPT_AOSOA32: return 4 * Mapping<L_AOSOA32>::index(cap, slot, int(field));
     case ADEPT_AOSOA64: return 4 * Mapping<L_AOSOA64>::index(cap, slot, int(field));
+    case ADEPT_SOA16: return 4 * Mapping<L_SOA16>::index(cap, slot, int(field));
     default: return UINT64_MAX;
   }
 }

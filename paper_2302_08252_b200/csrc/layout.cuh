@@ -20,7 +20,7 @@ enum Field : int {
   F_PX = 0, F_PY, F_PZ, F_DX, F_DY, F_DZ, F_EKIN, F_N0, F_N1, F_N2, F_VOL, F_IDLO, F_IDHI, F_STEP,
   kNumFields = 14
 };
-enum LayoutId : int { L_AOS = 0, L_SOA = 1, L_AOSOA32 = 2, L_AOSOA64 = 3 };
+enum LayoutId : int { L_AOS = 0, L_SOA = 1, L_AOSOA32 = 2, L_AOSOA64 = 3, L_SOA16 = 4 };
 
 // A track in registers.
 struct Trk {
@@ -89,6 +89,17 @@ template <int N> struct AoSoAMapping {  // blocks of N tracks, field-major insid
 };
 template <> struct Mapping<L_AOSOA32> : AoSoAMapping<32> {};  // "AoSoA-n"
 template <> struct Mapping<L_AOSOA64> : AoSoAMapping<64> {};  // the paper's fastest
+// SoA of 16-byte field groups (SURVEY.md §8(f) item 1 "grouped-SoA of 16-byte vectors"; BASELINE.json
+// north_star "coalesced, vectorised 16-byte loads of SoA fields"): four arrays of `cap` vectors --
+// {pos.xyz, dir.x}, {dir.y, dir.z, ekin, nial.0}, {nial.1, nial.2, vol, id_lo} (16 B each) and
+// {id_hi, step} (8 B) -- so that a record moves with four vector instructions instead of fourteen and
+// consecutive slots are consecutive vectors.
+template <> struct Mapping<L_SOA16> {
+  __host__ __device__ static constexpr size_t words(size_t cap) { return cap * kNumFields; }
+  __host__ __device__ static constexpr size_t index(size_t cap, size_t slot, int f) {
+    return (f < 12) ? size_t(f / 4) * 4 * cap + slot * 4 + (f % 4) : 12 * cap + slot * 2 + (f - 12);
+  }
+};
 
 // ---- access counting (instrumented build only) -----------------------------------------------
 // field_rw: shared-memory counters [14][2] of the CTA (flushed once per kernel);
@@ -137,10 +148,19 @@ template <int L, bool INSTR> struct TrackView {
   // whole record -> registers
   __device__ __forceinline__ Trk load(uint32_t slot) const {
     Trk t;
-    if constexpr (L == L_AOS) {
-      const uint4 *r = reinterpret_cast<const uint4 *>(base + size_t(slot) * Map::kStride);
-      const uint4 a = r[0], b = r[1], c = r[2];
-      const uint2 d = *reinterpret_cast<const uint2 *>(r + 3);
+    if constexpr (L == L_AOS || L == L_SOA16) {
+      uint4 a, b, c;
+      uint2 d;
+      if constexpr (L == L_AOS) {
+        const uint4 *r = reinterpret_cast<const uint4 *>(base + size_t(slot) * Map::kStride);
+        a = r[0]; b = r[1]; c = r[2];
+        d = *reinterpret_cast<const uint2 *>(r + 3);
+      } else {
+        a = *reinterpret_cast<const uint4 *>(base + Map::index(cap, slot, 0));
+        b = *reinterpret_cast<const uint4 *>(base + Map::index(cap, slot, 4));
+        c = *reinterpret_cast<const uint4 *>(base + Map::index(cap, slot, 8));
+        d = *reinterpret_cast<const uint2 *>(base + Map::index(cap, slot, 12));
+      }
       t.px = __uint_as_float(a.x); t.py = __uint_as_float(a.y); t.pz = __uint_as_float(a.z);
       t.dx = __uint_as_float(a.w); t.dy = __uint_as_float(b.x); t.dz = __uint_as_float(b.y);
       t.ekin = __uint_as_float(b.z); t.n0 = __uint_as_float(b.w);
@@ -159,12 +179,20 @@ template <int L, bool INSTR> struct TrackView {
 
   // registers -> whole record
   __device__ __forceinline__ void store(uint32_t slot, const Trk &t) const {
-    if constexpr (L == L_AOS) {
-      uint4 *r = reinterpret_cast<uint4 *>(base + size_t(slot) * Map::kStride);
-      r[0] = make_uint4(__float_as_uint(t.px), __float_as_uint(t.py), __float_as_uint(t.pz), __float_as_uint(t.dx));
-      r[1] = make_uint4(__float_as_uint(t.dy), __float_as_uint(t.dz), __float_as_uint(t.ekin), __float_as_uint(t.n0));
-      r[2] = make_uint4(__float_as_uint(t.n1), __float_as_uint(t.n2), t.vol, t.id_lo);
-      r[3] = make_uint4(t.id_hi, t.step, 0u, 0u);  // tail padding written so that sectors are whole
+    if constexpr (L == L_AOS || L == L_SOA16) {
+      const uint4 a = make_uint4(__float_as_uint(t.px), __float_as_uint(t.py), __float_as_uint(t.pz), __float_as_uint(t.dx));
+      const uint4 b = make_uint4(__float_as_uint(t.dy), __float_as_uint(t.dz), __float_as_uint(t.ekin), __float_as_uint(t.n0));
+      const uint4 c = make_uint4(__float_as_uint(t.n1), __float_as_uint(t.n2), t.vol, t.id_lo);
+      if constexpr (L == L_AOS) {
+        uint4 *r = reinterpret_cast<uint4 *>(base + size_t(slot) * Map::kStride);
+        r[0] = a; r[1] = b; r[2] = c;
+        r[3] = make_uint4(t.id_hi, t.step, 0u, 0u);  // tail padding written so that sectors are whole
+      } else {
+        *reinterpret_cast<uint4 *>(base + Map::index(cap, slot, 0)) = a;
+        *reinterpret_cast<uint4 *>(base + Map::index(cap, slot, 4)) = b;
+        *reinterpret_cast<uint4 *>(base + Map::index(cap, slot, 8)) = c;
+        *reinterpret_cast<uint2 *>(base + Map::index(cap, slot, 12)) = make_uint2(t.id_hi, t.step);
+      }
       if constexpr (INSTR) {
 #pragma unroll
         for (int f = 0; f < kNumFields; ++f) probe(f, 1, slot);

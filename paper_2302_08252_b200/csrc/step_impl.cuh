@@ -126,6 +126,13 @@ __device__ __forceinline__ void prefetch_tile(const Params &p, int kind, uint32_
             static_cast<uint32_t>(__cvta_generic_to_shared(in_buf))),
         "l"(reinterpret_cast<uint64_t>(&p.tile_map[kind][par])), "r"(0u), "r"(first), "r"(bar)
         : "memory");
+  } else if constexpr (L == L_SOA16) {  // four runs: three of 16-byte vectors, one of 8-byte vectors
+    const uint32_t n2 = (n + 1u) & ~1u;  // whole 16-byte pieces (slots are padded to whole tiles)
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(n2 * 56u) : "memory");
+#pragma unroll
+    for (int gI = 0; gI < 4; ++gI)
+      bulk_g2s(in_buf + Mapping<L>::index(kGroup, 0, 4 * gI), rec + Mapping<L>::index(p.capacity, first, 4 * gI),
+               n2 * (gI < 3 ? 16u : 8u), mbar);
   } else {  // AoSoA-n: whole blocks, one contiguous run
     constexpr uint32_t kL = Mapping<L>::kLanes;
     const uint32_t bytes = ((n + kL - 1u) / kL) * (kL * kNumFields * 4u);
@@ -149,6 +156,16 @@ template <int L> __device__ __forceinline__ Trk staged_load(const uint32_t *in_b
     asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(b.x), "=r"(b.y), "=r"(b.z), "=r"(b.w) : "r"(row + (16u ^ sw)));
     asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(c.x), "=r"(c.y), "=r"(c.z), "=r"(c.w) : "r"(row + (32u ^ sw)));
     asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(d.x), "=r"(d.y) : "r"(row + (48u ^ sw)));
+    t.px = __uint_as_float(a.x); t.py = __uint_as_float(a.y); t.pz = __uint_as_float(a.z);
+    t.dx = __uint_as_float(a.w); t.dy = __uint_as_float(b.x); t.dz = __uint_as_float(b.y);
+    t.ekin = __uint_as_float(b.z); t.n0 = __uint_as_float(b.w);
+    t.n1 = __uint_as_float(c.x); t.n2 = __uint_as_float(c.y);
+    t.vol = c.z; t.id_lo = c.w; t.id_hi = d.x; t.step = d.y;
+  } else if constexpr (L == L_SOA16) {
+    const uint4 a = *reinterpret_cast<const uint4 *>(in_buf + Mapping<L>::index(kGroup, gtid, 0));
+    const uint4 b = *reinterpret_cast<const uint4 *>(in_buf + Mapping<L>::index(kGroup, gtid, 4));
+    const uint4 c = *reinterpret_cast<const uint4 *>(in_buf + Mapping<L>::index(kGroup, gtid, 8));
+    const uint2 d = *reinterpret_cast<const uint2 *>(in_buf + Mapping<L>::index(kGroup, gtid, 12));
     t.px = __uint_as_float(a.x); t.py = __uint_as_float(a.y); t.pz = __uint_as_float(a.z);
     t.dx = __uint_as_float(a.w); t.dy = __uint_as_float(b.x); t.dz = __uint_as_float(b.y);
     t.ekin = __uint_as_float(b.z); t.n0 = __uint_as_float(b.w);
@@ -804,6 +821,6 @@ template <int L> struct OpsImpl {
   }
 };
 
-extern const LayoutOps kOpsAoS, kOpsSoA, kOpsAoSoA32, kOpsAoSoA64;
+extern const LayoutOps kOpsAoS, kOpsSoA, kOpsAoSoA32, kOpsAoSoA64, kOpsSoA16;
 
 }  // namespace adept

@@ -52,7 +52,7 @@ def test_workspace_bytes_is_host_arithmetic(L):
     base = size()
     assert base > 3 * 2 * 4096 * 56                                  # three kinds, two dense arrays
     assert size(capacity=8192) > base and size(capacity=4097) == size(capacity=4224)   # rounded to 128 slots (one tile)
-    assert size(layout=0) > size(layout=1) == size(layout=2) == size(layout=3)   # AoS records are padded to 64 B
+    assert size(layout=0) > size(layout=1) == size(layout=2) == size(layout=3) == size(layout=4)   # AoS records are padded to 64 B
     assert size(scheme=0) < base                                     # one slot array + two slot lists
     assert size(instrument=1) > base
     for bad in (dict(layout=7), dict(scheme=5), dict(capacity=0), dict(n_layers=0), dict(n_bins=0)):
@@ -67,9 +67,12 @@ def test_field_offset_follows_the_three_mappings(L):
             assert L.field_offset(L.ADEPT_SOA, cap, slot, f) == 4 * (f * cap + slot)       # 14 arrays
             assert L.field_offset(L.ADEPT_AOSOA32, cap, slot, f) == 4 * ((slot // 32) * 448 + f * 32 + slot % 32)
             assert L.field_offset(L.ADEPT_AOSOA64, cap, slot, f) == 4 * ((slot // 64) * 896 + f * 64 + slot % 64)
+            want = (f // 4) * 16 * cap + slot * 16 + (f % 4) * 4 if f < 12 else 48 * cap + slot * 8 + (f - 12) * 4
+            assert L.field_offset(L.ADEPT_SOA16, cap, slot, f) == want          # 16-byte field groups
     assert L.field_offset(L.ADEPT_SOA, cap, 0, 14) == 2**64 - 1 and L.field_offset(9, cap, 0, 0) == 2**64 - 1
     # every (slot, field) has its own word in every layout
-    for lay, words in ((L.ADEPT_AOS, 16), (L.ADEPT_SOA, 14), (L.ADEPT_AOSOA32, 14), (L.ADEPT_AOSOA64, 14)):
+    for lay, words in ((L.ADEPT_AOS, 16), (L.ADEPT_SOA, 14), (L.ADEPT_AOSOA32, 14), (L.ADEPT_AOSOA64, 14),
+                       (L.ADEPT_SOA16, 14)):
         offs = {L.field_offset(lay, 128, s, f) for s in range(128) for f in range(14)}
         assert len(offs) == 128 * 14 and max(offs) < 128 * words * 4
 

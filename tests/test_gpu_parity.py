@@ -11,7 +11,7 @@ from tests.helpers import make_tracks, sort_by_id
 
 pytestmark = pytest.mark.gpu
 
-LAYOUTS = ("aos", "soa", "aosoa32", "aosoa64")
+LAYOUTS = ("aos", "soa", "aosoa32", "aosoa64", "soa16")
 SCHEMES = ("dense", "sparse")
 INT_FIELDS = ("vol", "id_lo", "id_hi", "step")
 F32_FIELDS = ("pos", "dir", "ekin", "nial")
@@ -172,7 +172,8 @@ def test_tiny_shower_matches_oracle_every_iteration(layout, scheme):
     ctx.destroy()
 
 
-@pytest.mark.parametrize("layout,scheme", [("soa", "dense"), ("aosoa32", "dense"), ("aosoa64", "dense"), ("aos", "sparse")])
+@pytest.mark.parametrize("layout,scheme", [("soa", "dense"), ("aosoa32", "dense"), ("aosoa64", "dense"), ("soa16", "dense"),
+                                           ("aos", "sparse")])
 def test_full_showers_run_matches_oracle(layout, scheme):
     """Config 2 at reduced primaries (100 x 1 GeV) so that the oracle takes well under a second."""
     c = CONFIGS["full"]
@@ -358,7 +359,7 @@ def test_instrumented_sparse_writes_only_what_changed():
 
 
 # ------------------------------------------- BASELINE.json sizes, bench.py's launch configuration ---
-@pytest.mark.parametrize("layout,scheme,n", [("aosoa32", "dense", 1 << 24), ("soa", "dense", 1 << 23),
+@pytest.mark.parametrize("layout,scheme,n", [("aosoa32", "dense", 1 << 24), ("soa", "dense", 1 << 23), ("soa16", "dense", 1 << 23),
                                              ("aos", "sparse", 1 << 23)])
 def test_single_step_at_full_size_counts_and_sampled_tracks(layout, scheme, n):
     """Config 3 as bench.py times it: 2^24 tracks, dense double buffer, AoSoA-32, one adept_step --
