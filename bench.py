@@ -34,11 +34,11 @@ if ROOT not in sys.path:
 from workloads import CONFIGS, gen_tracks, geometry_for, tables_for  # noqa: E402
 
 WORKLOAD = "single_step"
-RECORD_BYTES = {"aos": 64, "soa": 56, "aosoa32": 56, "aosoa64": 56, "soa16": 56}     # bytes per record per layout
+RECORD_BYTES = {"aos": 64, "soa": 56, "aosoa32": 56, "aosoa64": 56, "soa16": 56, "aosoa16": 56, "aosoa128": 56}     # bytes per record per layout
 # dram__bytes_read.sum + dram__bytes_write.sum of one step_kernel launch on this workload, from the
 # `ncu --set full` captures summarised in profiles/r1_step_kernel.md (r1g: AoSoA-32)
 NCU_TRAFFIC_BYTES = {"aosoa32": 942.4e6 + 1043.9e6, "soa": None, "aos": None,
-                     "aosoa64": None, "soa16": None}
+                     "aosoa64": None, "soa16": None, "aosoa16": None, "aosoa128": None}
 
 
 def measured_peak():
@@ -488,7 +488,7 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--layout", default="all", choices=["soa", "aosoa32", "aosoa64", "soa16", "aos", "all"])
+    ap.add_argument("--layout", default="all", choices=["soa", "aosoa32", "aosoa64", "soa16", "aos", "aosoa16", "aosoa128", "all"])
     ap.add_argument("--tracks", type=int, default=CONFIGS[WORKLOAD]["n_tracks"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--workload", default="single_step", choices=["single_step", "tiny", "full", "heavy", "sweep"],

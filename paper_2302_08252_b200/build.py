@@ -14,7 +14,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libadept_b200.so")
-SOURCES = ["layout_aos.cu", "layout_soa.cu", "layout_aosoa32.cu", "layout_aosoa64.cu", "layout_soa16.cu", "adept_api.cu"]
+SOURCES = ["layout_aos.cu", "layout_soa.cu", "layout_aosoa32.cu", "layout_aosoa64.cu", "layout_soa16.cu", "layout_aosoa16.cu", "layout_aosoa128.cu",
+           "adept_api.cu"]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "--fmad=false", "--prec-div=true", "--prec-sqrt=true", "--ftz=false",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]

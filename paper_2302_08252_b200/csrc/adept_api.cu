@@ -51,6 +51,8 @@ static const LayoutOps *ops_for(int layout) {
     case ADEPT_AOSOA32: return &kOpsAoSoA32;
     case ADEPT_AOSOA64: return &kOpsAoSoA64;
     case ADEPT_SOA16: return &kOpsSoA16;
+    case ADEPT_AOSOA16: return &kOpsAoSoA16;
+    case ADEPT_AOSOA128: return &kOpsAoSoA128;
     default: return nullptr;
   }
 }
@@ -640,6 +642,8 @@ uint64_t adept_field_offset(int32_t layout, uint32_t capacity, uint32_t slot, ui
     case ADEPT_AOSOA32: return 4 * Mapping<L_AOSOA32>::index(cap, slot, int(field));
     case ADEPT_AOSOA64: return 4 * Mapping<L_AOSOA64>::index(cap, slot, int(field));
     case ADEPT_SOA16: return 4 * Mapping<L_SOA16>::index(cap, slot, int(field));
+    case ADEPT_AOSOA16: return 4 * Mapping<L_AOSOA16>::index(cap, slot, int(field));
+    case ADEPT_AOSOA128: return 4 * Mapping<L_AOSOA128>::index(cap, slot, int(field));
     default: return UINT64_MAX;
   }
 }

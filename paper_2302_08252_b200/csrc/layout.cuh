@@ -20,7 +20,7 @@ enum Field : int {
   F_PX = 0, F_PY, F_PZ, F_DX, F_DY, F_DZ, F_EKIN, F_N0, F_N1, F_N2, F_VOL, F_IDLO, F_IDHI, F_STEP,
   kNumFields = 14
 };
-enum LayoutId : int { L_AOS = 0, L_SOA = 1, L_AOSOA32 = 2, L_AOSOA64 = 3, L_SOA16 = 4 };
+enum LayoutId : int { L_AOS = 0, L_SOA = 1, L_AOSOA32 = 2, L_AOSOA64 = 3, L_SOA16 = 4, L_AOSOA16 = 5, L_AOSOA128 = 6 };
 
 // A track in registers.
 struct Trk {
@@ -89,6 +89,8 @@ template <int N> struct AoSoAMapping {  // blocks of N tracks, field-major insid
 };
 template <> struct Mapping<L_AOSOA32> : AoSoAMapping<32> {};  // "AoSoA-n"
 template <> struct Mapping<L_AOSOA64> : AoSoAMapping<64> {};  // the paper's fastest
+template <> struct Mapping<L_AOSOA16> : AoSoAMapping<16> {};  // "several lane counts"
+template <> struct Mapping<L_AOSOA128> : AoSoAMapping<128> {};  // one block per tile
 // SoA of 16-byte field groups (SURVEY.md §8(f) item 1 "grouped-SoA of 16-byte vectors"; BASELINE.json
 // north_star "coalesced, vectorised 16-byte loads of SoA fields"): four arrays of `cap` vectors --
 // {pos.xyz, dir.x}, {dir.y, dir.z, ekin, nial.0}, {nial.1, nial.2, vol, id_lo} (16 B each) and

@@ -821,6 +821,6 @@ template <int L> struct OpsImpl {
   }
 };
 
-extern const LayoutOps kOpsAoS, kOpsSoA, kOpsAoSoA32, kOpsAoSoA64, kOpsSoA16;
+extern const LayoutOps kOpsAoS, kOpsSoA, kOpsAoSoA32, kOpsAoSoA64, kOpsSoA16, kOpsAoSoA16, kOpsAoSoA128;
 
 }  // namespace adept

@@ -67,6 +67,8 @@ def test_field_offset_follows_the_three_mappings(L):
             assert L.field_offset(L.ADEPT_SOA, cap, slot, f) == 4 * (f * cap + slot)       # 14 arrays
             assert L.field_offset(L.ADEPT_AOSOA32, cap, slot, f) == 4 * ((slot // 32) * 448 + f * 32 + slot % 32)
             assert L.field_offset(L.ADEPT_AOSOA64, cap, slot, f) == 4 * ((slot // 64) * 896 + f * 64 + slot % 64)
+            for lay, n in ((5, 16), (6, 128)):                                      # more AoSoA lane counts
+                assert L.field_offset(lay, cap, slot, f) == 4 * ((slot // n) * 14 * n + f * n + slot % n)
             want = (f // 4) * 16 * cap + slot * 16 + (f % 4) * 4 if f < 12 else 48 * cap + slot * 8 + (f - 12) * 4
             assert L.field_offset(L.ADEPT_SOA16, cap, slot, f) == want          # 16-byte field groups
     assert L.field_offset(L.ADEPT_SOA, cap, 0, 14) == 2**64 - 1 and L.field_offset(9, cap, 0, 0) == 2**64 - 1
