@@ -577,7 +577,7 @@ int adept_run(adept_ctx *c, uint64_t max_iterations, adept_result *out) {
   // iteration with nothing alive is a no-op on the device (and is not counted), so over-shooting
   // the end of a shower by a few launches is harmless.
 #ifndef ADEPT_RUN_BURST
-#define ADEPT_RUN_BURST 8
+#define ADEPT_RUN_BURST 16
 #endif
   const uint64_t kBurst = ADEPT_RUN_BURST;
   uint64_t done = 0;
