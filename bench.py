@@ -36,8 +36,8 @@ from workloads import CONFIGS, gen_tracks, geometry_for, tables_for  # noqa: E40
 WORKLOAD = "single_step"
 RECORD_BYTES = {"aos": 64, "soa": 56, "aosoa32": 56, "aosoa64": 56, "soa16": 56, "aosoa16": 56, "aosoa128": 56}     # bytes per record per layout
 # dram__bytes_read.sum + dram__bytes_write.sum of one step_kernel launch on this workload, from the
-# `ncu --set full` captures summarised in profiles/r1_step_kernel.md (r1g: AoSoA-32)
-NCU_TRAFFIC_BYTES = {"aosoa32": 942.4e6 + 1043.9e6, "soa": None, "aos": None,
+# `ncu --set full` captures summarised in profiles/r1_step_kernel.md (r1i: AoSoA-32)
+NCU_TRAFFIC_BYTES = {"aosoa32": 944.8e6 + 1046.6e6, "soa": None, "aos": None,
                      "aosoa64": None, "soa16": None, "aosoa16": None, "aosoa128": None}
 
 
