@@ -103,7 +103,7 @@ def population(n_tracks: int, rank: int):
     return gen_tracks(n_tracks, c["seed"] + 1000 * rank, geometry_for(WORKLOAD), c["e_max"], c["fractions"])
 
 
-def oracle_single_step(pop, sample_tracks: int):
+def oracle_single_step(pop, sample_tracks: int, want_tracks: bool = False):
     """Time the oracle, as it stands, on the first `sample_tracks` tracks of each kind's share."""
     from oracle import Oracle
     c = CONFIGS[WORKLOAD]
@@ -119,16 +119,16 @@ def oracle_single_step(pop, sample_tracks: int):
     o.step()
     dt = time.perf_counter() - t0
     r = o.result()
-    r["sample"] = [sample_of(o.read_tracks(k, pop[0].dtype)) for k in range(3)]
+    if want_tracks:
+        r["tracks"] = [by_id(o.read_tracks(k, pop[0].dtype)) for k in range(3)]
     o.close()
     return n, dt, r
 
 
-def sample_of(tracks):
-    """1/64 of the tracks by id, in id order: what the full-size parity check compares word for word."""
-    t = tracks[(tracks["id_lo"] & 63) == 5]
-    key = t["id_hi"].astype(np.uint64) << np.uint64(32) | t["id_lo"].astype(np.uint64)
-    return t[np.argsort(key, kind="stable")]
+def by_id(tracks):
+    """All tracks in id order: the full-size parity check compares every one of them word for word."""
+    key = tracks["id_hi"].astype(np.uint64) << np.uint64(32) | tracks["id_lo"].astype(np.uint64)
+    return tracks[np.argsort(key, kind="stable")]
 
 
 def run_reference(args, rank: int):
@@ -186,7 +186,7 @@ def bench_layout(ctx, torch, pop, steps, warmup, flush, barrier):
     wall = time.perf_counter() - t0
     ms = [e0.elapsed_time(e1) for e0, e1 in ev]
     res = ctx.result()
-    res["sample"] = [sample_of(ctx.read_tracks(k)) for k in range(3)]
+    res["tracks"] = [by_id(ctx.read_tracks(k)) for k in range(3)]
     del pristine
     return ms, res, wall
 
@@ -325,7 +325,7 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
         "layouts": per_layout,
     }
     if world == 1 and not args.no_cpu:
-        n, dt, r = oracle_single_step(pop, n_tracks)
+        n, dt, r = oracle_single_step(pop, n_tracks, want_tracks=True)
         out["cpu_baseline"] = {"value": n / dt, "unit": "track-steps/s", "cores": 1, "kind": "oracle",
                                "sample": "one oracle iteration over all %d tracks of the same population" % n,
                                "seconds": dt}
@@ -333,7 +333,7 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
         # discrete-branch disagreements (north_star: to be reported): a track that took another branch
         # on the GPU has another fate -- it is missing, extra, or of another kind in the output sample
         n_cmp = n_missing = n_diff = 0
-        for a, b in zip(main_res["sample"], r["sample"]):
+        for a, b in zip(main_res["tracks"], r["tracks"]):
             ka = a["id_hi"].astype(np.uint64) << np.uint64(32) | a["id_lo"].astype(np.uint64)
             kb = b["id_hi"].astype(np.uint64) << np.uint64(32) | b["id_lo"].astype(np.uint64)
             common = np.intersect1d(ka, kb)
@@ -429,13 +429,15 @@ def run_sweep(args):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     layouts = ["aos", "soa", "aosoa32", "aosoa64", "soa16"] if args.layout == "all" else [args.layout]
     cells = []
-    for occ in c["occupancies"]:
+    occupancies = c["occupancies"] if args.occupancy is None else (args.occupancy,)
+    schemes = ("dense", "sparse") if args.scheme is None else (args.scheme,)
+    for occ in occupancies:
         pop = gen_sweep(occ)
         n_live = sum(p["tracks"].shape[0] for p in pop)
-        for scheme in ("dense", "sparse"):
+        for scheme in schemes:
             for layout in layouts:
                 cell = {"occupancy": occ, "scheme": scheme, "layout": layout, "tracks": n_live}
-                for instrument in (False, True):
+                for instrument in ((False,) if args.no_instr else (False, True)):
                     ctx = Context(geo, tab, layout=layout, scheme=scheme, capacity=cap, seed=c["seed"],
                                   instrument=instrument)
                     for k in range(3):
@@ -473,8 +475,8 @@ def run_sweep(args):
                     del ctx
                     torch.cuda.empty_cache()
                 cells.append(cell)
-                sys.stderr.write("%s\n" % json.dumps({k: cell[k] for k in ("occupancy", "scheme", "layout", "ms_per_step",
-                                                                            "bytes_touched_per_track_step")}))
+                sys.stderr.write("%s\n" % json.dumps({k: cell.get(k) for k in ("occupancy", "scheme", "layout", "ms_per_step",
+                                                                                "bytes_touched_per_track_step")}))
     best = max(cells, key=lambda x: x["track_steps_per_s"])
     print(json.dumps({"metric": "track-steps/sec", "value": best["track_steps_per_s"], "unit": "track-steps/s",
                       "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": best["ms_per_step"],
@@ -497,7 +499,10 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--workload", default="single_step", choices=["single_step", "tiny", "full", "heavy", "sweep"],
                     help="single_step = the headline (BASELINE.json configs[2]); the others are reported beside it")
-    ap.add_argument("--scheme", default="dense", choices=["dense", "sparse"], help="shower workloads only")
+    ap.add_argument("--scheme", default=None, choices=["dense", "sparse"],
+                    help="shower workloads: container (default dense); sweep: only this scheme (default both)")
+    ap.add_argument("--occupancy", type=float, default=None, help="sweep: only this occupancy (default 0.1 .. 0.9)")
+    ap.add_argument("--no-instr", action="store_true", help="sweep: skip the instrumented (counting) contexts")
     ap.add_argument("--batch", type=int, default=0, help="shower workloads: batch_primaries (0 = all at once)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
@@ -509,6 +514,7 @@ def main():
         return
     if args.workload in ("tiny", "full", "heavy"):
         if rank == 0:
+            args.scheme = args.scheme or "dense"
             run_showers(args, args.workload)
         return
     if args.workload == "sweep":

@@ -23,7 +23,8 @@
  *  - A context is not thread-safe.  Units: MeV, mm.  Particle kinds: 0 = e-, 1 = e+, 2 = gamma.
  *  - Capacity overflow: a full buffer/queue sets a device flag, the step completes without any
  *    out-of-bounds write (excess tracks are dropped), and the next synchronising call returns
- *    ADEPT_ECAPACITY; afterwards only adept_reset / adept_destroy are accepted.
+ *    ADEPT_ECAPACITY; afterwards only adept_reset / adept_destroy are accepted.  The same flag is
+ *    raised if an energy tally leaves its 64-bit fixed-point range (2^32 MeV in one slab).
  *
  * Workspace.  The workspace holds the complete device state of a context (control block, tables,
  * track buffers, queues, tallies).  A byte copy of it taken while no call is in flight may be
@@ -151,15 +152,24 @@ int adept_set_primary_index(adept_ctx *, uint64_t next_index);
 int adept_step(adept_ctx *, adept_counts *out);
 
 /* Iterate until no track is alive (and no primary is pending), or max_iterations (0 = no limit)
- * iterations were done in this call.  Fills *out (tallies are cumulative since create/reset). */
+ * iterations were done in this call -- iterations as adept_counts.iterations counts them: those in
+ * which at least one track was alive.  The limit is tested before a pending batch is injected, so no
+ * un-stepped batch is left behind.  Fills *out (tallies are cumulative since create/reset). */
 int adept_run(adept_ctx *, uint64_t max_iterations, adept_result *out);
 
 /* Fill *out with the current tallies without stepping (synchronises). */
 int adept_get_result(adept_ctx *, adept_result *out);
 
 /* Append n tracks (host array, 56-byte records) to kind's live set.  slots (host, n entries) is
- * used by the sparse scheme only: slot of each track, all distinct, free and < capacity; NULL =
- * next free slots.  The queue order is the array order. */
+ * used by the sparse scheme only: slot of each track, all distinct, free and < capacity (slots are
+ * handed out by a bump allocator, rule S30: the free ones are those at or above its top, i.e. above
+ * every slot used so far); NULL = next free slots.  The queue order is the array order.
+ * Preconditions on every record (the step indexes geometry and tallies by vol, packs flags into the
+ * top bits of step, and divides by the direction cosines): vol < 2*n_layers; step < 2^20;
+ * e_cut <= ekin <= e_max (an e+ may also have 0 <= ekin < e_cut: it annihilates at its next step,
+ * rule S17); pos and dir finite, dir not the zero vector; nial not NaN.
+ * EINVAL if a slot or a record breaks these (records are checked on the device while they are
+ * unpacked); nothing is changed then. */
 int adept_load_tracks(adept_ctx *, uint32_t kind, const adept_track *tracks, uint64_t n,
                       const uint32_t *slots);
 

@@ -230,7 +230,7 @@ class Context:
             assert out.dtype.itemsize == 56 and out.flags["C_CONTIGUOUS"]
             self._check(self._L.adept_read_tracks(self._h, kind, out.ctypes.data, out.shape[0], C.byref(n)))
             return int(n.value)
-        cap = self.capacity + 32 if cap is None else cap
+        cap = (self.capacity + 127) // 128 * 128 if cap is None else cap    # the library rounds capacity up to whole tiles
         buf = np.empty(cap, dtype=TRACK_DTYPE)
         self._check(self._L.adept_read_tracks(self._h, kind, buf.ctypes.data, cap, C.byref(n)))
         return buf[: n.value].copy()

@@ -108,6 +108,10 @@ struct adept_ctx {
   const LayoutOps *ops;
   Params params;
   cudaStream_t stream;
+  // host <-> device record transfers alternate between the two halves of the staging block: the copy
+  // of one half (on copy_stream) overlaps the pack/unpack kernel of the other (on `stream`)
+  cudaStream_t copy_stream;
+  cudaEvent_t ev_copied[2], ev_kernel[2];
   struct Shape { int threads; unsigned grid; size_t dyn_smem; } small, large;  // CTA shapes of the step kernel
   uint64_t live_hint;     // live tracks as last seen by the host: picks the shape
   unsigned char *ws;
@@ -123,6 +127,16 @@ struct adept_ctx {
 };
 
 namespace {
+
+void free_host_side(adept_ctx *c) {
+  if (c->pinned) cudaFreeHost(c->pinned);
+  if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+  for (int h = 0; h < 2; ++h) {
+    if (c->ev_copied[h]) cudaEventDestroy(c->ev_copied[h]);
+    if (c->ev_kernel[h]) cudaEventDestroy(c->ev_kernel[h]);
+  }
+  delete c;
+}
 
 int fail(adept_ctx *c, int code, const char *what, cudaError_t e = cudaSuccess) {
   if (c) {
@@ -183,6 +197,8 @@ void fill_result(const adept_ctx *c, adept_result *out) {
 }
 
 // write n_cur / slot_top / slots_used of one kind after a host-driven append
+__global__ void clear_bad_input_kernel(Ctl *ctl) { ctl->bad_input = 0u; }
+
 __global__ void set_counts_kernel(Ctl *ctl, int kind, uint32_t n_cur, uint32_t slot_top, unsigned long long used) {
   ctl->n_cur[kind] = n_cur;
   ctl->slot_top[kind] = slot_top;
@@ -262,18 +278,26 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
   c->stream = static_cast<cudaStream_t>(cfg->cuda_stream);
   c->ws = static_cast<unsigned char *>(cfg->workspace);
   c->pinned = nullptr;
+  c->copy_stream = nullptr;
+  for (int h = 0; h < 2; ++h) c->ev_copied[h] = c->ev_kernel[h] = nullptr;
   c->pitch = g->abs_mm + g->gap_mm;
   c->depth = static_cast<float>(g->n_layers) * c->pitch;
   auto die = [&](const char *what, cudaError_t e) {
     g_create_error = std::string(what) + ": " + cudaGetErrorString(e);
-    if (c->pinned) cudaFreeHost(c->pinned);
-    delete c;
+    free_host_side(c);
     return ADEPT_ECUDA;
   };
   cudaError_t e;
   c->pinned_bytes = kCtlHeaderBytes + (size_t(2) * g->n_layers + 1) * sizeof(unsigned long long);
   if ((e = cudaMallocHost(reinterpret_cast<void **>(&c->pinned), c->pinned_bytes)) != cudaSuccess)
     return die("cudaMallocHost", e);
+  if ((e = cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking)) != cudaSuccess)
+    return die("cudaStreamCreateWithFlags", e);
+  for (int h = 0; h < 2; ++h) {
+    if ((e = cudaEventCreateWithFlags(&c->ev_copied[h], cudaEventDisableTiming)) != cudaSuccess ||
+        (e = cudaEventCreateWithFlags(&c->ev_kernel[h], cudaEventDisableTiming)) != cudaSuccess)
+      return die("cudaEventCreateWithFlags", e);
+  }
 
   // tables: [mat][group][qty][node] (host, ABI) -> [group][mat][node]{q0,q1,q2,0} (device): a CTA
   // stages only the group of the particle kind it is stepping, and one 16-byte shared-memory load
@@ -295,7 +319,7 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
   p.tables = reinterpret_cast<const float4 *>(c->ws + pl.tables);
   p.table_bytes = static_cast<uint32_t>(pl.table_bytes / 2);  // per particle group
   p.nodes = nodes;
-  p.ln_e_min = t->ln_e_min; p.inv_dln = t->inv_dln; p.e_cut = t->e_cut;
+  p.ln_e_min = t->ln_e_min; p.inv_dln = t->inv_dln; p.e_cut = t->e_cut; p.e_max = t->e_max;
   p.n_slabs = 2 * g->n_layers;
   p.abs_mm = g->abs_mm; p.pitch = c->pitch; p.half_xy = g->half_xy_mm;
   p.mat_abs = g->mat_abs; p.mat_gap = g->mat_gap;
@@ -350,8 +374,7 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
   const int per_sm = c->ops->step_ctas_per_sm(cfg->scheme, instr, kBlockSmall, c->small.dyn_smem);
   if (per_sm <= 0) {
     g_create_error = "step kernel does not fit on an SM with these tables (shared memory)";
-    cudaFreeHost(c->pinned);
-    delete c;
+    free_host_side(c);
     return ADEPT_EINVAL;
   }
   c->small.grid = static_cast<unsigned>(sms * per_sm);
@@ -366,8 +389,7 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
   if (rc == ADEPT_OK && (e = cudaStreamSynchronize(c->stream)) != cudaSuccess) rc = ADEPT_ECUDA;
   if (rc != ADEPT_OK) {
     g_create_error = c->err.empty() ? "clearing the workspace failed" : c->err;
-    cudaFreeHost(c->pinned);
-    delete c;
+    free_host_side(c);
     return rc;
   }
   *out = c;
@@ -377,8 +399,8 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
 int adept_destroy(adept_ctx *c) {
   if (!c) return ADEPT_EINVAL;
   cudaStreamSynchronize(c->stream);
-  if (c->pinned) cudaFreeHost(c->pinned);
-  delete c;
+  cudaStreamSynchronize(c->copy_stream);
+  free_host_side(c);
   return ADEPT_OK;
 }
 
@@ -490,30 +512,55 @@ int adept_load_tracks(adept_ctx *c, uint32_t kind, const adept_track *tracks, ui
   uint32_t top = h.slot_top[kind];
   if (sparse) {
     if (slots) {
+      // "all distinct, free and < capacity": slots are handed out by a bump allocator (rule S30), so
+      // the free ones are exactly those at or above its top; distinctness by a bitmap over them
+      std::vector<uint64_t> seen((size_t(cap - h.slot_top[kind]) + 63) / 64, 0ull);
       for (uint64_t i = 0; i < n; ++i) {
         if (slots[i] >= cap) return fail(c, ADEPT_EINVAL, "adept_load_tracks: slot out of range");
+        if (slots[i] < h.slot_top[kind]) return fail(c, ADEPT_EINVAL, "adept_load_tracks: slot is not free");
+        const uint32_t r = slots[i] - h.slot_top[kind];
+        if (seen[r >> 6] & (1ull << (r & 63))) return fail(c, ADEPT_EINVAL, "adept_load_tracks: duplicate slot");
+        seen[r >> 6] |= 1ull << (r & 63);
         top = std::max(top, slots[i] + 1u);
       }
     } else {
       if (top + n > cap) return fail(c, ADEPT_EINVAL, "adept_load_tracks: more tracks than free slots");
     }
   }
+  // Chunks alternate between the two halves of the staging block: the host-to-device copy of one
+  // half (copy_stream) overlaps the unpack kernel of the other (the context's stream).  The records
+  // themselves are validated by the unpack kernel (Ctl::bad_input).
+  const uint32_t half = std::max<uint32_t>(1u, c->plan.stage_records / 2);
   uint32_t n_cur = h.n_cur[kind], next_slot = h.slot_top[kind];
-  for (uint64_t done = 0; done < n;) {
-    const uint32_t m = uint32_t(std::min<uint64_t>(n - done, c->plan.stage_records));
-    CU(c, cudaMemcpyAsync(c->ws + c->plan.stage, tracks + done, size_t(m) * sizeof(adept_track),
-                          cudaMemcpyHostToDevice, c->stream));
+  CU(c, cudaEventRecord(c->ev_kernel[0], c->stream));   // everything enqueued so far precedes the first copies
+  CU(c, cudaEventRecord(c->ev_kernel[1], c->stream));
+  int hb = 0;
+  for (uint64_t done = 0; done < n; hb ^= 1) {
+    const uint32_t m = uint32_t(std::min<uint64_t>(n - done, half));
+    unsigned char *stage = c->ws + c->plan.stage + size_t(hb) * half * kStageRecordBytes;
+    uint32_t *stage_slots = reinterpret_cast<uint32_t *>(c->ws + c->plan.stage_slots) + size_t(hb) * half;
+    CU(c, cudaStreamWaitEvent(c->copy_stream, c->ev_kernel[hb], 0));   // the half's previous chunk was consumed
+    CU(c, cudaMemcpyAsync(stage, tracks + done, size_t(m) * sizeof(adept_track), cudaMemcpyHostToDevice, c->copy_stream));
     const uint32_t *dslots = nullptr;
     if (sparse && slots) {
-      CU(c, cudaMemcpyAsync(c->ws + c->plan.stage_slots, slots + done, size_t(m) * 4, cudaMemcpyHostToDevice, c->stream));
-      dslots = reinterpret_cast<const uint32_t *>(c->ws + c->plan.stage_slots);
+      CU(c, cudaMemcpyAsync(stage_slots, slots + done, size_t(m) * 4, cudaMemcpyHostToDevice, c->copy_stream));
+      dslots = stage_slots;
     }
-    CU(c, c->ops->launch_load(c->cfg.scheme, c->params, c->ws + c->plan.stage, dslots, m, int(kind), h.parity, n_cur,
-                              next_slot, c->stream));
-    CU(c, cudaStreamSynchronize(c->stream));
+    CU(c, cudaEventRecord(c->ev_copied[hb], c->copy_stream));
+    CU(c, cudaStreamWaitEvent(c->stream, c->ev_copied[hb], 0));
+    CU(c, c->ops->launch_load(c->cfg.scheme, c->params, stage, dslots, m, int(kind), h.parity, n_cur, next_slot, c->stream));
+    CU(c, cudaEventRecord(c->ev_kernel[hb], c->stream));
     n_cur += m;
     next_slot += m;
     done += m;
+  }
+  rc = fetch_ctl(c, false);   // synchronises: the caller's arrays are free again
+  if (rc != ADEPT_OK) return rc;
+  if (host_ctl(c)->bad_input) {
+    clear_bad_input_kernel<<<1, 1, 0, c->stream>>>(c->params.ctl);
+    CU(c, cudaGetLastError());
+    CU(c, cudaStreamSynchronize(c->stream));
+    return fail(c, ADEPT_EINVAL, "adept_load_tracks: a record breaks the preconditions (vol, step, ekin, dir; see adept.h)");
   }
   if (sparse && !slots) top = next_slot;
   c->live_hint += n;
@@ -529,15 +576,25 @@ int adept_read_tracks(adept_ctx *c, uint32_t kind, adept_track *out, uint64_t ca
   const Ctl h = *host_ctl(c);
   *n = h.n_cur[kind];
   if (*n > cap || (*n && !out)) return fail(c, ADEPT_EINVAL, "adept_read_tracks: output array too small");
-  for (uint64_t done = 0; done < *n;) {
-    const uint32_t m = uint32_t(std::min<uint64_t>(*n - done, c->plan.stage_records));
-    CU(c, c->ops->launch_read(c->cfg.scheme, c->params, c->ws + c->plan.stage, uint32_t(done), m, int(kind), h.parity,
-                              c->stream));
-    CU(c, cudaMemcpyAsync(out + done, c->ws + c->plan.stage, size_t(m) * sizeof(adept_track), cudaMemcpyDeviceToHost,
-                          c->stream));
-    CU(c, cudaStreamSynchronize(c->stream));
+  // pack kernel of one half of the staging block (the context's stream) overlaps the device-to-host
+  // copy of the other (copy_stream)
+  const uint32_t half = std::max<uint32_t>(1u, c->plan.stage_records / 2);
+  CU(c, cudaEventRecord(c->ev_copied[0], c->copy_stream));
+  CU(c, cudaEventRecord(c->ev_copied[1], c->copy_stream));
+  int hb = 0;
+  for (uint64_t done = 0; done < *n; hb ^= 1) {
+    const uint32_t m = uint32_t(std::min<uint64_t>(*n - done, half));
+    unsigned char *stage = c->ws + c->plan.stage + size_t(hb) * half * kStageRecordBytes;
+    CU(c, cudaStreamWaitEvent(c->stream, c->ev_copied[hb], 0));   // the half's previous chunk has left
+    CU(c, c->ops->launch_read(c->cfg.scheme, c->params, stage, uint32_t(done), m, int(kind), h.parity, c->stream));
+    CU(c, cudaEventRecord(c->ev_kernel[hb], c->stream));
+    CU(c, cudaStreamWaitEvent(c->copy_stream, c->ev_kernel[hb], 0));
+    CU(c, cudaMemcpyAsync(out + done, stage, size_t(m) * sizeof(adept_track), cudaMemcpyDeviceToHost, c->copy_stream));
+    CU(c, cudaEventRecord(c->ev_copied[hb], c->copy_stream));
     done += m;
   }
+  CU(c, cudaStreamSynchronize(c->copy_stream));
+  CU(c, cudaStreamSynchronize(c->stream));
   return rc;
 }
 
@@ -574,17 +631,21 @@ int adept_run(adept_ctx *c, uint64_t max_iterations, adept_result *out) {
   int rc = check_alive(c);
   if (rc != ADEPT_OK) return rc;
   // Iterations are enqueued in bursts; the control block is read back after each burst.  An
-  // iteration with nothing alive is a no-op on the device (and is not counted), so over-shooting
-  // the end of a shower by a few launches is harmless.
+  // iteration with nothing alive is a no-op on the device and is not counted (Ctl::iterations), so
+  // over-shooting the end of a batch by a few launches is harmless; progress against
+  // max_iterations is what the device counted, not what the host enqueued.
 #ifndef ADEPT_RUN_BURST
 #define ADEPT_RUN_BURST 16
 #endif
   const uint64_t kBurst = ADEPT_RUN_BURST;
-  uint64_t done = 0;
-  for (;;) {
+  uint64_t first_iteration = 0;
+  for (bool first = true;; first = false) {
     rc = fetch_ctl(c, false);
     if (rc != ADEPT_OK) break;
     const Ctl *h = host_ctl(c);
+    if (first) first_iteration = h->iterations;
+    const uint64_t done = h->iterations - first_iteration;
+    if (max_iterations && done >= max_iterations) break;
     const uint64_t live = uint64_t(h->n_cur[0]) + h->n_cur[1] + h->n_cur[2];
     if (live == 0) {
       if (c->pending_done >= c->pending.size()) break;
@@ -595,12 +656,10 @@ int adept_run(adept_ctx *c, uint64_t max_iterations, adept_result *out) {
       c->pending_done += batch;
       if (c->pending_done >= c->pending.size()) { c->pending.clear(); c->pending_done = 0; }
     }
-    if (max_iterations && done >= max_iterations) break;
     uint64_t burst = kBurst;
     if (max_iterations) burst = std::min<uint64_t>(burst, max_iterations - done);
     for (uint64_t i = 0; i < burst && rc == ADEPT_OK; ++i) rc = launch_iteration(c);
     if (rc != ADEPT_OK) break;
-    done += burst;
   }
   if (out && (rc == ADEPT_OK || rc == ADEPT_ECAPACITY)) {
     const int rc2 = fetch_ctl(c, true);

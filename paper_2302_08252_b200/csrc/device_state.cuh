@@ -31,7 +31,7 @@ constexpr int kBlockSmall = 256, kBlockLarge = 1024;
 constexpr int kGroup = ADEPT_GROUP;
 constexpr int kMaxGroupsPerCta = kBlockLarge / kGroup;
 constexpr int kWarpsPerGroup = kGroup / 32;
-static_assert(kGroup == 64 || kGroup == 128, "a group is 2 or 4 warps (arrival word: 3 x 9-bit counts + 3-bit ticket)");
+static_assert(kGroup == 128, "a group is 4 warps (arrival word: 3 x 9-bit counts + 3-bit ticket; an AoSoA-128 block is one tile)");
 // Shared-memory queue (one per group) of tracks parked between the two halves of the step, entry-
 // major.  At most kGroup - 1 left over from earlier tiles plus kGroup from the current one.
 constexpr int kQueueCap = 2 * kGroup;
@@ -71,7 +71,7 @@ struct Ctl {
   uint32_t parity;       // which array / list is "current"
   uint32_t overflow;     // sticky
   uint32_t done_ctas;    // ticket counter: the last CTA of a step kernel ends the iteration
-  uint32_t pad0;
+  uint32_t bad_input;    // set by load_kernel when a record breaks the preconditions of adept_load_tracks
   uint32_t it_alive[4];    // this iteration: parents that survive, per kind (reset at iteration end)
   uint32_t it_escaped[4];  // this iteration: parents that left the calorimeter, per kind
   unsigned long long steps[3], secondaries[3], killed[3], escaped_n[3], slots_used[3];
@@ -96,7 +96,7 @@ struct Params {
   const float4 *tables;      // [group][material][node] {q0, q1, q2, 0}; group 0 = gamma, 1 = e+-
   uint32_t table_bytes;      // bytes of ONE group, multiple of 16
   uint32_t nodes;            // n_bins + 1
-  float ln_e_min, inv_dln, e_cut;
+  float ln_e_min, inv_dln, e_cut, e_max;
   uint32_t n_slabs;
   float abs_mm, pitch, half_xy;
   uint32_t mat_abs, mat_gap;

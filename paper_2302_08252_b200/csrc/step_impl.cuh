@@ -27,6 +27,9 @@
 //   A12     the instrumented instantiation counts every accessor call.
 #pragma once
 #include <cstdint>
+#include <map>
+#include <mutex>
+#include <utility>
 #include <cuda_runtime.h>
 
 #include "device_state.cuh"
@@ -135,6 +138,7 @@ __device__ __forceinline__ void prefetch_tile(const Params &p, int kind, uint32_
                n2 * (gI < 3 ? 16u : 8u), mbar);
   } else {  // AoSoA-n: whole blocks, one contiguous run
     constexpr uint32_t kL = Mapping<L>::kLanes;
+    static_assert(kL <= uint32_t(kGroup), "a staged tile holds whole AoSoA blocks");
     const uint32_t bytes = ((n + kL - 1u) / kL) * (kL * kNumFields * 4u);
     const uint32_t *src = rec + size_t(first / kL) * (kL * kNumFields);
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
@@ -638,7 +642,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == kBlockSmall) ? ADEPT_STEP
     __syncthreads();
     for (uint32_t s = tid; s <= p.n_slabs; s += kBlock) {
       const unsigned long long v = (static_cast<unsigned long long>(c.bins.hi[s]) << 32) + c.bins.lo[s];
-      if (v != 0ull) atomicAdd(&p.tally[s], v);
+      if (v != 0ull && atomicAdd(&p.tally[s], v) + v < v) ctl->overflow = 1u;  // 2^32 MeV in one bin: reported, not wrapped silently
     }
     if (tid < 3) {
       if (sh.alive[tid]) atomicAdd(&ctl->it_alive[tid], sh.alive[tid]);
@@ -737,9 +741,22 @@ __global__ void load_kernel(const __grid_constant__ Params p, const PackedTrack 
                             uint32_t n, int kind, uint32_t par, uint32_t entry_base, uint32_t slot_base) {
   const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
+  const PackedTrack a = src[i];
+  // preconditions of adept_load_tracks (include/adept.h): the step kernel indexes the slab geometry and
+  // the tally bins by `vol`, packs the pending interaction into the top bits of `step`, and divides by
+  // the direction cosines
+  const bool finite = isfinite(a.pos[0]) && isfinite(a.pos[1]) && isfinite(a.pos[2]) && isfinite(a.dir[0]) &&
+                      isfinite(a.dir[1]) && isfinite(a.dir[2]) && !isnan(a.nial[0]) && !isnan(a.nial[1]) &&
+                      !isnan(a.nial[2]);
+  const bool moving = a.dir[0] != 0.0f || a.dir[1] != 0.0f || a.dir[2] != 0.0f;
+  const bool energy = (a.ekin >= p.e_cut && a.ekin <= p.e_max) || (kind == K_EP && a.ekin >= 0.0f && a.ekin < p.e_cut);
+  if (!(finite && moving && energy && a.vol < p.n_slabs && a.step < (1u << 20))) {
+    p.ctl->bad_input = 1u;
+    return;
+  }
   int buf; uint32_t where;
   place<SCHEME>(p, kind, par, entry_base + i, slots ? slots[i] : slot_base + i, buf, where);
-  plain_view<L>(p, kind, buf).store(where, unpack(src[i]));
+  plain_view<L>(p, kind, buf).store(where, unpack(a));
 }
 
 template <int L, int SCHEME>
@@ -768,6 +785,23 @@ struct LayoutOps {
                              uint32_t par, cudaStream_t);
 };
 
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a property of (device, kernel instantiation), shared
+// by every context of the process: keep a running maximum and never lower it, so that a later context
+// with smaller tables cannot break the launches of an earlier, larger one.
+inline cudaError_t ensure_dynamic_smem(const void *kernel, size_t bytes) {
+  static std::mutex mu;
+  static std::map<std::pair<int, const void *>, size_t> granted;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  std::lock_guard<std::mutex> lock(mu);
+  size_t &have = granted[std::make_pair(dev, kernel)];
+  if (bytes <= have) return cudaSuccess;
+  e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(bytes));
+  if (e == cudaSuccess) have = bytes;
+  return e;
+}
+
 template <int L> struct OpsImpl {
   template <int T, typename F> static auto pick_t(int scheme, int instr, F f) {
     if (scheme == S_DENSE) return instr ? f(step_kernel<L, S_DENSE, true, T>) : f(step_kernel<L, S_DENSE, false, T>);
@@ -780,7 +814,7 @@ template <int L> struct OpsImpl {
   static int step_ctas_per_sm(int scheme, int instr, int threads, size_t dyn) {
     return pick(scheme, instr, threads, [&](auto *k) {
       int n = 0;
-      if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, int(dyn)) != cudaSuccess) return -1;
+      if (ensure_dynamic_smem(reinterpret_cast<const void *>(k), dyn) != cudaSuccess) return -1;
       if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k, threads, dyn) != cudaSuccess) return -1;
       return n;
     });
@@ -788,6 +822,8 @@ template <int L> struct OpsImpl {
   static cudaError_t launch_step(int scheme, int instr, const Params &p, int threads, unsigned grid, size_t dyn,
                                  cudaStream_t s) {
     return pick(scheme, instr, threads, [&](auto *k) {
+      const cudaError_t e = ensure_dynamic_smem(reinterpret_cast<const void *>(k), dyn);
+      if (e != cudaSuccess) return e;
       k<<<grid, threads, dyn, s>>>(p);
       return cudaGetLastError();
     });

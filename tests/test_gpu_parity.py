@@ -359,17 +359,39 @@ def test_instrumented_sparse_writes_only_what_changed():
 
 
 # ------------------------------------------- BASELINE.json sizes, bench.py's launch configuration ---
-@pytest.mark.parametrize("layout,scheme,n", [("aosoa32", "dense", 1 << 24), ("soa", "dense", 1 << 23), ("soa16", "dense", 1 << 23),
-                                             ("aos", "sparse", 1 << 23)])
-def test_single_step_at_full_size_counts_and_sampled_tracks(layout, scheme, n):
+_FULL_SIZE_CACHE = {}
+
+
+def _full_size_reference(n):
+    """Population and oracle step of config 3 at n tracks (computed once per size)."""
+    if n not in _FULL_SIZE_CACHE:
+        _FULL_SIZE_CACHE.clear()                       # one size at a time: the arrays are ~1 GB each
+        c = CONFIGS["single_step"]
+        geo, tab = geometry_for("single_step"), tables_for("single_step")
+        pop = gen_tracks(n, c["seed"], geo, c["e_max"], c["fractions"])
+        o = Oracle(geo, tab, seed=c["seed"])
+        for k in range(3):
+            o.load_tracks(k, pop[k])
+        o.step()
+        ref = [sort_by_id(o.read_tracks(k, pop[0].dtype)) for k in range(3)]
+        _FULL_SIZE_CACHE[n] = (geo, tab, pop, o.result(), ref)
+        o.close()
+    return _FULL_SIZE_CACHE[n]
+
+
+@pytest.mark.parametrize("layout,scheme,n", [("aosoa32", "dense", 1 << 24),
+                                             ("soa", "dense", 1 << 23), ("soa16", "dense", 1 << 23),
+                                             ("aos", "dense", 1 << 23), ("aosoa64", "dense", 1 << 23),
+                                             ("aos", "sparse", 1 << 23), ("soa", "sparse", 1 << 23),
+                                             ("aosoa32", "sparse", 1 << 23)])
+def test_single_step_at_full_size_counts_and_every_track(layout, scheme, n):
     """Config 3 as bench.py times it: 2^24 tracks, dense double buffer, AoSoA-32, one adept_step --
-    and 2^23 tracks in two more variants; all above the population at which the library switches to
-    its 1024-thread CTAs.  All integer counts and the per-slab deposits against the oracle's
-    full-size step, and every surviving / created track of a sample of 1/64 of the id space
-    compared word for word."""
+    and 2^23 tracks in seven more layout x scheme variants; all above the population at which the
+    library switches to its 1024-thread CTAs.  All integer counts and the per-slab deposits against
+    the oracle's full-size step, and EVERY surviving / created track compared word for word (sorted
+    by id), so that every lane position of the 1024-thread shape is covered."""
     c = CONFIGS["single_step"]
-    geo, tab = geometry_for("single_step"), tables_for("single_step")
-    pop = gen_tracks(n, c["seed"], geo, c["e_max"], c["fractions"])
+    geo, tab, pop, r, ref = _full_size_reference(n)
     cap = int(max(p.shape[0] for p in pop) * 1.25) + 4096
     if scheme == "sparse":
         cap = int(max(p.shape[0] for p in pop) * 1.6) + 4096      # slots of new tracks come on top of the old
@@ -377,20 +399,17 @@ def test_single_step_at_full_size_counts_and_sampled_tracks(layout, scheme, n):
     for k in range(3):
         ctx.load_tracks(k, pop[k])
     counts = ctx.step()
-    o = Oracle(geo, tab, seed=c["seed"])
-    for k in range(3):
-        o.load_tracks(k, pop[k])
-    o.step()
-    r = o.result()
     compare_counts(counts, r, what="full size")
     g = ctx.result()
     assert np.allclose(g["edep_slab"], r["edep_slab"], rtol=1e-9, atol=1e-6)
     assert abs(g["e_escaped"] - r["e_escaped"]) <= 1e-9 * r["e_escaped"]
+    if scheme == "sparse":       # rule S30: bump allocation on top of the loaded population
+        assert (g["slots_used"] == np.array([p.shape[0] for p in pop], dtype=np.uint64) + r["secondaries"]).all()
     for k in range(3):
-        a, b = ctx.read_tracks(k), o.read_tracks(k, pop[0].dtype)
-        assert a.shape[0] == b.shape[0] == int(counts["live"][k])
-        sa, sb = a[(a["id_lo"] & 63) == 5], b[(b["id_lo"] & 63) == 5]
-        assert compare_tracks(sa, sb, "full size kind %d" % k) == 0
+        a = sort_by_id(ctx.read_tracks(k))
+        assert a.shape[0] == ref[k].shape[0] == int(counts["live"][k])
+        same = a.view(np.uint8).reshape(-1, 56) == ref[k].view(np.uint8).reshape(-1, 56)
+        assert same.all(), "kind %d: %d tracks differ" % (k, int((~same.all(axis=1)).sum()))
     ctx.destroy()
 
 
@@ -447,3 +466,227 @@ def test_tallies_are_bit_identical_across_layouts_schemes_and_runs():
         if ref is None:
             ref = bits
         assert bits == ref, (layout, scheme)
+
+
+# ---------------------------------------------- rule R4 / locator / S31 / S24 on the device ---
+def _gun(kinds, zs, ekin=5.0):
+    from workloads import PRIMARY_DTYPE
+    p = np.zeros(len(zs), dtype=PRIMARY_DTYPE)
+    p["kind"] = kinds
+    p["pos"][:, 2] = np.asarray(zs, dtype=np.float32)
+    p["dir"][:, 2] = 1.0
+    p["ekin"] = np.float32(ekin)
+    return p
+
+
+@pytest.mark.parametrize("scheme", SCHEMES)
+def test_inject_mixed_kinds_ids_and_slabs(scheme):
+    """adept_inject: rule R4 ids (against the numpy Philox of tests/helpers.py and the oracle) for
+    p = 0, 1, 2^32 + 3 under two seeds, and the slab locator at z = 0, inside an absorber, exactly on
+    abs_mm, inside a gap, on a layer boundary and on the last plane, for a mixed e-/e+/gamma array."""
+    from tests.helpers import primary_ids_np
+    from workloads import Geometry
+    geo = Geometry(n_layers=3, abs_mm=2.5, gap_mm=5.5, half_xy_mm=50.0)       # pitch 8, exact in binary
+    tab = tables_for("tiny")
+    zs = [0.0, 1.0, 2.5, 5.0, 8.0, 10.5, 15.999, 16.0, 18.5, 24.0]
+    want_vol = np.array([0, 0, 1, 1, 2, 3, 3, 4, 5, 5])
+    kinds = np.array([2, 0, 1, 0, 2, 1, 0, 0, 2, 1])
+    prim = _gun(kinds, zs)
+    for seed in (0x1234, 0xABCDEF0123456789):
+        for first in (0, 1, (1 << 32) + 3):
+            ctx = _ctx(geo, tab, layout="aosoa32", scheme=scheme, capacity=256, seed=seed)
+            o = Oracle(geo, tab, seed=seed)
+            ctx.set_primary_index(first)
+            o.set_primary_index(first)
+            ctx.inject(prim)
+            o.inject(prim)
+            lo, hi = primary_ids_np(first + np.arange(len(zs), dtype=np.uint64), seed)
+            for k in range(3):
+                g = ctx.read_tracks(k)
+                sel = kinds == k
+                assert compare_tracks(g, o.read_tracks(k, g.dtype), "inject kind %d" % k) == 0
+                order = np.argsort(hi[sel].astype(np.uint64) << np.uint64(32) | lo[sel].astype(np.uint64))
+                gs = sort_by_id(g)
+                assert (gs["id_lo"] == lo[sel][order]).all() and (gs["id_hi"] == hi[sel][order]).all()
+                assert (gs["vol"] == want_vol[sel][order]).all()
+                assert (gs["step"] == 0).all() and (gs["nial"] == -1.0).all()
+            assert abs(ctx.result()["e_injected"] - o.result()["e_injected"]) < 1e-9
+            ctx.destroy()
+
+
+@pytest.mark.parametrize("scheme", SCHEMES)
+@pytest.mark.parametrize("layout", ("aos", "soa", "aosoa32"))
+def test_runaway_guard_and_continuous_loss_cases(layout, scheme):
+    """The oracle's S31 and S24 pins (tests/test_oracle_transport.py) through adept_load_tracks +
+    adept_step: tracks at step 2^20 - 2 / 2^20 - 1 of every kind (killed, energy into the post-step
+    slab); the midpoint rule on a two-node table; a step that reaches the range (E_post = 0)."""
+    from workloads import Geometry
+    from workloads.tables import GROUP_ELEC, Q_STOP, MC2, constant_tables
+    geo = Geometry(n_layers=2, abs_mm=2.5, gap_mm=5.5, half_xy_mm=50.0)
+    tab = constant_tables(16, 0.1, 100.0, 0.1)
+    e0 = np.float32(3.25)
+    for kind in range(3):
+        for step0, dies in (((1 << 20) - 2, False), ((1 << 20) - 1, True)):
+            t = make_tracks(130, ekin=e0, step=step0)
+            ctx = _ctx(geo, tab, layout=layout, scheme=scheme, capacity=512, seed=0)
+            o = Oracle(geo, tab, seed=0)
+            ctx.load_tracks(kind, t)
+            o.load_tracks(kind, t)
+            counts = ctx.step()
+            o.step()
+            compare_counts(counts, o.result(), what="S31 kind %d step0 %d" % (kind, step0))
+            assert compare_tracks(ctx.read_tracks(kind), o.read_tracks(kind, t.dtype)) == 0
+            g = ctx.result()
+            if dies:
+                rest = float(np.float32(2.0) * np.float32(MC2)) if kind == 1 else 0.0
+                assert int(counts["live"][kind]) == 0 and int(counts["killed"][kind]) == 130
+                assert abs(g["edep_slab"][1] - 130 * (float(e0) + rest)) < 1e-6 and g["edep_slab"][[0, 2, 3]].sum() == 0
+            else:
+                assert int(counts["live"][kind]) == 130 and g["edep_slab"].sum() == 0
+            ctx.destroy()
+    # S24 on a two-node table with S linear in ln E (closed form in the oracle's pin) and the stop rule
+    geo = Geometry(n_layers=1, abs_mm=1e3, gap_mm=1.0, half_xy_mm=1e6)
+    for rng_mm, s_lo, s_hi in ((50.0, 0.5, 1.5), (0.05, 1e-3, 1e-3), (0.3, 1e-3, 1e-3)):
+        tab = constant_tables(1, 0.1, 100.0, 0.1, brems=0.0, rng=rng_mm)
+        tab.data[:, GROUP_ELEC, Q_STOP, 0] = s_lo
+        tab.data[:, GROUP_ELEC, Q_STOP, 1] = s_hi
+        E = np.float32([90.0, 50.0, 20.0, 13.0, 2.0, 7.5])
+        for kind in (0, 1):
+            t = make_tracks(E.shape[0], ekin=E, pos=(0, 0, 500.0))
+            ctx = _ctx(geo, tab, layout=layout, scheme=scheme, capacity=128, seed=0)
+            o = Oracle(geo, tab, seed=0)
+            ctx.load_tracks(kind, t)
+            o.load_tracks(kind, t)
+            for it in range(2):        # second step: the stopped e+ (ekin = 0) annihilate (rule S17)
+                counts = ctx.step()
+                o.step()
+                compare_counts(counts, o.result(), what="S24 range %g kind %d" % (rng_mm, kind))
+                for k in range(3):
+                    assert compare_tracks(ctx.read_tracks(k), o.read_tracks(k, t.dtype)) == 0
+            assert np.allclose(ctx.result()["edep_slab"], o.result()["edep_slab"], rtol=1e-9, atol=1e-9)
+            ctx.destroy()
+
+
+def test_device_math_exhaustive_bit_equality():
+    """lg / ex / sincos2pi evaluated on the device for EVERY fp32 of the
+    used domains ([1e-8, 1e5]; +-[1e-6, 20]; the whole 2^23-point u grid) equal the oracle's bit for
+    bit; u01 over the whole grid."""
+    import torch
+    from paper_2302_08252_b200 import dev_math
+
+    def every_float(lo, hi, chunk=1 << 25):
+        a, b = int(np.float32(lo).view(np.uint32)), int(np.float32(hi).view(np.uint32))
+        for first in range(a, b, chunk):
+            yield np.arange(first, min(first + chunk, b), dtype=np.uint32).view(np.float32)
+
+    n = 0
+    for x in every_float(1e-8, 1e5):
+        y = dev_math(2, torch.from_numpy(x).cuda(), torch.float32, (x.shape[0],)).cpu().numpy()
+        assert (y.view(np.uint32) == math_fns.lg(x).view(np.uint32)).all()
+        n += x.shape[0]
+    for sign in (1.0, -1.0):
+        for x in every_float(1e-6, 20.0):
+            x = np.float32(sign) * x
+            y = dev_math(3, torch.from_numpy(x).cuda(), torch.float32, (x.shape[0],)).cpu().numpy()
+            assert (y.view(np.uint32) == math_fns.ex(x).view(np.uint32)).all()
+            n += x.shape[0]
+    assert n > 7.5e8
+    xs = (np.arange(1 << 23, dtype=np.uint64) << np.uint64(9)).astype(np.uint32)
+    u = dev_math(1, torch.from_numpy(xs.view(np.int32)).cuda(), torch.float32, (xs.shape[0],)).cpu().numpy()
+    assert (u.view(np.uint32) == math_fns.u01(xs).view(np.uint32)).all()
+    sc = dev_math(4, torch.from_numpy(u).cuda(), torch.float32, (u.shape[0], 2)).cpu().numpy()
+    s, c = math_fns.sincos2pi(u)
+    assert (sc[:, 0].view(np.uint32) == s.view(np.uint32)).all() and (sc[:, 1].view(np.uint32) == c.view(np.uint32)).all()
+    y = dev_math(2, torch.from_numpy(u).cuda(), torch.float32, (u.shape[0],)).cpu().numpy()
+    assert (y.view(np.uint32) == math_fns.lg(u).view(np.uint32)).all()
+
+
+# ------------------------------------------------------------- host-side contract (ADVICE r1) ---
+def test_two_live_contexts_with_different_tables_step_alternately():
+    """The dynamic shared-memory limit of a kernel instantiation is shared by all contexts of the
+    process: a later context with smaller tables must not lower it under an earlier, larger one."""
+    big_geo, big_tab = geometry_for("full"), tables_for("full")          # 257 nodes, 100 slabs
+    small_geo, small_tab = geometry_for("tiny"), tables_for("tiny")      # 65 nodes, 8 slabs
+    a = _ctx(big_geo, big_tab, layout="aosoa32", scheme="dense", capacity=1 << 16, seed=2)
+    b = _ctx(small_geo, small_tab, layout="aosoa32", scheme="dense", capacity=4096, seed=1)
+    a.inject(gen_primaries(3, 1000.0))
+    b.inject(gen_primaries(16, 10.0))
+    oa, ob = Oracle(big_geo, big_tab, seed=2), Oracle(small_geo, small_tab, seed=1)
+    oa.inject(gen_primaries(3, 1000.0))
+    ob.inject(gen_primaries(16, 10.0))
+    for it in range(30):
+        ca, cb = a.step(), b.step()
+        oa.step()
+        ob.step()
+        compare_counts(ca, oa.result(), what="big context, iteration %d" % it)
+        compare_counts(cb, ob.result(), what="small context, iteration %d" % it)
+    oa.run()
+    ob.run()
+    compare_counts(a.run(), oa.result())
+    compare_counts(b.run(), ob.result())
+    a.destroy()
+    b.destroy()
+
+
+def test_load_tracks_rejects_bad_records_and_slots():
+    from paper_2302_08252_b200 import AdeptError
+    geo, tab = geometry_for("tiny"), tables_for("tiny")
+    good = make_tracks(300, ekin=1.0)
+    for scheme in SCHEMES:
+        ctx = _ctx(geo, tab, layout="soa", scheme=scheme, capacity=1024, seed=1)
+        for field, value in (("vol", 2 * geo.n_layers), ("step", 1 << 20), ("ekin", 0.01), ("ekin", 1e5),
+                             ("ekin", np.nan), ("dir", (0.0, 0.0, 0.0)), ("dir", (np.inf, 0.0, 1.0)),
+                             ("pos", (np.nan, 0.0, 0.0)), ("nial", (np.nan, 1.0, 1.0))):
+            bad = good.copy()
+            bad[field][257] = value
+            with pytest.raises(AdeptError) as e:
+                ctx.load_tracks(0, bad)
+            assert e.value.code == -1, (field, value)
+            assert ctx.step()["live"].sum() == 0                     # nothing was changed
+        low = good.copy()
+        low["ekin"][::3] = 0.01                                      # allowed for e+ only (rule S17)
+        ctx.load_tracks(1, low)
+        assert int(ctx.step()["steps"][1]) == 300
+        ctx.destroy()
+    ctx = _ctx(geo, tab, layout="aos", scheme="sparse", capacity=1024, seed=1)
+    slots = np.arange(300, dtype=np.uint32) * 3
+    dup = slots.copy()
+    dup[200] = dup[17]
+    for bad_slots in (dup, slots + 200):                             # duplicate; beyond the capacity
+        with pytest.raises(AdeptError) as e:
+            ctx.load_tracks(0, good, bad_slots)
+        assert e.value.code == -1
+    ctx.load_tracks(0, good, slots)
+    with pytest.raises(AdeptError):                                  # slot 5 lies below the allocator's top: not free
+        ctx.load_tracks(0, good[:1], np.array([5], dtype=np.uint32))
+    ctx.load_tracks(0, good[:2], np.array([1000, 950], dtype=np.uint32))
+    o = Oracle(geo, tab, seed=1)
+    o.load_tracks(0, np.concatenate([good, good[:2]]))
+    o.step()
+    compare_counts(ctx.step(), o.result())
+    ctx.destroy()
+
+
+def test_run_counts_real_iterations_against_the_limit():
+    """adept_run(max_iterations): progress is what the device counted (iterations with something
+    alive), the limit is tested before the next batch is injected, and a run can be resumed."""
+    geo, tab = geometry_for("tiny"), tables_for("tiny")
+    prim = gen_primaries(6, 10.0)
+    o = Oracle(geo, tab, seed=9)
+    o.queue(prim)
+    o.run_batched(2)
+    r = o.result()
+    ctx = _ctx(geo, tab, layout="soa", scheme="dense", capacity=4096, seed=9, batch_primaries=2)
+    ctx.inject(prim)
+    done = 0
+    while True:
+        g = ctx.run(7)
+        assert g["iterations"] - done <= 7
+        if g["iterations"] == done:
+            break
+        assert g["iterations"] - done == 7 or g["live"].sum() == 0
+        done = g["iterations"]
+    compare_counts(g, r)
+    assert g["iterations"] == r["iterations"]
+    assert np.allclose(g["edep_layer"], r["edep_layer"], rtol=1e-4, atol=1e-12)
+    ctx.destroy()

@@ -13,7 +13,7 @@ import numpy as np
 import pytest
 
 from oracle import math_fns
-from tests.helpers import ulp_diff
+from tests.helpers import philox4x32_10_np, ulp_diff
 
 GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
 
@@ -26,6 +26,20 @@ def test_philox_known_answer_vectors():
         v = [int(x, 16) for x in r]
         out = math_fns.philox(v[0:4], v[4:6])
         assert [int(x) for x in out] == v[6:10]
+
+
+def test_numpy_philox_of_the_test_helpers_passes_the_same_vectors():
+    """tests/helpers.py philox4x32_10_np (used to pin rule R4 independently of the oracle's routine)
+    against the published vectors, and the oracle against it on random inputs."""
+    rows = [l.split() for l in open(os.path.join(GOLDEN, "philox4x32_10_kat.txt"))
+            if l.strip() and not l.startswith("#")]
+    for r in rows:
+        v = [int(x, 16) for x in r]
+        assert [int(x) for x in philox4x32_10_np([v[0:4]], [v[4:6]])[0]] == v[6:10]
+    rng = np.random.default_rng(1)
+    ctr = rng.integers(0, 2**32, size=(5000, 4), dtype=np.uint64).astype(np.uint32)
+    key = rng.integers(0, 2**32, size=(5000, 2), dtype=np.uint64).astype(np.uint32)
+    assert (math_fns.philox_array(ctr, key) == philox4x32_10_np(ctr, key)).all()
 
 
 def test_philox_array_matches_scalar_and_is_a_bijection_sample():
@@ -64,18 +78,26 @@ def _float_sweep(lo, hi, stride):
     return np.arange(int(a), int(b), stride, dtype=np.uint32).view(np.float32)
 
 
+def _every_float(lo, hi, chunk=1 << 23):
+    """Every fp32 in [lo, hi), in chunks (exhaustive sweep of the used domain)."""
+    a, b = int(np.float32(lo).view(np.uint32)), int(np.float32(hi).view(np.uint32))
+    for first in range(a, b, chunk):
+        yield np.arange(first, min(first + chunk, b), dtype=np.uint32).view(np.float32)
+
+
 def test_lg_against_libm():
-    # M8: <= 2 ulp on the used domain; the u grid gives finite positive -lg(u)
-    x = np.concatenate([_float_sweep(1e-8, 1e5, 37),
-                        _float_sweep(0.999, 1.001, 1),
-                        np.float32([1.0, 0.1, 1e4, 2.0**-24, 1 - 2.0**-24])])
-    y = math_fns.lg(x)
-    ref = np.log(x.astype(np.float64))
-    nz = ref != 0
-    # absolute floor of 2^-24 near x = 1 (ln is ~1e-7 there and the result comes from s = (m-1)/(m+1))
-    err = np.abs(y[nz].astype(np.float64) - ref[nz])
-    ok = (ulp_diff(y[nz], ref[nz]) <= 2.0) | (err <= 2.0**-24 * 0.5)
-    assert ok.all(), (x[nz][~ok][:5], y[nz][~ok][:5])
+    # M8: <= 2 ulp on EVERY fp32 of the used domain [1e-8, 1e5]; the u grid gives finite positive -lg(u)
+    n = 0
+    for x in _every_float(1e-8, 1e5):
+        y = math_fns.lg(x)
+        ref = np.log(x.astype(np.float64))
+        nz = ref != 0
+        # absolute floor of 2^-24 near x = 1 (ln is ~1e-7 there and the result comes from s = (m-1)/(m+1))
+        err = np.abs(y[nz].astype(np.float64) - ref[nz])
+        ok = (ulp_diff(y[nz], ref[nz]) <= 2.0) | (err <= 2.0**-24 * 0.5)
+        assert ok.all(), (x[nz][~ok][:5], y[nz][~ok][:5])
+        n += x.shape[0]
+    assert n > 3.6e8
     assert math_fns.lg(np.float32([1.0]))[0] == 0.0
     # exhaustive over the u grid: finite, positive, monotone non-increasing in u
     xs = (np.arange(1 << 23, dtype=np.uint64) << np.uint64(9)).astype(np.uint32)
@@ -86,18 +108,20 @@ def test_lg_against_libm():
 
 
 def test_ex_against_libm():
-    # M9: <= 1 ulp on [-20, 12] (the domain the step uses is [-17, 11.6])
-    x = _float_sweep(1e-6, 12.0, 53)
-    x = np.concatenate([x, -_float_sweep(1e-6, 20.0, 53), np.float32([0.0])])
-    y = math_fns.ex(x)
-    ref = np.exp(x.astype(np.float64))
-    assert ulp_diff(y, ref).max() <= 1.0
+    # M9: <= 1 ulp on EVERY fp32 of [-20, -1e-6] and [1e-6, 12] (the step uses [-17, 11.6]), and 0
+    n = 0
+    for sign, hi in ((1.0, 12.0), (-1.0, 20.0)):
+        for x in _every_float(1e-6, hi):
+            x = np.float32(sign) * x
+            assert ulp_diff(math_fns.ex(x), np.exp(x.astype(np.float64))).max() <= 1.0
+            n += x.shape[0]
+    assert n > 3.9e8
     assert math_fns.ex(np.float32([0.0]))[0] == 1.0
 
 
 def test_sincos2pi_against_libm():
     # M10: abs error <= 1e-7, |sin^2 + cos^2 - 1| <= 2e-7; exact at quadrant points
-    xs = (np.arange(0, 1 << 23, 5, dtype=np.uint64) << np.uint64(9)).astype(np.uint32)
+    xs = (np.arange(0, 1 << 23, 1, dtype=np.uint64) << np.uint64(9)).astype(np.uint32)   # the whole u grid
     u = math_fns.u01(xs)
     s, c = math_fns.sincos2pi(u)
     a = 2.0 * math.pi * u.astype(np.float64)

@@ -15,7 +15,7 @@ from oracle import Oracle, math_fns
 from workloads import CONFIGS, Geometry, gen_primaries, gen_sweep, geometry_for, tables_for
 from workloads.tables import (GROUP_ELEC, GROUP_GAMMA, MC2, Q_BREMS, Q_COMPT, Q_PAIR, Q_PHOTO,
                               Q_RANGE, Q_STOP, build_tables, constant_tables)
-from tests.helpers import make_tracks, sort_by_id
+from tests.helpers import make_tracks, primary_ids_np, sort_by_id
 
 E_CUT = 0.1
 W_ANNIH, W_GEOM, W_ELOSS = -2, -1, 3
@@ -378,6 +378,170 @@ def test_positron_annihilates_at_rest_with_two_back_to_back_photons():
     assert dsum < 3e-7
     cts = np.array(cts)
     assert np.allclose(cts, 1 - 2 * stream_u(t, 1, 2).astype(np.float64), atol=1e-7)   # isotropic in cos(theta)
+
+
+# ------------------------------------------- R4: primary ids and slab locator ---
+def _gun(kinds, zs, ekin=5.0):
+    from workloads import PRIMARY_DTYPE
+    p = np.zeros(len(zs), dtype=PRIMARY_DTYPE)
+    p["kind"] = kinds
+    p["pos"][:, 2] = np.asarray(zs, dtype=np.float32)
+    p["dir"][:, 2] = 1.0
+    p["ekin"] = np.float32(ekin)
+    return p
+
+
+@pytest.mark.parametrize("seed", [0x1234, 0xABCDEF0123456789])
+def test_inject_primary_ids_follow_rule_R4(seed):
+    """Rule R4: primary p gets words 0, 1 of Philox(ctr = (p_lo, p_hi, 0, 0x5052494D), key = seed),
+    evaluated here by the numpy Philox of tests/helpers.py (written from the published algorithm,
+    pinned to the known-answer vectors) -- not by the oracle's routine."""
+    geo, tab = geometry_for("tiny"), tables_for("tiny")
+    for first in (0, 1, (1 << 32) + 3):
+        o = Oracle(geo, tab, seed=seed)
+        o.set_primary_index(first)
+        o.inject(gen_primaries(3, 10.0))
+        t = o.read_tracks(0, make_tracks(1).dtype)
+        lo, hi = primary_ids_np([first, first + 1, first + 2], seed)
+        assert (t["id_lo"] == lo).all() and (t["id_hi"] == hi).all()
+        assert (t["step"] == 0).all() and (t["nial"] == -1.0).all() and (t["vol"] == 0).all()
+    # a swapped counter word, a missing tag or a swapped key half would give other ids
+    lo, hi = primary_ids_np([1, 1 << 32], 0x1234)
+    assert (int(lo[0]), int(hi[0])) != (int(lo[1]), int(hi[1]))
+
+
+def test_inject_locates_the_slab_from_z():
+    """DESIGN.md section 3 'locate' (rule R4): layer = int(z / pitch) clamped to the last layer,
+    gap iff z - layer * pitch >= abs_mm.  Thicknesses are exact in binary, slabs hand-computed."""
+    geo = Geometry(n_layers=3, abs_mm=2.5, gap_mm=5.5, half_xy_mm=50.0)       # pitch 8
+    tab = tables_for("tiny")
+    zs = [0.0, 1.0, 2.5, 5.0, 8.0, 10.5, 15.999, 16.0, 18.5, 24.0]
+    want = [0, 0, 1, 1, 2, 3, 3, 4, 5, 5]      # z = 24 is the last plane: clamped to layer 2, in its gap
+    for kind in (0, 1, 2):
+        o = Oracle(geo, tab, seed=1)
+        o.inject(_gun(kind, zs))
+        t = o.read_tracks(kind, make_tracks(1).dtype)
+        assert [int(v) for v in t["vol"]] == want
+        assert (t["pos"][:, 2] == np.float32(zs)).all()
+        assert all(o.live(k) == (len(zs) if k == kind else 0) for k in range(3))
+        r = o.result()
+        rest = float(np.float32(2.0) * np.float32(MC2)) if kind == 1 else 0.0   # S25 bookkeeping of e+
+        assert abs(r["e_injected"] - len(zs) * (5.0 + rest)) < 1e-9
+    # mixed kinds keep their global indices (ids) in injection order
+    o = Oracle(geo, tab, seed=1)
+    o.inject(_gun([2, 0, 1, 0, 2], [0.0, 1.0, 2.5, 8.0, 24.0]))
+    lo, _ = primary_ids_np(range(5), 1)
+    got = {k: o.read_tracks(k, make_tracks(1).dtype) for k in range(3)}
+    assert list(got[0]["id_lo"]) == [lo[1], lo[3]] and list(got[0]["vol"]) == [0, 2]
+    assert list(got[1]["id_lo"]) == [lo[2]] and list(got[1]["vol"]) == [1]
+    assert list(got[2]["id_lo"]) == [lo[0], lo[4]] and list(got[2]["vol"]) == [0, 5]
+    # outside the stack / box / energy grid: rejected
+    for bad in (_gun(0, [-0.001]), _gun(0, [24.001]), _gun(0, [1.0], ekin=0.05), _gun(0, [1.0], ekin=1e3)):
+        with pytest.raises(ValueError):
+            Oracle(geo, tab, seed=1).inject(bad)
+
+
+# ------------------------------------------------------- S31: runaway guard ---
+@pytest.mark.parametrize("kind", [0, 1, 2])
+def test_runaway_guard_kills_at_step_2_pow_20(kind):
+    """Rule S31: a track whose step counter reaches 2^20 is killed, its energy (+ 2 mc^2 for e+)
+    deposited in the slab it is in AFTER the step.  Vacuum-like tables: the step is a boundary
+    crossing 0 -> 1, so the deposit must land in slab 1; one step earlier nothing happens."""
+    geo = Geometry(n_layers=2, abs_mm=2.5, gap_mm=5.5, half_xy_mm=50.0)
+    tab = constant_tables(16, E_CUT, 100.0, E_CUT)
+    e0 = np.float32(3.25)
+    for step0, dies in (((1 << 20) - 2, False), ((1 << 20) - 1, True)):
+        o = Oracle(geo, tab, seed=0)
+        o.load_tracks(kind, make_tracks(2, ekin=e0, step=step0))
+        o.step()
+        r = o.result()
+        if not dies:
+            t = o.read_tracks(kind, make_tracks(1).dtype)
+            assert t.shape[0] == 2 and (t["step"] == step0 + 1).all() and (t["vol"] == 1).all()
+            assert r["edep_slab"].sum() == 0.0 and int(r["killed"][kind]) == 0
+            continue
+        assert o.live(kind) == 0 and int(r["killed"][kind]) == 2 and int(r["escaped_n"][kind]) == 0
+        rest = float(np.float32(2.0) * np.float32(MC2)) if kind == 1 else 0.0
+        assert r["edep_slab"][1] == 2 * (float(e0) + rest) and r["edep_slab"][[0, 2, 3]].sum() == 0.0
+        assert r["e_escaped"] == 0.0 and int(r["secondaries"].sum()) == 0
+    # an escaping track at the limit escapes (S25 comes first); a track killed by S24/S26 is not guarded twice
+    o = Oracle(geo, tab, seed=0)
+    o.load_tracks(kind, make_tracks(1, ekin=e0, step=(1 << 20) - 1, vol=3, pos=(0, 0, 12.0)))
+    o.step()
+    r = o.result()
+    assert int(r["escaped_n"][kind]) == 1 and r["edep_slab"].sum() == 0.0
+
+
+# ------------------------------------------- S24: midpoint rule and stop rule ---
+def _loss_tables(s_lo, s_hi, rng_mm):
+    """Two-node grid [0.1, 100] MeV on which S is linear in ln E; no bremsstrahlung; constant range."""
+    tab = constant_tables(1, E_CUT, 100.0, E_CUT, brems=0.0, rng=rng_mm)
+    tab.data[:, GROUP_ELEC, Q_STOP, 0] = s_lo
+    tab.data[:, GROUP_ELEC, Q_STOP, 1] = s_hi
+    return tab
+
+
+@pytest.mark.parametrize("kind", [0, 1])
+def test_continuous_loss_is_the_midpoint_rule_closed_form(kind):
+    """Rule S24 with S(E) = s_lo + (s_hi - s_lo) ln(E/0.1)/ln(1000): the step s = max(0.2 R, 0.1)
+    = 10 mm is ELOSS-limited and  E_post = E - s S(max(E - s S(E)/2, e_cut))  in closed form.
+    An Euler step (S at E) or the end-point rule is off by > 1e-3 here; the bar is 1e-6."""
+    s_lo, s_hi, R = 0.5, 1.5, 50.0
+    geo = Geometry(n_layers=1, abs_mm=1e3, gap_mm=1.0, half_xy_mm=1e6)
+    tab = _loss_tables(s_lo, s_hi, R)
+    E = np.float32([90.0, 50.0, 20.0, 13.0])
+    t = make_tracks(E.shape[0], ekin=E, pos=(0, 0, 500.0))
+    o = Oracle(geo, tab, seed=0)
+    o.set_trace(True)
+    o.load_tracks(kind, t)
+    o.step()
+    assert (o.trace()["winner"] == W_ELOSS).all()
+    S = lambda e: s_lo + (s_hi - s_lo) * np.log(e / 0.1) / math.log(1000.0)
+    E64 = E.astype(np.float64)
+    s = 0.2 * R
+    want = E64 - s * S(np.maximum(E64 - 0.5 * s * S(E64), E_CUT))
+    euler = E64 - s * S(E64)
+    assert (np.abs(euler / want - 1) > 1e-3).all()             # the pin can tell the two apart
+    g = sort_by_id(o.read_tracks(kind, t.dtype))
+    order = np.argsort(t["id_hi"].astype(np.uint64) << np.uint64(32) | t["id_lo"].astype(np.uint64))
+    assert np.abs(g["ekin"].astype(np.float64) / want[order] - 1).max() < 1e-6
+    assert np.abs(g["pos"][:, 2] - (500.0 + s)).max() < 1e-4 and (g["step"] == 1).all()
+    r = o.result()
+    assert abs(r["edep_slab"][0] - (E64 - want).sum()) < 1e-6 * E64.sum() and r["edep_slab"][1] == 0.0
+    # E_mid is clamped at the cut: E - s S(E)/2 < e_cut  ->  S is taken at e_cut, and dE = min(s S, E) = E
+    o = Oracle(geo, tab, seed=0)
+    o.load_tracks(kind, make_tracks(1, ekin=np.float32(2.0), pos=(0, 0, 500.0)))
+    o.step()
+    r = o.result()
+    assert r["edep_slab"][0] == 2.0                            # s S(e_cut) = 5 MeV > E: everything is lost
+    assert int(r["killed"][kind]) == (1 if kind == 0 else 0)   # e+ is kept for rule S17
+    if kind == 1:
+        assert o.read_tracks(1, t.dtype)["ekin"][0] == 0.0
+
+
+@pytest.mark.parametrize("kind", [0, 1])
+def test_track_stops_when_the_step_reaches_its_range(kind):
+    """Rule S20/S24: R <= r_min = 0.1 mm gives s_e = R, and an ELOSS-limited step with s >= R ends
+    the track: E_post = 0 exactly, whatever S says.  Just above r_min the step is 0.1 mm < R and
+    the midpoint rule applies instead."""
+    geo = Geometry(n_layers=1, abs_mm=1e3, gap_mm=1.0, half_xy_mm=1e6)
+    E = np.float32(7.5)
+    # S = 1e-3 MeV/mm: the midpoint rule alone would leave the energy almost untouched
+    o = Oracle(geo, _loss_tables(1e-3, 1e-3, 0.05), seed=0)
+    o.load_tracks(kind, make_tracks(3, ekin=E, pos=(0, 0, 500.0)))
+    o.step()
+    r = o.result()
+    assert r["edep_slab"][0] == 3 * float(E)
+    if kind == 0:
+        assert o.live(0) == 0 and int(r["killed"][0]) == 3
+    else:                                                       # S24: e+ survives with ekin = 0 until S17
+        t = o.read_tracks(1, make_tracks(1).dtype)
+        assert (t["ekin"] == 0.0).all() and np.allclose(t["pos"][:, 2], 500.05, atol=1e-4)
+    o = Oracle(geo, _loss_tables(1e-3, 1e-3, 0.3), seed=0)     # s_e = max(0.06, 0.1) = 0.1 < R
+    o.load_tracks(kind, make_tracks(3, ekin=E, pos=(0, 0, 500.0)))
+    o.step()
+    t = o.read_tracks(kind, make_tracks(1).dtype)
+    assert t.shape[0] == 3 and np.abs(t["ekin"].astype(np.float64) - (7.5 - 0.1 * 1e-3)).max() < 1e-6
 
 
 # ------------------------------------------------------ order independence ---
