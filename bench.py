@@ -8,6 +8,17 @@ interaction lengths; one adept_step per "step", dense double buffer, per layout.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--layout soa|aos|aosoa32|aosoa64|soa16|all] [--impl reference]
 
+`--gpus N` with N > 1 and no torchrun environment re-launches itself as N ranks (torch.distributed.run,
+rendezvous on 127.0.0.1); under torchrun it uses the ranks it was given.  `n_gpus` is the number of
+ranks that actually ran.
+
+The default line also carries, beside the headline (rank 0, one GPU): `showers` = BASELINE.json
+configs[1] ("full") and configs[4] ("heavy") through adept_inject + adept_run, each with the oracle
+timed on the same workload and the full-size parity of its counts and per-layer deposits; and
+`sweep` = configs[3], per scheme x layout x occupancy the step time, its roofline fraction and the
+time of slot allocation / compaction (section clocks of the timing variant of the library).
+`--extras none` prints the headline only.
+
 One JSON line on stdout (rank 0).  `value` is measured with the tracks resident in HBM: every timed
 step starts from a pristine copy of the workspace (restored outside the timed region, L2 flushed) and
 is timed with CUDA events on the stream the kernel is launched on.  `e2e` is the same step through
@@ -35,10 +46,27 @@ from workloads import CONFIGS, gen_tracks, geometry_for, tables_for  # noqa: E40
 
 WORKLOAD = "single_step"
 RECORD_BYTES = {"aos": 64, "soa": 56, "aosoa32": 56, "aosoa64": 56, "soa16": 56, "aosoa16": 56, "aosoa128": 56}     # bytes per record per layout
-# dram__bytes_read.sum + dram__bytes_write.sum of one step_kernel launch on this workload, from the
-# `ncu --set full` captures summarised in profiles/r1_step_kernel.md (r1i: AoSoA-32)
-NCU_TRAFFIC_BYTES = {"aosoa32": 944.8e6 + 1046.6e6, "soa": None, "aos": None,
-                     "aosoa64": None, "soa16": None, "aosoa16": None, "aosoa128": None}
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
+
+
+def ncu_traffic(workload: str, layout: str, scheme: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one step_kernel launch, from the committed table
+    of `ncu --set full` captures (profiles/ncu_traffic.csv; the .md beside it names the commands).
+    Returns (bytes, source) or (None, None) when no capture exists for this kernel and workload."""
+    try:
+        with open(TRAFFIC_CSV) as f:
+            rows = [l.strip().split(",") for l in f if l.strip() and not l.startswith("#")]
+    except OSError:
+        return None, None
+    head, best = rows[0], None
+    for r in rows[1:]:
+        d = dict(zip(head, r))
+        if d["workload"] == workload and d["layout"] == layout and d["scheme"] == scheme:
+            best = d                                   # later rows are later captures
+    if best is None:
+        return None, None
+    return float(best["dram_bytes_read"]) + float(best["dram_bytes_write"]), \
+        "profiles/ncu_traffic.csv (%s, commit %s)" % (best["capture"], best["commit"])
 
 
 def measured_peak():
@@ -131,8 +159,13 @@ def by_id(tracks):
     return tracks[np.argsort(key, kind="stable")]
 
 
-def run_reference(args, rank: int):
-    """--impl reference: the oracle on the host cores, same metric/config, bounded sample per step."""
+def host_cores() -> int:
+    return os.cpu_count() or 1
+
+
+def run_reference(args, rank: int, world: int):
+    """--impl reference: the oracle on the host cores, same metric/config, bounded sample per step.
+    Under torchrun rank 0 alone runs and prints; the other ranks exit without work."""
     if rank != 0:
         return
     sample = min(args.tracks, 1 << 21)
@@ -145,10 +178,10 @@ def run_reference(args, rank: int):
         n_tot += n
         t_tot += dt
     v = n_tot / t_tot
-    cpu = {"value": v, "unit": "track-steps/s", "cores": 1, "kind": "oracle",
+    cpu = {"value": v, "unit": "track-steps/s", "cores": 1, "host_cores": host_cores(), "kind": "oracle",
            "sample": "one adept_step-equivalent oracle iteration over %d tracks of the config-3 population per step" % sample}
     print(json.dumps({
-        "impl": "reference", "metric": "track-steps/sec", "value": v, "unit": "track-steps/s", "n_gpus": args.gpus,
+        "impl": "reference", "metric": "track-steps/sec", "value": v, "unit": "track-steps/s", "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_tot / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": "single-step microbenchmark (BASELINE.json configs[2]), oracle on host, "
@@ -289,8 +322,14 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
         if it > 0:
             e2e_c += dt
     ctx.destroy()
+    del ctx, pinned_in, pinned_out, host_in, host_out
     e2e_value = world * n_tracks * e2e_steps / e2e_t
     e2e_counts_only = world * n_tracks * e2e_steps / e2e_c
+
+    # ---- N > 1: the event-sharded heavy showers beside the weak-scaled step ----
+    sharded = None
+    if world > 1 and "showers" in args.extras:
+        sharded = sharded_showers(args, "heavy", rank, world, local_rank, dist, max_over_ranks)
 
     if rank != 0:
         if dist is not None:
@@ -298,6 +337,9 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
         return
     peak, peak_src = measured_peak()
     m = per_layout[main]
+    full_size = n_tracks == CONFIGS[WORKLOAD]["n_tracks"]
+    traffic, traffic_src = ncu_traffic("single_step", main, "dense") if full_size else (None, None)
+    shape = "1024 threads x 1 CTA/SM" if n_tracks >= (1 << 22) else "256 threads x 4 CTAs/SM"   # adept_api.cu launch_iteration
     out = {
         "metric": "track-steps/sec", "value": m["track_steps_per_s"], "unit": "track-steps/s", "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": m["ms_per_step"], "higher_is_better": True,
@@ -317,21 +359,23 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
                 "what": "adept_load_tracks x3 (pinned host) + adept_step + adept_read_tracks x3"},
         "roofline": {"bound": "hbm", "achieved": m["algorithmic_GBps"], "peak": peak, "unit": "GB/s",
                      "frac": m["algorithmic_GBps"] / peak,
-                     "traffic": NCU_TRAFFIC_BYTES[main] if n_tracks == CONFIGS[WORKLOAD]["n_tracks"] else None,
-                     "traffic_source": "profiles/r1_step_kernel.md (ncu --set full, bytes per launch)",
+                     "traffic": traffic, "traffic_source": traffic_src,
                      "peak_source": peak_src,
-                     "kernel": "adept::step_kernel<%s, dense, 1024 threads>" % main,
+                     "kernel": "adept::step_kernel<%s, dense, %s>" % (main, shape),
                      "bytes_per_launch": m["algorithmic_bytes_per_launch"]},
         "layouts": per_layout,
     }
+    if sharded is not None:
+        out["showers"] = {"heavy_sharded": sharded}
     if world == 1 and not args.no_cpu:
         n, dt, r = oracle_single_step(pop, n_tracks, want_tracks=True)
-        out["cpu_baseline"] = {"value": n / dt, "unit": "track-steps/s", "cores": 1, "kind": "oracle",
+        out["cpu_baseline"] = {"value": n / dt, "unit": "track-steps/s", "cores": 1, "host_cores": host_cores(),
+                               "kind": "oracle",
                                "sample": "one oracle iteration over all %d tracks of the same population" % n,
                                "seconds": dt}
         keys = ("steps", "secondaries", "killed", "escaped_n", "live")
         # discrete-branch disagreements (north_star: to be reported): a track that took another branch
-        # on the GPU has another fate -- it is missing, extra, or of another kind in the output sample
+        # on the GPU has another fate -- it is missing, extra, or of another kind in the output
         n_cmp = n_missing = n_diff = 0
         for a, b in zip(main_res["tracks"], r["tracks"]):
             ka = a["id_hi"].astype(np.uint64) << np.uint64(32) | a["id_lo"].astype(np.uint64)
@@ -347,57 +391,65 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
                                    "branch_disagreement_rate": (n_missing / max(1, n_cmp)),
                                    "edep_rel_err": float(np.max(np.abs(main_res["edep_layer"] - r["edep_layer"])
                                                                 / np.maximum(r["edep_layer"], 1e-30)))}
+        del r
+    del main_res, results, pop
+    torch.cuda.empty_cache()
+    if world == 1:
+        if "showers" in args.extras:
+            out["showers"] = {}
+            for name in ("full", "heavy") if "heavy" in args.extras else ("full",):
+                out["showers"][name] = showers(args, name, layout=main, scheme="dense", steps=3, warmup=1,
+                                               with_cpu=not args.no_cpu)
+        if "sweep" in args.extras:
+            out["sweep"] = sweep(args, layouts=("aos", "soa", "aosoa32"), steps=5, warmup=3, instr=False, sections=True)
     print(json.dumps(out))
     if dist is not None:
         dist.destroy_process_group()
 
 
-def run_showers(args, name: str):
-    """--workload tiny|full|heavy (BASELINE.json configs[0], [1], [4]): inject + adept_run to
-    completion; a "step" is one whole run.  These runs are launch-latency bound for most of their
-    iterations, so no roofline fraction is claimed for them."""
+def showers(args, name: str, *, layout: str, scheme: str, steps: int, warmup: int, with_cpu: bool, batch: int = 0,
+            flags: int = 0) -> dict:
+    """BASELINE.json configs[0], [1], [4] (tiny / full / heavy): adept_inject + adept_run to completion,
+    wall clock around the two calls (host primaries in, tallies out: this IS the end-to-end number).
+    These runs are launch-latency bound for most of their iterations, so no roofline
+    fraction is claimed for them."""
     import torch
     from paper_2302_08252_b200 import Context
     from workloads import gen_primaries
     c = CONFIGS[name]
     geo, tab = geometry_for(name), tables_for(name)
     prim = gen_primaries(c["n_primaries"], c["e_primary"])
-    layout = "aosoa32" if args.layout == "all" else args.layout
-    ctx = Context(geo, tab, layout=layout, scheme=args.scheme, capacity=c["capacity"], seed=c["seed"],
-                  batch_primaries=args.batch)
-    sampler = ClockSampler(0)
-    sampler.start()
+    ctx = Context(geo, tab, layout=layout, scheme=scheme, capacity=c["capacity"], seed=c["seed"],
+                  batch_primaries=batch, flags=flags)
     times, res = [], None
-    for it in range(args.warmup + args.steps):
+    for it in range(warmup + steps):
         ctx.reset()
         torch.cuda.synchronize()
         t0 = time.perf_counter()
         ctx.inject(prim)                      # host primaries -> device (H2D inside the timed region)
         res = ctx.run()                       # returns the tallies (D2H inside the timed region)
         dt = time.perf_counter() - t0
-        if it >= args.warmup:
+        if it >= warmup:
             times.append(dt)
-    clocks = sampler.stop()
     ctx.destroy()
-    steps = int(res["steps"].sum())
+    del ctx
+    torch.cuda.empty_cache()
+    n_steps = int(res["steps"].sum())
     t = float(np.mean(times))
-    out = {"metric": "track-steps/sec", "value": steps / t, "unit": "track-steps/s", "n_gpus": 1,
-           "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t, "higher_is_better": True,
-           "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-           "config": {"workload": "%s showers (BASELINE.json): %d x %g MeV e-, %d layers, adept_inject + adept_run "
-                                  "to completion, wall clock around the two calls" % (name, c["n_primaries"], c["e_primary"], c["n_layers"]),
-                      "layout": layout, "scheme": args.scheme, "capacity_per_kind": c["capacity"],
-                      "batch_primaries": args.batch},
-           "clocks": clocks, "gpu_launches": int(res["iterations"]),
-           "showers_per_s": c["n_primaries"] / t, "track_steps": steps, "iterations": int(res["iterations"]),
+    out = {"value": n_steps / t, "unit": "track-steps/s", "ms_per_run": 1e3 * t, "ms_min": 1e3 * float(np.min(times)),
+           "runs": steps, "warmup_runs": warmup,
+           "workload": "%s showers (BASELINE.json): %d x %g MeV e-, %d layers, adept_inject + adept_run to "
+                       "completion, wall clock around the two calls" % (name, c["n_primaries"], c["e_primary"], c["n_layers"]),
+           "layout": layout, "scheme": scheme, "capacity_per_kind": c["capacity"], "batch_primaries": batch,
+           "slot_recycling": bool(flags & 1),
+           "showers_per_s": c["n_primaries"] / t, "track_steps": n_steps, "iterations": int(res["iterations"]),
+           "us_per_iteration": 1e6 * t / max(1, int(res["iterations"])),
+           "gpu_launches_per_run": int(res["iterations"]),
            "secondaries": [int(x) for x in res["secondaries"]], "slots_used": [int(x) for x in res["slots_used"]],
            "edep_layer_MeV": [float(x) for x in res["edep_layer"]],
            "energy_balance_rel": float((res["edep_slab"].sum() + res["e_escaped"]) / res["e_injected"] - 1.0),
-           "e2e": {"value": steps / t, "unit": "track-steps/s", "h2d_bytes_per_step": 32 * c["n_primaries"],
-                   "d2h_bytes_per_step": 256 + 8 * (2 * c["n_layers"] + 1),
-                   "what": "same measurement: the timed region is the public API with host buffers"},
-           "roofline": None}
-    if not args.no_cpu:                                    # heavy: the oracle needs ~80 s (use --no-cpu to skip)
+           "h2d_bytes_per_run": 32 * c["n_primaries"], "d2h_bytes_per_run": 256 + 8 * (2 * c["n_layers"] + 1)}
+    if with_cpu:                                           # heavy: the oracle needs ~80 s
         from oracle import Oracle
         o = Oracle(geo, tab, seed=c["seed"])
         o.inject(prim)
@@ -405,21 +457,73 @@ def run_showers(args, name: str):
         o.run()
         dt = time.perf_counter() - t0
         r = o.result()
+        o.close()
         out["cpu_baseline"] = {"value": int(r["steps"].sum()) / dt, "unit": "track-steps/s", "cores": 1,
-                               "kind": "oracle", "sample": "the whole %s workload" % name, "seconds": dt}
+                               "host_cores": host_cores(), "kind": "oracle", "sample": "the whole %s workload" % name,
+                               "seconds": dt}
         keys = ("steps", "secondaries", "killed", "escaped_n")
         out["parity_full_size"] = {
             "counts_bit_exact": bool(all((res[k] == r[k]).all() for k in keys) and res["iterations"] == r["iterations"]),
-            "edep_layer_rel_err": float(np.max(np.abs(res["edep_layer"] - r["edep_layer"]) / np.maximum(r["edep_layer"], 1e-30)))}
-    print(json.dumps(out))
+            "edep_layer_rel_err": float(np.max(np.abs(res["edep_layer"] - r["edep_layer"]) / np.maximum(r["edep_layer"], 1e-30))),
+            "e_escaped_rel_err": float(abs(res["e_escaped"] - r["e_escaped"]) / max(r["e_escaped"], 1e-30))}
+    return out
 
 
-def run_sweep(args):
-    """--workload sweep (BASELINE.json configs[3]): 4 Mi slots per kind, occupancy 10..90 %, both
-    schemes x three layouts.  Per cell: time of one adept_step (CUDA events, state restored and L2
-    flushed between repetitions; slot allocation / compaction is fused into the step kernel, so it is
-    part of this time), and from an instrumented context of the same population the per-field
-    read/write counts and the slots / 128-byte lines touched."""
+def sharded_showers(args, name, rank, world, local_rank, dist, max_over_ranks) -> dict:
+    """N > 1: the primaries of `name` split over the ranks, one context per GPU, one
+    all-reduce of the tallies at the end (paper_2302_08252_b200/sharding.py).  Strong scaling: the
+    total work is fixed."""
+    import torch
+    from paper_2302_08252_b200 import Context
+    from paper_2302_08252_b200.sharding import run_sharded
+    from workloads import gen_primaries
+    c = CONFIGS[name]
+    prim = gen_primaries(c["n_primaries"], c["e_primary"])
+    ctx = Context(geometry_for(name), tables_for(name), layout="aosoa32", scheme="dense", capacity=c["capacity"],
+                  seed=c["seed"], device="cuda:%d" % local_rank)
+    times, res = [], None
+    for it in range(1 + 3):
+        ctx.reset()
+        torch.cuda.synchronize()
+        dist.barrier()
+        t0 = time.perf_counter()
+        res = run_sharded(ctx, prim, rank, world)
+        torch.cuda.synchronize()
+        dt = max_over_ranks(time.perf_counter() - t0)
+        if it > 0:
+            times.append(dt)
+    ctx.destroy()
+    n_steps = int(res["steps"].sum())
+    t = float(np.mean(times))
+    return {"value": n_steps / t, "unit": "track-steps/s", "ms_per_run": 1e3 * t, "scaling": "strong",
+            "workload": "%s showers, primaries sharded over %d ranks, one all-reduce of the tallies" % (name, world),
+            "track_steps": n_steps, "iterations": int(res["iterations"]), "showers_per_s": c["n_primaries"] / t}
+
+
+# SURVEY.md §8(d): algorithmic bytes per track-step of one cell of the sweep.  Dense: every record is
+# read once and every output record (survivor or secondary) written once.  Sparse: per input track one
+# slot-list entry and the record (AoS: its two sectors; SoA family: its 14 words -- the sector
+# amplification of scattered slots comes on top and is what the paper's finding is about); per
+# survivor the record's dirty words as whole records (AoS: two sectors) and one slot-list entry; per
+# secondary a whole record and one slot-list entry.
+def sweep_bytes(scheme: str, layout: str, n_in: int, n_surv: int, n_sec: int) -> int:
+    rec = RECORD_BYTES[layout]
+    if scheme == "dense":
+        return rec * (n_in + n_surv + n_sec)
+    return n_in * (4 + rec) + n_surv * (rec + 4) + n_sec * (rec + 4)
+
+
+SECTION_NAMES = ("other", "load", "move", "interact", "alloc", "store")
+
+
+def sweep(args, *, layouts, steps, warmup, instr, sections, occupancies=None, schemes=("dense", "sparse")) -> dict:
+    """BASELINE.json configs[3]: 4 Mi slots per kind, occupancy 10..90 %, both schemes x layouts.  Per
+    cell: time of one adept_step (CUDA events, state restored and L2 flushed between repetitions) with
+    its roofline fraction; the share of that time spent in slot allocation / compaction (rows A9, A10;
+    section clocks of the timing variant of the library, include/adept.h) -- the step does both inside
+    one kernel, so "step plus allocation/compaction time" is one time and its split; and, with
+    `instr`, the per-field read/write counts and slots / 128-byte lines touched
+     from an instrumented context of the same population."""
     import torch
     from paper_2302_08252_b200 import Context, FIELD_NAMES
     from workloads import gen_sweep
@@ -427,26 +531,29 @@ def run_sweep(args):
     geo, tab = geometry_for("sweep"), tables_for("sweep")
     span, cap = c["span"], c["span"] + c["reserve"]
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
-    layouts = ["aos", "soa", "aosoa32", "aosoa64", "soa16"] if args.layout == "all" else [args.layout]
+    peak, peak_src = measured_peak()
     cells = []
-    occupancies = c["occupancies"] if args.occupancy is None else (args.occupancy,)
-    schemes = ("dense", "sparse") if args.scheme is None else (args.scheme,)
-    for occ in occupancies:
+    for occ in (occupancies or c["occupancies"]):
         pop = gen_sweep(occ)
         n_live = sum(p["tracks"].shape[0] for p in pop)
         for scheme in schemes:
             for layout in layouts:
                 cell = {"occupancy": occ, "scheme": scheme, "layout": layout, "tracks": n_live}
-                for instrument in ((False,) if args.no_instr else (False, True)):
+                variants = [("time", False, None)]
+                if sections:
+                    variants.append(("sections", False, "timing"))
+                if instr:
+                    variants.append(("instr", True, None))
+                for what, instrument, variant in variants:
                     ctx = Context(geo, tab, layout=layout, scheme=scheme, capacity=cap, seed=c["seed"],
-                                  instrument=instrument)
+                                  instrument=instrument, variant=variant)
                     for k in range(3):
                         ctx.load_tracks(k, pop[k]["tracks"], pop[k]["slots"] if scheme == "sparse" else None)
                     torch.cuda.synchronize()
-                    if not instrument:
+                    if what == "time":
                         pristine = ctx.workspace.clone()
                         ms = []
-                        for it in range(args.warmup + args.steps):
+                        for it in range(warmup + steps):
                             ctx.workspace.copy_(pristine)
                             flush.zero_()
                             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -454,14 +561,28 @@ def run_sweep(args):
                             ctx.step(sync=False)
                             e1.record(ctx.stream)
                             torch.cuda.synchronize()
-                            if it >= args.warmup:
+                            if it >= warmup:
                                 ms.append(e0.elapsed_time(e1))
                         res = ctx.result()
                         del pristine
-                        cell.update(ms_per_step=float(np.mean(ms)), ms_min=float(np.min(ms)),
-                                    track_steps_per_s=n_live / (float(np.mean(ms)) * 1e-3),
+                        t = float(np.mean(ms))
+                        n_sec = int(res["secondaries"].sum())
+                        n_surv = int(res["live"].sum()) - n_sec
+                        nbytes = sweep_bytes(scheme, layout, n_live, n_surv, n_sec)
+                        cell.update(ms_per_step=t, ms_min=float(np.min(ms)), track_steps_per_s=n_live / (t * 1e-3),
                                     secondaries=[int(x) for x in res["secondaries"]],
-                                    slots_used=[int(x) for x in res["slots_used"]])
+                                    slots_used=[int(x) for x in res["slots_used"]],
+                                    algorithmic_bytes=nbytes,
+                                    roofline={"bound": "hbm", "achieved": nbytes / (t * 1e-3) / 1e9, "peak": peak,
+                                              "unit": "GB/s", "frac": nbytes / (t * 1e-3) / 1e9 / peak})
+                    elif what == "sections":
+                        ctx.step()
+                        cyc = ctx.read_sections().astype(np.float64)[:len(SECTION_NAMES)]
+                        share = cyc / max(1.0, cyc.sum())
+                        cell["section_share"] = {n: float(v) for n, v in zip(SECTION_NAMES, share)}
+                        cell["alloc_compaction_ms"] = float((share[4] + share[5]) * cell["ms_per_step"])
+                        cell["alloc_ms"] = float(share[4] * cell["ms_per_step"])
+                        cell["store_ms"] = float(share[5] * cell["ms_per_step"])
                     else:
                         ctx.step()
                         cnt = ctx.read_counters()
@@ -476,16 +597,67 @@ def run_sweep(args):
                     torch.cuda.empty_cache()
                 cells.append(cell)
                 sys.stderr.write("%s\n" % json.dumps({k: cell.get(k) for k in ("occupancy", "scheme", "layout", "ms_per_step",
-                                                                                "bytes_touched_per_track_step")}))
+                                                                                "alloc_compaction_ms", "bytes_touched_per_track_step")}))
+        del pop
     best = max(cells, key=lambda x: x["track_steps_per_s"])
-    print(json.dumps({"metric": "track-steps/sec", "value": best["track_steps_per_s"], "unit": "track-steps/s",
-                      "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": best["ms_per_step"],
-                      "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
-                      "data": "synthetic",
-                      "config": {"workload": "buffer-scheme sweep (BASELINE.json configs[3]): %d slots per kind, "
-                                             "5 %% of live tracks spawn one secondary; value = best cell" % span,
-                                 "layout": best["layout"], "scheme": best["scheme"], "occupancy": best["occupancy"]},
-                      "gpu_launches": args.steps, "roofline": None, "cells": cells}))
+    return {"workload": "buffer-scheme sweep (BASELINE.json configs[3]): %d slots per kind, 5 %% of live tracks "
+                        "spawn one secondary; one adept_step per cell" % span,
+            "peak_source": peak_src,
+            "sections": "share of per-warp cycles per kernel section from libadept_b200_timing.so (section clocks), "
+                        "applied to the cell's ms_per_step; alloc = rows A9 (ballots, arrival word, reservation, "
+                        "group barrier), store = row A10 (record and slot-list writes)" if sections else None,
+            "best": {k: best[k] for k in ("occupancy", "scheme", "layout", "ms_per_step", "track_steps_per_s")},
+            "cells": cells}
+
+
+def run_showers_cli(args, name: str):
+    """--workload tiny|full|heavy: the shower block as a contract line of its own."""
+    layout = "aosoa32" if args.layout == "all" else args.layout
+    sampler = ClockSampler(0)
+    sampler.start()
+    b = showers(args, name, layout=layout, scheme=args.scheme, steps=args.steps, warmup=args.warmup,
+                with_cpu=not args.no_cpu, batch=args.batch, flags=1 if args.recycle else 0)
+    clocks = sampler.stop()
+    out = {"metric": "track-steps/sec", "value": b["value"], "unit": "track-steps/s", "n_gpus": 1,
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": b["ms_per_run"], "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+           "config": {"workload": b["workload"], "layout": layout, "scheme": args.scheme,
+                      "capacity_per_kind": b["capacity_per_kind"], "batch_primaries": args.batch},
+           "clocks": clocks, "gpu_launches": b["gpu_launches_per_run"],
+           "e2e": {"value": b["value"], "unit": "track-steps/s", "h2d_bytes_per_step": b["h2d_bytes_per_run"],
+                   "d2h_bytes_per_step": b["d2h_bytes_per_run"],
+                   "what": "same measurement: the timed region is the public API with host buffers"},
+           "roofline": None}
+    out.update({k: v for k, v in b.items() if k not in ("value", "unit", "workload")})
+    print(json.dumps(out))
+
+
+def run_sweep_cli(args):
+    layouts = ("aos", "soa", "aosoa32", "aosoa64", "soa16") if args.layout == "all" else (args.layout,)
+    sw = sweep(args, layouts=layouts, steps=args.steps, warmup=args.warmup, instr=not args.no_instr,
+               sections=not args.no_sections,
+               occupancies=None if args.occupancy is None else (args.occupancy,),
+               schemes=("dense", "sparse") if args.scheme is None else (args.scheme,))
+    best = sw["best"]
+    out = {"metric": "track-steps/sec", "value": best["track_steps_per_s"], "unit": "track-steps/s",
+           "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": best["ms_per_step"],
+           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+           "config": {"workload": sw["workload"] + "; value = best cell", "layout": best["layout"],
+                      "scheme": best["scheme"], "occupancy": best["occupancy"]},
+           "gpu_launches": args.steps, "roofline": None}
+    out.update({k: sw[k] for k in ("peak_source", "sections", "cells")})
+    print(json.dumps(out))
+
+
+def relaunch_as_ranks(n: int) -> int:
+    """`python bench.py --gpus N` outside torchrun: run the same command line as N ranks of one node."""
+    import socket
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(n),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
 
 
 def main():
@@ -496,30 +668,42 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--layout", default="all", choices=["soa", "aosoa32", "aosoa64", "soa16", "aos", "aosoa16", "aosoa128", "all"])
     ap.add_argument("--tracks", type=int, default=CONFIGS[WORKLOAD]["n_tracks"])
-    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline legs")
+    ap.add_argument("--extras", default=None,
+                    help="comma list of what the default line carries beside the headline: showers, heavy, sweep "
+                         "(default: all three at the full population, none otherwise); 'none' = headline only")
     ap.add_argument("--workload", default="single_step", choices=["single_step", "tiny", "full", "heavy", "sweep"],
-                    help="single_step = the headline (BASELINE.json configs[2]); the others are reported beside it")
+                    help="single_step = the headline (BASELINE.json configs[2]); the others as a line of their own")
     ap.add_argument("--scheme", default=None, choices=["dense", "sparse"],
                     help="shower workloads: container (default dense); sweep: only this scheme (default both)")
     ap.add_argument("--occupancy", type=float, default=None, help="sweep: only this occupancy (default 0.1 .. 0.9)")
     ap.add_argument("--no-instr", action="store_true", help="sweep: skip the instrumented (counting) contexts")
+    ap.add_argument("--no-sections", action="store_true", help="sweep: skip the section-clock contexts")
     ap.add_argument("--batch", type=int, default=0, help="shower workloads: batch_primaries (0 = all at once)")
+    ap.add_argument("--recycle", action="store_true", help="shower workloads, sparse scheme: recycle freed slots")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
+    if "WORLD_SIZE" not in os.environ and args.gpus > 1:
+        sys.exit(relaunch_as_ranks(args.gpus))
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus and rank == 0:
+        sys.stderr.write("bench.py: --gpus %d but %d rank(s) were launched; reporting n_gpus = %d\n" % (args.gpus, world, world))
+    if args.extras is None:
+        args.extras = "showers,heavy,sweep" if args.tracks == CONFIGS[WORKLOAD]["n_tracks"] else "none"
+    args.extras = set(x for x in args.extras.split(",") if x and x != "none")
     if args.impl == "reference":
-        run_reference(args, rank)
+        run_reference(args, rank, world)
         return
     if args.workload in ("tiny", "full", "heavy"):
         if rank == 0:
             args.scheme = args.scheme or "dense"
-            run_showers(args, args.workload)
+            run_showers_cli(args, args.workload)
         return
     if args.workload == "sweep":
         if rank == 0:
-            run_sweep(args)
+            run_sweep_cli(args)
         return
     run_gpu(args, rank, world, local_rank)
 

@@ -187,6 +187,19 @@ int adept_read_counters(adept_ctx *, uint64_t *field_rw, uint32_t *lines, uint32
 uint64_t adept_instr_lines(const adept_ctx *);
 uint64_t adept_instr_slots(const adept_ctx *);
 
+/* Timing variant of the library (built with -DADEPT_TIMING_SECTIONS as libadept_b200_timing.so;
+ * BASELINE.json configs[3]: "each scheme reports step plus slot-allocation/compaction time").
+ * Allocation and compaction are fused into the step kernel, so the
+ * variant brackets the sections of every tile with the SM clock and sums, over lane 0 of every
+ * warp, the cycles spent in each: cycles[0] other (prologue, table staging, tally flush),
+ * [1] A1 record load, [2] A2-A7 move half, [3] A8 interact half, [4] A9 allocation (ballots, arrival
+ * word, range/slot reservation, group barrier, ranks), [5] A10 stores (records, slot lists, parked
+ * queue); [6], [7] unused.  Cumulative since create/reset.  adept_timing_sections() returns 1 in
+ * the timing variant, 0 otherwise (all cycles then read 0).  cycles: host, ADEPT_N_SECTIONS entries. */
+#define ADEPT_N_SECTIONS 8
+int adept_timing_sections(void);
+int adept_read_sections(adept_ctx *, uint64_t *cycles);
+
 /* Byte offset of word `field` (0..13: pos xyz, dir xyz, ekin, nial 0-2, vol, id_lo, id_hi, step) of
  * slot `slot` inside one record buffer of `capacity` slots under `layout` (Fig. 3:
  * where each field is placed).  Pure host arithmetic; UINT64_MAX on invalid arguments. */

@@ -49,7 +49,7 @@ class _Config(C.Structure):
     _fields_ = [("layout", C.c_int32), ("scheme", C.c_int32), ("capacity_per_kind", C.c_uint32),
                 ("batch_primaries", C.c_uint32), ("seed", C.c_uint64), ("workspace", C.c_void_p),
                 ("workspace_bytes", C.c_size_t), ("cuda_stream", C.c_void_p), ("instrument", C.c_uint32),
-                ("reserved", C.c_uint32)]
+                ("flags", C.c_uint32)]
 
 
 class _Counts(C.Structure):
@@ -63,17 +63,19 @@ class _Result(C.Structure):
                 ("edep_slab", C.POINTER(C.c_double)), ("edep_layer", C.POINTER(C.c_double))]
 
 
-_LIB = None
+_SO_TIMING = os.path.join(_HERE, "libadept_b200_timing.so")   # -DADEPT_TIMING_SECTIONS variant (adept.h)
+_LIBS: dict = {}
 
 
-def lib():
-    """Load the C-ABI library.  Raises if it has not been built: there is no fallback path."""
-    global _LIB
-    if _LIB is None:
-        if not os.path.exists(_SO):
+def lib(variant: str | None = None):
+    """Load the C-ABI library (`variant="timing"`: the section-clock build of the same sources).
+    Raises if it has not been built: there is no fallback path."""
+    so = _SO_TIMING if variant == "timing" else _SO
+    if so not in _LIBS:
+        if not os.path.exists(so):
             raise ImportError("%s is missing: run `python -m paper_2302_08252_b200.build` (or "
-                              "__graft_entry__.build()); there is no CPU fallback" % _SO)
-        L = C.CDLL(_SO)
+                              "__graft_entry__.build()); there is no CPU fallback" % so)
+        L = C.CDLL(so)
         vp, u64, u32 = C.c_void_p, C.c_uint64, C.c_uint32
         L.adept_workspace_bytes.restype = C.c_size_t
         L.adept_workspace_bytes.argtypes = [C.POINTER(_Geometry), C.POINTER(_Tables), C.POINTER(_Config)]
@@ -97,8 +99,11 @@ def lib():
         L.adept_last_error.restype = C.c_char_p
         L.adept_last_error.argtypes = [vp]
         L.adept_dev_math.argtypes = [C.c_int, vp, vp, u64, vp]
-        _LIB = L
-    return _LIB
+        L.adept_timing_sections.restype = C.c_int
+        L.adept_timing_sections.argtypes = []
+        L.adept_read_sections.argtypes = [vp, vp]
+        _LIBS[so] = L
+    return _LIBS[so]
 
 
 def field_offset(layout: int, capacity: int, slot: int, field: int) -> int:
@@ -129,9 +134,9 @@ class Context:
     """adept_create ... adept_destroy.  `geometry`/`tables` are the workloads.* objects (plain data)."""
 
     def __init__(self, geometry, tables, *, layout="soa", scheme="dense", capacity, seed=0,
-                 batch_primaries=0, instrument=False, device="cuda:0", stream=None):
+                 batch_primaries=0, instrument=False, device="cuda:0", stream=None, variant=None, flags=0):
         import torch
-        self._L = lib()
+        self._L = lib(variant)
         self._torch = torch
         self.layout = LAYOUTS[layout] if isinstance(layout, str) else int(layout)
         self.scheme = SCHEMES[scheme] if isinstance(scheme, str) else int(scheme)
@@ -142,7 +147,7 @@ class Context:
         self._t = _Tables(tables.n_bins, tables.n_materials, tables.e_min, tables.e_max, float(tables.ln_e_min),
                           float(tables.inv_dln), tables.e_cut, data.ctypes.data_as(C.POINTER(C.c_float)))
         cfg = _Config(self.layout, self.scheme, capacity, batch_primaries, seed, None, 0, None,
-                      1 if instrument else 0, 0)
+                      1 if instrument else 0, flags)
         nbytes = self._L.adept_workspace_bytes(C.byref(self._g), C.byref(self._t), C.byref(cfg))
         if nbytes == 0:
             raise AdeptError(-1, "adept_workspace_bytes rejected the arguments")
@@ -243,6 +248,12 @@ class Context:
         slots = np.zeros((3, n_slots), dtype=np.uint32)
         self._check(self._L.adept_read_counters(self._h, rw.ctypes.data, lines.ctypes.data, slots.ctypes.data))
         return dict(field_rw=rw, lines=lines, slots=slots)
+
+    def read_sections(self):
+        """Timing variant: warp-cycles per kernel section (adept.h adept_read_sections)."""
+        out = np.zeros(8, dtype=np.uint64)
+        self._check(self._L.adept_read_sections(self._h, out.ctypes.data))
+        return out
 
     def reset(self):
         self._check(self._L.adept_reset(self._h))

@@ -14,6 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libadept_b200.so")
+LIB_TIMING = os.path.join(HERE, "libadept_b200_timing.so")   # same sources, -DADEPT_TIMING_SECTIONS (include/adept.h)
 SOURCES = ["layout_aos.cu", "layout_soa.cu", "layout_aosoa32.cu", "layout_aosoa64.cu", "layout_soa16.cu", "layout_aosoa16.cu", "layout_aosoa128.cu",
            "adept_api.cu"]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
@@ -27,11 +28,18 @@ def _deps():
     return out
 
 
-def is_stale() -> bool:
-    if not os.path.exists(LIB):
+def is_stale(lib: str = LIB) -> bool:
+    if not os.path.exists(lib):
         return True
-    t = os.path.getmtime(LIB)
+    t = os.path.getmtime(lib)
     return any(os.path.getmtime(d) > t for d in _deps())
+
+
+def build_all(force: bool = False) -> None:
+    """The library and its timing variant."""
+    build(force=force)
+    if force or is_stale(LIB_TIMING):
+        build(extra_flags=("-DADEPT_TIMING_SECTIONS",), out=LIB_TIMING)
 
 
 def build(force: bool = False, verbose: bool = False, extra_flags=(), out: str | None = None) -> str:
@@ -68,3 +76,5 @@ def build(force: bool = False, verbose: bool = False, extra_flags=(), out: str |
 
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--no-variants" not in sys.argv:
+        build_all()

@@ -71,7 +71,8 @@ static bool make_plan(const adept_geometry *g, const adept_tables *t, const adep
   pl.table_bytes = size_t(t->n_materials) * 2 * (t->n_bins + 1) * sizeof(float4);
   pl.stage_records = std::min<uint32_t>(pl.capacity, kStageRecords);
   size_t off = 0;
-  pl.ctl = off; off = align_up(off + kCtlHeaderBytes + (size_t(2) * g->n_layers + 1) * sizeof(unsigned long long));
+  // control header, tallies (per slab + escaped), section clocks of the timing build
+  pl.ctl = off; off = align_up(off + kCtlHeaderBytes + (size_t(2) * g->n_layers + 1 + kNumSections) * sizeof(unsigned long long));
   pl.tables = off; off = align_up(off + pl.table_bytes);
   pl.stage = off; off = align_up(off + size_t(pl.stage_records) * kStageRecordBytes);
   pl.stage_slots = off; off = align_up(off + size_t(pl.stage_records) * 4);
@@ -288,7 +289,7 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
     return ADEPT_ECUDA;
   };
   cudaError_t e;
-  c->pinned_bytes = kCtlHeaderBytes + (size_t(2) * g->n_layers + 1) * sizeof(unsigned long long);
+  c->pinned_bytes = kCtlHeaderBytes + (size_t(2) * g->n_layers + 1 + kNumSections) * sizeof(unsigned long long);
   if ((e = cudaMallocHost(reinterpret_cast<void **>(&c->pinned), c->pinned_bytes)) != cudaSuccess)
     return die("cudaMallocHost", e);
   if ((e = cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking)) != cudaSuccess)
@@ -316,6 +317,7 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
   Params &p = c->params;
   p.ctl = reinterpret_cast<Ctl *>(c->ws + pl.ctl);
   p.tally = reinterpret_cast<unsigned long long *>(c->ws + pl.ctl + kCtlHeaderBytes);
+  p.sections = p.tally + (size_t(2) * g->n_layers + 1);
   p.tables = reinterpret_cast<const float4 *>(c->ws + pl.tables);
   p.table_bytes = static_cast<uint32_t>(pl.table_bytes / 2);  // per particle group
   p.nodes = nodes;
@@ -689,6 +691,24 @@ int adept_read_counters(adept_ctx *c, uint64_t *field_rw, uint32_t *lines, uint3
                        cudaMemcpyDeviceToHost));
   }
   return ADEPT_OK;
+}
+
+int adept_timing_sections(void) {
+#ifdef ADEPT_TIMING_SECTIONS
+  return 1;
+#else
+  return 0;
+#endif
+}
+
+int adept_read_sections(adept_ctx *c, uint64_t *cycles) {
+  if (!c || !cycles) return c ? fail(c, ADEPT_EINVAL, "adept_read_sections: cycles is NULL") : ADEPT_EINVAL;
+  const int rc = fetch_ctl(c, true);
+  if (rc != ADEPT_OK && rc != ADEPT_ECAPACITY) return rc;
+  const unsigned long long *s = reinterpret_cast<const unsigned long long *>(c->pinned + kCtlHeaderBytes) +
+                                (size_t(2) * c->geo.n_layers + 1);
+  for (int i = 0; i < kNumSections; ++i) cycles[i] = s[i];
+  return rc;
 }
 
 uint64_t adept_field_offset(int32_t layout, uint32_t capacity, uint32_t slot, uint32_t field) {

@@ -93,6 +93,7 @@ struct KindStorage {
 struct Params {
   Ctl *ctl;
   unsigned long long *tally; // [n_slabs + 1] fixed point, right after the control header
+  unsigned long long *sections;  // [kNumSections] warp-cycles per kernel section (timing build; after the tallies)
   const float4 *tables;      // [group][material][node] {q0, q1, q2, 0}; group 0 = gamma, 1 = e+-
   uint32_t table_bytes;      // bytes of ONE group, multiple of 16
   uint32_t nodes;            // n_bins + 1

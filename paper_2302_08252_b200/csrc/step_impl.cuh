@@ -44,6 +44,41 @@ __device__ __forceinline__ void group_sync(int group) {
   asm volatile("bar.sync %0, %1;" ::"r"(group + 1), "n"(kGroup) : "memory");
 }
 
+// ---- section clocks (timing build only) ------------------------------------------------------------
+// BASELINE.json configs[3]: "each scheme reports step plus slot-allocation/compaction time".  Allocation
+// and compaction are fused into the step kernel (rows A9, A10), so a variant of the library compiled
+// with -DADEPT_TIMING_SECTIONS brackets the sections of a tile with clock64(): lane 0 of every warp adds
+// the cycles it spent in each section to CTA counters, flushed to Params::sections at kernel end.
+// The shares of the per-warp cycles, applied to the kernel time of the normal build, are the reported
+// per-section times.  In the normal build the clock is an empty object.
+enum Section : int {
+  SEC_OTHER = 0,     // launch prologue, table staging, loop control, tally flush
+  SEC_LOAD = 1,      // A1: waiting for / fetching the records of a tile
+  SEC_PHYSICS = 2,   // A2-A7: the move half and its scoring
+  SEC_INTERACT = 3,  // A8: the interact half (queue read, sampling, scoring)
+  SEC_ALLOC = 4,     // A9: ballots, arrival word, range / slot reservation, the group barrier, ranks
+  SEC_STORE = 5,     // A10: survivor and secondary writes, slot-list pushes, parked-queue writes
+  kNumSections = 8
+};
+#ifdef ADEPT_TIMING_SECTIONS
+struct SectClock {
+  long long t;
+  uint32_t *acc;  // shared, [kNumSections]
+  bool lead;
+  __device__ __forceinline__ void start(uint32_t *a, bool l) { acc = a; lead = l; t = clock64(); }
+  __device__ __forceinline__ void mark(int s) {
+    const long long n = clock64();
+    if (lead) atomicAdd(&acc[s], static_cast<uint32_t>(n - t));
+    t = n;
+  }
+};
+#else
+struct SectClock {
+  __device__ __forceinline__ void start(uint32_t *, bool) {}
+  __device__ __forceinline__ void mark(int) {}
+};
+#endif
+
 // ---- tally bins (row A6) -------------------------------------------------------------------------
 struct Bins {
   uint32_t *lo, *hi;  // shared, n_slabs + 1 entries each
@@ -258,6 +293,7 @@ struct CtaShared {
   uint32_t alive[4];
   uint32_t escaped[4];
   uint32_t probe[3 * kNumFields * 2];
+  uint32_t sect[kNumSections];  // timing build: cycles per section (lane 0 of every warp)
   GroupShared grp[kMaxGroupsPerCta];
 };
 
@@ -310,6 +346,7 @@ struct GroupRefs {
   uint32_t *queue;   // shared, [kQueueCap][queue_words]
   uint32_t *in_buf;  // shared, one staged tile (dense scheme)
   int group, gtid;   // group index inside the CTA, thread index inside the group
+  SectClock *clk;    // timing build: this thread's section clock
 };
 
 // S25 / S31 energy of a track that leaves the simulation
@@ -333,6 +370,7 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
   GroupShared &g = *c.g;
 
   // A1: load
+  c.clk->mark(SEC_OTHER);
   uint32_t slot = i;
   if (SCHEME == S_SPARSE && active) slot = p.kind[KIND].queue[par][i];
   const TrackView<L, INSTR> cur = make_view<L, INSTR>(p, KIND, (SCHEME == S_DENSE) ? int(par) : 0, c.cta->probe);
@@ -363,6 +401,7 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
       t = cur.load(slot);
     }
     old = t;
+    c.clk->mark(SEC_LOAD);
     if constexpr (KIND == K_GAMMA) move_gamma(t, env, o);
     else move_elec<KIND>(t, env, o);
     // A6: scoring into the CTA's bins (pre-step slab; the S31 guard uses the post-step slab).  A
@@ -374,6 +413,7 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
       if (o.guard) bin_add_track_energy<KIND>(c.bins, t.vol, t.ekin);
     }
   }
+  c.clk->mark(SEC_PHYSICS);
   const bool parked = active && o.pending != P_NONE;
   const bool survives = active && !parked && o.alive;
   const uint32_t m_surv = __ballot_sync(0xFFFFFFFFu, survives);
@@ -398,6 +438,7 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
   }
   word = __shfl_sync(0xFFFFFFFFu, word, 0);
 
+  c.clk->mark(SEC_ALLOC);
   // park the tracks that still owe an interaction
   if (parked) {
     const uint32_t q = queued + count_of(word, 1) + __popc(m_park & lt_mask);
@@ -407,7 +448,9 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
   // later writes only what it changes)
   if (SCHEME == S_SPARSE && (survives || parked)) cur.store_changed(slot, t, old);
 
+  c.clk->mark(SEC_STORE);
   group_sync(c.group);
+  c.clk->mark(SEC_ALLOC);
   if (survives) {
     const uint32_t dst = g.base[sbuf][0] + count_of(word, 0) + __popc(m_surv & lt_mask);
     if (dst < p.capacity) {
@@ -417,6 +460,7 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
       ctl->overflow = 1u;
     }
   }
+  c.clk->mark(SEC_STORE);
   return g.qtot[sbuf];
 }
 
@@ -432,6 +476,7 @@ __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &e
   const uint32_t batch = queued < uint32_t(kGroup) ? queued : uint32_t(kGroup);
   const uint32_t first = queued - batch;
 
+  c.clk->mark(SEC_OTHER);
   const bool have = uint32_t(gtid) < batch;
   Trk t, before_interaction;
   InteractOut o;
@@ -449,6 +494,7 @@ __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &e
     if (o.dep_b != 0.0f) bin_add(c.bins, t.vol, o.dep_b);
     if (o.guard) bin_add_track_energy<KIND>(c.bins, t.vol, t.ekin);
   }
+  c.clk->mark(SEC_INTERACT);
   constexpr int Q0 = kid_kind<KIND>(0), Q1 = kid_kind<KIND>(1);  // never KIND itself
   const uint32_t m_alive = __ballot_sync(0xFFFFFFFFu, o.alive);
   const uint32_t m_k0 = __ballot_sync(0xFFFFFFFFu, o.kid[0].kind >= 0);
@@ -483,6 +529,7 @@ __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &e
   const uint32_t r_k1 = count_of(word, Q1) + ((Q0 == Q1) ? uint32_t(__popc(m_k0)) : 0u) + __popc(m_k1 & lt_mask);
   const int nbuf = int(par ^ 1u);
   bool dropped = false;
+  c.clk->mark(SEC_ALLOC);
   if (SCHEME == S_DENSE) {
     // A10: whole records into the next arrays
     if (o.alive) {
@@ -524,6 +571,7 @@ __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &e
     }
   }
   if (dropped) ctl->overflow = 1u;
+  c.clk->mark(SEC_STORE);
   return first;
 }
 
@@ -603,6 +651,8 @@ __global__ void __launch_bounds__(THREADS, (THREADS == kBlockSmall) ? ADEPT_STEP
   unsigned char *mine = dyn_smem + units_offset(p.table_bytes, p.n_slabs) + size_t(c.group) * kPerGroup;
   c.in_buf = reinterpret_cast<uint32_t *>(mine);
   c.queue = reinterpret_cast<uint32_t *>(mine + kInBuf);
+  SectClock clk;
+  c.clk = &clk;
 
   // A0: what is alive (written by the previous iteration's last CTA; constant during this launch)
   const uint32_t par = ctl->parity;
@@ -623,7 +673,9 @@ __global__ void __launch_bounds__(THREADS, (THREADS == kBlockSmall) ? ADEPT_STEP
     if (tid < 4) { sh.alive[tid] = 0u; sh.escaped[tid] = 0u; }
     if (tid < kGroupsPerCta) { sh.grp[tid].loaded = 0u; sh.grp[tid].acc[0] = 0u; sh.grp[tid].acc[1] = 0u; }
     if (INSTR) for (int s = tid; s < 3 * kNumFields * 2; s += kBlock) sh.probe[s] = 0u;
+    if (tid < kNumSections) sh.sect[tid] = 0u;
     __syncthreads();
+    clk.start(sh.sect, (tid & 31) == 0);
 
     Env env;
     env.tab = s_tab; env.nodes = p.nodes;
@@ -639,7 +691,11 @@ __global__ void __launch_bounds__(THREADS, (THREADS == kBlockSmall) ? ADEPT_STEP
     run_kind<L, SCHEME, INSTR, K_GAMMA>(p, env, c, par, t0 + t1, t2, n2, sbuf, in_phase, tab_phase, staged_group);
 
     // flush the CTA's tallies
+    clk.mark(SEC_OTHER);
     __syncthreads();
+#ifdef ADEPT_TIMING_SECTIONS
+    if (tid < kNumSections && sh.sect[tid]) atomicAdd(&p.sections[tid], static_cast<unsigned long long>(sh.sect[tid]));
+#endif
     for (uint32_t s = tid; s <= p.n_slabs; s += kBlock) {
       const unsigned long long v = (static_cast<unsigned long long>(c.bins.hi[s]) << 32) + c.bins.lo[s];
       if (v != 0ull && atomicAdd(&p.tally[s], v) + v < v) ctl->overflow = 1u;  // 2^32 MeV in one bin: reported, not wrapped silently

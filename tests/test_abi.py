@@ -14,7 +14,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 @pytest.fixture(scope="module")
 def L():
     from paper_2302_08252_b200 import build
-    build.build()
+    build.build_all()
     from paper_2302_08252_b200 import binding
     return binding
 
@@ -31,7 +31,16 @@ def test_library_exports_every_declared_function(L):
     lib = L.lib()
     for n in names:
         assert hasattr(lib, n), "libadept_b200.so does not export %s" % n
-    assert len(names) >= 17
+    assert len(names) >= 19
+
+
+def test_timing_variant_exports_the_same_abi(L):
+    """libadept_b200_timing.so (section clocks, -DADEPT_TIMING_SECTIONS) is the same library."""
+    lib, timing = L.lib(), L.lib("timing")
+    for n in declared_functions():
+        assert hasattr(timing, n), "libadept_b200_timing.so does not export %s" % n
+    assert lib.adept_timing_sections() == 0 and timing.adept_timing_sections() == 1
+    assert timing.adept_read_sections(None, None) == -1
 
 
 def test_record_sizes_match_the_header(L):

@@ -8,11 +8,12 @@ import sys
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def _run(extra_env=None):
-    env = dict(os.environ)
+def _run(extra_env=None, extra_args=()):
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK")}
     env.update(extra_env or {})
     out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--steps", "2",
-                          "--warmup", "1", "--tracks", "65536"], capture_output=True, text=True, env=env, timeout=300)
+                          "--warmup", "1", "--tracks", "65536", *extra_args], capture_output=True, text=True, env=env,
+                         timeout=600)
     assert out.returncode == 0, out.stderr[-2000:]
     return out.stdout.strip()
 
@@ -28,11 +29,21 @@ def test_reference_arm_prints_one_contract_line():
     assert "workload" in d["config"] and "model" not in d["config"]
     cb = d["cpu_baseline"]
     assert cb["kind"] == "oracle" and cb["cores"] == 1 and cb["value"] == d["value"] and "sample" in cb
+    assert cb["host_cores"] == os.cpu_count() and d["n_gpus"] == 1
     assert d["e2e"] == {"value": d["value"], "unit": d["unit"], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
 
 
 def test_reference_arm_other_ranks_stay_silent():
     assert _run({"RANK": "1", "WORLD_SIZE": "2", "LOCAL_RANK": "1"}) == ""
+
+
+def test_gpus_flag_launches_the_ranks_itself():
+    """`python bench.py --gpus 2` outside torchrun runs two ranks (127.0.0.1 rendezvous); rank 0 alone
+    prints, and n_gpus is the number of ranks that ran."""
+    lines = [l for l in _run(extra_args=("--gpus", "2")).split("\n") if l.strip().startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["n_gpus"] == 2
 
 
 import pytest
@@ -58,7 +69,8 @@ def test_gpu_arm_prints_one_contract_line():
     e = d["e2e"]
     assert e["h2d_bytes_per_step"] == 56 * 262144 and e["d2h_bytes_per_step"] > 56 * 262144 and e["value"] < d["value"]
     cb = d["cpu_baseline"]
-    assert cb["kind"] == "oracle" and cb["cores"] == 1 and cb["value"] > 1e5
+    assert cb["kind"] == "oracle" and cb["cores"] == 1 and cb["value"] > 1e5 and cb["host_cores"] >= 1
+    assert "showers" not in d and "sweep" not in d      # reduced population: headline only
     p = d["parity_full_size"]
     assert p["counts_bit_exact"] and p["tracks_with_another_fate"] == 0 and p["tracks_with_any_word_differing"] == 0
     assert set(d["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
