@@ -91,8 +91,17 @@ typedef struct {
   size_t workspace_bytes;
   void *cuda_stream;          /* cudaStream_t */
   uint32_t instrument;        /* 1 = counting build of the same kernels */
-  uint32_t reserved;
+  uint32_t flags;             /* 0 or ADEPT_FLAG_*; unknown bits are rejected */
 } adept_config;
+
+/* Sparse single buffer only (ignored by the dense double buffer).  The paper's container hands out
+ * slots "atomically" and never reuses one within a batch (2044 dense slots against
+ * 45509 sparse ones for the same run) -- that policy is the default (DESIGN.md rule S30).  With this
+ * flag the slot of every track that ends is pushed onto a per-kind ring of free slots, and secondaries
+ * take slots from the ring (those freed up to the previous iteration) before bump-allocating new
+ * ones.  Results are unchanged (slots carry no physics); adept_counts.slots_used
+ * then reports the real footprint. */
+#define ADEPT_FLAG_RECYCLE_SLOTS 1u
 
 typedef struct { uint32_t kind; float pos[3], dir[3], ekin; } adept_primary; /* 32 B */
 

@@ -33,7 +33,7 @@ inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 struct Plan {  // carve-up of the workspace
   size_t ctl, tables, stage, stage_slots;
-  size_t rec[3], queue[3][2];
+  size_t rec[3], queue[3][2], ring[3];
   size_t instr_rw, instr_lines[3], instr_slots[3];
   size_t total;
   uint32_t capacity;       // rounded up to a multiple of 128 (one tile)
@@ -49,10 +49,12 @@ static const LayoutOps *ops_for(int layout) {
     case ADEPT_AOS: return &kOpsAoS;
     case ADEPT_SOA: return &kOpsSoA;
     case ADEPT_AOSOA32: return &kOpsAoSoA32;
+#ifndef ADEPT_FEW_LAYOUTS   // experiment builds instantiate the three paper layouts only
     case ADEPT_AOSOA64: return &kOpsAoSoA64;
     case ADEPT_SOA16: return &kOpsSoA16;
     case ADEPT_AOSOA16: return &kOpsAoSoA16;
     case ADEPT_AOSOA128: return &kOpsAoSoA128;
+#endif
     default: return nullptr;
   }
 }
@@ -62,6 +64,7 @@ static bool make_plan(const adept_geometry *g, const adept_tables *t, const adep
   const LayoutOps *ops = ops_for(c->layout);
   if (!ops) return false;
   if (c->scheme != ADEPT_SPARSE_SINGLE && c->scheme != ADEPT_DENSE_DOUBLE) return false;
+  if (c->flags & ~uint32_t(ADEPT_FLAG_RECYCLE_SLOTS)) return false;
   if (g->n_layers == 0 || g->n_layers > 2048) return false;
   if (t->n_bins == 0 || t->n_bins > 4096 || t->n_materials == 0 || t->n_materials > 8) return false;
   if (c->capacity_per_kind == 0 || c->capacity_per_kind > (1u << 30)) return false;
@@ -82,6 +85,8 @@ static bool make_plan(const adept_geometry *g, const adept_tables *t, const adep
       pl.queue[k][q] = off;
       if (c->scheme == ADEPT_SPARSE_SINGLE) off = align_up(off + size_t(pl.capacity) * 4);
     }
+    pl.ring[k] = off;   // freed slots (ADEPT_FLAG_RECYCLE_SLOTS)
+    if (c->scheme == ADEPT_SPARSE_SINGLE && (c->flags & ADEPT_FLAG_RECYCLE_SLOTS)) off = align_up(off + size_t(pl.capacity) * 4);
   }
   pl.lines_per_kind = (pl.rec_words * 4 * pl.nbuf + 127) / 128;
   pl.slots_per_kind = size_t(pl.capacity) * pl.nbuf;
@@ -326,12 +331,14 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
   p.abs_mm = g->abs_mm; p.pitch = c->pitch; p.half_xy = g->half_xy_mm;
   p.mat_abs = g->mat_abs; p.mat_gap = g->mat_gap;
   p.capacity = pl.capacity;
+  p.recycle = (cfg->scheme == ADEPT_SPARSE_SINGLE && (cfg->flags & ADEPT_FLAG_RECYCLE_SLOTS)) ? 1u : 0u;
   for (int k = 0; k < 3; ++k) {
     uint32_t *r = reinterpret_cast<uint32_t *>(c->ws + pl.rec[k]);
     p.kind[k].rec[0] = r;
     p.kind[k].rec[1] = (pl.nbuf == 2) ? r + pl.rec_words : r;
     p.kind[k].queue[0] = reinterpret_cast<uint32_t *>(c->ws + pl.queue[k][0]);
     p.kind[k].queue[1] = reinterpret_cast<uint32_t *>(c->ws + pl.queue[k][1]);
+    p.kind[k].free_ring = reinterpret_cast<uint32_t *>(c->ws + pl.ring[k]);
     p.kind[k].instr_lines = reinterpret_cast<uint32_t *>(c->ws + pl.instr_lines[k]);
     p.kind[k].instr_slots = reinterpret_cast<uint32_t *>(c->ws + pl.instr_slots[k]);
   }
@@ -373,7 +380,7 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
   const size_t tile_words = c->ops->record_words(kGroup);
   c->small.threads = kBlockSmall;
   c->small.dyn_smem = step_smem_bytes(cfg->scheme, pl.table_bytes / 2, p.n_slabs, tile_words, kBlockSmall);
-  const int per_sm = c->ops->step_ctas_per_sm(cfg->scheme, instr, kBlockSmall, c->small.dyn_smem);
+  const int per_sm = c->ops->step_ctas_per_sm(cfg->scheme, instr, int(p.recycle), kBlockSmall, c->small.dyn_smem);
   if (per_sm <= 0) {
     g_create_error = "step kernel does not fit on an SM with these tables (shared memory)";
     free_host_side(c);
@@ -382,7 +389,7 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
   c->small.grid = static_cast<unsigned>(sms * per_sm);
   c->large.threads = kBlockLarge;
   c->large.dyn_smem = step_smem_bytes(cfg->scheme, pl.table_bytes / 2, p.n_slabs, tile_words, kBlockLarge);
-  const int per_sm_large = c->ops->step_ctas_per_sm(cfg->scheme, instr, kBlockLarge, c->large.dyn_smem);
+  const int per_sm_large = c->ops->step_ctas_per_sm(cfg->scheme, instr, int(p.recycle), kBlockLarge, c->large.dyn_smem);
   cudaGetLastError();  // a failed attribute query of the optional shape is not an error of the context
   c->large.grid = per_sm_large > 0 ? static_cast<unsigned>(sms * per_sm_large) : 0u;
   c->live_hint = 0;

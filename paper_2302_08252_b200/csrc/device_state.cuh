@@ -41,6 +41,8 @@ constexpr int kQueueCap = 2 * kGroup;
 __host__ __device__ constexpr int queue_words(int scheme) { return scheme == S_DENSE ? 14 : 16; }
 __host__ __device__ constexpr size_t queue_bytes(int scheme) { return size_t(kQueueCap) * queue_words(scheme) * 4; }
 // Dense scheme: one tile staged in shared memory by TMA (record_words(kGroup) words of the layout).
+// The sparse scheme stages nothing: its kernels leave the rest of the SM's memory to L1 (measured:
+// the scattered 16-byte pieces of AoS records depend on it -- DESIGN.md §10).
 __host__ __device__ constexpr size_t in_buf_bytes(int scheme, size_t tile_words) {
   return scheme == S_DENSE ? tile_words * 4 : 0;
 }
@@ -76,16 +78,21 @@ struct Ctl {
   uint32_t it_escaped[4];  // this iteration: parents that left the calorimeter, per kind
   unsigned long long steps[3], secondaries[3], killed[3], escaped_n[3], slots_used[3];
   unsigned long long iterations;
-  unsigned long long pad1[3];
+  // sparse scheme with ADEPT_FLAG_RECYCLE_SLOTS: ring of freed slots per kind (KindStorage::free_ring).
+  // Monotonic counters, ring index = counter % capacity.  Slots freed in iteration n are pushed at
+  // `free_tail` and become allocatable in iteration n + 1: an iteration pops only below
+  // `free_tail_start` (the tail at its start), so pushes and pops never meet inside a launch.
+  uint32_t free_head[4], free_tail[4], free_tail_start[4];
   // unsigned long long tally[n_slabs + 1] follows at byte kCtlHeaderBytes: fixed-point energy
   // deposit per slab, then the energy carried out of the calorimeter
 };
-constexpr size_t kCtlHeaderBytes = 256;
+constexpr size_t kCtlHeaderBytes = 512;
 static_assert(sizeof(Ctl) <= kCtlHeaderBytes, "control block header");
 
 struct KindStorage {
   uint32_t *rec[2];    // dense: current/next arrays by parity; sparse: rec[0] only
   uint32_t *queue[2];  // sparse: slot lists by parity
+  uint32_t *free_ring;    // sparse + slot recycling: [capacity] freed slots (Ctl::free_head / free_tail)
   uint32_t *instr_lines;  // instrumented build: per 128-B line of this kind's record storage
   uint32_t *instr_slots;  // instrumented build: per slot (dense: 2 * capacity)
 };
@@ -102,6 +109,7 @@ struct Params {
   float abs_mm, pitch, half_xy;
   uint32_t mat_abs, mat_gap;
   uint32_t capacity;         // slots per kind (multiple of 128)
+  uint32_t recycle;          // sparse scheme: 1 = freed slots are reused (ADEPT_FLAG_RECYCLE_SLOTS)
   KindStorage kind[3];
   unsigned long long *instr_field_rw;  // [3][14][2], instrumented build
   // SoA and AoS layouts, dense scheme: tensor maps of the record buffers, [kind][parity] (see

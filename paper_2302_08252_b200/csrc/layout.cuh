@@ -205,8 +205,75 @@ template <int L, bool INSTR> struct TrackView {
     }
   }
 
+  // registers -> the words the move half of a step assigns (sparse single buffer: in-place update,
+  // PAPER.md:115 "writes concentrated on ..."): pos, nial of the kind's processes, step -- and ekin
+  // for e+-, vol when the step crossed into another slab.  dir never changes in the move half, ids
+  // never.  A word assigned the value it already had (a zero-length step) is written again; the
+  // counting build uses store_changed below instead and counts only real changes.
+  template <bool GAMMA> __device__ __forceinline__ void store_moved(uint32_t slot, const Trk &t, bool vol_changed) const {
+    if constexpr (L == L_AOS || L == L_SOA16) {
+      // 16-byte pieces {pos, dir.x} {dir.yz, ekin, nial0} {nial12, vol, id_lo} {id_hi, step}: a photon
+      // rewrites all four, e+- three and the third only with vol
+      uint4 *q0, *q1, *q2;
+      uint2 *q3;
+      if constexpr (L == L_AOS) {
+        uint4 *r = reinterpret_cast<uint4 *>(base + size_t(slot) * Map::kStride);
+        q0 = r; q1 = r + 1; q2 = r + 2; q3 = reinterpret_cast<uint2 *>(r + 3);
+      } else {
+        q0 = reinterpret_cast<uint4 *>(base + Map::index(cap, slot, 0));
+        q1 = reinterpret_cast<uint4 *>(base + Map::index(cap, slot, 4));
+        q2 = reinterpret_cast<uint4 *>(base + Map::index(cap, slot, 8));
+        q3 = reinterpret_cast<uint2 *>(base + Map::index(cap, slot, 12));
+      }
+      *q0 = make_uint4(__float_as_uint(t.px), __float_as_uint(t.py), __float_as_uint(t.pz), __float_as_uint(t.dx));
+      *q1 = make_uint4(__float_as_uint(t.dy), __float_as_uint(t.dz), __float_as_uint(t.ekin), __float_as_uint(t.n0));
+      if (GAMMA || vol_changed) *q2 = make_uint4(__float_as_uint(t.n1), __float_as_uint(t.n2), t.vol, t.id_lo);
+      *q3 = make_uint2(t.id_hi, t.step);
+    } else {
+      base[Map::index(cap, slot, F_PX)] = __float_as_uint(t.px);
+      base[Map::index(cap, slot, F_PY)] = __float_as_uint(t.py);
+      base[Map::index(cap, slot, F_PZ)] = __float_as_uint(t.pz);
+      base[Map::index(cap, slot, F_N0)] = __float_as_uint(t.n0);
+      if constexpr (GAMMA) {
+        base[Map::index(cap, slot, F_N1)] = __float_as_uint(t.n1);
+        base[Map::index(cap, slot, F_N2)] = __float_as_uint(t.n2);
+      } else {
+        base[Map::index(cap, slot, F_EKIN)] = __float_as_uint(t.ekin);
+      }
+      if (vol_changed) base[Map::index(cap, slot, F_VOL)] = t.vol;
+      base[Map::index(cap, slot, F_STEP)] = t.step;
+    }
+  }
+
   // registers -> only the words that differ from `old` (sparse single buffer: in-place update)
   __device__ __forceinline__ void store_changed(uint32_t slot, const Trk &t, const Trk &old) const {
+    if constexpr ((L == L_AOS || L == L_SOA16) && !INSTR) {
+      // layouts that keep a record's words in 16-byte pieces: a piece with a changed word is rewritten
+      // whole (the thread owns the record; the unchanged words of the piece are written back as they
+      // are), so an update costs two to four vector stores instead of seven to fourteen scalar ones.
+      // The counting build below keeps the word-by-word form: it counts the words the step changes.
+      auto differ = [&](int f) { return trk_word(t, f) != trk_word(old, f); };  // bit patterns, as below
+      const bool c0 = differ(F_PX) || differ(F_PY) || differ(F_PZ) || differ(F_DX);
+      const bool c1 = differ(F_DY) || differ(F_DZ) || differ(F_EKIN) || differ(F_N0);
+      const bool c2 = differ(F_N1) || differ(F_N2) || differ(F_VOL) || differ(F_IDLO);
+      const bool c3 = differ(F_IDHI) || differ(F_STEP);
+      uint4 *q0, *q1, *q2;
+      uint2 *q3;
+      if constexpr (L == L_AOS) {
+        uint4 *r = reinterpret_cast<uint4 *>(base + size_t(slot) * Map::kStride);
+        q0 = r; q1 = r + 1; q2 = r + 2; q3 = reinterpret_cast<uint2 *>(r + 3);
+      } else {
+        q0 = reinterpret_cast<uint4 *>(base + Map::index(cap, slot, 0));
+        q1 = reinterpret_cast<uint4 *>(base + Map::index(cap, slot, 4));
+        q2 = reinterpret_cast<uint4 *>(base + Map::index(cap, slot, 8));
+        q3 = reinterpret_cast<uint2 *>(base + Map::index(cap, slot, 12));
+      }
+      if (c0) *q0 = make_uint4(__float_as_uint(t.px), __float_as_uint(t.py), __float_as_uint(t.pz), __float_as_uint(t.dx));
+      if (c1) *q1 = make_uint4(__float_as_uint(t.dy), __float_as_uint(t.dz), __float_as_uint(t.ekin), __float_as_uint(t.n0));
+      if (c2) *q2 = make_uint4(__float_as_uint(t.n1), __float_as_uint(t.n2), t.vol, t.id_lo);
+      if (c3) *q3 = make_uint2(t.id_hi, t.step);
+      return;
+    }
 #pragma unroll
     for (int f = 0; f < kNumFields; ++f) {
       const uint32_t w = trk_word(t, f);

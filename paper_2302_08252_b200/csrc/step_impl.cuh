@@ -285,7 +285,14 @@ struct GroupShared {
   uint32_t acc[2];       // arrival words, alternating between consecutive tiles / batches
   uint32_t qtot[2];      // parked tracks after the tile
   uint32_t base[2][4];   // first output entry per destination kind (dense: next array; sparse: next slot list)
-  uint32_t sbase[2][4];  // sparse: first new slot per destination kind
+  uint32_t sbase[2][4];  // sparse: first new (bump-allocated) slot per destination kind
+  // sparse scheme with slot recycling: tracks that end in each warp of the tile / batch, where the
+  // group's freed slots go in the ring, and per destination kind the ring position and number of
+  // recycled slots its children take before bump-allocated ones
+  uint32_t kcnt[2][kWarpsPerGroup];
+  uint32_t fbase[2];
+  uint32_t rbase[2][4], rn[2][4];
+  uint32_t sgot[2][4];   // sparse: children per destination kind that got a slot (the rest are dropped: overflow)
 };
 // Per-CTA shared state.
 struct CtaShared {
@@ -298,7 +305,7 @@ struct CtaShared {
 };
 
 // A9 + A11: the last CTA closes the iteration.
-template <int SCHEME> __device__ void finish_iteration(const Params &p) {
+template <int SCHEME, bool RECYCLE> __device__ void finish_iteration(const Params &p) {
   Ctl *c = p.ctl;
   uint32_t live_before = 0, live_after = 0;
   for (int k = 0; k < 3; ++k) {
@@ -327,8 +334,17 @@ template <int SCHEME> __device__ void finish_iteration(const Params &p) {
   }
   c->parity ^= 1u;
   if (live_before) c->iterations += 1ull;
-  if (SCHEME == S_SPARSE && live_after == 0u) {  // rule S30: slots are recycled only when the buffer is empty
-    for (int k = 0; k < 3; ++k) c->slot_top[k] = 0u;
+  if (SCHEME == S_SPARSE && RECYCLE) {
+    // slots freed in this iteration become allocatable in the next one; pops that ran past the
+    // allocatable part of the ring took bump-allocated slots instead (interact_batch)
+    for (int k = 0; k < 3; ++k) {
+      const uint32_t head = __ldcg(&c->free_head[k]), start = c->free_tail_start[k];
+      if (static_cast<int32_t>(head - start) > 0) c->free_head[k] = start;
+      c->free_tail_start[k] = __ldcg(&c->free_tail[k]);
+    }
+  }
+  if (SCHEME == S_SPARSE && live_after == 0u) {  // rule S30: without recycling, slots are reused only when the buffer is empty
+    for (int k = 0; k < 3; ++k) { c->slot_top[k] = 0u; c->free_head[k] = 0u; c->free_tail[k] = 0u; c->free_tail_start[k] = 0u; }
   }
   c->done_ctas = 0u;
 }
@@ -358,7 +374,7 @@ template <int KIND> __device__ __forceinline__ void bin_add_track_energy(const B
 // First half of the step for tile `tile` of kind KIND's current set (rows A1-A7, A10 for the
 // tracks whose step ends without an interaction).  `queued` = parked tracks of the group before
 // the tile; returns the number after it (the same value in every thread of the group).
-template <int L, int SCHEME, bool INSTR, int KIND>
+template <int L, int SCHEME, bool INSTR, bool RECYCLE, int KIND>
 __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, const GroupRefs &c, uint32_t par,
                                               uint32_t tile, uint32_t next_tile, uint32_t n_kind, int sbuf,
                                               uint32_t &in_phase, uint32_t queued) {
@@ -375,6 +391,7 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
   if (SCHEME == S_SPARSE && active) slot = p.kind[KIND].queue[par][i];
   const TrackView<L, INSTR> cur = make_view<L, INSTR>(p, KIND, (SCHEME == S_DENSE) ? int(par) : 0, c.cta->probe);
   Trk t, old;
+  uint32_t vol_before = 0u;
   MoveOut o;
   move_out_init(o);
   o.alive = false;
@@ -391,24 +408,24 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
         prefetch_tile<L>(p, KIND, par, next_tile, n_kind, c.in_buf, &g.mbar_in);
     }
   }
+  // sparse scheme: plain loads of the record the list entry names (no shared-memory staging: the
+  // sparse kernels leave the SM's memory to L1, which the scattered record pieces hit in)
+  if (SCHEME == S_SPARSE && active) t = cur.load(slot);
   if (active) {
-    if (SCHEME == S_DENSE) {
-      if (INSTR) {
+    if (INSTR && SCHEME == S_DENSE) {
 #pragma unroll
-        for (int f = 0; f < kNumFields; ++f) cur.probe(f, 0, slot);
-      }
-    } else {
-      t = cur.load(slot);
+      for (int f = 0; f < kNumFields; ++f) cur.probe(f, 0, slot);
     }
-    old = t;
+    if (INSTR && SCHEME == S_SPARSE) old = t;  // the counting build compares against the pre-step record
+    vol_before = t.vol;
     c.clk->mark(SEC_LOAD);
     if constexpr (KIND == K_GAMMA) move_gamma(t, env, o);
     else move_elec<KIND>(t, env, o);
     // A6: scoring into the CTA's bins (pre-step slab; the S31 guard uses the post-step slab).  A
     // photon deposits nothing in this half; the rare terms share one branch.
-    if (KIND != K_GAMMA && o.dep != 0.0f) bin_add(c.bins, old.vol, o.dep);
+    if (KIND != K_GAMMA && o.dep != 0.0f) bin_add(c.bins, vol_before, o.dep);
     if ((KIND != K_GAMMA && o.dep_b != 0.0f) || o.escaped || o.guard) {
-      if (KIND != K_GAMMA && o.dep_b != 0.0f) bin_add(c.bins, old.vol, o.dep_b);
+      if (KIND != K_GAMMA && o.dep_b != 0.0f) bin_add(c.bins, vol_before, o.dep_b);
       if (o.escaped) bin_add_track_energy<KIND>(c.bins, env.n_slabs, t.ekin);
       if (o.guard) bin_add_track_energy<KIND>(c.bins, t.vol, t.ekin);
     }
@@ -416,9 +433,27 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
   c.clk->mark(SEC_PHYSICS);
   const bool parked = active && o.pending != P_NONE;
   const bool survives = active && !parked && o.alive;
+  // A10 sparse: in-place update of the words that changed (parked tracks too: the interaction later
+  // writes only what it changes).  Done first: it needs no rank, and the pre-step copy of the record
+  // dies here instead of living through the ranking.
+  if (SCHEME == S_SPARSE) {
+    if (survives || parked) {
+      if constexpr (INSTR) cur.store_changed(slot, t, old);  // counts exactly the words that changed
+      else cur.template store_moved<KIND == K_GAMMA>(slot, t, t.vol != vol_before);
+    }
+    c.clk->mark(SEC_STORE);
+  }
   const uint32_t m_surv = __ballot_sync(0xFFFFFFFFu, survives);
   const uint32_t m_esc = __ballot_sync(0xFFFFFFFFu, o.escaped);
   const uint32_t m_park = __ballot_sync(0xFFFFFFFFu, parked);
+  // sparse scheme with slot recycling: a track that ends here frees its slot
+  constexpr bool recycle = SCHEME == S_SPARSE && RECYCLE;
+  const bool ends = recycle && active && !parked && !survives;
+  uint32_t m_end = 0u;
+  if (SCHEME == S_SPARSE && recycle) {
+    m_end = __ballot_sync(0xFFFFFFFFu, ends);
+    if (lane == 0) g.kcnt[sbuf][gtid >> 5] = uint32_t(__popc(m_end));
+  }
 
   // A9: rank survivors and parked tracks of the warp inside the group (the third count, escapes, is
   // only totalled); last warp reserves the range and books the tile's counts
@@ -434,6 +469,12 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
       g.base[sbuf][0] = n_out ? atomicAdd(&ctl->n_next[KIND], n_out) : 0u;
       if (n_out) atomicAdd(&c.cta->alive[KIND], n_out);
       if (n_esc) atomicAdd(&c.cta->escaped[KIND], n_esc);
+      if (SCHEME == S_SPARSE && recycle) {
+        const uint32_t first = tile * kGroup;
+        const uint32_t n_tile = (n_kind - first < uint32_t(kGroup)) ? n_kind - first : uint32_t(kGroup);
+        const uint32_t n_end = n_tile - n_out - count_of(total, 1);
+        if (n_end) g.fbase[sbuf] = atomicAdd(&ctl->free_tail[KIND], n_end);
+      }
     }
   }
   word = __shfl_sync(0xFFFFFFFFu, word, 0);
@@ -444,10 +485,6 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
     const uint32_t q = queued + count_of(word, 1) + __popc(m_park & lt_mask);
     park_store<SCHEME>(c.queue, q, t, o.pending, slot);
   }
-  // A10 sparse: in-place update of the words that changed (parked tracks too: the interaction
-  // later writes only what it changes)
-  if (SCHEME == S_SPARSE && (survives || parked)) cur.store_changed(slot, t, old);
-
   c.clk->mark(SEC_STORE);
   group_sync(c.group);
   c.clk->mark(SEC_ALLOC);
@@ -460,13 +497,18 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
       ctl->overflow = 1u;
     }
   }
+  if (SCHEME == S_SPARSE && ends) {  // freed slot -> the kind's ring, in warp order inside the tile
+    uint32_t r = uint32_t(__popc(m_end & lt_mask));
+    for (int w = 0; w < (gtid >> 5); ++w) r += g.kcnt[sbuf][w];
+    p.kind[KIND].free_ring[(g.fbase[sbuf] + r) % p.capacity] = slot;
+  }
   c.clk->mark(SEC_STORE);
   return g.qtot[sbuf];
 }
 
 // Second half of the step on a dense batch of up to kGroup parked tracks taken from the top of the
 // group's queue (rows A8, A9, A10).  Returns the number of tracks left in the queue.
-template <int L, int SCHEME, bool INSTR, int KIND>
+template <int L, int SCHEME, bool INSTR, bool RECYCLE, int KIND>
 __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &env, const GroupRefs &c, uint32_t par,
                                                    uint32_t queued, int sbuf) {
   const int gtid = c.gtid, lane = gtid & 31;
@@ -497,6 +539,13 @@ __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &e
   c.clk->mark(SEC_INTERACT);
   constexpr int Q0 = kid_kind<KIND>(0), Q1 = kid_kind<KIND>(1);  // never KIND itself
   const uint32_t m_alive = __ballot_sync(0xFFFFFFFFu, o.alive);
+  constexpr bool recycle = SCHEME == S_SPARSE && RECYCLE;
+  const bool ends = recycle && have && !o.alive;  // the parent's slot is free from the next iteration on
+  uint32_t m_end = 0u;
+  if (SCHEME == S_SPARSE && recycle) {
+    m_end = __ballot_sync(0xFFFFFFFFu, ends);
+    if (lane == 0) g.kcnt[sbuf][gtid >> 5] = uint32_t(__popc(m_end));
+  }
   const uint32_t m_k0 = __ballot_sync(0xFFFFFFFFu, o.kid[0].kind >= 0);
   const uint32_t m_k1 = __ballot_sync(0xFFFFFFFFu, o.kid[1].kind >= 0);
 
@@ -513,9 +562,33 @@ __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &e
 #pragma unroll
       for (int q = 0; q < 3; ++q) {
         const uint32_t want = count_of(total, q);
-        g.base[sbuf][q] = want ? atomicAdd(&ctl->n_next[q], want) : 0u;
-        // sparse: children get bump-allocated, never recycled slots (rule S30)
-        if (SCHEME == S_SPARSE && q != KIND) g.sbase[sbuf][q] = want ? atomicAdd(&ctl->slot_top[q], want) : 0u;
+        uint32_t got = want;
+        if (SCHEME == S_SPARSE && q != KIND) {
+          // sparse: children get bump-allocated, never recycled slots (rule S30) -- or, with slot
+          // recycling, first the slots freed up to the previous iteration (the kind's ring below
+          // free_tail_start), then bump-allocated ones
+          uint32_t n_ring = 0u, h = 0u;
+          if (recycle && want) {
+            h = atomicAdd(&ctl->free_head[q], want);
+            const int32_t avail = static_cast<int32_t>(ctl->free_tail_start[q] - h);
+            n_ring = avail <= 0 ? 0u : (uint32_t(avail) < want ? uint32_t(avail) : want);
+          }
+          g.rbase[sbuf][q] = h;
+          g.rn[sbuf][q] = n_ring;
+          const uint32_t rest = want - n_ring;
+          const uint32_t sb = rest ? atomicAdd(&ctl->slot_top[q], rest) : 0u;
+          g.sbase[sbuf][q] = sb;
+          // slots past the end of the buffer do not exist: those children are dropped (overflow), and
+          // only children that have a slot get a list entry, so every list entry names a real slot
+          const uint32_t usable = (sb >= p.capacity) ? 0u : ((p.capacity - sb < rest) ? p.capacity - sb : rest);
+          got = n_ring + usable;
+          g.sgot[sbuf][q] = got;
+        }
+        g.base[sbuf][q] = got ? atomicAdd(&ctl->n_next[q], got) : 0u;
+      }
+      if (SCHEME == S_SPARSE && recycle) {
+        const uint32_t n_end = batch - count_of(total, KIND);
+        if (n_end) g.fbase[sbuf] = atomicAdd(&ctl->free_tail[KIND], n_end);
       }
     }
   }
@@ -555,16 +628,29 @@ __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &e
       if (qpos < p.capacity) p.kind[KIND].queue[nbuf][qpos] = slot;
       else dropped = true;
     }
+    // slot of the child with rank r among the group's children of kind q
+    auto child_slot = [&](int q, uint32_t r) -> uint32_t {
+      const uint32_t nr = g.rn[sbuf][q];
+      if (r < nr) return p.kind[q].free_ring[(g.rbase[sbuf][q] + r) % p.capacity];
+      return g.sbase[sbuf][q] + (r - nr);
+    };
+    if (ends) {
+      uint32_t r = uint32_t(__popc(m_end & lt_mask));
+      for (int w = 0; w < (gtid >> 5); ++w) r += g.kcnt[sbuf][w];
+      p.kind[KIND].free_ring[(g.fbase[sbuf] + r) % p.capacity] = slot;
+    }
     if (o.kid[0].kind >= 0) {
-      const uint32_t s_new = g.sbase[sbuf][Q0] + r_k0, qpos = g.base[sbuf][Q0] + r_k0;
-      if (s_new < p.capacity && qpos < p.capacity) {
+      const uint32_t qpos = g.base[sbuf][Q0] + r_k0;
+      if (r_k0 < g.sgot[sbuf][Q0] && qpos < p.capacity) {
+        const uint32_t s_new = child_slot(Q0, r_k0);
         make_view<L, INSTR>(p, Q0, 0, c.cta->probe).store(s_new, kid_track(t, o.kid[0]));
         p.kind[Q0].queue[nbuf][qpos] = s_new;
       } else dropped = true;
     }
     if (o.kid[1].kind >= 0) {
-      const uint32_t s_new = g.sbase[sbuf][Q1] + r_k1, qpos = g.base[sbuf][Q1] + r_k1;
-      if (s_new < p.capacity && qpos < p.capacity) {
+      const uint32_t qpos = g.base[sbuf][Q1] + r_k1;
+      if (r_k1 < g.sgot[sbuf][Q1] && qpos < p.capacity) {
+        const uint32_t s_new = child_slot(Q1, r_k1);
         make_view<L, INSTR>(p, Q1, 0, c.cta->probe).store(s_new, kid_track(t, o.kid[1]));
         p.kind[Q1].queue[nbuf][qpos] = s_new;
       } else dropped = true;
@@ -577,7 +663,7 @@ __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &e
 
 // All tiles of one kind that belong to this group, then the left-over parked tracks.
 // `first_global_tile` = tiles of the kinds before this one; n_tiles, n_kind are launch-uniform.
-template <int L, int SCHEME, bool INSTR, int KIND>
+template <int L, int SCHEME, bool INSTR, bool RECYCLE, int KIND>
 __device__ __forceinline__ void run_kind(const Params &p, const Env &env, const GroupRefs &c, uint32_t par,
                                          uint32_t first_global_tile, uint32_t n_tiles, uint32_t n_kind, int &sbuf,
                                          uint32_t &in_phase, uint32_t &tab_phase, int &staged_group) {
@@ -611,15 +697,15 @@ __device__ __forceinline__ void run_kind(const Params &p, const Env &env, const 
   uint32_t queued = 0u;
   for (uint32_t tile = shift; tile < n_tiles; tile += n_groups) {
     const uint32_t next_tile = (tile + n_groups < n_tiles) ? tile + n_groups : 0xFFFFFFFFu;
-    queued = move_tile<L, SCHEME, INSTR, KIND>(p, env, c, par, tile, next_tile, n_kind, sbuf, in_phase, queued);
+    queued = move_tile<L, SCHEME, INSTR, RECYCLE, KIND>(p, env, c, par, tile, next_tile, n_kind, sbuf, in_phase, queued);
     sbuf ^= 1;
     if (queued >= uint32_t(kGroup)) {
-      queued = interact_batch<L, SCHEME, INSTR, KIND>(p, env, c, par, queued, sbuf);
+      queued = interact_batch<L, SCHEME, INSTR, RECYCLE, KIND>(p, env, c, par, queued, sbuf);
       sbuf ^= 1;
     }
   }
   while (queued != 0u) {
-    queued = interact_batch<L, SCHEME, INSTR, KIND>(p, env, c, par, queued, sbuf);
+    queued = interact_batch<L, SCHEME, INSTR, RECYCLE, KIND>(p, env, c, par, queued, sbuf);
     sbuf ^= 1;
   }
 }
@@ -630,7 +716,7 @@ __device__ __forceinline__ void run_kind(const Params &p, const Env &env, const 
 #ifndef ADEPT_STEP_MIN_CTAS
 #define ADEPT_STEP_MIN_CTAS 4
 #endif
-template <int L, int SCHEME, bool INSTR, int THREADS>
+template <int L, int SCHEME, bool INSTR, int THREADS, bool RECYCLE = false>
 __global__ void __launch_bounds__(THREADS, (THREADS == kBlockSmall) ? ADEPT_STEP_MIN_CTAS : 1) step_kernel(const __grid_constant__ Params p) {
   constexpr int kBlock = THREADS;
   constexpr int kGroupsPerCta = THREADS / kGroup;
@@ -686,9 +772,9 @@ __global__ void __launch_bounds__(THREADS, (THREADS == kBlockSmall) ? ADEPT_STEP
     int sbuf = 0;
     uint32_t in_phase = 0u, tab_phase = 0u;
     int staged_group = -1;
-    run_kind<L, SCHEME, INSTR, K_EM>(p, env, c, par, 0u, t0, n0, sbuf, in_phase, tab_phase, staged_group);
-    run_kind<L, SCHEME, INSTR, K_EP>(p, env, c, par, t0, t1, n1, sbuf, in_phase, tab_phase, staged_group);
-    run_kind<L, SCHEME, INSTR, K_GAMMA>(p, env, c, par, t0 + t1, t2, n2, sbuf, in_phase, tab_phase, staged_group);
+    run_kind<L, SCHEME, INSTR, RECYCLE, K_EM>(p, env, c, par, 0u, t0, n0, sbuf, in_phase, tab_phase, staged_group);
+    run_kind<L, SCHEME, INSTR, RECYCLE, K_EP>(p, env, c, par, t0, t1, n1, sbuf, in_phase, tab_phase, staged_group);
+    run_kind<L, SCHEME, INSTR, RECYCLE, K_GAMMA>(p, env, c, par, t0 + t1, t2, n2, sbuf, in_phase, tab_phase, staged_group);
 
     // flush the CTA's tallies
     clk.mark(SEC_OTHER);
@@ -717,7 +803,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == kBlockSmall) ? ADEPT_STEP
     const uint32_t ticket = atomicAdd(&ctl->done_ctas, 1u);
     if (ticket == gridDim.x - 1) {
       __threadfence();
-      finish_iteration<SCHEME>(p);
+      finish_iteration<SCHEME, RECYCLE>(p);
     }
   }
 }
@@ -830,9 +916,9 @@ __global__ void read_kernel(const __grid_constant__ Params p, PackedTrack *dst, 
 // scheme and instrumentation are compile-time parameters of every kernel.)
 struct LayoutOps {
   size_t (*record_words)(size_t capacity);
-  int (*step_ctas_per_sm)(int scheme, int instr, int threads, size_t dyn_smem);
+  int (*step_ctas_per_sm)(int scheme, int instr, int recycle, int threads, size_t dyn_smem);
   cudaError_t (*launch_step)(int scheme, int instr, const Params &, int threads, unsigned grid, size_t dyn_smem,
-                             cudaStream_t);
+                             cudaStream_t);  // Params::recycle picks the slot-recycling instantiation (sparse scheme)
   cudaError_t (*launch_inject)(int scheme, const Params &, const void *staged, uint32_t n, int kind, uint32_t par,
                                uint32_t entry_base, uint32_t slot_base, unsigned long long seed, cudaStream_t);
   cudaError_t (*launch_load)(int scheme, const Params &, const void *staged, const uint32_t *slots, uint32_t n,
@@ -859,16 +945,17 @@ inline cudaError_t ensure_dynamic_smem(const void *kernel, size_t bytes) {
 }
 
 template <int L> struct OpsImpl {
-  template <int T, typename F> static auto pick_t(int scheme, int instr, F f) {
+  template <int T, typename F> static auto pick_t(int scheme, int instr, int recycle, F f) {
     if (scheme == S_DENSE) return instr ? f(step_kernel<L, S_DENSE, true, T>) : f(step_kernel<L, S_DENSE, false, T>);
+    if (recycle) return instr ? f(step_kernel<L, S_SPARSE, true, T, true>) : f(step_kernel<L, S_SPARSE, false, T, true>);
     return instr ? f(step_kernel<L, S_SPARSE, true, T>) : f(step_kernel<L, S_SPARSE, false, T>);
   }
-  template <typename F> static auto pick(int scheme, int instr, int threads, F f) {
-    return threads == kBlockLarge ? pick_t<kBlockLarge>(scheme, instr, f) : pick_t<kBlockSmall>(scheme, instr, f);
+  template <typename F> static auto pick(int scheme, int instr, int recycle, int threads, F f) {
+    return threads == kBlockLarge ? pick_t<kBlockLarge>(scheme, instr, recycle, f) : pick_t<kBlockSmall>(scheme, instr, recycle, f);
   }
   static size_t record_words(size_t cap) { return Mapping<L>::words(cap); }
-  static int step_ctas_per_sm(int scheme, int instr, int threads, size_t dyn) {
-    return pick(scheme, instr, threads, [&](auto *k) {
+  static int step_ctas_per_sm(int scheme, int instr, int recycle, int threads, size_t dyn) {
+    return pick(scheme, instr, recycle, threads, [&](auto *k) {
       int n = 0;
       if (ensure_dynamic_smem(reinterpret_cast<const void *>(k), dyn) != cudaSuccess) return -1;
       if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k, threads, dyn) != cudaSuccess) return -1;
@@ -877,7 +964,7 @@ template <int L> struct OpsImpl {
   }
   static cudaError_t launch_step(int scheme, int instr, const Params &p, int threads, unsigned grid, size_t dyn,
                                  cudaStream_t s) {
-    return pick(scheme, instr, threads, [&](auto *k) {
+    return pick(scheme, instr, int(p.recycle), threads, [&](auto *k) {
       const cudaError_t e = ensure_dynamic_smem(reinterpret_cast<const void *>(k), dyn);
       if (e != cudaSuccess) return e;
       k<<<grid, threads, dyn, s>>>(p);

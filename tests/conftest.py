@@ -11,6 +11,7 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (B200); run with -m gpu")
+    config.addinivalue_line("markers", "slow: takes minutes (the oracle on a full-size shower workload)")
 
 
 def pytest_collection_modifyitems(config, items):

@@ -690,3 +690,113 @@ def test_run_counts_real_iterations_against_the_limit():
     assert g["iterations"] == r["iterations"]
     assert np.allclose(g["edep_layer"], r["edep_layer"], rtol=1e-4, atol=1e-12)
     ctx.destroy()
+
+
+# ----------------------------------------------------------- slot recycling --
+@pytest.mark.parametrize("layout", ("aos", "soa", "aosoa32", "soa16"))
+def test_sparse_slot_recycling_keeps_results_and_bounds_the_footprint(layout):
+    """ADEPT_FLAG_RECYCLE_SLOTS (include/adept.h): the slot of every track that ends goes onto a ring
+    and secondaries take recycled slots first.  Slots carry no physics, so every count, every tally and
+    every surviving track must equal the oracle's -- iteration by iteration on the tiny shower, and
+    over 100 x 1 GeV showers in a buffer far smaller than the never-recycle policy needs (PAPER.md:137:
+    2044 against 45509 slots)."""
+    RECYCLE = 1
+    c = CONFIGS["tiny"]
+    geo, tab = geometry_for("tiny"), tables_for("tiny")
+    prim = gen_primaries(c["n_primaries"], c["e_primary"])
+    o = Oracle(geo, tab, seed=c["seed"])
+    o.inject(prim)
+    ctx = _ctx(geo, tab, layout=layout, scheme="sparse", capacity=c["capacity"], seed=c["seed"], flags=RECYCLE)
+    ctx.inject(prim)
+    it = 0
+    while sum(o.live(k) for k in range(3)):
+        o.step()
+        compare_counts(ctx.step(), o.result(), what="iteration %d" % it)
+        for k in range(3):
+            compare_tracks(ctx.read_tracks(k), o.read_tracks(k, make_tracks(1).dtype), "iteration %d kind %d" % (it, k))
+        it += 1
+    r, g = o.result(), ctx.result()
+    assert np.allclose(g["edep_layer"], r["edep_layer"], rtol=1e-4, atol=1e-12)
+    never = np.array([c["n_primaries"], 0, 0], dtype=np.uint64) + r["secondaries"]
+    assert (g["slots_used"] <= never).all() and g["slots_used"].sum() < never.sum()
+    ctx.destroy()
+
+    c = CONFIGS["full"]
+    geo, tab = geometry_for("full"), tables_for("full")
+    prim = gen_primaries(100, c["e_primary"])
+    o = Oracle(geo, tab, seed=c["seed"])
+    o.inject(prim)
+    o.run()
+    r = o.result()
+    cap = 1 << 14                                   # peak live per kind is ~6e3; e- created in total ~5.8e4
+    assert r["secondaries"][0] > 3 * cap
+    ctx = _ctx(geo, tab, layout=layout, scheme="sparse", capacity=cap, seed=c["seed"], flags=RECYCLE)
+    ctx.inject(prim)
+    g = ctx.run()
+    compare_counts(g, r)
+    assert g["iterations"] == r["iterations"] and g["overflow"] == 0
+    assert np.allclose(g["edep_layer"], r["edep_layer"], rtol=1e-4, atol=1e-9)
+    assert (g["slots_used"] <= cap).all()
+    ctx.destroy()
+    # the paper's policy in the same buffer: it overflows, and says so
+    from paper_2302_08252_b200 import AdeptError
+    ctx = _ctx(geo, tab, layout=layout, scheme="sparse", capacity=cap, seed=c["seed"])
+    ctx.inject(prim)
+    with pytest.raises(AdeptError) as e:
+        ctx.run()
+    assert e.value.code == -2
+    ctx.destroy()
+
+
+def test_recycling_flag_is_validated_and_ignored_by_the_dense_scheme():
+    from paper_2302_08252_b200 import AdeptError
+    geo, tab = geometry_for("tiny"), tables_for("tiny")
+    with pytest.raises(AdeptError):
+        _ctx(geo, tab, layout="soa", scheme="sparse", capacity=4096, flags=2)
+    prim = gen_primaries(16, 10.0)
+    a = _ctx(geo, tab, layout="soa", scheme="dense", capacity=4096, seed=1, flags=1)
+    b = _ctx(geo, tab, layout="soa", scheme="dense", capacity=4096, seed=1)
+    a.inject(prim); b.inject(prim)
+    ra, rb = a.run(), b.run()
+    compare_counts(ra, rb)
+    assert (ra["edep_slab"] == rb["edep_slab"]).all() and (ra["slots_used"] == rb["slots_used"]).all()
+    a.destroy(); b.destroy()
+
+
+# ------------------------------------------------------------------ config 5 at full size ----------
+@pytest.mark.slow
+@pytest.mark.parametrize("layout,scheme,flags", [("aosoa32", "dense", 0), ("aos", "sparse", 1)])
+def test_heavy_showers_at_full_size_match_the_oracle(layout, scheme, flags):
+    """BASELINE.json configs[4]: 10 000 x 10 GeV e-, 8 Mi slots per kind, run to completion -- every
+    count bit-exact, per-layer deposits within 1e-4 (the oracle needs ~80 s on one host core).  The
+    sparse single buffer holds the run in the same 8 Mi slots only with slot recycling (the e- created
+    in total are ~5.7e7, SURVEY.md:583)."""
+    c = CONFIGS["heavy"]
+    geo, tab = geometry_for("heavy"), tables_for("heavy")
+    prim = gen_primaries(c["n_primaries"], c["e_primary"])
+    r = _heavy_reference()
+    ctx = _ctx(geo, tab, layout=layout, scheme=scheme, capacity=c["capacity"], seed=c["seed"], flags=flags)
+    ctx.inject(prim)
+    g = ctx.run()
+    compare_counts(g, r)
+    assert g["iterations"] == r["iterations"] and g["overflow"] == 0
+    assert np.allclose(g["edep_layer"], r["edep_layer"], rtol=1e-4, atol=1e-9)
+    assert abs(g["e_escaped"] - r["e_escaped"]) <= 1e-9 * r["e_injected"]
+    assert abs(g["edep_slab"].sum() + g["e_escaped"] - g["e_injected"]) < 1e-6 * g["e_injected"]
+    if scheme == "sparse":
+        assert (g["slots_used"] <= c["capacity"]).all() and r["secondaries"][0] > 4 * c["capacity"]
+    ctx.destroy()
+
+
+_HEAVY = {}
+
+
+def _heavy_reference():
+    if not _HEAVY:
+        c = CONFIGS["heavy"]
+        o = Oracle(geometry_for("heavy"), tables_for("heavy"), seed=c["seed"])
+        o.inject(gen_primaries(c["n_primaries"], c["e_primary"]))
+        o.run()
+        _HEAVY.update(o.result())
+        o.close()
+    return _HEAVY
