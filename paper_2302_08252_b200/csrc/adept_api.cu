@@ -75,7 +75,7 @@ static bool make_plan(const adept_geometry *g, const adept_tables *t, const adep
   pl.stage_records = std::min<uint32_t>(pl.capacity, kStageRecords);
   size_t off = 0;
   // control header, tallies (per slab + escaped), section clocks of the timing build
-  pl.ctl = off; off = align_up(off + kCtlHeaderBytes + (size_t(2) * g->n_layers + 1 + kNumSections) * sizeof(unsigned long long));
+  pl.ctl = off; off = align_up(off + kCtlHeaderBytes + (size_t(2) * g->n_layers + 1 + kNumSections + 1) * sizeof(unsigned long long));
   pl.tables = off; off = align_up(off + pl.table_bytes);
   pl.stage = off; off = align_up(off + size_t(pl.stage_records) * kStageRecordBytes);
   pl.stage_slots = off; off = align_up(off + size_t(pl.stage_records) * 4);
@@ -254,6 +254,12 @@ static int clear_state(adept_ctx *c) {
   CU(c, cudaMemsetAsync(c->ws + pl.ctl, 0, pl.tables - pl.ctl, c->stream));
   if (c->cfg.instrument && pl.total > pl.instr_rw)
     CU(c, cudaMemsetAsync(c->ws + pl.instr_rw, 0, pl.total - pl.instr_rw, c->stream));
+#ifdef ADEPT_TIMING_SECTIONS
+  {  // scratch word of the launch timeline: earliest CTA start of the running launch (atomicMin)
+    static const unsigned long long kNever = ~0ull;
+    CU(c, cudaMemcpyAsync(c->params.sections + kNumSections, &kNever, sizeof kNever, cudaMemcpyHostToDevice, c->stream));
+  }
+#endif
   c->pending.clear();
   c->pending_done = 0;
   c->next_primary = 0;
@@ -294,7 +300,7 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
     return ADEPT_ECUDA;
   };
   cudaError_t e;
-  c->pinned_bytes = kCtlHeaderBytes + (size_t(2) * g->n_layers + 1 + kNumSections) * sizeof(unsigned long long);
+  c->pinned_bytes = kCtlHeaderBytes + (size_t(2) * g->n_layers + 1 + kNumSections + 1) * sizeof(unsigned long long);
   if ((e = cudaMallocHost(reinterpret_cast<void **>(&c->pinned), c->pinned_bytes)) != cudaSuccess)
     return die("cudaMallocHost", e);
   if ((e = cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking)) != cudaSuccess)

@@ -27,6 +27,7 @@
 //   A12     the instrumented instantiation counts every accessor call.
 #pragma once
 #include <cstdint>
+#include <cstdlib>
 #include <map>
 #include <mutex>
 #include <utility>
@@ -305,48 +306,58 @@ struct CtaShared {
 };
 
 // A9 + A11: the last CTA closes the iteration.
-template <int SCHEME, bool RECYCLE> __device__ void finish_iteration(const Params &p) {
+// Run by the first warp of the last CTA: lane k < 3 closes kind k, so that the dependent global
+// accesses of the three kinds overlap (an iteration of a small population is a chain of memory round
+// trips; this is its last link).
+template <int SCHEME, bool RECYCLE> __device__ void finish_iteration(const Params &p, int lane) {
   Ctl *c = p.ctl;
-  uint32_t live_before = 0, live_after = 0;
-  for (int k = 0; k < 3; ++k) {
-    const uint32_t n = c->n_cur[k];
-    uint32_t nn = __ldcg(&c->n_next[k]);
+  uint32_t n = 0u, nn = 0u;
+  if (lane < 3) {
+    const int k = lane;
+    n = c->n_cur[k];
+    nn = __ldcg(&c->n_next[k]);
     const uint32_t alive = __ldcg(&c->it_alive[k]);
     const uint32_t esc = __ldcg(&c->it_escaped[k]);
-    live_before += n;
-    c->steps[k] += n;
-    c->killed[k] += n - alive;
-    c->escaped_n[k] += esc;
-    c->secondaries[k] += nn - alive;
+    uint32_t top = 0u, head = 0u, start = 0u, tail = 0u;
+    if (SCHEME == S_SPARSE) top = __ldcg(&c->slot_top[k]);
+    if (SCHEME == S_SPARSE && RECYCLE) {
+      head = __ldcg(&c->free_head[k]); start = c->free_tail_start[k]; tail = __ldcg(&c->free_tail[k]);
+    }
+    const unsigned long long steps = c->steps[k], killed = c->killed[k], escaped = c->escaped_n[k],
+                             secondaries = c->secondaries[k], used = c->slots_used[k];
+    c->steps[k] = steps + n;
+    c->killed[k] = killed + (n - alive);
+    c->escaped_n[k] = escaped + esc;
+    c->secondaries[k] = secondaries + (nn - alive);
     if (nn > p.capacity) { nn = p.capacity; c->overflow = 1u; }
     if (SCHEME == S_SPARSE) {
-      uint32_t top = __ldcg(&c->slot_top[k]);
       if (top > p.capacity) { top = p.capacity; c->slot_top[k] = top; c->overflow = 1u; }
-      if (top > c->slots_used[k]) c->slots_used[k] = top;
+      if (top > used) c->slots_used[k] = top;
     } else {
-      if (nn > c->slots_used[k]) c->slots_used[k] = nn;
+      if (nn > used) c->slots_used[k] = nn;
     }
     c->n_cur[k] = nn;
     c->n_next[k] = 0u;
     c->it_alive[k] = 0u;
     c->it_escaped[k] = 0u;
-    live_after += nn;
-  }
-  c->parity ^= 1u;
-  if (live_before) c->iterations += 1ull;
-  if (SCHEME == S_SPARSE && RECYCLE) {
-    // slots freed in this iteration become allocatable in the next one; pops that ran past the
-    // allocatable part of the ring took bump-allocated slots instead (interact_batch)
-    for (int k = 0; k < 3; ++k) {
-      const uint32_t head = __ldcg(&c->free_head[k]), start = c->free_tail_start[k];
+    if (SCHEME == S_SPARSE && RECYCLE) {
+      // slots freed in this iteration become allocatable in the next one; pops that ran past the
+      // allocatable part of the ring took bump-allocated slots instead (interact_batch)
       if (static_cast<int32_t>(head - start) > 0) c->free_head[k] = start;
-      c->free_tail_start[k] = __ldcg(&c->free_tail[k]);
+      c->free_tail_start[k] = tail;
     }
   }
-  if (SCHEME == S_SPARSE && live_after == 0u) {  // rule S30: without recycling, slots are reused only when the buffer is empty
-    for (int k = 0; k < 3; ++k) { c->slot_top[k] = 0u; c->free_head[k] = 0u; c->free_tail[k] = 0u; c->free_tail_start[k] = 0u; }
+  const uint32_t live_before = __reduce_add_sync(0xFFFFFFFFu, n), live_after = __reduce_add_sync(0xFFFFFFFFu, nn);
+  if (SCHEME == S_SPARSE && live_after == 0u && lane < 3) {
+    // rule S30: slots are reused (without recycling: only) once the buffer is empty
+    const int k = lane;
+    c->slot_top[k] = 0u; c->free_head[k] = 0u; c->free_tail[k] = 0u; c->free_tail_start[k] = 0u;
   }
-  c->done_ctas = 0u;
+  if (lane == 0) {
+    c->parity ^= 1u;
+    if (live_before) c->iterations += 1ull;
+    c->done_ctas = 0u;
+  }
 }
 
 // ------------------------------------------------------------------- tile = kGroup tracks -----
@@ -672,6 +683,12 @@ __device__ __forceinline__ void run_kind(const Params &p, const Env &env, const 
   const uint32_t n_groups = gridDim.x * groups_per_cta;
   const uint32_t me = blockIdx.x * groups_per_cta + c.group;
   const uint32_t shift = (me + n_groups - first_global_tile % n_groups) % n_groups;
+  // a CTA none of whose groups has a tile of this kind skips it altogether -- in particular the
+  // CTA-wide staging of the kind's tables (small populations: most CTAs hold one tile of one kind)
+  bool cta_has = false;
+  for (uint32_t gI = 0; gI < groups_per_cta; ++gI)
+    cta_has |= (blockIdx.x * groups_per_cta + gI + n_groups - first_global_tile % n_groups) % n_groups < n_tiles;
+  if (!cta_has) return;
   // the group's first tile of this kind is requested before the tables are: the two copies overlap
   // (small populations -- the head and tail of a shower -- are latency-bound, one tile per group)
   if (SCHEME == S_DENSE && shift < n_tiles && c.gtid == 0)  // the staging buffer is free: its last reader passed a barrier
@@ -679,7 +696,7 @@ __device__ __forceinline__ void run_kind(const Params &p, const Env &env, const 
   // A3: the cross-section tables of this kind's particle group -> shared memory, one TMA bulk copy
   // (e- and e+ share a group).  CTA-wide: every group is done with the previous tables.
   constexpr int group = (KIND == K_GAMMA) ? 0 : 1;
-  if (n_tiles != 0u && staged_group != group) {
+  if (staged_group != group) {
     __syncthreads();
     if (threadIdx.x == 0) {
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -740,27 +757,37 @@ __global__ void __launch_bounds__(THREADS, (THREADS == kBlockSmall) ? ADEPT_STEP
   SectClock clk;
   c.clk = &clk;
 
+  // Everything that does not depend on the previous launch comes first: with programmatic dependent
+  // launch (launch_step) this prologue overlaps the tail of the previous iteration's kernel.
+  if (tid == 0) {  // barriers of the asynchronous copies (tables of a particle group, staged tiles)
+    mbar_init(&sh.mbar, 1u);
+#pragma unroll
+    for (int gI = 0; gI < kGroupsPerCta; ++gI) mbar_init(&sh.grp[gI].mbar_in, 1u);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  for (uint32_t s = tid; s < 2u * (p.n_slabs + 1u); s += kBlock) c.bins.lo[s] = 0u;  // tally bins, counters
+  if (tid < 4) { sh.alive[tid] = 0u; sh.escaped[tid] = 0u; }
+  if (tid < kGroupsPerCta) { sh.grp[tid].loaded = 0u; sh.grp[tid].acc[0] = 0u; sh.grp[tid].acc[1] = 0u; }
+  if (INSTR) for (int s = tid; s < 3 * kNumFields * 2; s += kBlock) sh.probe[s] = 0u;
+  if (tid < kNumSections) sh.sect[tid] = 0u;
+  asm volatile("griddepcontrol.wait;" ::: "memory");  // the previous launch has completed and its writes are visible
+#ifdef ADEPT_TIMING_SECTIONS
+  // launch timeline (timing build): sections[6] += first CTA start -> last CTA done (ns),
+  // sections[7] += the last CTA's end-of-iteration work (ns); sections[kNumSections] = scratch
+  unsigned long long t_cta_start = 0ull;
+  if (tid == 0) {
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_cta_start));
+    atomicMin(&p.sections[kNumSections], t_cta_start);
+  }
+#endif
   // A0: what is alive (written by the previous iteration's last CTA; constant during this launch)
   const uint32_t par = ctl->parity;
   const uint32_t n0 = ctl->n_cur[0], n1 = ctl->n_cur[1], n2 = ctl->n_cur[2];
   const uint32_t t0 = (n0 + kGroup - 1) / kGroup, t1 = (n1 + kGroup - 1) / kGroup, t2 = (n2 + kGroup - 1) / kGroup;
   const uint32_t tiles = t0 + t1 + t2;
+  __syncthreads();
 
   if (blockIdx.x * kGroupsPerCta < tiles) {  // CTA-uniform: at least one group of this CTA has a tile
-    // barriers of the asynchronous copies (tables of a particle group, staged tiles); bins and
-    // counters cleared
-    if (tid == 0) {
-      mbar_init(&sh.mbar, 1u);
-#pragma unroll
-      for (int gI = 0; gI < kGroupsPerCta; ++gI) mbar_init(&sh.grp[gI].mbar_in, 1u);
-      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    for (uint32_t s = tid; s < 2u * (p.n_slabs + 1u); s += kBlock) c.bins.lo[s] = 0u;
-    if (tid < 4) { sh.alive[tid] = 0u; sh.escaped[tid] = 0u; }
-    if (tid < kGroupsPerCta) { sh.grp[tid].loaded = 0u; sh.grp[tid].acc[0] = 0u; sh.grp[tid].acc[1] = 0u; }
-    if (INSTR) for (int s = tid; s < 3 * kNumFields * 2; s += kBlock) sh.probe[s] = 0u;
-    if (tid < kNumSections) sh.sect[tid] = 0u;
-    __syncthreads();
     clk.start(sh.sect, (tid & 31) == 0);
 
     Env env;
@@ -798,12 +825,29 @@ __global__ void __launch_bounds__(THREADS, (THREADS == kBlockSmall) ? ADEPT_STEP
 
   // A11: the last CTA to arrive ends the iteration
   __syncthreads();
-  if (tid == 0) {
-    __threadfence();
-    const uint32_t ticket = atomicAdd(&ctl->done_ctas, 1u);
+  if (tid < 32) {
+    uint32_t ticket = 0u;
+    if (tid == 0) {
+      __threadfence();
+      ticket = atomicAdd(&ctl->done_ctas, 1u);
+    }
+    ticket = __shfl_sync(0xFFFFFFFFu, ticket, 0);
     if (ticket == gridDim.x - 1) {
       __threadfence();
-      finish_iteration<SCHEME, RECYCLE>(p);
+#ifdef ADEPT_TIMING_SECTIONS
+      unsigned long long t0 = 0ull, t1 = 0ull;
+      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+      finish_iteration<SCHEME, RECYCLE>(p, tid);
+      __threadfence();
+      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
+      if (tid == 0) {
+        p.sections[6] += t0 - p.sections[kNumSections];
+        p.sections[7] += t1 - t0;
+        p.sections[kNumSections] = ~0ull;
+      }
+#else
+      finish_iteration<SCHEME, RECYCLE>(p, tid);
+#endif
     }
   }
 }
@@ -967,8 +1011,22 @@ template <int L> struct OpsImpl {
     return pick(scheme, instr, int(p.recycle), threads, [&](auto *k) {
       const cudaError_t e = ensure_dynamic_smem(reinterpret_cast<const void *>(k), dyn);
       if (e != cudaSuccess) return e;
-      k<<<grid, threads, dyn, s>>>(p);
-      return cudaGetLastError();
+      // Programmatic dependent launch: the CTAs of this launch may become resident, and run their
+      // prologue up to griddepcontrol.wait, while the previous kernel of the stream is still finishing
+      // (its last CTA closes the iteration alone) -- iterations of small populations are a chain of
+      // latencies, and this takes the launch latency out of it.
+      cudaLaunchConfig_t cfg = {};
+      cfg.gridDim = dim3(grid);
+      cfg.blockDim = dim3(unsigned(threads));
+      cfg.dynamicSmemBytes = dyn;
+      cfg.stream = s;
+      cudaLaunchAttribute attr[1];
+      attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+      attr[0].val.programmaticStreamSerializationAllowed = 1;
+      static const bool no_pdl = std::getenv("ADEPT_NO_PDL") != nullptr;
+      cfg.attrs = attr;
+      cfg.numAttrs = no_pdl ? 0u : 1u;
+      return cudaLaunchKernelEx(&cfg, k, p);
     });
   }
   static cudaError_t launch_inject(int scheme, const Params &p, const void *staged, uint32_t n, int kind,
