@@ -25,7 +25,7 @@
 // the next slab boundary, applies continuous energy loss and discrete
 // interactions, emits secondaries"; Philox-4x32 keyed by (track id, step, draw
 // index)).  Every point on which those two sources are silent is a numbered
-// reading in DESIGN.md §3 (rules R1-R6, M7-M11, T12-T14, S16-S31); the code
+// reading in DESIGN.md §3 (rules R1-R6, M7-M11, T12-T14, S16-S31, X35-X37); the code
 // below follows those rules one by one, in their order and notation, with no
 // blocking, fusion or reordering.
 //
@@ -37,6 +37,14 @@
 // per-event energy conservation; <T(x)> = T0 exp(-x/X0) for brems; Compton
 // energy-momentum conservation and Compton edge; CSDA range; pair/photo
 // branch energies; lockstep == depth-first order independence.
+// Extended physics (tables.physics = 1; DESIGN.md rules X35-X37, SURVEY.md
+// §8(f) item 3): delta-ray production on nial[1] of e+- (X36) and the Compton
+// energy fraction from the full Klein-Nishina distribution by composition and
+// rejection (X37).  Pins (tests/test_oracle_extended.py): the eps distribution
+// against quadrature of the textbook Klein-Nishina density (KS distance, mean);
+// the delta-ray energy against the closed-form 1/T^2 CDF; exact two-body
+// energy-momentum closure; S_restricted + int T dSigma_delta = S; per-event
+// energy conservation; lockstep == depth-first.
 // Parity unpinned (no external closed form exists): the full-shower
 // longitudinal profile — only sanity checks (P-table).
 //
@@ -78,6 +86,8 @@ struct TablesIn {          // as passed over the C interface
   uint32_t n_bins, n_materials;
   float e_min, e_max, ln_e_min, inv_dln, e_cut;
   const float *data;       // [mat][group][qty][n_bins+1]
+  uint32_t physics;        // rule X35: 0 = rules S16-S32, 1 = with the extended rules X36, X37
+  const float *data_x;     // physics 1: [mat][n_bins+1] Sigma_delta [1/mm] of the e+- group
 };
 
 struct Result {
@@ -203,9 +213,12 @@ struct Tables {
   uint32_t n_bins = 0, n_materials = 0;
   float e_min = 0, e_max = 0, ln_e_min = 0, inv_dln = 0, e_cut = 0;
   std::vector<float> data;
+  uint32_t physics = 0;       // X35
+  std::vector<float> data_x;  // X36: Sigma_delta per material
   const float *q(uint32_t mat, int group, int qty) const {
     return data.data() + ((size_t)(mat * 2 + group) * 3 + qty) * (n_bins + 1);
   }
+  const float *qx(uint32_t mat) const { return data_x.data() + (size_t)mat * (n_bins + 1); }
 };
 
 struct Bin { int j; float f; };
@@ -267,11 +280,11 @@ struct Oracle {
   }
 };
 
-struct Rng {                       // R2: lazy, fixed-purpose draws
+struct Rng {                       // R2: lazy, fixed-purpose draws (calls 3..18: the tries of rule X37)
   uint32_t key[2];
   uint32_t step;
-  bool have[3] = {false, false, false};
-  uint32_t blk[3][4];
+  bool have[19] = {};
+  uint32_t blk[19][4];
   uint32_t word(int call, int w) {
     if (!have[call]) {
       const uint32_t ctr[4] = {step, (uint32_t)call, 0u, 0u};
@@ -344,7 +357,8 @@ bool step_track(Oracle &o, int kind, Track &t, Child children[2], int &n_childre
     return finish(false);
   }
 
-  const int NP = (kind == KIND_GAMMA) ? 3 : 1;
+  const bool extended = tab.physics == 1u;                       // X35
+  const int NP = (kind == KIND_GAMMA) ? 3 : (extended ? 2 : 1);  // X36: e+- process 1 = delta-ray production
   const int group = (kind == KIND_GAMMA) ? GROUP_GAMMA : GROUP_ELEC;
 
   // S18: re-sample spent interaction lengths.
@@ -359,7 +373,8 @@ bool step_track(Oracle &o, int kind, Track &t, Child children[2], int &n_childre
   float sig[3] = {0.0f, 0.0f, 0.0f};
   float sj[3] = {INF, INF, INF};
   for (int j = 0; j < NP; ++j) {
-    sig[j] = interp(tab.q(mat, group, j), bin);
+    sig[j] = (kind != KIND_GAMMA && j == 1) ? interp(tab.qx(mat), bin)   // X36: Sigma_delta
+                                            : interp(tab.q(mat, group, j), bin);
     sj[j] = (sig[j] > 0.0f) ? t.nial[j] / sig[j] : INF;
   }
 
@@ -456,7 +471,32 @@ bool step_track(Oracle &o, int kind, Track &t, Child children[2], int &n_childre
   } else if (w != W_ELOSS) {
     // S26: discrete interaction of process w.
     t.nial[w] = -1.0f;
-    if (kind != KIND_GAMMA) {
+    if (kind != KIND_GAMMA && w == 1) {
+      // X36: delta-ray production (the 1/T^2 term common to Moller and Bhabha scattering) on
+      // [e_cut, E/2], two-body kinematics on a free electron at rest
+      const float E = t.ekin;
+      const float a = e_cut, b = 0.5f * E;
+      float T = (a * b) / (b - rng.u(1, 0) * (b - a));
+      if (!(T > a)) T = a;
+      if (!(T < b)) T = b;
+      const float E1 = E - T;
+      const float tau = E + o.two_mc2;
+      float cd = sqrtf((T * tau) / (E * (T + o.two_mc2)));
+      float cp = sqrtf((E1 * tau) / (E * (E1 + o.two_mc2)));
+      if (cd > 1.0f) cd = 1.0f;
+      if (cp > 1.0f) cp = 1.0f;
+      const float sd = sqrtf(fmaf(-cd, cd, 1.0f));
+      const float sp = sqrtf(fmaf(-cp, cp, 1.0f));
+      float sphi, cphi;
+      sincos2pi(rng.u(1, 1), &sphi, &cphi);
+      float dd[3], dp[3];
+      rotate(t.dir, sd, cd, sphi, cphi, dd);
+      rotate(t.dir, sp, cp, -sphi, -cphi, dp);
+      children[0].kind = KIND_EM; children[0].t = make_child(t, rng, 0, dd, T);
+      n_children = 1;
+      t.ekin = E1;
+      for (int c = 0; c < 3; ++c) t.dir[c] = dp[c];
+    } else if (kind != KIND_GAMMA) {
       // bremsstrahlung, 1/k spectrum on [e_cut, E]
       const float E = t.ekin;
       float k = e_cut * ex(rng.u(1, 0) * lg(E / e_cut));
@@ -489,7 +529,30 @@ bool step_track(Oracle &o, int kind, Track &t, Child children[2], int &n_childre
       const float E = t.ekin;
       const float kappa = E / o.mc2;
       const float L = lg(fmaf(2.0f, kappa, 1.0f));
-      const float eps = ex(-(rng.u(1, 0) * L));
+      float eps;
+      if (!extended) {
+        eps = ex(-(rng.u(1, 0) * L));
+      } else {
+        // X37: eps from the Klein-Nishina distribution f(eps) ~ (1/eps + eps)(1 - eps sin^2/(1 + eps^2))
+        // by composition and rejection (try k draws call 3 + k, words 0..2; at most 16 tries)
+        const float eps0 = 1.0f / fmaf(2.0f, kappa, 1.0f);
+        const float eps0sq = eps0 * eps0;
+        const float a1 = L;                              // ln(1/eps0)
+        const float a2 = 0.5f * (1.0f - eps0sq);
+        const float thr = a1 / (a1 + a2);
+        eps = 1.0f;
+        for (int k = 0; k < 16; ++k) {
+          const float u1 = rng.u(3 + k, 0), u2 = rng.u(3 + k, 1), u3 = rng.u(3 + k, 2);
+          if (thr > u1) eps = ex(-(a1 * u2));
+          else eps = sqrtf(fmaf(1.0f - eps0sq, u2, eps0sq));
+          if (eps < eps0) eps = eps0;
+          if (eps > 1.0f) eps = 1.0f;
+          const float tt = (1.0f - eps) / (kappa * eps);
+          const float sin2 = tt * (2.0f - tt);
+          const float g = 1.0f - (eps * sin2) / fmaf(eps, eps, 1.0f);
+          if (g >= u3) break;
+        }
+      }
       const float E1 = eps * E;
       const float T = E - E1;
       float ct = 1.0f - (((1.0f / eps) - 1.0f) / kappa);
@@ -658,6 +721,9 @@ orc_ctx *orc_create(const Geometry *g, const TablesIn *tin, uint64_t seed) {
   o->tab.e_min = tin->e_min; o->tab.e_max = tin->e_max; o->tab.ln_e_min = tin->ln_e_min;
   o->tab.inv_dln = tin->inv_dln; o->tab.e_cut = tin->e_cut;
   o->tab.data.assign(tin->data, tin->data + (size_t)tin->n_materials * 6 * (tin->n_bins + 1));
+  o->tab.physics = tin->physics;
+  if (tin->physics > 1u || (tin->physics == 1u && !tin->data_x)) { delete o; return nullptr; }
+  if (tin->physics == 1u) o->tab.data_x.assign(tin->data_x, tin->data_x + (size_t)tin->n_materials * (tin->n_bins + 1));
   o->seed = seed;
   o->pitch = g->abs_mm + g->gap_mm;
   o->two_mc2 = 2.0f * o->mc2;

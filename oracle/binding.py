@@ -34,7 +34,8 @@ class _Geometry(C.Structure):
 class _Tables(C.Structure):
     _fields_ = [("n_bins", C.c_uint32), ("n_materials", C.c_uint32), ("e_min", C.c_float),
                 ("e_max", C.c_float), ("ln_e_min", C.c_float), ("inv_dln", C.c_float),
-                ("e_cut", C.c_float), ("data", C.POINTER(C.c_float))]
+                ("e_cut", C.c_float), ("data", C.POINTER(C.c_float)),
+                ("physics", C.c_uint32), ("data_x", C.POINTER(C.c_float))]
 
 
 class _Result(C.Structure):
@@ -97,10 +98,13 @@ def _ptr(a: np.ndarray):
 
 def _tables_struct(tables):
     data = np.ascontiguousarray(tables.data, dtype=np.float32)
+    physics = int(getattr(tables, "physics", 0))
+    data_x = np.ascontiguousarray(tables.data_x, dtype=np.float32) if physics else None
     t = _Tables(tables.n_bins, tables.n_materials, tables.e_min, tables.e_max,
                 float(tables.ln_e_min), float(tables.inv_dln), tables.e_cut,
-                data.ctypes.data_as(C.POINTER(C.c_float)))
-    return t, data
+                data.ctypes.data_as(C.POINTER(C.c_float)), physics,
+                data_x.ctypes.data_as(C.POINTER(C.c_float)) if physics else None)
+    return t, (data, data_x)
 
 
 class math_fns:

@@ -42,7 +42,7 @@ class _Geometry(C.Structure):
 class _Tables(C.Structure):
     _fields_ = [("n_bins", C.c_uint32), ("n_materials", C.c_uint32), ("e_min", C.c_float), ("e_max", C.c_float),
                 ("ln_e_min", C.c_float), ("inv_dln", C.c_float), ("e_cut", C.c_float),
-                ("data", C.POINTER(C.c_float))]
+                ("data", C.POINTER(C.c_float)), ("physics", C.c_uint32), ("data_x", C.POINTER(C.c_float))]
 
 
 class _Config(C.Structure):
@@ -144,8 +144,11 @@ class Context:
         self._g = _Geometry(geometry.n_layers, geometry.abs_mm, geometry.gap_mm, geometry.half_xy_mm,
                             geometry.mat_abs, geometry.mat_gap)
         data = np.ascontiguousarray(tables.data, dtype=np.float32)
+        physics = int(getattr(tables, "physics", 0))
+        data_x = np.ascontiguousarray(tables.data_x, dtype=np.float32) if physics else None
         self._t = _Tables(tables.n_bins, tables.n_materials, tables.e_min, tables.e_max, float(tables.ln_e_min),
-                          float(tables.inv_dln), tables.e_cut, data.ctypes.data_as(C.POINTER(C.c_float)))
+                          float(tables.inv_dln), tables.e_cut, data.ctypes.data_as(C.POINTER(C.c_float)), physics,
+                          data_x.ctypes.data_as(C.POINTER(C.c_float)) if physics else None)
         cfg = _Config(self.layout, self.scheme, capacity, batch_primaries, seed, None, 0, None,
                       1 if instrument else 0, flags)
         nbytes = self._L.adept_workspace_bytes(C.byref(self._g), C.byref(self._t), C.byref(cfg))

@@ -67,6 +67,7 @@ static bool make_plan(const adept_geometry *g, const adept_tables *t, const adep
   if (c->flags & ~uint32_t(ADEPT_FLAG_RECYCLE_SLOTS)) return false;
   if (g->n_layers == 0 || g->n_layers > 2048) return false;
   if (t->n_bins == 0 || t->n_bins > 4096 || t->n_materials == 0 || t->n_materials > 8) return false;
+  if (t->physics > 1u || (t->physics == 1u && (c->instrument || (c->flags & ADEPT_FLAG_RECYCLE_SLOTS)))) return false;
   if (c->capacity_per_kind == 0 || c->capacity_per_kind > (1u << 30)) return false;
   pl.capacity = (c->capacity_per_kind + 127u) / 128u * 128u;
   pl.nbuf = (c->scheme == ADEPT_DENSE_DOUBLE) ? 2 : 1;
@@ -277,6 +278,7 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
   Plan pl;
   if (!make_plan(g, t, cfg, pl)) return bad("invalid geometry, tables or configuration");
   if (!t->data) return bad("tables.data is NULL");
+  if (t->physics == 1u && !t->data_x) return bad("tables.physics = 1 needs tables.data_x");
   if (!(g->abs_mm > 0.0f) || !(g->gap_mm > 0.0f) || !(g->half_xy_mm > 0.0f)) return bad("non-positive geometry");
   if (g->mat_abs >= t->n_materials || g->mat_gap >= t->n_materials) return bad("material index out of range");
   if (!(t->e_cut > 0.0f) || !(t->e_max > t->e_min) || !(t->e_min > 0.0f)) return bad("invalid energy grid");
@@ -285,7 +287,7 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
 
   adept_ctx *c = new (std::nothrow) adept_ctx();
   if (!c) return bad("out of host memory");
-  c->geo = *g; c->tab = *t; c->tab.data = nullptr; c->cfg = *cfg; c->plan = pl;
+  c->geo = *g; c->tab = *t; c->tab.data = nullptr; c->tab.data_x = nullptr; c->cfg = *cfg; c->plan = pl;
   c->ops = ops_for(cfg->layout);
   c->stream = static_cast<cudaStream_t>(cfg->cuda_stream);
   c->ws = static_cast<unsigned char *>(cfg->workspace);
@@ -321,6 +323,10 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
       for (uint32_t q = 0; q < 3; ++q)
         for (uint32_t j = 0; j < nodes; ++j)
           packed[((size_t(grp) * t->n_materials + m) * nodes + j) * 4 + q] = t->data[((size_t(m) * 2 + grp) * 3 + q) * nodes + j];
+  if (t->physics == 1u)  // X36: Sigma_delta in the fourth lane of the e+- group
+    for (uint32_t m = 0; m < t->n_materials; ++m)
+      for (uint32_t j = 0; j < nodes; ++j)
+        packed[((size_t(1) * t->n_materials + m) * nodes + j) * 4 + 3] = t->data_x[size_t(m) * nodes + j];
   if ((e = cudaMemcpyAsync(c->ws + pl.tables, packed.data(), pl.table_bytes, cudaMemcpyHostToDevice, c->stream)) != cudaSuccess)
     return die("cudaMemcpyAsync(tables)", e);
   if ((e = cudaStreamSynchronize(c->stream)) != cudaSuccess) return die("cudaStreamSynchronize", e);
@@ -338,6 +344,8 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
   p.mat_abs = g->mat_abs; p.mat_gap = g->mat_gap;
   p.capacity = pl.capacity;
   p.recycle = (cfg->scheme == ADEPT_SPARSE_SINGLE && (cfg->flags & ADEPT_FLAG_RECYCLE_SLOTS)) ? 1u : 0u;
+  p.physics = t->physics;
+  const int variant = (p.recycle ? V_RECYCLE : 0) | (p.physics ? V_PHYS : 0);
   for (int k = 0; k < 3; ++k) {
     uint32_t *r = reinterpret_cast<uint32_t *>(c->ws + pl.rec[k]);
     p.kind[k].rec[0] = r;
@@ -386,7 +394,7 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
   const size_t tile_words = c->ops->record_words(kGroup);
   c->small.threads = kBlockSmall;
   c->small.dyn_smem = step_smem_bytes(cfg->scheme, pl.table_bytes / 2, p.n_slabs, tile_words, kBlockSmall);
-  const int per_sm = c->ops->step_ctas_per_sm(cfg->scheme, instr, int(p.recycle), kBlockSmall, c->small.dyn_smem);
+  const int per_sm = c->ops->step_ctas_per_sm(cfg->scheme, instr, variant, kBlockSmall, c->small.dyn_smem);
   if (per_sm <= 0) {
     g_create_error = "step kernel does not fit on an SM with these tables (shared memory)";
     free_host_side(c);
@@ -395,7 +403,7 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
   c->small.grid = static_cast<unsigned>(sms * per_sm);
   c->large.threads = kBlockLarge;
   c->large.dyn_smem = step_smem_bytes(cfg->scheme, pl.table_bytes / 2, p.n_slabs, tile_words, kBlockLarge);
-  const int per_sm_large = c->ops->step_ctas_per_sm(cfg->scheme, instr, int(p.recycle), kBlockLarge, c->large.dyn_smem);
+  const int per_sm_large = c->ops->step_ctas_per_sm(cfg->scheme, instr, variant, kBlockLarge, c->large.dyn_smem);
   cudaGetLastError();  // a failed attribute query of the optional shape is not an error of the context
   c->large.grid = per_sm_large > 0 ? static_cast<unsigned>(sms * per_sm_large) : 0u;
   c->live_hint = 0;

@@ -110,6 +110,7 @@ struct Params {
   uint32_t mat_abs, mat_gap;
   uint32_t capacity;         // slots per kind (multiple of 128)
   uint32_t recycle;          // sparse scheme: 1 = freed slots are reused (ADEPT_FLAG_RECYCLE_SLOTS)
+  uint32_t physics;          // adept_tables.physics: 1 = extended rules X36, X37
   KindStorage kind[3];
   unsigned long long *instr_field_rw;  // [3][14][2], instrumented build
   // SoA and AoS layouts, dense scheme: tensor maps of the record buffers, [kind][parity] (see

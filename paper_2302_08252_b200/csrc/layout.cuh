@@ -210,7 +210,8 @@ template <int L, bool INSTR> struct TrackView {
   // for e+-, vol when the step crossed into another slab.  dir never changes in the move half, ids
   // never.  A word assigned the value it already had (a zero-length step) is written again; the
   // counting build uses store_changed below instead and counts only real changes.
-  template <bool GAMMA> __device__ __forceinline__ void store_moved(uint32_t slot, const Trk &t, bool vol_changed) const {
+  // N1: e+- also assign nial[1] (extended physics, rule X36).
+  template <bool GAMMA, bool N1 = false> __device__ __forceinline__ void store_moved(uint32_t slot, const Trk &t, bool vol_changed) const {
     if constexpr (L == L_AOS || L == L_SOA16) {
       // 16-byte pieces {pos, dir.x} {dir.yz, ekin, nial0} {nial12, vol, id_lo} {id_hi, step}: a photon
       // rewrites all four, e+- three and the third only with vol
@@ -227,7 +228,7 @@ template <int L, bool INSTR> struct TrackView {
       }
       *q0 = make_uint4(__float_as_uint(t.px), __float_as_uint(t.py), __float_as_uint(t.pz), __float_as_uint(t.dx));
       *q1 = make_uint4(__float_as_uint(t.dy), __float_as_uint(t.dz), __float_as_uint(t.ekin), __float_as_uint(t.n0));
-      if (GAMMA || vol_changed) *q2 = make_uint4(__float_as_uint(t.n1), __float_as_uint(t.n2), t.vol, t.id_lo);
+      if (GAMMA || N1 || vol_changed) *q2 = make_uint4(__float_as_uint(t.n1), __float_as_uint(t.n2), t.vol, t.id_lo);
       *q3 = make_uint2(t.id_hi, t.step);
     } else {
       base[Map::index(cap, slot, F_PX)] = __float_as_uint(t.px);
@@ -239,6 +240,7 @@ template <int L, bool INSTR> struct TrackView {
         base[Map::index(cap, slot, F_N2)] = __float_as_uint(t.n2);
       } else {
         base[Map::index(cap, slot, F_EKIN)] = __float_as_uint(t.ekin);
+        if constexpr (N1) base[Map::index(cap, slot, F_N1)] = __float_as_uint(t.n1);
       }
       if (vol_changed) base[Map::index(cap, slot, F_VOL)] = t.vol;
       base[Map::index(cap, slot, F_STEP)] = t.step;

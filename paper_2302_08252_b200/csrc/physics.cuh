@@ -241,7 +241,8 @@ __device__ __forceinline__ void move_gamma(Trk &t, const Env &g, MoveOut &o) {
 }
 
 // S26 for a photon whose step (already taken: t.step is the post-increment value) ended in process w.
-__device__ __forceinline__ void interact_gamma(Trk &t, int w, const Env &g, InteractOut &o) {
+// PHYS = 1: the Compton energy fraction comes from the full Klein-Nishina distribution (rule X37).
+template <int PHYS> __device__ __forceinline__ void interact_gamma(Trk &t, int w, const Env &g, InteractOut &o) {
   interact_out_init(o);
   const Stream rs{t.id_lo, t.id_hi, t.step - 1u};  // draws are addressed by the pre-increment step (R2)
   const uint4 r1 = rs.call(1), r2 = rs.call(2);
@@ -265,7 +266,31 @@ __device__ __forceinline__ void interact_gamma(Trk &t, int w, const Env &g, Inte
   const float E = t.ekin;
   const float kappa = E / kMc2;
   const float L = lg(fmaf(2.0f, kappa, 1.0f));
-  const float eps = ex(-(u01(r1.x) * L));
+  float eps;
+  if constexpr (PHYS == 0) {
+    eps = ex(-(u01(r1.x) * L));
+  } else {
+    // X37: composition (1/eps on [eps0, 1] with weight a1, eps on [eps0, 1] with weight a2) and
+    // rejection by g = 1 - eps sin^2(theta) / (1 + eps^2); try k draws call 3 + k, at most 16 tries
+    const float eps0 = 1.0f / fmaf(2.0f, kappa, 1.0f);
+    const float eps0sq = eps0 * eps0;
+    const float a1 = L;
+    const float a2 = 0.5f * (1.0f - eps0sq);
+    const float thr = a1 / (a1 + a2);
+    eps = 1.0f;
+    for (int k = 0; k < 16; ++k) {
+      const uint4 r = rs.call(3u + uint32_t(k));
+      const float u1 = u01(r.x), u2 = u01(r.y), u3 = u01(r.z);
+      if (thr > u1) eps = ex(-(a1 * u2));
+      else eps = sqrtf(fmaf(1.0f - eps0sq, u2, eps0sq));
+      if (eps < eps0) eps = eps0;
+      if (eps > 1.0f) eps = 1.0f;
+      const float tt = (1.0f - eps) / (kappa * eps);
+      const float sin2 = tt * (2.0f - tt);
+      const float gg = 1.0f - (eps * sin2) / fmaf(eps, eps, 1.0f);
+      if (gg >= u3) break;
+    }
+  }
   const float E1 = eps * E;
   const float T = E - E1;
   float ct = 1.0f - (((1.0f / eps) - 1.0f) / kappa);
@@ -293,7 +318,8 @@ __device__ __forceinline__ void interact_gamma(Trk &t, int w, const Env &g, Inte
 }
 
 // --------------------------------------------------------------------- electron / positron ---
-template <int KIND> __device__ __forceinline__ void move_elec(Trk &t, const Env &g, MoveOut &o) {
+// PHYS = 1: delta-ray production is a second discrete process, on nial[1] (rule X36).
+template <int KIND, int PHYS> __device__ __forceinline__ void move_elec(Trk &t, const Env &g, MoveOut &o) {
   static_assert(KIND == K_EM || KIND == K_EP, "e- or e+");
   move_out_init(o);
   const Stream rs{t.id_lo, t.id_hi, t.step};
@@ -307,7 +333,16 @@ template <int KIND> __device__ __forceinline__ void move_elec(Trk &t, const Env 
   }
 
   // S18: bremsstrahlung is the only discrete process; nial[1], nial[2] are carried unchanged
-  if (t.n0 <= 0.0f) t.n0 = -lg(u01(rs.call(0).x));
+  // (X36: delta-ray production is the second one, nial[2] is carried unchanged)
+  if constexpr (PHYS == 0) {
+    if (t.n0 <= 0.0f) t.n0 = -lg(u01(rs.call(0).x));
+  } else {
+    if (t.n0 <= 0.0f || t.n1 <= 0.0f) {
+      const uint4 r = rs.call(0);
+      if (t.n0 <= 0.0f) t.n0 = -lg(u01(r.x));
+      if (t.n1 <= 0.0f) t.n1 = -lg(u01(r.y));
+    }
+  }
 
   // S19, S20
   const uint32_t vol0 = t.vol;
@@ -320,6 +355,11 @@ template <int KIND> __device__ __forceinline__ void move_elec(Trk &t, const Env 
   const float S0 = lerp_node(b.f, A.y, B.y);
   const float R = lerp_node(b.f, A.z, B.z);
   const float s0 = quotient_or_inf(t.n0, sig0, sig0 > 0.0f);
+  float sig1 = 0.0f, s1 = kInf;
+  if constexpr (PHYS != 0) {
+    sig1 = lerp_node(b.f, A.w, B.w);  // X36: Sigma_delta rides in the fourth lane of the e+- group
+    s1 = quotient_or_inf(t.n1, sig1, sig1 > 0.0f);
+  }
   float s_e;
   {
     const float r_min = 0.1f, f_r = 0.2f;
@@ -336,12 +376,14 @@ template <int KIND> __device__ __forceinline__ void move_elec(Trk &t, const Env 
   int w = -1;
   if (s_e < s) { s = s_e; w = 3; }
   if (s0 < s) { s = s0; w = 0; }
+  if (PHYS != 0 && s1 < s) { s = s1; w = 1; }
 
   // S23
   t.px = fmaf(s, t.dx, t.px);
   t.py = fmaf(s, t.dy, t.py);
   t.pz = fmaf(s, t.dz, t.pz);
   t.n0 = fmaf(-s, sig0, t.n0);
+  if constexpr (PHYS != 0) t.n1 = fmaf(-s, sig1, t.n1);
   t.step = rs.step + 1u;
 
   // S24: continuous loss by the midpoint rule, deposit in the pre-step slab
@@ -360,17 +402,17 @@ template <int KIND> __device__ __forceinline__ void move_elec(Trk &t, const Env 
   t.ekin = E_post;
   // what the step ends in, as flags (no early exits: the outcomes of a warp's lanes differ)
   const bool below = E_post < e_cut;            // S24: e- deposits the rest and dies; e+ is kept for S17
-  const bool brems = !below && w == 0;          // S26 follows in interact_elec
+  const bool brems = !below && (w == 0 || w == 1);  // S26 (X36: w == 1) follows in interact_elec
   const bool geom = !below && w < 0;
   o.dep_b = (below && KIND == K_EM) ? E_post : 0.0f;
-  o.pending = brems ? int(P_PROC0) : int(P_NONE);
+  o.pending = brems ? w : int(P_NONE);
   o.escaped = cross_boundary(geom, t, g, vol0, face, z_lo, z_hi);  // S25
   o.guard = !below && !brems && !o.escaped && t.step >= (1u << 20);  // S31
   o.alive = !((below && KIND == K_EM) || o.escaped || o.guard);
 }
 
 // S17 annihilation (pending == P_ANNIH: track untouched) or S26 bremsstrahlung (step already taken).
-template <int KIND> __device__ __forceinline__ void interact_elec(Trk &t, int pending, const Env &g, InteractOut &o) {
+template <int KIND, int PHYS> __device__ __forceinline__ void interact_elec(Trk &t, int pending, const Env &g, InteractOut &o) {
   interact_out_init(o);
   const bool annih = (KIND == K_EP) && (pending == P_ANNIH);
   const Stream rs{t.id_lo, t.id_hi, annih ? t.step : t.step - 1u};
@@ -387,8 +429,35 @@ template <int KIND> __device__ __forceinline__ void interact_elec(Trk &t, int pe
     o.alive = false;
     return;
   }
-  // bremsstrahlung: k from the 1/k spectrum on [e_cut, E], photon along dir
   const float e_cut = g.e_cut;
+  if (PHYS != 0 && pending == P_PROC1) {
+    // X36: delta ray from the 1/T^2 spectrum on [e_cut, E/2], two-body kinematics on a free electron
+    t.n1 = -1.0f;
+    const float E = t.ekin;
+    const float a = e_cut, b = 0.5f * E;
+    float T = (a * b) / (b - u01(r1.x) * (b - a));
+    if (!(T > a)) T = a;
+    if (!(T < b)) T = b;
+    const float E1 = E - T;
+    const float tau = E + two_mc2();
+    float cd = sqrtf((T * tau) / (E * (T + two_mc2())));
+    float cp = sqrtf((E1 * tau) / (E * (E1 + two_mc2())));
+    if (cd > 1.0f) cd = 1.0f;
+    if (cp > 1.0f) cp = 1.0f;
+    const float sd = sqrtf(fmaf(-cd, cd, 1.0f));
+    const float sp = sqrtf(fmaf(-cp, cp, 1.0f));
+    float sphi, cphi;
+    sincos2pi(u01(r1.y), sphi, cphi);
+    float ax, ay, az, bx, by, bz;
+    rotate_dir(t.dx, t.dy, t.dz, sd, cd, sphi, cphi, ax, ay, az);
+    rotate_dir(t.dx, t.dy, t.dz, sp, cp, -sphi, -cphi, bx, by, bz);
+    make_kid(o.kid[0], K_EM, ax, ay, az, T, r2.x, r2.y);
+    t.ekin = E1;
+    t.dx = bx; t.dy = by; t.dz = bz;
+    runaway_guard<KIND>(t, o);
+    return;
+  }
+  // bremsstrahlung: k from the 1/k spectrum on [e_cut, E], photon along dir
   t.n0 = -1.0f;
   const float E = t.ekin;
   float k = e_cut * ex(u01(r1.x) * lg(E / e_cut));

@@ -45,6 +45,10 @@ __device__ __forceinline__ void group_sync(int group) {
   asm volatile("bar.sync %0, %1;" ::"r"(group + 1), "n"(kGroup) : "memory");
 }
 
+// Variant bits of the step kernel (template parameter VAR): slot recycling of the sparse scheme
+// (ADEPT_FLAG_RECYCLE_SLOTS) and the extended physics rules X36, X37 (adept_tables.physics = 1).
+enum Variant : int { V_RECYCLE = 1, V_PHYS = 2 };
+
 // ---- section clocks (timing build only) ------------------------------------------------------------
 // BASELINE.json configs[3]: "each scheme reports step plus slot-allocation/compaction time".  Allocation
 // and compaction are fused into the step kernel (rows A9, A10), so a variant of the library compiled
@@ -309,9 +313,10 @@ struct CtaShared {
 // Run by the first warp of the last CTA: lane k < 3 closes kind k, so that the dependent global
 // accesses of the three kinds overlap (an iteration of a small population is a chain of memory round
 // trips; this is its last link).
-template <int SCHEME, bool RECYCLE> __device__ void finish_iteration(const Params &p, int lane) {
+template <int SCHEME, int VAR> __device__ void finish_iteration(const Params &p, int lane) {
   Ctl *c = p.ctl;
   uint32_t n = 0u, nn = 0u;
+  constexpr bool RECYCLE = (VAR & V_RECYCLE) != 0;
   if (lane < 3) {
     const int k = lane;
     n = c->n_cur[k];
@@ -385,7 +390,7 @@ template <int KIND> __device__ __forceinline__ void bin_add_track_energy(const B
 // First half of the step for tile `tile` of kind KIND's current set (rows A1-A7, A10 for the
 // tracks whose step ends without an interaction).  `queued` = parked tracks of the group before
 // the tile; returns the number after it (the same value in every thread of the group).
-template <int L, int SCHEME, bool INSTR, bool RECYCLE, int KIND>
+template <int L, int SCHEME, bool INSTR, int VAR, int KIND>
 __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, const GroupRefs &c, uint32_t par,
                                               uint32_t tile, uint32_t next_tile, uint32_t n_kind, int sbuf,
                                               uint32_t &in_phase, uint32_t queued) {
@@ -431,7 +436,7 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
     vol_before = t.vol;
     c.clk->mark(SEC_LOAD);
     if constexpr (KIND == K_GAMMA) move_gamma(t, env, o);
-    else move_elec<KIND>(t, env, o);
+    else move_elec<KIND, (VAR & V_PHYS) ? 1 : 0>(t, env, o);
     // A6: scoring into the CTA's bins (pre-step slab; the S31 guard uses the post-step slab).  A
     // photon deposits nothing in this half; the rare terms share one branch.
     if (KIND != K_GAMMA && o.dep != 0.0f) bin_add(c.bins, vol_before, o.dep);
@@ -450,7 +455,7 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
   if (SCHEME == S_SPARSE) {
     if (survives || parked) {
       if constexpr (INSTR) cur.store_changed(slot, t, old);  // counts exactly the words that changed
-      else cur.template store_moved<KIND == K_GAMMA>(slot, t, t.vol != vol_before);
+      else cur.template store_moved<KIND == K_GAMMA, (VAR & V_PHYS) != 0>(slot, t, t.vol != vol_before);
     }
     c.clk->mark(SEC_STORE);
   }
@@ -458,7 +463,7 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
   const uint32_t m_esc = __ballot_sync(0xFFFFFFFFu, o.escaped);
   const uint32_t m_park = __ballot_sync(0xFFFFFFFFu, parked);
   // sparse scheme with slot recycling: a track that ends here frees its slot
-  constexpr bool recycle = SCHEME == S_SPARSE && RECYCLE;
+  constexpr bool recycle = SCHEME == S_SPARSE && (VAR & V_RECYCLE) != 0;
   const bool ends = recycle && active && !parked && !survives;
   uint32_t m_end = 0u;
   if (SCHEME == S_SPARSE && recycle) {
@@ -519,7 +524,7 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
 
 // Second half of the step on a dense batch of up to kGroup parked tracks taken from the top of the
 // group's queue (rows A8, A9, A10).  Returns the number of tracks left in the queue.
-template <int L, int SCHEME, bool INSTR, bool RECYCLE, int KIND>
+template <int L, int SCHEME, bool INSTR, int VAR, int KIND>
 __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &env, const GroupRefs &c, uint32_t par,
                                                    uint32_t queued, int sbuf) {
   const int gtid = c.gtid, lane = gtid & 31;
@@ -541,8 +546,8 @@ __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &e
     int pending;
     park_load<SCHEME>(c.queue, q, t, pending, slot);
     before_interaction = t;
-    if constexpr (KIND == K_GAMMA) interact_gamma(t, pending, env, o);
-    else interact_elec<KIND>(t, pending, env, o);
+    if constexpr (KIND == K_GAMMA) interact_gamma<(VAR & V_PHYS) ? 1 : 0>(t, pending, env, o);
+    else interact_elec<KIND, (VAR & V_PHYS) ? 1 : 0>(t, pending, env, o);
     if (o.dep != 0.0f) bin_add(c.bins, t.vol, o.dep);
     if (o.dep_b != 0.0f) bin_add(c.bins, t.vol, o.dep_b);
     if (o.guard) bin_add_track_energy<KIND>(c.bins, t.vol, t.ekin);
@@ -550,21 +555,29 @@ __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &e
   c.clk->mark(SEC_INTERACT);
   constexpr int Q0 = kid_kind<KIND>(0), Q1 = kid_kind<KIND>(1);  // never KIND itself
   const uint32_t m_alive = __ballot_sync(0xFFFFFFFFu, o.alive);
-  constexpr bool recycle = SCHEME == S_SPARSE && RECYCLE;
+  constexpr bool recycle = SCHEME == S_SPARSE && (VAR & V_RECYCLE) != 0;
   const bool ends = recycle && have && !o.alive;  // the parent's slot is free from the next iteration on
   uint32_t m_end = 0u;
   if (SCHEME == S_SPARSE && recycle) {
     m_end = __ballot_sync(0xFFFFFFFFu, ends);
     if (lane == 0) g.kcnt[sbuf][gtid >> 5] = uint32_t(__popc(m_end));
   }
-  const uint32_t m_k0 = __ballot_sync(0xFFFFFFFFu, o.kid[0].kind >= 0);
+  // Extended physics (rule X36): child 0 of an e+- is a photon (bremsstrahlung) or an e- (delta ray).
+  // Delta rays are ranked in a field of their own: field 0 = e- for e+ parents; for e- parents
+  // field 1 (the e+ field, which an e- parent never uses), with destination kind e-.
+  constexpr bool kDelta = (VAR & V_PHYS) != 0 && KIND != K_GAMMA;
+  constexpr int FD = (KIND == K_EM) ? 1 : 0;
+  const bool k0d = kDelta && o.kid[0].kind == K_EM;
+  const uint32_t m_k0 = __ballot_sync(0xFFFFFFFFu, o.kid[0].kind >= 0 && !k0d);
+  const uint32_t m_kd = kDelta ? __ballot_sync(0xFFFFFFFFu, k0d) : 0u;
   const uint32_t m_k1 = __ballot_sync(0xFFFFFFFFu, o.kid[1].kind >= 0);
+  auto dest_of = [](int field) -> int { return (kDelta && field == FD) ? int(K_EM) : field; };
 
   // A9: one arrival per warp with its output counts per destination kind
   uint32_t word = 0;
   if (lane == 0) {
     const uint32_t mine = (uint32_t(__popc(m_alive)) << (9 * KIND)) + (uint32_t(__popc(m_k0)) << (9 * Q0)) +
-                          (uint32_t(__popc(m_k1)) << (9 * Q1)) + kTicket;
+                          (uint32_t(__popc(m_k1)) << (9 * Q1)) + (uint32_t(__popc(m_kd)) << (9 * FD)) + kTicket;
     word = atomicAdd(&g.acc[sbuf], mine);
     if (last_ticket(word)) {
       const uint32_t total = word + mine;
@@ -573,6 +586,7 @@ __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &e
 #pragma unroll
       for (int q = 0; q < 3; ++q) {
         const uint32_t want = count_of(total, q);
+        const int d = dest_of(q);  // destination kind of field q
         uint32_t got = want;
         if (SCHEME == S_SPARSE && q != KIND) {
           // sparse: children get bump-allocated, never recycled slots (rule S30) -- or, with slot
@@ -580,14 +594,14 @@ __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &e
           // free_tail_start), then bump-allocated ones
           uint32_t n_ring = 0u, h = 0u;
           if (recycle && want) {
-            h = atomicAdd(&ctl->free_head[q], want);
-            const int32_t avail = static_cast<int32_t>(ctl->free_tail_start[q] - h);
+            h = atomicAdd(&ctl->free_head[d], want);
+            const int32_t avail = static_cast<int32_t>(ctl->free_tail_start[d] - h);
             n_ring = avail <= 0 ? 0u : (uint32_t(avail) < want ? uint32_t(avail) : want);
           }
           g.rbase[sbuf][q] = h;
           g.rn[sbuf][q] = n_ring;
           const uint32_t rest = want - n_ring;
-          const uint32_t sb = rest ? atomicAdd(&ctl->slot_top[q], rest) : 0u;
+          const uint32_t sb = rest ? atomicAdd(&ctl->slot_top[d], rest) : 0u;
           g.sbase[sbuf][q] = sb;
           // slots past the end of the buffer do not exist: those children are dropped (overflow), and
           // only children that have a slot get a list entry, so every list entry names a real slot
@@ -595,7 +609,7 @@ __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &e
           got = n_ring + usable;
           g.sgot[sbuf][q] = got;
         }
-        g.base[sbuf][q] = got ? atomicAdd(&ctl->n_next[q], got) : 0u;
+        g.base[sbuf][q] = got ? atomicAdd(&ctl->n_next[d], got) : 0u;
       }
       if (SCHEME == S_SPARSE && recycle) {
         const uint32_t n_end = batch - count_of(total, KIND);
@@ -609,7 +623,9 @@ __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &e
   // position of this thread's outputs among its warp's: survivor; child 0; child 1 (after the warp's
   // children 0 when both go to the same kind)
   const uint32_t r_alive = count_of(word, KIND) + __popc(m_alive & lt_mask);
-  const uint32_t r_k0 = count_of(word, Q0) + __popc(m_k0 & lt_mask);
+  const int f0 = k0d ? FD : Q0;             // arrival-word field and destination kind of child 0
+  const int d0 = k0d ? int(K_EM) : Q0;
+  const uint32_t r_k0 = count_of(word, f0) + __popc((k0d ? m_kd : m_k0) & lt_mask);
   const uint32_t r_k1 = count_of(word, Q1) + ((Q0 == Q1) ? uint32_t(__popc(m_k0)) : 0u) + __popc(m_k1 & lt_mask);
   const int nbuf = int(par ^ 1u);
   bool dropped = false;
@@ -622,8 +638,8 @@ __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &e
       else dropped = true;
     }
     if (o.kid[0].kind >= 0) {
-      const uint32_t dst = g.base[sbuf][Q0] + r_k0;
-      if (dst < p.capacity) make_view<L, INSTR>(p, Q0, nbuf, c.cta->probe).store(dst, kid_track(t, o.kid[0]));
+      const uint32_t dst = g.base[sbuf][f0] + r_k0;
+      if (dst < p.capacity) make_view<L, INSTR>(p, d0, nbuf, c.cta->probe).store(dst, kid_track(t, o.kid[0]));
       else dropped = true;
     }
     if (o.kid[1].kind >= 0) {
@@ -639,10 +655,10 @@ __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &e
       if (qpos < p.capacity) p.kind[KIND].queue[nbuf][qpos] = slot;
       else dropped = true;
     }
-    // slot of the child with rank r among the group's children of kind q
+    // slot of the child with rank r among the group's children of field q
     auto child_slot = [&](int q, uint32_t r) -> uint32_t {
       const uint32_t nr = g.rn[sbuf][q];
-      if (r < nr) return p.kind[q].free_ring[(g.rbase[sbuf][q] + r) % p.capacity];
+      if (r < nr) return p.kind[dest_of(q)].free_ring[(g.rbase[sbuf][q] + r) % p.capacity];
       return g.sbase[sbuf][q] + (r - nr);
     };
     if (ends) {
@@ -651,11 +667,11 @@ __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &e
       p.kind[KIND].free_ring[(g.fbase[sbuf] + r) % p.capacity] = slot;
     }
     if (o.kid[0].kind >= 0) {
-      const uint32_t qpos = g.base[sbuf][Q0] + r_k0;
-      if (r_k0 < g.sgot[sbuf][Q0] && qpos < p.capacity) {
-        const uint32_t s_new = child_slot(Q0, r_k0);
-        make_view<L, INSTR>(p, Q0, 0, c.cta->probe).store(s_new, kid_track(t, o.kid[0]));
-        p.kind[Q0].queue[nbuf][qpos] = s_new;
+      const uint32_t qpos = g.base[sbuf][f0] + r_k0;
+      if (r_k0 < g.sgot[sbuf][f0] && qpos < p.capacity) {
+        const uint32_t s_new = child_slot(f0, r_k0);
+        make_view<L, INSTR>(p, d0, 0, c.cta->probe).store(s_new, kid_track(t, o.kid[0]));
+        p.kind[d0].queue[nbuf][qpos] = s_new;
       } else dropped = true;
     }
     if (o.kid[1].kind >= 0) {
@@ -674,7 +690,7 @@ __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &e
 
 // All tiles of one kind that belong to this group, then the left-over parked tracks.
 // `first_global_tile` = tiles of the kinds before this one; n_tiles, n_kind are launch-uniform.
-template <int L, int SCHEME, bool INSTR, bool RECYCLE, int KIND>
+template <int L, int SCHEME, bool INSTR, int VAR, int KIND>
 __device__ __forceinline__ void run_kind(const Params &p, const Env &env, const GroupRefs &c, uint32_t par,
                                          uint32_t first_global_tile, uint32_t n_tiles, uint32_t n_kind, int &sbuf,
                                          uint32_t &in_phase, uint32_t &tab_phase, int &staged_group) {
@@ -714,15 +730,15 @@ __device__ __forceinline__ void run_kind(const Params &p, const Env &env, const 
   uint32_t queued = 0u;
   for (uint32_t tile = shift; tile < n_tiles; tile += n_groups) {
     const uint32_t next_tile = (tile + n_groups < n_tiles) ? tile + n_groups : 0xFFFFFFFFu;
-    queued = move_tile<L, SCHEME, INSTR, RECYCLE, KIND>(p, env, c, par, tile, next_tile, n_kind, sbuf, in_phase, queued);
+    queued = move_tile<L, SCHEME, INSTR, VAR, KIND>(p, env, c, par, tile, next_tile, n_kind, sbuf, in_phase, queued);
     sbuf ^= 1;
     if (queued >= uint32_t(kGroup)) {
-      queued = interact_batch<L, SCHEME, INSTR, RECYCLE, KIND>(p, env, c, par, queued, sbuf);
+      queued = interact_batch<L, SCHEME, INSTR, VAR, KIND>(p, env, c, par, queued, sbuf);
       sbuf ^= 1;
     }
   }
   while (queued != 0u) {
-    queued = interact_batch<L, SCHEME, INSTR, RECYCLE, KIND>(p, env, c, par, queued, sbuf);
+    queued = interact_batch<L, SCHEME, INSTR, VAR, KIND>(p, env, c, par, queued, sbuf);
     sbuf ^= 1;
   }
 }
@@ -733,7 +749,7 @@ __device__ __forceinline__ void run_kind(const Params &p, const Env &env, const 
 #ifndef ADEPT_STEP_MIN_CTAS
 #define ADEPT_STEP_MIN_CTAS 4
 #endif
-template <int L, int SCHEME, bool INSTR, int THREADS, bool RECYCLE = false>
+template <int L, int SCHEME, bool INSTR, int THREADS, int VAR = 0>
 __global__ void __launch_bounds__(THREADS, (THREADS == kBlockSmall) ? ADEPT_STEP_MIN_CTAS : 1) step_kernel(const __grid_constant__ Params p) {
   constexpr int kBlock = THREADS;
   constexpr int kGroupsPerCta = THREADS / kGroup;
@@ -799,9 +815,9 @@ __global__ void __launch_bounds__(THREADS, (THREADS == kBlockSmall) ? ADEPT_STEP
     int sbuf = 0;
     uint32_t in_phase = 0u, tab_phase = 0u;
     int staged_group = -1;
-    run_kind<L, SCHEME, INSTR, RECYCLE, K_EM>(p, env, c, par, 0u, t0, n0, sbuf, in_phase, tab_phase, staged_group);
-    run_kind<L, SCHEME, INSTR, RECYCLE, K_EP>(p, env, c, par, t0, t1, n1, sbuf, in_phase, tab_phase, staged_group);
-    run_kind<L, SCHEME, INSTR, RECYCLE, K_GAMMA>(p, env, c, par, t0 + t1, t2, n2, sbuf, in_phase, tab_phase, staged_group);
+    run_kind<L, SCHEME, INSTR, VAR, K_EM>(p, env, c, par, 0u, t0, n0, sbuf, in_phase, tab_phase, staged_group);
+    run_kind<L, SCHEME, INSTR, VAR, K_EP>(p, env, c, par, t0, t1, n1, sbuf, in_phase, tab_phase, staged_group);
+    run_kind<L, SCHEME, INSTR, VAR, K_GAMMA>(p, env, c, par, t0 + t1, t2, n2, sbuf, in_phase, tab_phase, staged_group);
 
     // flush the CTA's tallies
     clk.mark(SEC_OTHER);
@@ -837,7 +853,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == kBlockSmall) ? ADEPT_STEP
 #ifdef ADEPT_TIMING_SECTIONS
       unsigned long long t0 = 0ull, t1 = 0ull;
       asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
-      finish_iteration<SCHEME, RECYCLE>(p, tid);
+      finish_iteration<SCHEME, VAR>(p, tid);
       __threadfence();
       asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
       if (tid == 0) {
@@ -846,7 +862,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == kBlockSmall) ? ADEPT_STEP
         p.sections[kNumSections] = ~0ull;
       }
 #else
-      finish_iteration<SCHEME, RECYCLE>(p, tid);
+      finish_iteration<SCHEME, VAR>(p, tid);
 #endif
     }
   }
@@ -960,9 +976,9 @@ __global__ void read_kernel(const __grid_constant__ Params p, PackedTrack *dst, 
 // scheme and instrumentation are compile-time parameters of every kernel.)
 struct LayoutOps {
   size_t (*record_words)(size_t capacity);
-  int (*step_ctas_per_sm)(int scheme, int instr, int recycle, int threads, size_t dyn_smem);
+  int (*step_ctas_per_sm)(int scheme, int instr, int variant, int threads, size_t dyn_smem);
   cudaError_t (*launch_step)(int scheme, int instr, const Params &, int threads, unsigned grid, size_t dyn_smem,
-                             cudaStream_t);  // Params::recycle picks the slot-recycling instantiation (sparse scheme)
+                             cudaStream_t);  // Params::recycle / physics pick the kernel variant
   cudaError_t (*launch_inject)(int scheme, const Params &, const void *staged, uint32_t n, int kind, uint32_t par,
                                uint32_t entry_base, uint32_t slot_base, unsigned long long seed, cudaStream_t);
   cudaError_t (*launch_load)(int scheme, const Params &, const void *staged, const uint32_t *slots, uint32_t n,
@@ -989,17 +1005,20 @@ inline cudaError_t ensure_dynamic_smem(const void *kernel, size_t bytes) {
 }
 
 template <int L> struct OpsImpl {
-  template <int T, typename F> static auto pick_t(int scheme, int instr, int recycle, F f) {
+  // The extended physics is instantiated for the plain (non-counting) kernels without slot recycling.
+  template <int T, typename F> static auto pick_t(int scheme, int instr, int var, F f) {
+    if (var & V_PHYS)
+      return scheme == S_DENSE ? f(step_kernel<L, S_DENSE, false, T, V_PHYS>) : f(step_kernel<L, S_SPARSE, false, T, V_PHYS>);
     if (scheme == S_DENSE) return instr ? f(step_kernel<L, S_DENSE, true, T>) : f(step_kernel<L, S_DENSE, false, T>);
-    if (recycle) return instr ? f(step_kernel<L, S_SPARSE, true, T, true>) : f(step_kernel<L, S_SPARSE, false, T, true>);
+    if (var & V_RECYCLE) return instr ? f(step_kernel<L, S_SPARSE, true, T, V_RECYCLE>) : f(step_kernel<L, S_SPARSE, false, T, V_RECYCLE>);
     return instr ? f(step_kernel<L, S_SPARSE, true, T>) : f(step_kernel<L, S_SPARSE, false, T>);
   }
-  template <typename F> static auto pick(int scheme, int instr, int recycle, int threads, F f) {
-    return threads == kBlockLarge ? pick_t<kBlockLarge>(scheme, instr, recycle, f) : pick_t<kBlockSmall>(scheme, instr, recycle, f);
+  template <typename F> static auto pick(int scheme, int instr, int var, int threads, F f) {
+    return threads == kBlockLarge ? pick_t<kBlockLarge>(scheme, instr, var, f) : pick_t<kBlockSmall>(scheme, instr, var, f);
   }
   static size_t record_words(size_t cap) { return Mapping<L>::words(cap); }
-  static int step_ctas_per_sm(int scheme, int instr, int recycle, int threads, size_t dyn) {
-    return pick(scheme, instr, recycle, threads, [&](auto *k) {
+  static int step_ctas_per_sm(int scheme, int instr, int var, int threads, size_t dyn) {
+    return pick(scheme, instr, var, threads, [&](auto *k) {
       int n = 0;
       if (ensure_dynamic_smem(reinterpret_cast<const void *>(k), dyn) != cudaSuccess) return -1;
       if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k, threads, dyn) != cudaSuccess) return -1;
@@ -1008,7 +1027,7 @@ template <int L> struct OpsImpl {
   }
   static cudaError_t launch_step(int scheme, int instr, const Params &p, int threads, unsigned grid, size_t dyn,
                                  cudaStream_t s) {
-    return pick(scheme, instr, int(p.recycle), threads, [&](auto *k) {
+    return pick(scheme, instr, (p.recycle ? V_RECYCLE : 0) | (p.physics ? V_PHYS : 0), threads, [&](auto *k) {
       const cudaError_t e = ensure_dynamic_smem(reinterpret_cast<const void *>(k), dyn);
       if (e != cudaSuccess) return e;
       // Programmatic dependent launch: the CTAs of this launch may become resident, and run their

@@ -50,7 +50,7 @@ def test_record_sizes_match_the_header(L):
 
 def _args(L, layout=1, scheme=1, capacity=4096, n_layers=50, n_bins=256, instrument=0):
     g = L._Geometry(n_layers, 2.3, 5.7, 200.0, 0, 1)
-    t = L._Tables(n_bins, 2, 0.1, 1e4, 0.0, 1.0, 0.1, None)
+    t = L._Tables(n_bins, 2, 0.1, 1e4, 0.0, 1.0, 0.1, None, 0, None)
     c = L._Config(layout, scheme, capacity, 0, 0, None, 0, None, instrument, 0)
     return g, t, c
 

@@ -800,3 +800,75 @@ def _heavy_reference():
         _HEAVY.update(o.result())
         o.close()
     return _HEAVY
+
+
+# ------------------------------------------------- extended physics ----------
+@pytest.mark.parametrize("scheme", SCHEMES)
+@pytest.mark.parametrize("layout", ("aos", "soa", "aosoa32", "soa16"))
+def test_extended_physics_matches_oracle(layout, scheme):
+    """adept_tables.physics = 1 (rules X36 delta rays on nial[1], X37 Klein-Nishina rejection sampling):
+    the tiny shower track by track in every iteration, then 100 x 1 GeV showers to completion."""
+    c = CONFIGS["tiny"]
+    geo, tab = geometry_for("tiny"), tables_for("tiny", physics=1)
+    prim = gen_primaries(c["n_primaries"], c["e_primary"])
+    o = Oracle(geo, tab, seed=c["seed"])
+    o.inject(prim)
+    ctx = _ctx(geo, tab, layout=layout, scheme=scheme, capacity=c["capacity"], seed=c["seed"])
+    ctx.inject(prim)
+    it = 0
+    while sum(o.live(k) for k in range(3)):
+        o.step()
+        compare_counts(ctx.step(), o.result(), what="iteration %d" % it)
+        for k in range(3):
+            compare_tracks(ctx.read_tracks(k), o.read_tracks(k, make_tracks(1).dtype), "iteration %d kind %d" % (it, k))
+        it += 1
+    r, g = o.result(), ctx.result()
+    assert np.allclose(g["edep_layer"], r["edep_layer"], rtol=1e-4, atol=1e-12)
+    ctx.destroy()
+    basic = Oracle(geo, tables_for("tiny"), seed=c["seed"])
+    basic.inject(prim)
+    basic.run()
+    assert r["secondaries"][0] > basic.result()["secondaries"][0]        # the delta rays are there
+
+    c = CONFIGS["full"]
+    geo, tab = geometry_for("full"), tables_for("full", physics=1)
+    prim = gen_primaries(100, c["e_primary"])
+    o = Oracle(geo, tab, seed=c["seed"])
+    o.inject(prim)
+    o.run()
+    r = o.result()
+    ctx = _ctx(geo, tab, layout=layout, scheme=scheme, capacity=1 << 19, seed=c["seed"])
+    ctx.inject(prim)
+    g = ctx.run()
+    compare_counts(g, r)
+    assert g["iterations"] == r["iterations"]
+    assert np.allclose(g["edep_layer"], r["edep_layer"], rtol=1e-4, atol=1e-9)
+    assert abs(g["edep_slab"].sum() + g["e_escaped"] - g["e_injected"]) < 1e-6 * g["e_injected"]
+    ctx.destroy()
+
+
+def test_extended_physics_single_step_population_and_validation():
+    """One step of a config-3-like population under the extended rules, every track compared; the
+    variant is refused where it is not built (instrumented contexts, slot recycling)."""
+    from paper_2302_08252_b200 import AdeptError
+    geo, tab = geometry_for("single_step"), tables_for("single_step", physics=1)
+    pop = gen_tracks(300_001, 11, geo, CONFIGS["single_step"]["e_max"])
+    for p in pop:                                   # spent interaction lengths: everything re-samples
+        p["nial"][::3] = -1.0
+    o = Oracle(geo, tab, seed=3)
+    for k in range(3):
+        o.load_tracks(k, pop[k])
+    o.step()
+    r = o.result()
+    for layout, scheme in (("aosoa32", "dense"), ("soa", "dense"), ("aos", "sparse"), ("soa", "sparse")):
+        ctx = _ctx(geo, tab, layout=layout, scheme=scheme, capacity=1 << 19, seed=3)
+        for k in range(3):
+            ctx.load_tracks(k, pop[k])
+        compare_counts(ctx.step(), r, what=layout + scheme)
+        for k in range(3):
+            assert compare_tracks(ctx.read_tracks(k), o.read_tracks(k, pop[k].dtype), "%s %s kind %d" % (layout, scheme, k)) == 0
+        ctx.destroy()
+    with pytest.raises(AdeptError):
+        _ctx(geo, tab, layout="soa", scheme="dense", capacity=4096, instrument=True)
+    with pytest.raises(AdeptError):
+        _ctx(geo, tab, layout="soa", scheme="sparse", capacity=4096, flags=1)

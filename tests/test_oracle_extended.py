@@ -1,0 +1,202 @@
+"""Pins of the oracle's extended physics (DESIGN.md rules X35-X37), against
+what the mathematics fixes: the Klein-Nishina energy distribution by quadrature of the textbook
+differential cross-section, the 1/T^2 delta-ray spectrum by its closed-form CDF, exact two-body
+energy-momentum conservation, and the table identities of the restricted stopping power.  CPU only."""
+import math
+
+import numpy as np
+
+from oracle import Oracle
+from workloads import CONFIGS, Geometry, gen_primaries, geometry_for, tables_for
+from workloads.tables import (GROUP_ELEC, MATERIALS, MC2, Q_STOP, build_tables, constant_tables, sigma_delta,
+                              stopping_power)
+from tests.helpers import make_tracks, sort_by_id
+
+E_CUT = 0.1
+
+
+def _isotropic(n, seed):
+    rng = np.random.default_rng(seed)
+    ct = rng.uniform(-1, 1, n)
+    ph = rng.uniform(0, 2 * math.pi, n)
+    d = np.stack([np.sqrt(1 - ct * ct) * np.cos(ph), np.sqrt(1 - ct * ct) * np.sin(ph), ct], 1)
+    return (d / np.linalg.norm(d, axis=1, keepdims=True)).astype(np.float32)
+
+
+def _ks(sample, cdf):
+    """Kolmogorov distance between the empirical distribution of `sample` and `cdf`."""
+    x = np.sort(sample)
+    n = x.shape[0]
+    F = cdf(x)
+    return max(np.max(np.arange(1, n + 1) / n - F), np.max(F - np.arange(0, n) / n))
+
+
+# ------------------------------------------------------------------ X37: Klein-Nishina --------
+def kn_density(eps, kappa):
+    """Klein-Nishina differential cross-section in eps = E'/E (textbook form, unnormalised):
+    d sigma / d eps ~ 1/eps + eps - sin^2(theta), cos(theta) = 1 - (1/eps - 1)/kappa."""
+    t = (1.0 - eps) / (kappa * eps)
+    return 1.0 / eps + eps - t * (2.0 - t)
+
+
+def test_compton_energy_fraction_follows_klein_nishina():
+    """Forced Compton steps under physics = 1: the distribution of eps = E'/E must be the
+    Klein-Nishina one (quadrature of the textbook density: KS distance and mean), which the basic
+    rule's 1/eps spectrum is not; the kinematics stay those of rule S26/S27."""
+    geo = Geometry(n_layers=1, abs_mm=1e3, gap_mm=1.0, half_xy_mm=1e6)
+    n = 60000
+    for E0 in (0.3, 3.0, 30.0):
+        kappa = E0 / MC2
+        eps0 = 1.0 / (1.0 + 2.0 * kappa)
+        grid = np.linspace(eps0, 1.0, 200001)
+        dens = kn_density(grid, kappa)
+        cum = np.concatenate([[0.0], np.cumsum(0.5 * (dens[1:] + dens[:-1]) * np.diff(grid))])
+        mean_kn = float(np.trapezoid(grid * dens, grid) / cum[-1])
+        cdf = lambda x: np.interp(x, grid, cum / cum[-1])
+        dist = {}
+        for physics in (0, 1):
+            tab = constant_tables(16, E_CUT, 100.0, E_CUT, compt=1.0, physics=physics)
+            t = make_tracks(n, pos=(0, 0, 500.0), ekin=E0, nial=(1e6, 1e-30, 1e6))
+            t["dir"] = _isotropic(n, 5)
+            o = Oracle(geo, tab, seed=0)
+            o.load_tracks(2, t)
+            o.step()
+            g = sort_by_id(o.read_tracks(2, t.dtype))
+            eps = g["ekin"].astype(np.float64) / E0
+            assert eps.min() >= eps0 * (1 - 1e-6) and eps.max() <= 1.0
+            if E0 * eps0 >= E_CUT:
+                assert g.shape[0] == n                     # every scattered photon is above the cut
+                dist[physics] = (_ks(eps, cdf), abs(eps.mean() - mean_kn) / eps.std() * math.sqrt(n))
+            # Compton relation between angle and energy (rule S26), from the output directions
+            order = np.argsort(t["id_hi"].astype(np.uint64) << np.uint64(32) | t["id_lo"].astype(np.uint64))
+            par = {(int(a), int(b)): i for i, (a, b) in enumerate(zip(t["id_lo"], t["id_hi"]))}
+            idx = np.array([par[(int(a), int(b))] for a, b in zip(g["id_lo"][:4000], g["id_hi"][:4000])])
+            cth = np.einsum("ij,ij->i", t["dir"][idx].astype(np.float64), g["dir"][:4000].astype(np.float64))
+            want = 1.0 - (1.0 / eps[:4000] - 1.0) / kappa
+            assert np.abs(cth - want).max() < 5e-5
+        if dist:
+            assert dist[1][0] < 1.63 / math.sqrt(n) and dist[1][1] < 4.0       # KS at 1 %, mean within 4 sigma
+            assert dist[0][0] > 5 * dist[1][0]                                   # the 1/eps rule is visibly not KN
+
+
+def test_klein_nishina_rejection_keeps_energy_and_momentum():
+    geo = Geometry(n_layers=1, abs_mm=1e3, gap_mm=1.0, half_xy_mm=1e6)
+    tab = constant_tables(16, E_CUT, 100.0, E_CUT, compt=1.0, physics=1)
+    n, E0 = 20000, 2.0
+    t = make_tracks(n, pos=(0, 0, 500.0), ekin=E0, nial=(1e6, 1e-30, 1e6))
+    t["dir"] = _isotropic(n, 8)
+    o = Oracle(geo, tab, seed=0)
+    o.load_tracks(2, t)
+    o.step()
+    r = o.result()
+    g, el = o.read_tracks(2, t.dtype), o.read_tracks(0, t.dtype)
+    dep = r["edep_slab"].sum()
+    assert abs(g["ekin"].astype(np.float64).sum() + el["ekin"].astype(np.float64).sum() + dep - n * E0) < 1e-6 * n * E0
+    assert np.abs(np.linalg.norm(g["dir"].astype(np.float64), axis=1) - 1).max() < 3e-7
+    assert np.abs(np.linalg.norm(el["dir"].astype(np.float64), axis=1) - 1).max() < 3e-7
+
+
+# ------------------------------------------------------------------ X36: delta rays ------------
+def _delta_step(kind, E0, n, seed):
+    geo = Geometry(n_layers=1, abs_mm=1e3, gap_mm=1.0, half_xy_mm=1e6)
+    tab = constant_tables(16, E_CUT, 100.0, E_CUT, physics=1, delta=1.0, stop=0.0)
+    t = make_tracks(n, pos=(0, 0, 500.0), ekin=E0, nial=(1e6, 1e-30, 1e6))
+    t["dir"] = _isotropic(n, seed)
+    o = Oracle(geo, tab, seed=0)
+    o.load_tracks(kind, t)
+    o.step()
+    return t, o
+
+
+def test_delta_ray_spectrum_and_two_body_kinematics():
+    """Forced delta-ray steps (rule X36) of e- and e+: T follows 1/T^2 on [e_cut, E/2] (closed-form
+    CDF), E' + T = E, and the three momenta close: p(E) d = p(T) d_delta + p(E') d' with
+    p(x)^2 = x (x + 2 mc^2).  The child is an e- at the parent's position, the parent keeps going."""
+    n = 40000
+    p_of = lambda x: np.sqrt(x * (x + 2 * MC2))
+    for kind, E0 in ((0, 5.0), (1, 5.0), (0, 0.5), (0, 800.0)):
+        t, o = _delta_step(kind, E0, n, 21 + kind)
+        r = o.result()
+        assert r["secondaries"][0] == n and r["secondaries"][1] == 0 and r["secondaries"][2] == 0
+        assert r["killed"].sum() == 0 and r["edep_slab"].sum() == 0.0
+        allk = o.read_tracks(0, t.dtype) if kind == 0 else None
+        parents = sort_by_id(o.read_tracks(kind, t.dtype))
+        if kind == 0:                              # parents and children share the e- buffer
+            ids = set(zip(t["id_lo"].tolist(), t["id_hi"].tolist()))
+            is_parent = np.array([(a, b) in ids for a, b in zip(allk["id_lo"].tolist(), allk["id_hi"].tolist())])
+            parents, kids = sort_by_id(allk[is_parent]), allk[~is_parent]
+        else:
+            kids = o.read_tracks(0, t.dtype)
+        assert parents.shape[0] == n and kids.shape[0] == n
+        assert (parents["step"] == 1).all() and (kids["step"] == 0).all() and (kids["nial"] == -1.0).all()
+        assert (parents["nial"][:, 1] == -1.0).all()           # spent: re-sampled at the next step
+        T = kids["ekin"].astype(np.float64)
+        a, b = E_CUT, 0.5 * E0
+        assert T.min() >= a * (1 - 1e-6) and T.max() <= b * (1 + 1e-6)
+        cdf = lambda x: (1 / a - 1 / x) / (1 / a - 1 / b)
+        assert _ks(T, cdf) < 1.63 / math.sqrt(n)
+        # match children to parents through rule R5 (call 2, ordinal 0) and close the kinematics
+        from tests.test_oracle_transport import child_ids
+        ts = sort_by_id(t)
+        lo, hi = child_ids(ts, 0)
+        where = {(int(x), int(y)): i for i, (x, y) in enumerate(zip(lo, hi))}
+        idx = np.array([where[(int(x), int(y))] for x, y in zip(kids["id_lo"], kids["id_hi"])])
+        E1 = parents["ekin"].astype(np.float64)[idx]
+        assert np.abs(E1 + T - E0).max() < 2e-7 * E0
+        d = ts["dir"][idx].astype(np.float64)
+        lhs = p_of(E0) * d
+        rhs = p_of(T)[:, None] * kids["dir"].astype(np.float64) + p_of(E1)[:, None] * parents["dir"][idx].astype(np.float64)
+        # along the parent's direction the balance is tight; across it the rule takes sin from
+        # sqrt(1 - cos^2) in fp32, so a near-forward partner carries an error of ~ p sqrt(ulp): bounded,
+        # and far below that for the bulk (a wrong sign or azimuth would be O(p sin theta) everywhere)
+        miss = lhs - rhs
+        along = np.einsum("ij,ij->i", miss, d)
+        across = np.linalg.norm(miss - along[:, None] * d, axis=1)
+        # (rule S27 divides by sqrt(1 - d.z^2): for parents within a few degrees of the z axis the
+        # rotated polar angle is only good to ~1e-3 relative -- those are held to the loose bound)
+        off_axis = 1.0 - d[:, 2] ** 2 > 1e-2
+        assert np.abs(along[off_axis]).max() < 3e-5 * p_of(E0) + 2e-6
+        assert np.abs(along).max() < 1.5e-3 * p_of(E0)
+        assert across.max() < 1.5e-3 * p_of(E0) and np.median(across) < 1e-4 * p_of(E0)
+        assert (kids["pos"] == parents["pos"][idx]).all() and (kids["vol"] == parents["vol"][idx]).all()   # R6: born where the parent is
+
+
+def test_delta_ray_tables_split_the_collision_loss_exactly():
+    """Sigma_delta is the integral of C/T^2 over [e_cut, T/2], and the restricted stopping power plus
+    the energy carried by the delta rays is the unrestricted one: S_1 + C ln(T / 2 e_cut) = S_0."""
+    for mat in MATERIALS:
+        for T in (0.15, 0.2, 0.25, 1.0, 10.0, 1e3, 1e4):
+            sd = float(sigma_delta(mat, T, E_CUT))
+            s0, s1 = float(stopping_power(mat, T, E_CUT, 0)), float(stopping_power(mat, T, E_CUT, 1))
+            if T <= 2 * E_CUT:
+                assert sd == 0.0 and s0 == s1
+                continue
+            x = np.exp(np.linspace(math.log(E_CUT), math.log(0.5 * T), 20001))
+            gamma = 1 + T / MC2
+            C = 0.5 * 30.7075 * mat.rho * 1e-3 * mat.Z / mat.A / (1 - 1 / gamma ** 2)
+            assert abs(np.trapezoid(C / x ** 2, x) - sd) < 1e-6 * sd
+            assert abs(s1 + np.trapezoid(C / x, x) - s0) < 1e-7 * s0 and s1 > 0
+    tab = build_tables(64, E_CUT, 100.0, E_CUT, physics=1)
+    assert tab.physics == 1 and tab.data_x.shape == (2, 65) and tab.data_x.dtype == np.float32
+    assert (tab.data[:, GROUP_ELEC, Q_STOP] <= build_tables(64, E_CUT, 100.0, E_CUT).data[:, GROUP_ELEC, Q_STOP]).all()
+
+
+def test_extended_physics_conserves_energy_and_is_order_independent():
+    c = CONFIGS["tiny"]
+    geo, tab = geometry_for("tiny"), tables_for("tiny", physics=1)
+    worst = 0.0
+    for ev in range(6):
+        o = Oracle(geo, tab, seed=100 + ev)
+        o.inject(gen_primaries(1, 50.0))
+        o.run()
+        r = o.result()
+        worst = max(worst, abs(r["edep_slab"].sum() + r["e_escaped"] - r["e_injected"]) / r["e_injected"])
+    assert worst < 1e-6
+    a, b = Oracle(geo, tab, seed=c["seed"]), Oracle(geo, tab, seed=c["seed"])
+    prim = gen_primaries(c["n_primaries"], c["e_primary"])
+    a.inject(prim); b.inject(prim)
+    a.run(); b.run(depth_first=True)
+    ra, rb = a.result(), b.result()
+    for k in ("steps", "secondaries", "killed", "escaped_n"):
+        assert (ra[k] == rb[k]).all()
+    assert np.allclose(ra["edep_slab"], rb["edep_slab"], rtol=1e-12, atol=1e-12)

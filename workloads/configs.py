@@ -48,9 +48,10 @@ def geometry_for(name: str) -> Geometry:
 _TABLE_CACHE: dict = {}
 
 
-def tables_for(name: str) -> TableSet:
+def tables_for(name: str, physics: int = 0) -> TableSet:
+    """Tables of a config; physics = 1: the extended rule set (DESIGN.md rules X35-X37)."""
     c = CONFIGS[name]
-    key = (c["n_bins"], c["e_max"])
+    key = (c["n_bins"], c["e_max"], physics)
     if key not in _TABLE_CACHE:
-        _TABLE_CACHE[key] = build_tables(c["n_bins"], E_CUT, c["e_max"], E_CUT)
+        _TABLE_CACHE[key] = build_tables(c["n_bins"], E_CUT, c["e_max"], E_CUT, physics=physics)
     return _TABLE_CACHE[key]

@@ -82,15 +82,38 @@ def sigma_photo(mat: Material, E):
             * SIGMA_THOMSON * (MC2 / E) ** 3.5)
 
 
-def stopping_power(mat: Material, T, e_cut: float):
+def _beta2(T):
+    gamma = 1.0 + np.asarray(T, dtype=np.float64) / MC2
+    return 1.0 - 1.0 / (gamma * gamma)
+
+
+def _delta_prefactor(mat: Material, T):
+    """n Z 2 pi r_e^2 mc^2 / beta^2 [MeV/mm]: prefactor of dSigma/dT_delta = C / T_delta^2."""
+    return 0.5 * K_BB * mat.rho * 1e-3 * (mat.Z / mat.A) / _beta2(T)
+
+
+def sigma_delta(mat: Material, T, e_cut: float):
+    """Rule X36: delta-ray production above the cut, the 1/T^2 term common to Moller and Bhabha
+    scattering, integrated over [e_cut, T/2]; zero for T <= 2 e_cut."""
+    T = np.asarray(T, dtype=np.float64)
+    t_max = np.maximum(0.5 * T, e_cut)
+    return np.where(T > 2.0 * e_cut, _delta_prefactor(mat, T) * (1.0 / e_cut - 1.0 / t_max), 0.0)
+
+
+def stopping_power(mat: Material, T, e_cut: float, physics: int = 0):
     """Restricted stopping power [MeV/mm]: Bethe-Bloch collision term (no
-    density correction) plus the radiative loss to photons below the cut."""
+    density correction) plus the radiative loss to photons below the cut.
+    physics 1 (rule X36): minus the energy carried by the delta rays that are
+    then produced explicitly, int_{e_cut}^{T/2} T' dSigma = C ln(T / (2 e_cut))."""
     T = np.asarray(T, dtype=np.float64)
     gamma = 1.0 + T / MC2
     beta2 = 1.0 - 1.0 / (gamma * gamma)
     I = mat.I_eV * 1e-6
     col = (K_BB * mat.rho * 1e-3 * (mat.Z / mat.A) / beta2
            * (np.log(2.0 * MC2 * beta2 * gamma * gamma / I) - beta2))
+    if physics:
+        col = col - np.where(T > 2.0 * e_cut,
+                             _delta_prefactor(mat, T) * np.log(np.maximum(0.5 * T, e_cut) / e_cut), 0.0)
     return col + e_cut / mat.X0
 
 
@@ -100,12 +123,12 @@ def sigma_brems(mat: Material, T, e_cut: float):
     return np.where(T > e_cut, np.log(np.maximum(T, e_cut) / e_cut) / mat.X0, 0.0)
 
 
-def csda_range(mat: Material, nodes, e_cut: float, panels: int = 32):
+def csda_range(mat: Material, nodes, e_cut: float, panels: int = 32, physics: int = 0):
     """R(T) = e_cut/S(e_cut) + int_{e_cut}^{T} dT'/S(T') on the table nodes,
     composite Simpson in ln T with `panels` panels per bin."""
     nodes = np.asarray(nodes, dtype=np.float64)
     out = np.empty_like(nodes)
-    acc = e_cut / float(stopping_power(mat, e_cut, e_cut))
+    acc = e_cut / float(stopping_power(mat, e_cut, e_cut, physics))
     prev = e_cut
     for i, T in enumerate(nodes):
         if T > prev:
@@ -115,7 +138,7 @@ def csda_range(mat: Material, nodes, e_cut: float, panels: int = 32):
             w[1:-1:2] = 4.0
             w[2:-1:2] = 2.0
             Tx = np.exp(x)
-            acc += float(np.sum(w * Tx / stopping_power(mat, Tx, e_cut))) * (hi - lo) / (6.0 * panels)
+            acc += float(np.sum(w * Tx / stopping_power(mat, Tx, e_cut, physics))) * (hi - lo) / (6.0 * panels)
             prev = T
         out[i] = acc
     return out
@@ -133,13 +156,15 @@ class TableSet:
     inv_dln: np.float32
     nodes: np.ndarray           # float64 [n_bins+1]
     data: np.ndarray            # float32 [mat][group][qty][n_bins+1], C-contiguous
+    physics: int = 0            # rule X35: 0 = basic rules; 1 = delta rays (X36) + Klein-Nishina sampling (X37)
+    data_x: np.ndarray | None = None    # physics 1: float32 [mat][n_bins+1] Sigma_delta of the e+- group
 
     def q(self, mat: int, group: int, qty: int) -> np.ndarray:
         return self.data[mat, group, qty]
 
 
 def build_tables(n_bins: int, e_min: float, e_max: float, e_cut: float,
-                 materials=MATERIALS) -> TableSet:
+                 materials=MATERIALS, physics: int = 0) -> TableSet:
     j = np.arange(n_bins + 1, dtype=np.float64)
     nodes = e_min * (e_max / e_min) ** (j / n_bins)
     nodes[0], nodes[-1] = e_min, e_max
@@ -149,9 +174,12 @@ def build_tables(n_bins: int, e_min: float, e_max: float, e_cut: float,
         data[m, GROUP_GAMMA, Q_COMPT] = sigma_compton(mat, nodes)
         data[m, GROUP_GAMMA, Q_PHOTO] = sigma_photo(mat, nodes)
         data[m, GROUP_ELEC, Q_BREMS] = sigma_brems(mat, nodes, e_cut)
-        data[m, GROUP_ELEC, Q_STOP] = stopping_power(mat, nodes, e_cut)
-        data[m, GROUP_ELEC, Q_RANGE] = csda_range(mat, nodes, e_cut)
-    return TableSet(
+        data[m, GROUP_ELEC, Q_STOP] = stopping_power(mat, nodes, e_cut, physics)
+        data[m, GROUP_ELEC, Q_RANGE] = csda_range(mat, nodes, e_cut, physics=physics)
+    data_x = None
+    if physics:
+        data_x = np.ascontiguousarray(np.stack([sigma_delta(mat, nodes, e_cut) for mat in materials]).astype(np.float32))
+    return TableSet(physics=physics, data_x=data_x,
         n_bins=n_bins, n_materials=len(materials), e_min=e_min, e_max=e_max, e_cut=e_cut,
         ln_e_min=np.float32(math.log(e_min)),
         inv_dln=np.float32(n_bins / math.log(e_max / e_min)),
@@ -160,7 +188,7 @@ def build_tables(n_bins: int, e_min: float, e_max: float, e_cut: float,
 
 def constant_tables(n_bins: int, e_min: float, e_max: float, e_cut: float, *,
                     pair=0.0, compt=0.0, photo=0.0, brems=0.0, stop=0.0, rng=1e30,
-                    n_materials: int = 2) -> TableSet:
+                    n_materials: int = 2, physics: int = 0, delta=0.0) -> TableSet:
     """Energy-independent tables for closed-form checks (pure absorber,
     vacuum-like geometry tests, brems-only slabs)."""
     j = np.arange(n_bins + 1, dtype=np.float64)
@@ -172,6 +200,7 @@ def constant_tables(n_bins: int, e_min: float, e_max: float, e_cut: float, *,
     data[:, GROUP_ELEC, Q_BREMS] = brems
     data[:, GROUP_ELEC, Q_STOP] = stop
     data[:, GROUP_ELEC, Q_RANGE] = rng
+    data_x = np.full((n_materials, n_bins + 1), delta, dtype=np.float32) if physics else None
     return TableSet(n_bins, n_materials, e_min, e_max, e_cut,
                     np.float32(math.log(e_min)), np.float32(n_bins / math.log(e_max / e_min)),
-                    nodes, data)
+                    nodes, data, physics, data_x)
