@@ -49,9 +49,9 @@ static const LayoutOps *ops_for(int layout) {
     case ADEPT_AOS: return &kOpsAoS;
     case ADEPT_SOA: return &kOpsSoA;
     case ADEPT_AOSOA32: return &kOpsAoSoA32;
-#ifndef ADEPT_FEW_LAYOUTS   // experiment builds instantiate the three paper layouts only
-    case ADEPT_AOSOA64: return &kOpsAoSoA64;
     case ADEPT_SOA16: return &kOpsSoA16;
+#ifndef ADEPT_FEW_LAYOUTS   // experiment builds instantiate four layouts only
+    case ADEPT_AOSOA64: return &kOpsAoSoA64;
     case ADEPT_AOSOA16: return &kOpsAoSoA16;
     case ADEPT_AOSOA128: return &kOpsAoSoA128;
 #endif
@@ -393,7 +393,7 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
   const int instr = cfg->instrument ? 1 : 0;
   const size_t tile_words = c->ops->record_words(kGroup);
   c->small.threads = kBlockSmall;
-  c->small.dyn_smem = step_smem_bytes(cfg->scheme, pl.table_bytes / 2, p.n_slabs, tile_words, kBlockSmall);
+  c->small.dyn_smem = step_smem_bytes(cfg->scheme, pl.table_bytes / 2, p.n_slabs, tile_words, kBlockSmall, c->ops->sparse_gather);
   const int per_sm = c->ops->step_ctas_per_sm(cfg->scheme, instr, variant, kBlockSmall, c->small.dyn_smem);
   if (per_sm <= 0) {
     g_create_error = "step kernel does not fit on an SM with these tables (shared memory)";
@@ -402,7 +402,7 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
   }
   c->small.grid = static_cast<unsigned>(sms * per_sm);
   c->large.threads = kBlockLarge;
-  c->large.dyn_smem = step_smem_bytes(cfg->scheme, pl.table_bytes / 2, p.n_slabs, tile_words, kBlockLarge);
+  c->large.dyn_smem = step_smem_bytes(cfg->scheme, pl.table_bytes / 2, p.n_slabs, tile_words, kBlockLarge, c->ops->sparse_gather);
   const int per_sm_large = c->ops->step_ctas_per_sm(cfg->scheme, instr, variant, kBlockLarge, c->large.dyn_smem);
   cudaGetLastError();  // a failed attribute query of the optional shape is not an error of the context
   c->large.grid = per_sm_large > 0 ? static_cast<unsigned>(sms * per_sm_large) : 0u;

@@ -40,11 +40,17 @@ constexpr int kQueueCap = 2 * kGroup;
 // 64 bytes, written and read as 64-bit words (7 or 8 shared-memory instructions, conflict-free).
 __host__ __device__ constexpr int queue_words(int scheme) { return scheme == S_DENSE ? 14 : 16; }
 __host__ __device__ constexpr size_t queue_bytes(int scheme) { return size_t(kQueueCap) * queue_words(scheme) * 4; }
-// Dense scheme: one tile staged in shared memory by TMA (record_words(kGroup) words of the layout).
-// The sparse scheme stages nothing: its kernels leave the rest of the SM's memory to L1 (measured:
-// the scattered 16-byte pieces of AoS records depend on it -- DESIGN.md §10).
-__host__ __device__ constexpr size_t in_buf_bytes(int scheme, size_t tile_words) {
-  return scheme == S_DENSE ? tile_words * 4 : 0;
+// One tile of records staged in shared memory per group (record_words(kGroup) words of the layout):
+// dense scheme, by TMA bulk / tiled copies of the contiguous tile; sparse scheme, by per-thread
+// asynchronous copies (cp.async) of the records the group's list entries name, followed by two words
+// per thread -- the slot of the gathered record and the thread's list entry for the tile after it,
+// which also arrives by cp.async.  Both schemes fetch one tile ahead of the tile being stepped.
+// `gather`: the layout keeps a record's words in 16-byte pieces (layout.cuh Mapping<L>::kSparseGather);
+// the word-by-word layouts load their records directly and stage nothing (measured: 14 four-byte
+// asynchronous copies per record and the L1 capacity given up for the staging buffer cost them more
+// than the latency they hide -- DESIGN.md §10).
+__host__ __device__ constexpr size_t in_buf_bytes(int scheme, size_t tile_words, bool gather) {
+  return scheme == S_DENSE ? tile_words * 4 : (gather ? tile_words * 4 + 2 * size_t(kGroup) * 4 : 0);
 }
 // Tally bins of a CTA: per slab (+ one bin for the energy carried out of the calorimeter) a 64-bit
 // fixed-point sum kept as two 32-bit limbs, [lo limbs][hi limbs].
@@ -55,8 +61,8 @@ __host__ __device__ constexpr size_t units_offset(size_t table_bytes, uint32_t n
   return (table_bytes + bins_bytes(n_slabs) + 127) / 128 * 128;
 }
 __host__ __device__ constexpr size_t step_smem_bytes(int scheme, size_t table_bytes, uint32_t n_slabs, size_t tile_words,
-                                                     int threads) {
-  return units_offset(table_bytes, n_slabs) + size_t(threads / kGroup) * (in_buf_bytes(scheme, tile_words) + queue_bytes(scheme));
+                                                     int threads, bool gather) {
+  return units_offset(table_bytes, n_slabs) + size_t(threads / kGroup) * (in_buf_bytes(scheme, tile_words, gather) + queue_bytes(scheme));
 }
 
 // Energy tallies (rule M7: sums of fp32 terms) are accumulated in 64-bit fixed point, unit

@@ -70,18 +70,23 @@ __device__ __forceinline__ void trk_set_word(Trk &t, int f, uint32_t w) {
 // Capacities are multiples of 128 slots (one tile), so every SoA field array and every AoSoA block
 // starts on a 128-byte line.
 template <int L> struct Mapping;
+// Mapping<L>::kSparseGather: the sparse scheme fetches this layout's records one tile ahead by
+// asynchronous 16-byte copies (step_impl.cuh gather_record); false = direct loads.
 
 template <> struct Mapping<L_AOS> {  // 14 words padded to 16: one record = 64 B = 2 sectors = 4 x 16 B
   static constexpr int kStride = 16;
+  static constexpr bool kSparseGather = true;
   __host__ __device__ static constexpr size_t words(size_t cap) { return cap * kStride; }
   __host__ __device__ static constexpr size_t index(size_t, size_t slot, int f) { return slot * kStride + f; }
 };
 template <> struct Mapping<L_SOA> {  // 14 arrays of `cap` words
+  static constexpr bool kSparseGather = false;
   __host__ __device__ static constexpr size_t words(size_t cap) { return cap * kNumFields; }
   __host__ __device__ static constexpr size_t index(size_t cap, size_t slot, int f) { return f * cap + slot; }
 };
 template <int N> struct AoSoAMapping {  // blocks of N tracks, field-major inside a block (N * 56 B)
   static constexpr int kLanes = N;
+  static constexpr bool kSparseGather = false;
   __host__ __device__ static constexpr size_t words(size_t cap) { return cap * kNumFields; }
   __host__ __device__ static constexpr size_t index(size_t, size_t slot, int f) {
     return (slot / kLanes) * (kLanes * kNumFields) + f * kLanes + (slot % kLanes);
@@ -97,6 +102,7 @@ template <> struct Mapping<L_AOSOA128> : AoSoAMapping<128> {};  // one block per
 // {id_hi, step} (8 B) -- so that a record moves with four vector instructions instead of fourteen and
 // consecutive slots are consecutive vectors.
 template <> struct Mapping<L_SOA16> {
+  static constexpr bool kSparseGather = false;  // measured: faster only above ~80 % occupancy
   __host__ __device__ static constexpr size_t words(size_t cap) { return cap * kNumFields; }
   __host__ __device__ static constexpr size_t index(size_t cap, size_t slot, int f) {
     return (f < 12) ? size_t(f / 4) * 4 * cap + slot * 4 + (f % 4) : 12 * cap + slot * 2 + (f - 12);

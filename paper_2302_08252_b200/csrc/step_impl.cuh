@@ -222,6 +222,76 @@ template <int L> __device__ __forceinline__ Trk staged_load(const uint32_t *in_b
   return t;
 }
 
+// ---- asynchronous record gather (sparse scheme) --------------------------------------------------
+// The slot list is dense, the records it names are not.  One tile ahead of the tile being stepped,
+// every thread copies the record of ITS next list entry into the group's staging buffer with cp.async,
+// and its list entry for the tile after that into a stash word -- no register holds a value that is
+// still in flight, so nothing waits for a load until the tile is reached (cp.async.wait_group).
+//   AoS: four lanes fetch one 64-byte record (lane l: piece l & 3 of the record of lane 8 j + (l >> 2),
+//        j = 0..3), so that a warp's copy asks for 8 whole records = whole sectors; the pieces land
+//        record-major with the 64-byte swizzle of the dense tiles (staged_load<L_AOS> undoes it).
+//   The other layouts load their records directly (Mapping<L>::kSparseGather = false): for SoA / AoSoA-n
+//        a record is 14 scattered words -- the sector amplification the paper reports (PAPER.md:111,
+//        145) -- and 14 four-byte copies plus the L1 capacity given up for the staging buffer cost more
+//        than the latency they hide; SoA16 gains only above ~80 % occupancy.
+constexpr uint32_t kNoSlot = 0xFFFFFFFFu;
+__device__ __forceinline__ void cp_async_16(uint32_t smem_dst, const void *gmem_src) {  // .cg: not kept in L1
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_dst), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_4(uint32_t smem_dst, const void *gmem_src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_dst), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+// `slot` = kNoSlot for a thread without a list entry (ragged last tile).  Called by whole warps.
+template <int L>
+__device__ __forceinline__ void gather_record(const uint32_t *rec, uint32_t cap, uint32_t slot, uint32_t *in_buf, int gtid) {
+  const uint32_t row = static_cast<uint32_t>(__cvta_generic_to_shared(in_buf));
+  if constexpr (L == L_AOS) {
+    const int lane = gtid & 31, piece = lane & 3;
+    const uint32_t warp_row = uint32_t(gtid & ~31);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const int src = 8 * j + (lane >> 2);
+      const uint32_t s_src = __shfl_sync(0xFFFFFFFFu, slot, src);
+      const uint32_t dst_row = row + (warp_row + uint32_t(src)) * 64u;
+      const uint32_t sw = ((dst_row >> 7) & 3u) << 4;
+      if (s_src != kNoSlot)
+        cp_async_16(dst_row + ((uint32_t(piece) << 4) ^ sw), rec + size_t(s_src) * Mapping<L>::kStride + piece * 4);
+    }
+  } else {  // generic form (no layout uses it today: the word-by-word layouts load directly)
+    if (slot != kNoSlot) {
+#pragma unroll
+      for (int f = 0; f < kNumFields; ++f)
+        cp_async_4(row + uint32_t(f * kGroup + gtid) * 4u, rec + Mapping<L>::index(cap, slot, f));
+    }
+  }
+}
+// The thread's gathered record out of the staging buffer.
+template <int L> __device__ __forceinline__ Trk gathered_load(const uint32_t *in_buf, int gtid) {
+  if constexpr (L == L_AOS) return staged_load<L>(in_buf, gtid);
+  Trk t;
+#pragma unroll
+  for (int f = 0; f < kNumFields; ++f) trk_set_word(t, f, in_buf[f * kGroup + gtid]);
+  return t;
+}
+// Issue the gather of the record in `slot` (this thread's entry of tile `tile_next`), remember the slot,
+// and fetch the thread's list entry of the tile after that into the stash.  stash = in_buf + tile words:
+// [0][gtid] slot of the gathered record, [1][gtid] list entry of the following tile.
+template <int L>
+__device__ __forceinline__ void gather_ahead(const Params &p, int kind, uint32_t par, uint32_t slot, uint32_t i_after,
+                                             uint32_t n_kind, uint32_t *in_buf, int gtid) {
+  uint32_t *stash = in_buf + Mapping<L>::words(kGroup);
+  gather_record<L>(p.kind[kind].rec[0], p.capacity, slot, in_buf, gtid);
+  stash[gtid] = slot;
+  if (i_after < n_kind)
+    cp_async_4(static_cast<uint32_t>(__cvta_generic_to_shared(stash + kGroup + gtid)), p.kind[kind].queue[par] + i_after);
+  else
+    stash[kGroup + gtid] = kNoSlot;
+  cp_async_commit();
+}
+
 template <int L, bool INSTR>
 __device__ __forceinline__ TrackView<L, INSTR> make_view(const Params &p, int kind, int buf, uint32_t *cta_probe) {
   TrackView<L, INSTR> v;
@@ -404,7 +474,8 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
   // A1: load
   c.clk->mark(SEC_OTHER);
   uint32_t slot = i;
-  if (SCHEME == S_SPARSE && active) slot = p.kind[KIND].queue[par][i];
+  constexpr bool kGather = SCHEME == S_SPARSE && Mapping<L>::kSparseGather;
+  if (SCHEME == S_SPARSE && !kGather && active) slot = p.kind[KIND].queue[par][i];
   const TrackView<L, INSTR> cur = make_view<L, INSTR>(p, KIND, (SCHEME == S_DENSE) ? int(par) : 0, c.cta->probe);
   Trk t, old;
   uint32_t vol_before = 0u;
@@ -424,11 +495,23 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
         prefetch_tile<L>(p, KIND, par, next_tile, n_kind, c.in_buf, &g.mbar_in);
     }
   }
-  // sparse scheme: plain loads of the record the list entry names (no shared-memory staging: the
-  // sparse kernels leave the SM's memory to L1, which the scattered record pieces hit in)
-  if (SCHEME == S_SPARSE && active) t = cur.load(slot);
+  if constexpr (kGather) {  // the record was gathered into the staging buffer one tile ago (gather_ahead)
+    uint32_t *stash = c.in_buf + Mapping<L>::words(kGroup);
+    cp_async_wait_all();
+    if (L == L_AOS) __syncwarp();  // the pieces of a record were copied by four lanes of the warp
+    slot = stash[gtid];
+    const uint32_t s_next = stash[kGroup + gtid];
+    if (active) t = gathered_load<L>(c.in_buf, gtid);
+    if (next_tile != 0xFFFFFFFFu) {
+      if (L == L_AOS) __syncwarp();  // every lane has read its record: the rows may be refilled
+      const uint32_t i_after = (2u * next_tile - tile) * kGroup + gtid;  // next_tile - tile = groups of the grid
+      gather_ahead<L>(p, KIND, par, s_next, i_after, n_kind, c.in_buf, gtid);
+    }
+  } else if (SCHEME == S_SPARSE && active) {
+    t = cur.load(slot);  // word-by-word layouts: plain loads of the record the list entry names
+  }
   if (active) {
-    if (INSTR && SCHEME == S_DENSE) {
+    if (INSTR && (SCHEME == S_DENSE || kGather)) {
 #pragma unroll
       for (int f = 0; f < kNumFields; ++f) cur.probe(f, 0, slot);
     }
@@ -709,6 +792,11 @@ __device__ __forceinline__ void run_kind(const Params &p, const Env &env, const 
   // (small populations -- the head and tail of a shower -- are latency-bound, one tile per group)
   if (SCHEME == S_DENSE && shift < n_tiles && c.gtid == 0)  // the staging buffer is free: its last reader passed a barrier
     prefetch_tile<L>(p, KIND, par, shift, n_kind, c.in_buf, &c.g->mbar_in);
+  if (SCHEME == S_SPARSE && Mapping<L>::kSparseGather && shift < n_tiles) {  // each thread: its record of the first tile, its list entry of the second
+    const uint32_t i0 = shift * kGroup + c.gtid;
+    const uint32_t slot0 = (i0 < n_kind) ? __ldg(&p.kind[KIND].queue[par][i0]) : kNoSlot;
+    gather_ahead<L>(p, KIND, par, slot0, i0 + n_groups * kGroup, n_kind, c.in_buf, c.gtid);
+  }
   // A3: the cross-section tables of this kind's particle group -> shared memory, one TMA bulk copy
   // (e- and e+ share a group).  CTA-wide: every group is done with the previous tables.
   constexpr int group = (KIND == K_GAMMA) ? 0 : 1;
@@ -758,7 +846,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == kBlockSmall) ? ADEPT_STEP
   float4 *s_tab = reinterpret_cast<float4 *>(dyn_smem);
   const int tid = threadIdx.x;
   Ctl *ctl = p.ctl;
-  constexpr size_t kInBuf = in_buf_bytes(SCHEME, Mapping<L>::words(kGroup));
+  constexpr size_t kInBuf = in_buf_bytes(SCHEME, Mapping<L>::words(kGroup), Mapping<L>::kSparseGather);
   constexpr size_t kPerGroup = kInBuf + queue_bytes(SCHEME);
   GroupRefs c;
   c.cta = &sh;
@@ -976,6 +1064,7 @@ __global__ void read_kernel(const __grid_constant__ Params p, PackedTrack *dst, 
 // scheme and instrumentation are compile-time parameters of every kernel.)
 struct LayoutOps {
   size_t (*record_words)(size_t capacity);
+  bool sparse_gather;  // Mapping<L>::kSparseGather
   int (*step_ctas_per_sm)(int scheme, int instr, int variant, int threads, size_t dyn_smem);
   cudaError_t (*launch_step)(int scheme, int instr, const Params &, int threads, unsigned grid, size_t dyn_smem,
                              cudaStream_t);  // Params::recycle / physics pick the kernel variant
@@ -1073,7 +1162,7 @@ template <int L> struct OpsImpl {
     return cudaGetLastError();
   }
   static LayoutOps make() {
-    return LayoutOps{record_words, step_ctas_per_sm, launch_step, launch_inject, launch_load, launch_read};
+    return LayoutOps{record_words, Mapping<L>::kSparseGather, step_ctas_per_sm, launch_step, launch_inject, launch_load, launch_read};
   }
 };
 
