@@ -50,7 +50,8 @@ __host__ __device__ constexpr size_t queue_bytes(int scheme) { return size_t(kQu
 // asynchronous copies per record and the L1 capacity given up for the staging buffer cost them more
 // than the latency they hide -- DESIGN.md §10).
 __host__ __device__ constexpr size_t in_buf_bytes(int scheme, size_t tile_words, bool gather) {
-  return scheme == S_DENSE ? tile_words * 4 : (gather ? tile_words * 4 + 2 * size_t(kGroup) * 4 : 0);
+  // sparse, direct loads: only the two stash words per thread (list entries of the next two tiles)
+  return scheme == S_DENSE ? tile_words * 4 : (gather ? tile_words * 4 : 0) + 2 * size_t(kGroup) * 4;
 }
 // Tally bins of a CTA: per slab (+ one bin for the energy carried out of the calorimeter) a 64-bit
 // fixed-point sum kept as two 32-bit limbs, [lo limbs][hi limbs].
