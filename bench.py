@@ -400,6 +400,17 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
             for name in ("full", "heavy") if "heavy" in args.extras else ("full",):
                 out["showers"][name] = showers(args, name, layout=main, scheme="dense", steps=3, warmup=1,
                                                with_cpu=not args.no_cpu)
+            # the paper's default container on the same workloads: sparse single buffer, AoS, with slot
+            # recycling (without it config 5 needs ~5.7e7 e- slots, SURVEY.md:583); parity against the
+            # oracle result already computed above
+            for name in ("full", "heavy") if "heavy" in args.extras else ("full",):
+                b = showers(args, name, layout="aos", scheme="sparse", steps=3, warmup=1, with_cpu=False, flags=1)
+                ref = out["showers"][name]
+                b["same_counts_as_dense"] = bool(b["track_steps"] == ref["track_steps"] and b["iterations"] == ref["iterations"]
+                                                 and b["secondaries"] == ref["secondaries"])
+                b["edep_layer_rel_diff_to_dense"] = float(np.max(np.abs(np.array(b["edep_layer_MeV"]) - np.array(ref["edep_layer_MeV"]))
+                                                                 / np.maximum(np.array(ref["edep_layer_MeV"]), 1e-30)))
+                out["showers"][name + "_sparse_recycle"] = b
         if "sweep" in args.extras:
             out["sweep"] = sweep(args, layouts=("aos", "soa", "aosoa32"), steps=5, warmup=3, instr=False, sections=True)
     print(json.dumps(out))
@@ -569,12 +580,14 @@ def sweep(args, *, layouts, steps, warmup, instr, sections, occupancies=None, sc
                         n_sec = int(res["secondaries"].sum())
                         n_surv = int(res["live"].sum()) - n_sec
                         nbytes = sweep_bytes(scheme, layout, n_live, n_surv, n_sec)
+                        traffic, traffic_src = ncu_traffic("sweep_%g" % occ, layout, scheme)
                         cell.update(ms_per_step=t, ms_min=float(np.min(ms)), track_steps_per_s=n_live / (t * 1e-3),
                                     secondaries=[int(x) for x in res["secondaries"]],
                                     slots_used=[int(x) for x in res["slots_used"]],
                                     algorithmic_bytes=nbytes,
                                     roofline={"bound": "hbm", "achieved": nbytes / (t * 1e-3) / 1e9, "peak": peak,
-                                              "unit": "GB/s", "frac": nbytes / (t * 1e-3) / 1e9 / peak})
+                                              "unit": "GB/s", "frac": nbytes / (t * 1e-3) / 1e9 / peak,
+                                              "traffic": traffic, "traffic_source": traffic_src})
                     elif what == "sections":
                         ctx.step()
                         cyc = ctx.read_sections().astype(np.float64)[:len(SECTION_NAMES)]

@@ -872,3 +872,31 @@ def test_extended_physics_single_step_population_and_validation():
         _ctx(geo, tab, layout="soa", scheme="dense", capacity=4096, instrument=True)
     with pytest.raises(AdeptError):
         _ctx(geo, tab, layout="soa", scheme="sparse", capacity=4096, flags=1)
+
+
+# ------------------------------------------------------------------ timing variant -----------------
+def test_timing_variant_computes_the_same_and_fills_its_section_clocks():
+    """libadept_b200_timing.so (-DADEPT_TIMING_SECTIONS, include/adept.h): same results as the plain
+    library, and the per-section warp-cycle sums bench.py's sweep reads are there."""
+    from paper_2302_08252_b200 import lib
+    assert lib().adept_timing_sections() == 0 and lib("timing").adept_timing_sections() == 1
+    pop = gen_sweep(0.3, span=1 << 16)
+    geo, tab = geometry_for("sweep"), tables_for("sweep")
+    for scheme in SCHEMES:
+        res = []
+        for variant in (None, "timing"):
+            ctx = _ctx(geo, tab, layout="aosoa32", scheme=scheme, capacity=1 << 17, seed=4, variant=variant)
+            for k in range(3):
+                ctx.load_tracks(k, pop[k]["tracks"], pop[k]["slots"] if scheme == "sparse" else None)
+            counts = ctx.step()
+            sec = ctx.read_sections()
+            res.append((counts, ctx.result(), [sort_by_id(ctx.read_tracks(k)) for k in range(3)], sec))
+            ctx.destroy()
+        compare_counts(res[0][0], res[1][0])
+        assert (res[0][1]["edep_slab"] == res[1][1]["edep_slab"]).all()
+        for a, b in zip(res[0][2], res[1][2]):
+            assert (a.view(np.uint8) == b.view(np.uint8)).all()
+        assert res[0][3].sum() == 0                                   # the plain library keeps no clocks
+        s = res[1][3]
+        assert (s[1:6] > 0).all() and s[4] + s[5] < s[:6].sum()       # load, move, interact, alloc, store all ran
+        assert s[6] > 0 and s[7] > 0                                  # launch timeline (ns)
