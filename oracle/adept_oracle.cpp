@@ -25,7 +25,7 @@
 // the next slab boundary, applies continuous energy loss and discrete
 // interactions, emits secondaries"; Philox-4x32 keyed by (track id, step, draw
 // index)).  Every point on which those two sources are silent is a numbered
-// reading in DESIGN.md §3 (rules R1-R6, M7-M11, T12-T14, S16-S31, X35-X37); the code
+// reading in DESIGN.md §3 (rules R1-R6, M7-M11, T12-T14, S16-S31, X35-X38); the code
 // below follows those rules one by one, in their order and notation, with no
 // blocking, fusion or reordering.
 //
@@ -37,10 +37,10 @@
 // per-event energy conservation; <T(x)> = T0 exp(-x/X0) for brems; Compton
 // energy-momentum conservation and Compton edge; CSDA range; pair/photo
 // branch energies; lockstep == depth-first order independence.
-// Extended physics (tables.physics = 1; DESIGN.md rules X35-X37, SURVEY.md
-// §8(f) item 3): delta-ray production on nial[1] of e+- (X36) and the Compton
+// Extended physics (tables.physics = 1; DESIGN.md rules X35-X38, SURVEY.md
+// §8(f) item 3): delta-ray production on nial[1] of e+- (X36), the Compton
 // energy fraction from the full Klein-Nishina distribution by composition and
-// rejection (X37).  Pins (tests/test_oracle_extended.py): the eps distribution
+// rejection (X37), annihilation in flight on nial[2] of e+ (X38).  Pins (tests/test_oracle_extended.py): the eps distribution
 // against quadrature of the textbook Klein-Nishina density (KS distance, mean);
 // the delta-ray energy against the closed-form 1/T^2 CDF; exact two-body
 // energy-momentum closure; S_restricted + int T dSigma_delta = S; per-event
@@ -87,7 +87,7 @@ struct TablesIn {          // as passed over the C interface
   float e_min, e_max, ln_e_min, inv_dln, e_cut;
   const float *data;       // [mat][group][qty][n_bins+1]
   uint32_t physics;        // rule X35: 0 = rules S16-S32, 1 = with the extended rules X36, X37
-  const float *data_x;     // physics 1: [mat][n_bins+1] Sigma_delta [1/mm] of the e+- group
+  const float *data_x;     // physics 1: [mat][2][n_bins+1]: Sigma_delta of e+- (X36), Sigma_annihilation of e+ (X38) [1/mm]
 };
 
 struct Result {
@@ -218,7 +218,7 @@ struct Tables {
   const float *q(uint32_t mat, int group, int qty) const {
     return data.data() + ((size_t)(mat * 2 + group) * 3 + qty) * (n_bins + 1);
   }
-  const float *qx(uint32_t mat) const { return data_x.data() + (size_t)mat * (n_bins + 1); }
+  const float *qx(uint32_t mat, int which) const { return data_x.data() + ((size_t)mat * 2 + which) * (n_bins + 1); }
 };
 
 struct Bin { int j; float f; };
@@ -358,7 +358,8 @@ bool step_track(Oracle &o, int kind, Track &t, Child children[2], int &n_childre
   }
 
   const bool extended = tab.physics == 1u;                       // X35
-  const int NP = (kind == KIND_GAMMA) ? 3 : (extended ? 2 : 1);  // X36: e+- process 1 = delta-ray production
+  // X36: e+- process 1 = delta-ray production; X38: e+ process 2 = annihilation in flight
+  const int NP = (kind == KIND_GAMMA) ? 3 : (extended ? (kind == KIND_EP ? 3 : 2) : 1);
   const int group = (kind == KIND_GAMMA) ? GROUP_GAMMA : GROUP_ELEC;
 
   // S18: re-sample spent interaction lengths.
@@ -373,7 +374,7 @@ bool step_track(Oracle &o, int kind, Track &t, Child children[2], int &n_childre
   float sig[3] = {0.0f, 0.0f, 0.0f};
   float sj[3] = {INF, INF, INF};
   for (int j = 0; j < NP; ++j) {
-    sig[j] = (kind != KIND_GAMMA && j == 1) ? interp(tab.qx(mat), bin)   // X36: Sigma_delta
+    sig[j] = (kind != KIND_GAMMA && j >= 1) ? interp(tab.qx(mat, j - 1), bin)   // X36: Sigma_delta, X38: Sigma_annihilation
                                             : interp(tab.q(mat, group, j), bin);
     sj[j] = (sig[j] > 0.0f) ? t.nial[j] / sig[j] : INF;
   }
@@ -471,7 +472,44 @@ bool step_track(Oracle &o, int kind, Track &t, Child children[2], int &n_childre
   } else if (w != W_ELOSS) {
     // S26: discrete interaction of process w.
     t.nial[w] = -1.0f;
-    if (kind != KIND_GAMMA && w == 1) {
+    if (kind == KIND_EP && w == 2) {
+      // X38: annihilation in flight on an electron at rest: two photons, isotropic in the centre-of-
+      // momentum frame, boosted to the laboratory; the positron dies
+      const float E = t.ekin;
+      const float e_tot = E + o.two_mc2;
+      const float pp = sqrtf(E * e_tot);                   // positron momentum, p^2 = E (E + 2 mc^2)
+      const float beta = pp / e_tot;                       // velocity of the centre of momentum
+      const float cs = 1.0f - 2.0f * rng.u(1, 2);
+      const float k1 = (0.5f * e_tot) * fmaf(beta, cs, 1.0f);
+      const float k2 = e_tot - k1;
+      float c1 = (cs + beta) / fmaf(beta, cs, 1.0f);
+      if (c1 > 1.0f) c1 = 1.0f;
+      if (c1 < -1.0f) c1 = -1.0f;
+      const float s1 = sqrtf(fmaf(-c1, c1, 1.0f));
+      float sphi, cphi;
+      sincos2pi(rng.u(1, 3), &sphi, &cphi);
+      float d1[3];
+      rotate(t.dir, s1, c1, sphi, cphi, d1);
+      float q[3];
+      for (int c = 0; c < 3; ++c) q[c] = fmaf(pp, t.dir[c], -(k1 * d1[c]));
+      const float qn = sqrtf(fmaf(q[0], q[0], fmaf(q[1], q[1], q[2] * q[2])));
+      note_margin(margin, k1, e_cut);
+      if (k1 >= e_cut) {
+        children[n_children].kind = KIND_GAMMA; children[n_children].t = make_child(t, rng, 0, d1, k1);
+        ++n_children;
+      } else {
+        deposit(vol0, k1);
+      }
+      note_margin(margin, k2, e_cut);
+      if (k2 >= e_cut && qn > 0.0f) {
+        const float d2[3] = {q[0] / qn, q[1] / qn, q[2] / qn};
+        children[n_children].kind = KIND_GAMMA; children[n_children].t = make_child(t, rng, 1, d2, k2);
+        ++n_children;
+      } else {
+        deposit(vol0, k2);
+      }
+      return finish(false);
+    } else if (kind != KIND_GAMMA && w == 1) {
       // X36: delta-ray production (the 1/T^2 term common to Moller and Bhabha scattering) on
       // [e_cut, E/2], two-body kinematics on a free electron at rest
       const float E = t.ekin;
@@ -723,7 +761,7 @@ orc_ctx *orc_create(const Geometry *g, const TablesIn *tin, uint64_t seed) {
   o->tab.data.assign(tin->data, tin->data + (size_t)tin->n_materials * 6 * (tin->n_bins + 1));
   o->tab.physics = tin->physics;
   if (tin->physics > 1u || (tin->physics == 1u && !tin->data_x)) { delete o; return nullptr; }
-  if (tin->physics == 1u) o->tab.data_x.assign(tin->data_x, tin->data_x + (size_t)tin->n_materials * (tin->n_bins + 1));
+  if (tin->physics == 1u) o->tab.data_x.assign(tin->data_x, tin->data_x + (size_t)tin->n_materials * 2 * (tin->n_bins + 1));
   o->seed = seed;
   o->pitch = g->abs_mm + g->gap_mm;
   o->two_mc2 = 2.0f * o->mc2;

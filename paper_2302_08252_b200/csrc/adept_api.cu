@@ -72,7 +72,8 @@ static bool make_plan(const adept_geometry *g, const adept_tables *t, const adep
   pl.capacity = (c->capacity_per_kind + 127u) / 128u * 128u;
   pl.nbuf = (c->scheme == ADEPT_DENSE_DOUBLE) ? 2 : 1;
   pl.rec_words = ops->record_words(pl.capacity);
-  pl.table_bytes = size_t(t->n_materials) * 2 * (t->n_bins + 1) * sizeof(float4);
+  // device tables: group 0 = gamma, 1 = e+-, and under the extended physics 2 = e+ extras (rule X38)
+  pl.table_bytes = size_t(t->n_materials) * (t->physics ? 3 : 2) * (t->n_bins + 1) * sizeof(float4);
   pl.stage_records = std::min<uint32_t>(pl.capacity, kStageRecords);
   size_t off = 0;
   // control header, tallies (per slab + escaped), section clocks of the timing build
@@ -326,7 +327,10 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
   if (t->physics == 1u)  // X36: Sigma_delta in the fourth lane of the e+- group
     for (uint32_t m = 0; m < t->n_materials; ++m)
       for (uint32_t j = 0; j < nodes; ++j)
-        packed[((size_t(1) * t->n_materials + m) * nodes + j) * 4 + 3] = t->data_x[size_t(m) * nodes + j];
+      {  // data_x[mat][2][node]: Sigma_delta -> fourth lane of the e+- group, Sigma_annihilation -> first lane of group 2
+        packed[((size_t(1) * t->n_materials + m) * nodes + j) * 4 + 3] = t->data_x[(size_t(m) * 2 + 0) * nodes + j];
+        packed[((size_t(2) * t->n_materials + m) * nodes + j) * 4 + 0] = t->data_x[(size_t(m) * 2 + 1) * nodes + j];
+      }
   if ((e = cudaMemcpyAsync(c->ws + pl.tables, packed.data(), pl.table_bytes, cudaMemcpyHostToDevice, c->stream)) != cudaSuccess)
     return die("cudaMemcpyAsync(tables)", e);
   if ((e = cudaStreamSynchronize(c->stream)) != cudaSuccess) return die("cudaStreamSynchronize", e);
@@ -336,7 +340,8 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
   p.tally = reinterpret_cast<unsigned long long *>(c->ws + pl.ctl + kCtlHeaderBytes);
   p.sections = p.tally + (size_t(2) * g->n_layers + 1);
   p.tables = reinterpret_cast<const float4 *>(c->ws + pl.tables);
-  p.table_bytes = static_cast<uint32_t>(pl.table_bytes / 2);  // per particle group
+  p.table_bytes = static_cast<uint32_t>(size_t(t->n_materials) * nodes * sizeof(float4));  // per particle group
+  p.table_area = p.table_bytes * (t->physics ? 2u : 1u);
   p.nodes = nodes;
   p.ln_e_min = t->ln_e_min; p.inv_dln = t->inv_dln; p.e_cut = t->e_cut; p.e_max = t->e_max;
   p.n_slabs = 2 * g->n_layers;
@@ -393,7 +398,7 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
   const int instr = cfg->instrument ? 1 : 0;
   const size_t tile_words = c->ops->record_words(kGroup);
   c->small.threads = kBlockSmall;
-  c->small.dyn_smem = step_smem_bytes(cfg->scheme, pl.table_bytes / 2, p.n_slabs, tile_words, kBlockSmall, c->ops->sparse_gather);
+  c->small.dyn_smem = step_smem_bytes(cfg->scheme, p.table_area, p.n_slabs, tile_words, kBlockSmall, c->ops->sparse_gather);
   const int per_sm = c->ops->step_ctas_per_sm(cfg->scheme, instr, variant, kBlockSmall, c->small.dyn_smem);
   if (per_sm <= 0) {
     g_create_error = "step kernel does not fit on an SM with these tables (shared memory)";
@@ -402,7 +407,7 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
   }
   c->small.grid = static_cast<unsigned>(sms * per_sm);
   c->large.threads = kBlockLarge;
-  c->large.dyn_smem = step_smem_bytes(cfg->scheme, pl.table_bytes / 2, p.n_slabs, tile_words, kBlockLarge, c->ops->sparse_gather);
+  c->large.dyn_smem = step_smem_bytes(cfg->scheme, p.table_area, p.n_slabs, tile_words, kBlockLarge, c->ops->sparse_gather);
   const int per_sm_large = c->ops->step_ctas_per_sm(cfg->scheme, instr, variant, kBlockLarge, c->large.dyn_smem);
   cudaGetLastError();  // a failed attribute query of the optional shape is not an error of the context
   c->large.grid = per_sm_large > 0 ? static_cast<unsigned>(sms * per_sm_large) : 0u;

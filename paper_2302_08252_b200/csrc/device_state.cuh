@@ -110,6 +110,8 @@ struct Params {
   unsigned long long *sections;  // [kNumSections] warp-cycles per kernel section (timing build; after the tallies)
   const float4 *tables;      // [group][material][node] {q0, q1, q2, 0}; group 0 = gamma, 1 = e+-
   uint32_t table_bytes;      // bytes of ONE group, multiple of 16
+  uint32_t table_area;       // shared-memory bytes of the staged tables: one group, or (extended physics) the
+                             // e+- group followed by the e+ extras
   uint32_t nodes;            // n_bins + 1
   float ln_e_min, inv_dln, e_cut, e_max;
   uint32_t n_slabs;
@@ -117,7 +119,7 @@ struct Params {
   uint32_t mat_abs, mat_gap;
   uint32_t capacity;         // slots per kind (multiple of 128)
   uint32_t recycle;          // sparse scheme: 1 = freed slots are reused (ADEPT_FLAG_RECYCLE_SLOTS)
-  uint32_t physics;          // adept_tables.physics: 1 = extended rules X36, X37
+  uint32_t physics;          // adept_tables.physics: 1 = extended rules X36-X38
   KindStorage kind[3];
   unsigned long long *instr_field_rw;  // [3][14][2], instrumented build
   // SoA and AoS layouts, dense scheme: tensor maps of the record buffers, [kind][parity] (see

@@ -216,8 +216,8 @@ template <int L, bool INSTR> struct TrackView {
   // for e+-, vol when the step crossed into another slab.  dir never changes in the move half, ids
   // never.  A word assigned the value it already had (a zero-length step) is written again; the
   // counting build uses store_changed below instead and counts only real changes.
-  // N1: e+- also assign nial[1] (extended physics, rule X36).
-  template <bool GAMMA, bool N1 = false> __device__ __forceinline__ void store_moved(uint32_t slot, const Trk &t, bool vol_changed) const {
+  // N1: e+- also assign nial[1] (extended physics, rule X36); N2: e+ also nial[2] (rule X38).
+  template <bool GAMMA, bool N1 = false, bool N2 = false> __device__ __forceinline__ void store_moved(uint32_t slot, const Trk &t, bool vol_changed) const {
     if constexpr (L == L_AOS || L == L_SOA16) {
       // 16-byte pieces {pos, dir.x} {dir.yz, ekin, nial0} {nial12, vol, id_lo} {id_hi, step}: a photon
       // rewrites all four, e+- three and the third only with vol
@@ -247,6 +247,7 @@ template <int L, bool INSTR> struct TrackView {
       } else {
         base[Map::index(cap, slot, F_EKIN)] = __float_as_uint(t.ekin);
         if constexpr (N1) base[Map::index(cap, slot, F_N1)] = __float_as_uint(t.n1);
+        if constexpr (N2) base[Map::index(cap, slot, F_N2)] = __float_as_uint(t.n2);
       }
       if (vol_changed) base[Map::index(cap, slot, F_VOL)] = t.vol;
       base[Map::index(cap, slot, F_STEP)] = t.step;

@@ -23,7 +23,8 @@ enum Kind : int { K_EM = 0, K_EP = 1, K_GAMMA = 2 };
 
 // What the step needs besides the track: tables (shared memory) and geometry (registers).
 struct Env {
-  const float4 *tab;  // the particle group's tables: [material][node] -> {qty0, qty1, qty2, 0}
+  const float4 *tab;  // the particle group's tables: [material][node] -> {qty0, qty1, qty2, qty3 or 0}
+  uint32_t group_nodes;  // nodes of one staged group (materials * nodes): the e+ extras follow the e+- group
   uint32_t nodes;     // n_bins + 1
   float ln_e_min, inv_dln, e_cut;
   uint32_t n_slabs;   // 2 * n_layers
@@ -337,10 +338,11 @@ template <int KIND, int PHYS> __device__ __forceinline__ void move_elec(Trk &t, 
   if constexpr (PHYS == 0) {
     if (t.n0 <= 0.0f) t.n0 = -lg(u01(rs.call(0).x));
   } else {
-    if (t.n0 <= 0.0f || t.n1 <= 0.0f) {
+    if (t.n0 <= 0.0f || t.n1 <= 0.0f || (KIND == K_EP && t.n2 <= 0.0f)) {
       const uint4 r = rs.call(0);
       if (t.n0 <= 0.0f) t.n0 = -lg(u01(r.x));
       if (t.n1 <= 0.0f) t.n1 = -lg(u01(r.y));
+      if (KIND == K_EP && t.n2 <= 0.0f) t.n2 = -lg(u01(r.z));
     }
   }
 
@@ -355,10 +357,15 @@ template <int KIND, int PHYS> __device__ __forceinline__ void move_elec(Trk &t, 
   const float S0 = lerp_node(b.f, A.y, B.y);
   const float R = lerp_node(b.f, A.z, B.z);
   const float s0 = quotient_or_inf(t.n0, sig0, sig0 > 0.0f);
-  float sig1 = 0.0f, s1 = kInf;
+  float sig1 = 0.0f, s1 = kInf, sig2 = 0.0f, s2 = kInf;
   if constexpr (PHYS != 0) {
     sig1 = lerp_node(b.f, A.w, B.w);  // X36: Sigma_delta rides in the fourth lane of the e+- group
     s1 = quotient_or_inf(t.n1, sig1, sig1 > 0.0f);
+    if constexpr (KIND == K_EP) {     // X38: Sigma_annihilation, first lane of the e+ extras staged behind the group
+      const float4 *tx = tab + g.group_nodes;
+      sig2 = lerp_node(b.f, tx[b.j].x, tx[b.j + 1].x);
+      s2 = quotient_or_inf(t.n2, sig2, sig2 > 0.0f);
+    }
   }
   float s_e;
   {
@@ -377,6 +384,7 @@ template <int KIND, int PHYS> __device__ __forceinline__ void move_elec(Trk &t, 
   if (s_e < s) { s = s_e; w = 3; }
   if (s0 < s) { s = s0; w = 0; }
   if (PHYS != 0 && s1 < s) { s = s1; w = 1; }
+  if (PHYS != 0 && KIND == K_EP && s2 < s) { s = s2; w = 2; }
 
   // S23
   t.px = fmaf(s, t.dx, t.px);
@@ -384,6 +392,7 @@ template <int KIND, int PHYS> __device__ __forceinline__ void move_elec(Trk &t, 
   t.pz = fmaf(s, t.dz, t.pz);
   t.n0 = fmaf(-s, sig0, t.n0);
   if constexpr (PHYS != 0) t.n1 = fmaf(-s, sig1, t.n1);
+  if constexpr (PHYS != 0 && KIND == K_EP) t.n2 = fmaf(-s, sig2, t.n2);
   t.step = rs.step + 1u;
 
   // S24: continuous loss by the midpoint rule, deposit in the pre-step slab
@@ -402,7 +411,7 @@ template <int KIND, int PHYS> __device__ __forceinline__ void move_elec(Trk &t, 
   t.ekin = E_post;
   // what the step ends in, as flags (no early exits: the outcomes of a warp's lanes differ)
   const bool below = E_post < e_cut;            // S24: e- deposits the rest and dies; e+ is kept for S17
-  const bool brems = !below && (w == 0 || w == 1);  // S26 (X36: w == 1) follows in interact_elec
+  const bool brems = !below && (w == 0 || w == 1 || w == 2);  // S26 (X36: w == 1, X38: w == 2) follows in interact_elec
   const bool geom = !below && w < 0;
   o.dep_b = (below && KIND == K_EM) ? E_post : 0.0f;
   o.pending = brems ? w : int(P_NONE);
@@ -430,6 +439,34 @@ template <int KIND, int PHYS> __device__ __forceinline__ void interact_elec(Trk 
     return;
   }
   const float e_cut = g.e_cut;
+  if (PHYS != 0 && KIND == K_EP && pending == P_PROC2) {
+    // X38: annihilation in flight, two photons isotropic in the centre-of-momentum frame
+    const float E = t.ekin;
+    const float e_tot = E + two_mc2();
+    const float pp = sqrtf(E * e_tot);
+    const float beta = pp / e_tot;
+    const float cs = 1.0f - 2.0f * u01(r1.z);
+    const float k1 = (0.5f * e_tot) * fmaf(beta, cs, 1.0f);
+    const float k2 = e_tot - k1;
+    float c1 = (cs + beta) / fmaf(beta, cs, 1.0f);
+    if (c1 > 1.0f) c1 = 1.0f;
+    if (c1 < -1.0f) c1 = -1.0f;
+    const float s1 = sqrtf(fmaf(-c1, c1, 1.0f));
+    float sphi, cphi;
+    sincos2pi(u01(r1.w), sphi, cphi);
+    float ax, ay, az;
+    rotate_dir(t.dx, t.dy, t.dz, s1, c1, sphi, cphi, ax, ay, az);
+    const float qx = fmaf(pp, t.dx, -(k1 * ax));
+    const float qy = fmaf(pp, t.dy, -(k1 * ay));
+    const float qz = fmaf(pp, t.dz, -(k1 * az));
+    const float qn = sqrtf(fmaf(qx, qx, fmaf(qy, qy, qz * qz)));
+    if (k1 >= e_cut) make_kid(o.kid[0], K_GAMMA, ax, ay, az, k1, r2.x, r2.y);
+    else o.dep = k1;
+    if (k2 >= e_cut && qn > 0.0f) make_kid(o.kid[1], K_GAMMA, qx / qn, qy / qn, qz / qn, k2, r2.z, r2.w);
+    else o.dep_b = k2;
+    o.alive = false;
+    return;
+  }
   if (PHYS != 0 && pending == P_PROC1) {
     // X36: delta ray from the 1/T^2 spectrum on [e_cut, E/2], two-body kinematics on a free electron
     t.n1 = -1.0f;

@@ -46,7 +46,7 @@ __device__ __forceinline__ void group_sync(int group) {
 }
 
 // Variant bits of the step kernel (template parameter VAR): slot recycling of the sparse scheme
-// (ADEPT_FLAG_RECYCLE_SLOTS) and the extended physics rules X36, X37 (adept_tables.physics = 1).
+// (ADEPT_FLAG_RECYCLE_SLOTS) and the extended physics rules X36-X38 (adept_tables.physics = 1).
 enum Variant : int { V_RECYCLE = 1, V_PHYS = 2 };
 
 // ---- section clocks (timing build only) ------------------------------------------------------------
@@ -562,7 +562,7 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
   if (SCHEME == S_SPARSE) {
     if (survives || parked) {
       if constexpr (INSTR) cur.store_changed(slot, t, old);  // counts exactly the words that changed
-      else cur.template store_moved<KIND == K_GAMMA, (VAR & V_PHYS) != 0>(slot, t, t.vol != vol_before);
+      else cur.template store_moved<KIND == K_GAMMA, (VAR & V_PHYS) != 0, (VAR & V_PHYS) != 0 && KIND == K_EP>(slot, t, t.vol != vol_before);
     }
     c.clk->mark(SEC_STORE);
   }
@@ -840,14 +840,16 @@ __device__ __forceinline__ void run_kind(const Params &p, const Env &env, const 
   constexpr int group = (KIND == K_GAMMA) ? 0 : 1;
   if (staged_group != group) {
     __syncthreads();
+    // extended physics: the e+ extras (group 2, rule X38) lie behind the e+- group and are staged with it
+    const uint32_t stage_bytes = ((VAR & V_PHYS) != 0 && group == 1) ? 2u * p.table_bytes : p.table_bytes;
     if (threadIdx.x == 0) {
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
       asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(
                        static_cast<uint32_t>(__cvta_generic_to_shared(&c.cta->mbar))),
-                   "r"(p.table_bytes)
+                   "r"(stage_bytes)
                    : "memory");
       bulk_g2s(const_cast<float4 *>(env.tab), reinterpret_cast<const unsigned char *>(p.tables) + size_t(group) * p.table_bytes,
-               p.table_bytes, &c.cta->mbar);
+               stage_bytes, &c.cta->mbar);
     }
     mbar_wait(&c.cta->mbar, tab_phase);
     tab_phase ^= 1u;
@@ -891,9 +893,9 @@ __global__ void __launch_bounds__(THREADS, (THREADS == kBlockSmall) ? ADEPT_STEP
   c.group = tid / kGroup;
   c.gtid = tid % kGroup;
   c.g = &sh.grp[c.group];
-  c.bins.lo = reinterpret_cast<uint32_t *>(dyn_smem + p.table_bytes);
+  c.bins.lo = reinterpret_cast<uint32_t *>(dyn_smem + p.table_area);
   c.bins.hi = c.bins.lo + (p.n_slabs + 1u);
-  unsigned char *mine = dyn_smem + units_offset(p.table_bytes, p.n_slabs) + size_t(c.group) * kPerGroup;
+  unsigned char *mine = dyn_smem + units_offset(p.table_area, p.n_slabs) + size_t(c.group) * kPerGroup;
   c.in_buf = reinterpret_cast<uint32_t *>(mine);
   c.queue = reinterpret_cast<uint32_t *>(mine + kInBuf);
   SectClock clk;
@@ -933,7 +935,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == kBlockSmall) ? ADEPT_STEP
     clk.start(sh.sect, (tid & 31) == 0);
 
     Env env;
-    env.tab = s_tab; env.nodes = p.nodes;
+    env.tab = s_tab; env.nodes = p.nodes; env.group_nodes = p.table_bytes / 16u;
     env.ln_e_min = p.ln_e_min; env.inv_dln = p.inv_dln; env.e_cut = p.e_cut;
     env.n_slabs = p.n_slabs; env.abs_mm = p.abs_mm; env.pitch = p.pitch; env.half_xy = p.half_xy;
     env.mat_abs = p.mat_abs; env.mat_gap = p.mat_gap;

@@ -900,3 +900,37 @@ def test_timing_variant_computes_the_same_and_fills_its_section_clocks():
         s = res[1][3]
         assert (s[1:6] > 0).all() and s[4] + s[5] < s[:6].sum()       # load, move, interact, alloc, store all ran
         assert s[6] > 0 and s[7] > 0                                  # launch timeline (ns)
+
+
+@pytest.mark.parametrize("scheme", SCHEMES)
+def test_extended_physics_forced_interactions(scheme):
+    """Every track's step ends in the process under test: delta rays of e- and e+ (X36), annihilation
+    in flight (X38), Klein-Nishina Compton (X37) -- counts and all track words against the oracle."""
+    from workloads.tables import constant_tables
+    from workloads import Geometry
+    geo = Geometry(n_layers=2, abs_mm=50.0, gap_mm=50.0, half_xy_mm=1e4)
+    tab = constant_tables(16, 0.1, 100.0, 0.1, physics=1, delta=1.0, annih=1.0, compt=1.0, stop=0.0)
+    n = 5000 + 77
+    rng = np.random.default_rng(12)
+    cases = ((0, (1e6, 1e-30, 1e6)), (1, (1e6, 1e-30, 1e6)), (1, (1e6, 1e6, 1e-30)), (2, (1e6, 1e-30, 1e6)))
+    for layout in ("aosoa32", "aos"):
+        for kind, nial in cases:
+            t = make_tracks(n, pos=(0, 0, 25.0), ekin=1.0, nial=nial, id0=1 + 100000 * kind)
+            t["ekin"] = np.exp(rng.uniform(np.log(0.25), np.log(90.0), n)).astype(np.float32)
+            ct = rng.uniform(-1, 1, n)
+            ph = rng.uniform(0, 2 * np.pi, n)
+            d = np.stack([np.sqrt(1 - ct * ct) * np.cos(ph), np.sqrt(1 - ct * ct) * np.sin(ph), ct], 1)
+            t["dir"] = (d / np.linalg.norm(d, axis=1, keepdims=True)).astype(np.float32)
+            o = Oracle(geo, tab, seed=0)
+            o.load_tracks(kind, t)
+            o.step()
+            r = o.result()
+            assert r["secondaries"].sum() >= n // 2
+            ctx = _ctx(geo, tab, layout=layout, scheme=scheme, capacity=1 << 14, seed=0)
+            ctx.load_tracks(kind, t)
+            compare_counts(ctx.step(), r, what="%s kind %d %s" % (layout, kind, nial))
+            for k in range(3):
+                assert compare_tracks(ctx.read_tracks(k), o.read_tracks(k, t.dtype), "kind %d" % k) == 0
+            g = ctx.result()
+            assert np.allclose(g["edep_slab"], r["edep_slab"], rtol=1e-9, atol=1e-9)
+            ctx.destroy()

@@ -1,4 +1,4 @@
-"""Pins of the oracle's extended physics (DESIGN.md rules X35-X37), against
+"""Pins of the oracle's extended physics (DESIGN.md rules X35-X38), against
 what the mathematics fixes: the Klein-Nishina energy distribution by quadrature of the textbook
 differential cross-section, the 1/T^2 delta-ray spectrum by its closed-form CDF, exact two-body
 energy-momentum conservation, and the table identities of the restricted stopping power.  CPU only."""
@@ -177,7 +177,7 @@ def test_delta_ray_tables_split_the_collision_loss_exactly():
             assert abs(np.trapezoid(C / x ** 2, x) - sd) < 1e-6 * sd
             assert abs(s1 + np.trapezoid(C / x, x) - s0) < 1e-7 * s0 and s1 > 0
     tab = build_tables(64, E_CUT, 100.0, E_CUT, physics=1)
-    assert tab.physics == 1 and tab.data_x.shape == (2, 65) and tab.data_x.dtype == np.float32
+    assert tab.physics == 1 and tab.data_x.shape == (2, 2, 65) and tab.data_x.dtype == np.float32
     assert (tab.data[:, GROUP_ELEC, Q_STOP] <= build_tables(64, E_CUT, 100.0, E_CUT).data[:, GROUP_ELEC, Q_STOP]).all()
 
 
@@ -200,3 +200,67 @@ def test_extended_physics_conserves_energy_and_is_order_independent():
     for k in ("steps", "secondaries", "killed", "escaped_n"):
         assert (ra[k] == rb[k]).all()
     assert np.allclose(ra["edep_slab"], rb["edep_slab"], rtol=1e-12, atol=1e-12)
+
+
+# ------------------------------------------------------------------ X38: annihilation in flight --
+def test_annihilation_in_flight_closes_energy_and_momentum():
+    """Forced rule-X38 steps: the positron dies, two photons carry E + 2 mc^2 and the positron's
+    momentum; k1 is uniform on [E_tot (1 - beta)/2, E_tot (1 + beta)/2] (isotropic in the centre-of-
+    momentum frame); a photon below the cut is deposited instead."""
+    geo = Geometry(n_layers=1, abs_mm=1e3, gap_mm=1.0, half_xy_mm=1e6)
+    tab = constant_tables(16, E_CUT, 100.0, E_CUT, physics=1, annih=1.0, stop=0.0)
+    n = 40000
+    for E0 in (0.2, 2.0, 60.0):
+        t = make_tracks(n, pos=(0, 0, 500.0), ekin=E0, nial=(1e6, 1e6, 1e-30))
+        t["dir"] = _isotropic(n, 31)
+        o = Oracle(geo, tab, seed=0)
+        o.load_tracks(1, t)
+        o.step()
+        r = o.result()
+        assert r["killed"][1] == n and o.live(1) == 0 and r["secondaries"][0] == 0 and r["secondaries"][1] == 0
+        g = o.read_tracks(2, t.dtype)
+        e_tot, pp = E0 + 2 * MC2, math.sqrt(E0 * (E0 + 2 * MC2))
+        beta = pp / e_tot
+        lo, hi = 0.5 * e_tot * (1 - beta), 0.5 * e_tot * (1 + beta)
+        dep = r["edep_slab"].sum()
+        assert abs(g["ekin"].astype(np.float64).sum() + dep - n * e_tot) < 1e-6 * n * e_tot
+        assert g["ekin"].min() >= E_CUT and (dep > 0) == (lo < E_CUT)
+        # pair the two photons of each positron through rule R5 (call 2, ordinals 0 and 1)
+        from tests.test_oracle_transport import child_ids
+        ts = sort_by_id(t)
+        ids = {(int(a), int(b)): i for i, (a, b) in enumerate(zip(g["id_lo"], g["id_hi"]))}
+        l0, h0 = child_ids(ts, 0)
+        l1, h1 = child_ids(ts, 1)
+        k1s, closed = [], 0
+        for i in range(n):
+            a, b = ids.get((int(l0[i]), int(h0[i]))), ids.get((int(l1[i]), int(h1[i])))
+            if a is not None:
+                k1s.append(float(g["ekin"][a]))
+            if a is None or b is None:
+                continue
+            k1, k2 = float(g["ekin"][a]), float(g["ekin"][b])
+            assert abs(k1 + k2 - e_tot) < 3e-7 * e_tot
+            miss = pp * ts["dir"][i].astype(np.float64) - k1 * g["dir"][a].astype(np.float64) - k2 * g["dir"][b].astype(np.float64)
+            assert np.abs(miss).max() < 2e-3 * max(pp, k2) + 1e-6      # rule S27 near the z axis: see the delta-ray test
+            closed += 1
+        assert closed > 0.5 * n
+        k1s = np.array(k1s)
+        assert k1s.min() >= max(lo, E_CUT) * (1 - 1e-6) and k1s.max() <= hi * (1 + 1e-6)
+        a_ = max(lo, E_CUT)
+        assert _ks(k1s, lambda x: (x - a_) / (hi - a_)) < 1.63 / math.sqrt(k1s.shape[0])
+
+
+def test_annihilation_cross_section_limits():
+    """Heitler's formula: sigma -> pi r_e^2 / beta at low energy (Dirac's limit), ~ ln(2 gamma)/gamma at high."""
+    from workloads.tables import R_E, sigma_annihilation
+    mat = MATERIALS[0]
+    for T in (1e-4, 1e-3):
+        g = 1 + T / MC2
+        beta = math.sqrt(1 - 1 / g ** 2)
+        assert abs(float(sigma_annihilation(mat, T)) / (mat.n_atoms * mat.Z * math.pi * R_E ** 2 / beta) - 1) < 0.02
+    for T in (1e4, 1e5):
+        g = 1 + T / MC2
+        want = mat.n_atoms * mat.Z * math.pi * R_E ** 2 / g * (math.log(2 * g) - 1)
+        assert abs(float(sigma_annihilation(mat, T)) / want - 1) < 0.01
+    tab = build_tables(64, E_CUT, 100.0, E_CUT, physics=1)
+    assert tab.data_x.shape == (2, 2, 65) and (tab.data_x[:, 1] > 0).all()

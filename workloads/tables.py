@@ -100,6 +100,15 @@ def sigma_delta(mat: Material, T, e_cut: float):
     return np.where(T > 2.0 * e_cut, _delta_prefactor(mat, T) * (1.0 / e_cut - 1.0 / t_max), 0.0)
 
 
+def sigma_annihilation(mat: Material, T):
+    """Rule X38: annihilation in flight of a positron of kinetic energy T on an electron at rest,
+    Heitler's total cross-section per electron times the electron density [1/mm]."""
+    g = 1.0 + np.asarray(T, dtype=np.float64) / MC2
+    r = np.sqrt(g * g - 1.0)
+    per_e = math.pi * R_E * R_E / (g + 1.0) * ((g * g + 4.0 * g + 1.0) / (g * g - 1.0) * np.log(g + r) - (g + 3.0) / r)
+    return mat.n_atoms * mat.Z * per_e
+
+
 def stopping_power(mat: Material, T, e_cut: float, physics: int = 0):
     """Restricted stopping power [MeV/mm]: Bethe-Bloch collision term (no
     density correction) plus the radiative loss to photons below the cut.
@@ -156,8 +165,8 @@ class TableSet:
     inv_dln: np.float32
     nodes: np.ndarray           # float64 [n_bins+1]
     data: np.ndarray            # float32 [mat][group][qty][n_bins+1], C-contiguous
-    physics: int = 0            # rule X35: 0 = basic rules; 1 = delta rays (X36) + Klein-Nishina sampling (X37)
-    data_x: np.ndarray | None = None    # physics 1: float32 [mat][n_bins+1] Sigma_delta of the e+- group
+    physics: int = 0            # rule X35: 0 = basic rules; 1 = delta rays (X36), Klein-Nishina sampling (X37), annihilation in flight (X38)
+    data_x: np.ndarray | None = None    # physics 1: float32 [mat][2][n_bins+1]: Sigma_delta (e+-), Sigma_annihilation (e+)
 
     def q(self, mat: int, group: int, qty: int) -> np.ndarray:
         return self.data[mat, group, qty]
@@ -178,7 +187,8 @@ def build_tables(n_bins: int, e_min: float, e_max: float, e_cut: float,
         data[m, GROUP_ELEC, Q_RANGE] = csda_range(mat, nodes, e_cut, physics=physics)
     data_x = None
     if physics:
-        data_x = np.ascontiguousarray(np.stack([sigma_delta(mat, nodes, e_cut) for mat in materials]).astype(np.float32))
+        data_x = np.ascontiguousarray(np.stack([np.stack([sigma_delta(mat, nodes, e_cut), sigma_annihilation(mat, nodes)])
+                                                for mat in materials]).astype(np.float32))
     return TableSet(physics=physics, data_x=data_x,
         n_bins=n_bins, n_materials=len(materials), e_min=e_min, e_max=e_max, e_cut=e_cut,
         ln_e_min=np.float32(math.log(e_min)),
@@ -188,7 +198,7 @@ def build_tables(n_bins: int, e_min: float, e_max: float, e_cut: float,
 
 def constant_tables(n_bins: int, e_min: float, e_max: float, e_cut: float, *,
                     pair=0.0, compt=0.0, photo=0.0, brems=0.0, stop=0.0, rng=1e30,
-                    n_materials: int = 2, physics: int = 0, delta=0.0) -> TableSet:
+                    n_materials: int = 2, physics: int = 0, delta=0.0, annih=0.0) -> TableSet:
     """Energy-independent tables for closed-form checks (pure absorber,
     vacuum-like geometry tests, brems-only slabs)."""
     j = np.arange(n_bins + 1, dtype=np.float64)
@@ -200,7 +210,10 @@ def constant_tables(n_bins: int, e_min: float, e_max: float, e_cut: float, *,
     data[:, GROUP_ELEC, Q_BREMS] = brems
     data[:, GROUP_ELEC, Q_STOP] = stop
     data[:, GROUP_ELEC, Q_RANGE] = rng
-    data_x = np.full((n_materials, n_bins + 1), delta, dtype=np.float32) if physics else None
+    data_x = None
+    if physics:
+        data_x = np.zeros((n_materials, 2, n_bins + 1), dtype=np.float32)
+        data_x[:, 0], data_x[:, 1] = delta, annih
     return TableSet(n_bins, n_materials, e_min, e_max, e_cut,
                     np.float32(math.log(e_min)), np.float32(n_bins / math.log(e_max / e_min)),
                     nodes, data, physics, data_x)
