@@ -45,7 +45,7 @@ if ROOT not in sys.path:
 from workloads import CONFIGS, gen_tracks, geometry_for, tables_for  # noqa: E402
 
 WORKLOAD = "single_step"
-RECORD_BYTES = {"aos": 64, "soa": 56, "aosoa32": 56, "aosoa64": 56, "soa16": 56, "aosoa16": 56, "aosoa128": 56}     # bytes per record per layout
+RECORD_BYTES = {"aos": 64, "soa": 56, "aosoa32": 56, "aosoa64": 56, "soa16": 56, "aosoa16": 56, "aosoa128": 56, "hc16": 56}     # bytes per record per layout
 TRAFFIC_CSV = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
 
 
@@ -253,7 +253,7 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
     biggest = max(p.shape[0] for p in pop)
     capacity = int(biggest * 1.25) + 4096                  # one step grows the photon set by ~16 %
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-    layouts = ["aosoa32", "aosoa64", "soa16", "soa", "aos"] if args.layout == "all" else [args.layout]
+    layouts = ["aosoa32", "aosoa64", "soa16", "hc16", "soa", "aos"] if args.layout == "all" else [args.layout]
     per_layout, results = {}, {}
     sampler = ClockSampler(local_rank)
     sampler.start()
@@ -412,7 +412,7 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
                                                                  / np.maximum(np.array(ref["edep_layer_MeV"]), 1e-30)))
                 out["showers"][name + "_sparse_recycle"] = b
         if "sweep" in args.extras:
-            out["sweep"] = sweep(args, layouts=("aos", "soa", "aosoa32"), steps=5, warmup=3, instr=False, sections=True)
+            out["sweep"] = sweep(args, layouts=("aos", "soa", "aosoa32", "hc16"), steps=5, warmup=3, instr=False, sections=True)
     print(json.dumps(out))
     if dist is not None:
         dist.destroy_process_group()
@@ -515,13 +515,19 @@ def sharded_showers(args, name, rank, world, local_rank, dist, max_over_ranks) -
 # read once and every output record (survivor or secondary) written once.  Sparse: per input track one
 # slot-list entry and the record (AoS: its two sectors; SoA family: its 14 words -- the sector
 # amplification of scattered slots comes on top and is what the paper's finding is about); per
-# survivor the record's dirty words as whole records (AoS: two sectors) and one slot-list entry; per
-# secondary a whole record and one slot-list entry.
+# survivor the record's dirty bytes (SPARSE_DIRTY_BYTES) and one slot-list entry; per secondary a whole
+# record and one slot-list entry.
+# Bytes of a record the move half of a step must write back in place (sparse scheme): AoS rewrites
+# its two sectors; SoA16 its vectors with a changed word (all four for a photon); HC16 its two hot
+# vectors; the word-by-word layouts the 7-8 words a step assigns (pos, nial of the kind, step, ekin / vol).
+SPARSE_DIRTY_BYTES = {"aos": 64, "soa16": 56, "hc16": 32}
+
+
 def sweep_bytes(scheme: str, layout: str, n_in: int, n_surv: int, n_sec: int) -> int:
     rec = RECORD_BYTES[layout]
     if scheme == "dense":
         return rec * (n_in + n_surv + n_sec)
-    return n_in * (4 + rec) + n_surv * (rec + 4) + n_sec * (rec + 4)
+    return n_in * (4 + rec) + n_surv * (SPARSE_DIRTY_BYTES.get(layout, 32) + 4) + n_sec * (rec + 4)
 
 
 SECTION_NAMES = ("other", "load", "move", "interact", "alloc", "store")
@@ -646,7 +652,7 @@ def run_showers_cli(args, name: str):
 
 
 def run_sweep_cli(args):
-    layouts = ("aos", "soa", "aosoa32", "aosoa64", "soa16") if args.layout == "all" else (args.layout,)
+    layouts = ("aos", "soa", "aosoa32", "aosoa64", "soa16", "hc16") if args.layout == "all" else (args.layout,)
     sw = sweep(args, layouts=layouts, steps=args.steps, warmup=args.warmup, instr=not args.no_instr,
                sections=not args.no_sections,
                occupancies=None if args.occupancy is None else (args.occupancy,),
@@ -679,7 +685,7 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--layout", default="all", choices=["soa", "aosoa32", "aosoa64", "soa16", "aos", "aosoa16", "aosoa128", "all"])
+    ap.add_argument("--layout", default="all", choices=["soa", "aosoa32", "aosoa64", "soa16", "aos", "aosoa16", "aosoa128", "hc16", "all"])
     ap.add_argument("--tracks", type=int, default=CONFIGS[WORKLOAD]["n_tracks"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline legs")
     ap.add_argument("--extras", default=None,

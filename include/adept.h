@@ -56,7 +56,13 @@ typedef enum {
  * 16-byte field groups {pos.xyz, dir.x} {dir.y, dir.z, ekin, nial.0} {nial.1, nial.2, vol, id_lo}
  * {id_hi, step} -- the hot/cold grouping the paper's conclusion points to. */
 typedef enum { ADEPT_AOS = 0, ADEPT_SOA = 1, ADEPT_AOSOA32 = 2, ADEPT_AOSOA64 = 3, ADEPT_SOA16 = 4,
-               ADEPT_AOSOA16 = 5, ADEPT_AOSOA128 = 6 } adept_layout;
+               ADEPT_AOSOA16 = 5, ADEPT_AOSOA128 = 6, ADEPT_HC16 = 7 } adept_layout;
+/* ADEPT_HC16: hot/cold split with per-kind grouping ("a separation of hot and cold data
+ * would be a first step", "different layouts per particle type"): the SoA16 geometry with the words of a
+ * record regrouped, per particle kind, into two vectors the step rewrites every time ({pos, step} and
+ * gamma: {nial.0-2, vol} / e+-: {ekin, nial.0, nial.1, vol}), one it only reads unless an interaction
+ * happens (gamma: {dir, ekin} / e+-: {dir, nial.2}) and the cold {id_lo, id_hi}.  The sparse single
+ * buffer then rewrites 32 bytes of a record per step instead of 56-64. */
 /* Track container (PAPER.md:29 / PAPER.md:31). */
 typedef enum { ADEPT_SPARSE_SINGLE = 0, ADEPT_DENSE_DOUBLE = 1 } adept_scheme;
 
@@ -222,6 +228,9 @@ int adept_read_sections(adept_ctx *, uint64_t *cycles);
  * slot `slot` inside one record buffer of `capacity` slots under `layout` (Fig. 3:
  * where each field is placed).  Pure host arithmetic; UINT64_MAX on invalid arguments. */
 uint64_t adept_field_offset(int32_t layout, uint32_t capacity, uint32_t slot, uint32_t field);
+/* The same for layouts whose placement depends on the particle kind (ADEPT_HC16; for the others `kind`
+ * only has to be valid).  adept_field_offset itself returns UINT64_MAX for ADEPT_HC16. */
+uint64_t adept_field_offset_kind(int32_t layout, uint32_t kind, uint32_t capacity, uint32_t slot, uint32_t field);
 
 /* Drop all tracks, pending primaries and tallies; keeps geometry, tables and configuration. */
 int adept_reset(adept_ctx *);

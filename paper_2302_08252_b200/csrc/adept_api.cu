@@ -50,6 +50,7 @@ static const LayoutOps *ops_for(int layout) {
     case ADEPT_SOA: return &kOpsSoA;
     case ADEPT_AOSOA32: return &kOpsAoSoA32;
     case ADEPT_SOA16: return &kOpsSoA16;
+    case ADEPT_HC16: return &kOpsHC16;
 #ifndef ADEPT_FEW_LAYOUTS   // experiment builds instantiate four layouts only
     case ADEPT_AOSOA64: return &kOpsAoSoA64;
     case ADEPT_AOSOA16: return &kOpsAoSoA16;
@@ -735,6 +736,15 @@ int adept_read_sections(adept_ctx *c, uint64_t *cycles) {
                                 (size_t(2) * c->geo.n_layers + 1);
   for (int i = 0; i < kNumSections; ++i) cycles[i] = s[i];
   return rc;
+}
+
+uint64_t adept_field_offset_kind(int32_t layout, uint32_t kind, uint32_t capacity, uint32_t slot, uint32_t field) {
+  if (kind > 2u) return UINT64_MAX;
+  if (layout != ADEPT_HC16) return adept_field_offset(layout, capacity, slot, field);
+  if (field >= uint32_t(kNumFields) || capacity == 0) return UINT64_MAX;
+  const size_t cap = (size_t(capacity) + 127) / 128 * 128;
+  if (slot >= cap) return UINT64_MAX;
+  return 4 * Mapping<L_HC16>::index(cap, slot, int(field), int(kind));
 }
 
 uint64_t adept_field_offset(int32_t layout, uint32_t capacity, uint32_t slot, uint32_t field) {

@@ -20,7 +20,8 @@ enum Field : int {
   F_PX = 0, F_PY, F_PZ, F_DX, F_DY, F_DZ, F_EKIN, F_N0, F_N1, F_N2, F_VOL, F_IDLO, F_IDHI, F_STEP,
   kNumFields = 14
 };
-enum LayoutId : int { L_AOS = 0, L_SOA = 1, L_AOSOA32 = 2, L_AOSOA64 = 3, L_SOA16 = 4, L_AOSOA16 = 5, L_AOSOA128 = 6 };
+enum LayoutId : int { L_AOS = 0, L_SOA = 1, L_AOSOA32 = 2, L_AOSOA64 = 3, L_SOA16 = 4, L_AOSOA16 = 5, L_AOSOA128 = 6,
+                      L_HC16 = 7 };
 
 // A track in registers.
 struct Trk {
@@ -77,18 +78,18 @@ template <> struct Mapping<L_AOS> {  // 14 words padded to 16: one record = 64 B
   static constexpr int kStride = 16;
   static constexpr bool kSparseGather = true;
   __host__ __device__ static constexpr size_t words(size_t cap) { return cap * kStride; }
-  __host__ __device__ static constexpr size_t index(size_t, size_t slot, int f) { return slot * kStride + f; }
+  __host__ __device__ static constexpr size_t index(size_t, size_t slot, int f, int = 0) { return slot * kStride + f; }
 };
 template <> struct Mapping<L_SOA> {  // 14 arrays of `cap` words
   static constexpr bool kSparseGather = false;
   __host__ __device__ static constexpr size_t words(size_t cap) { return cap * kNumFields; }
-  __host__ __device__ static constexpr size_t index(size_t cap, size_t slot, int f) { return f * cap + slot; }
+  __host__ __device__ static constexpr size_t index(size_t cap, size_t slot, int f, int = 0) { return f * cap + slot; }
 };
 template <int N> struct AoSoAMapping {  // blocks of N tracks, field-major inside a block (N * 56 B)
   static constexpr int kLanes = N;
   static constexpr bool kSparseGather = false;
   __host__ __device__ static constexpr size_t words(size_t cap) { return cap * kNumFields; }
-  __host__ __device__ static constexpr size_t index(size_t, size_t slot, int f) {
+  __host__ __device__ static constexpr size_t index(size_t, size_t slot, int f, int = 0) {
     return (slot / kLanes) * (kLanes * kNumFields) + f * kLanes + (slot % kLanes);
   }
 };
@@ -104,10 +105,60 @@ template <> struct Mapping<L_AOSOA128> : AoSoAMapping<128> {};  // one block per
 template <> struct Mapping<L_SOA16> {
   static constexpr bool kSparseGather = false;  // measured: faster only above ~80 % occupancy
   __host__ __device__ static constexpr size_t words(size_t cap) { return cap * kNumFields; }
-  __host__ __device__ static constexpr size_t index(size_t cap, size_t slot, int f) {
+  __host__ __device__ static constexpr size_t index(size_t cap, size_t slot, int f, int = 0) {
     return (f < 12) ? size_t(f / 4) * 4 * cap + slot * 4 + (f % 4) : 12 * cap + slot * 2 + (f - 12);
   }
 };
+// Hot/cold split with per-kind grouping ("Individualizing,
+// splitting and regrouping ... A separation of hot and cold data would be a first step ... different
+// layouts per particle type"): the SoA16 geometry -- three arrays of 16-byte vectors and one of
+// 8-byte vectors -- with the record's words regrouped by how the step of each particle kind uses them:
+//   vector A (hot, rewritten every step)   {pos.x, pos.y, pos.z, step}                 all kinds
+//   vector B (hot, rewritten every step)   gamma: {nial.0, nial.1, nial.2, vol}   e+-: {ekin, nial.0, nial.1, vol}
+//   vector C (read; written by an interaction only)  gamma: {dir.x, dir.y, dir.z, ekin}   e+-: {dir.x, dir.y, dir.z, nial.2}
+//   vector D (cold: read only when a draw is made)   {id_lo, id_hi}
+// In the sparse single buffer the move half of a step then rewrites 32 bytes of a record (A and B)
+// instead of 56-64.  `kind` = 2 (gamma) selects the first grouping.
+template <> struct Mapping<L_HC16> {
+  static constexpr bool kSparseGather = false;
+  __host__ __device__ static constexpr size_t words(size_t cap) { return cap * kNumFields; }
+  __host__ __device__ static constexpr int position(int f, int kind) {
+    constexpr int kGamma[kNumFields] = {0, 1, 2, 8, 9, 10, 11, 4, 5, 6, 7, 12, 13, 3};
+    constexpr int kElec[kNumFields] = {0, 1, 2, 8, 9, 10, 4, 5, 6, 11, 7, 12, 13, 3};
+    return kind == 2 ? kGamma[f] : kElec[f];
+  }
+  __host__ __device__ static constexpr size_t index(size_t cap, size_t slot, int f, int kind = 2) {
+    return Mapping<L_SOA16>::index(cap, slot, position(f, kind));
+  }
+};
+
+// ---- L_HC16: a record <-> its four vectors, by particle kind ----------------------------------
+__device__ __forceinline__ void hc16_pack(bool gamma, const Trk &t, uint4 &a, uint4 &b, uint4 &c, uint2 &d) {
+  a = make_uint4(__float_as_uint(t.px), __float_as_uint(t.py), __float_as_uint(t.pz), t.step);
+  if (gamma) {
+    b = make_uint4(__float_as_uint(t.n0), __float_as_uint(t.n1), __float_as_uint(t.n2), t.vol);
+    c = make_uint4(__float_as_uint(t.dx), __float_as_uint(t.dy), __float_as_uint(t.dz), __float_as_uint(t.ekin));
+  } else {
+    b = make_uint4(__float_as_uint(t.ekin), __float_as_uint(t.n0), __float_as_uint(t.n1), t.vol);
+    c = make_uint4(__float_as_uint(t.dx), __float_as_uint(t.dy), __float_as_uint(t.dz), __float_as_uint(t.n2));
+  }
+  d = make_uint2(t.id_lo, t.id_hi);
+}
+__device__ __forceinline__ Trk hc16_unpack(bool gamma, const uint4 &a, const uint4 &b, const uint4 &c, const uint2 &d) {
+  Trk t;
+  t.px = __uint_as_float(a.x); t.py = __uint_as_float(a.y); t.pz = __uint_as_float(a.z); t.step = a.w;
+  t.dx = __uint_as_float(c.x); t.dy = __uint_as_float(c.y); t.dz = __uint_as_float(c.z);
+  if (gamma) {
+    t.n0 = __uint_as_float(b.x); t.n1 = __uint_as_float(b.y); t.n2 = __uint_as_float(b.z);
+    t.ekin = __uint_as_float(c.w);
+  } else {
+    t.ekin = __uint_as_float(b.x); t.n0 = __uint_as_float(b.y); t.n1 = __uint_as_float(b.z);
+    t.n2 = __uint_as_float(c.w);
+  }
+  t.vol = b.w;
+  t.id_lo = d.x; t.id_hi = d.y;
+  return t;
+}
 
 // ---- access counting (instrumented build only) -----------------------------------------------
 // field_rw: shared-memory counters [14][2] of the CTA (flushed once per kernel);
@@ -136,27 +187,39 @@ template <int L, bool INSTR> struct TrackView {
   uint32_t cap;        // slots
   size_t storage_off;  // byte offset of this buffer inside the kind's record storage (probe only)
   uint32_t buf_index;  // 0/1 (probe only)
+  int kind;            // particle kind of the buffer (per-kind layouts)
   ProbeSink sink;
 
   using Map = Mapping<L>;
 
   __device__ __forceinline__ void probe(int f, int w, size_t slot) const {
-    Probe<INSTR>().touch(sink, f, w, storage_off + Map::index(cap, slot, f) * 4, size_t(buf_index) * cap + slot);
+    Probe<INSTR>().touch(sink, f, w, storage_off + Map::index(cap, slot, f, kind) * 4, size_t(buf_index) * cap + slot);
   }
 
   __device__ __forceinline__ uint32_t load_word(uint32_t slot, int f) const {
     probe(f, 0, slot);
-    return base[Map::index(cap, slot, f)];
+    return base[Map::index(cap, slot, f, kind)];
   }
   __device__ __forceinline__ void store_word(uint32_t slot, int f, uint32_t w) const {
     probe(f, 1, slot);
-    base[Map::index(cap, slot, f)] = w;
+    base[Map::index(cap, slot, f, kind)] = w;
   }
 
   // whole record -> registers
   __device__ __forceinline__ Trk load(uint32_t slot) const {
     Trk t;
-    if constexpr (L == L_AOS || L == L_SOA16) {
+    if constexpr (L == L_HC16) {
+      using V = Mapping<L_SOA16>;
+      const uint4 a = *reinterpret_cast<const uint4 *>(base + V::index(cap, slot, 0));
+      const uint4 b = *reinterpret_cast<const uint4 *>(base + V::index(cap, slot, 4));
+      const uint4 c = *reinterpret_cast<const uint4 *>(base + V::index(cap, slot, 8));
+      const uint2 d = *reinterpret_cast<const uint2 *>(base + V::index(cap, slot, 12));
+      t = hc16_unpack(kind == 2, a, b, c, d);
+      if constexpr (INSTR) {
+#pragma unroll
+        for (int f = 0; f < kNumFields; ++f) probe(f, 0, slot);
+      }
+    } else if constexpr (L == L_AOS || L == L_SOA16) {
       uint4 a, b, c;
       uint2 d;
       if constexpr (L == L_AOS) {
@@ -187,7 +250,20 @@ template <int L, bool INSTR> struct TrackView {
 
   // registers -> whole record
   __device__ __forceinline__ void store(uint32_t slot, const Trk &t) const {
-    if constexpr (L == L_AOS || L == L_SOA16) {
+    if constexpr (L == L_HC16) {
+      using V = Mapping<L_SOA16>;
+      uint4 a, b, c;
+      uint2 d;
+      hc16_pack(kind == 2, t, a, b, c, d);
+      *reinterpret_cast<uint4 *>(base + V::index(cap, slot, 0)) = a;
+      *reinterpret_cast<uint4 *>(base + V::index(cap, slot, 4)) = b;
+      *reinterpret_cast<uint4 *>(base + V::index(cap, slot, 8)) = c;
+      *reinterpret_cast<uint2 *>(base + V::index(cap, slot, 12)) = d;
+      if constexpr (INSTR) {
+#pragma unroll
+        for (int f = 0; f < kNumFields; ++f) probe(f, 1, slot);
+      }
+    } else if constexpr (L == L_AOS || L == L_SOA16) {
       const uint4 a = make_uint4(__float_as_uint(t.px), __float_as_uint(t.py), __float_as_uint(t.pz), __float_as_uint(t.dx));
       const uint4 b = make_uint4(__float_as_uint(t.dy), __float_as_uint(t.dz), __float_as_uint(t.ekin), __float_as_uint(t.n0));
       const uint4 c = make_uint4(__float_as_uint(t.n1), __float_as_uint(t.n2), t.vol, t.id_lo);
@@ -218,7 +294,17 @@ template <int L, bool INSTR> struct TrackView {
   // counting build uses store_changed below instead and counts only real changes.
   // N1: e+- also assign nial[1] (extended physics, rule X36); N2: e+ also nial[2] (rule X38).
   template <bool GAMMA, bool N1 = false, bool N2 = false> __device__ __forceinline__ void store_moved(uint32_t slot, const Trk &t, bool vol_changed) const {
-    if constexpr (L == L_AOS || L == L_SOA16) {
+    if constexpr (L == L_HC16) {
+      // the two hot vectors; e+ under the extended physics also assigns nial[2], which lives in vector C
+      using V = Mapping<L_SOA16>;
+      uint4 a, b, c;
+      uint2 d;
+      hc16_pack(GAMMA, t, a, b, c, d);
+      *reinterpret_cast<uint4 *>(base + V::index(cap, slot, 0)) = a;
+      *reinterpret_cast<uint4 *>(base + V::index(cap, slot, 4)) = b;
+      if constexpr (N2) *reinterpret_cast<uint4 *>(base + V::index(cap, slot, 8)) = c;
+      (void)vol_changed; (void)d;
+    } else if constexpr (L == L_AOS || L == L_SOA16) {
       // 16-byte pieces {pos, dir.x} {dir.yz, ekin, nial0} {nial12, vol, id_lo} {id_hi, step}: a photon
       // rewrites all four, e+- three and the third only with vol
       uint4 *q0, *q1, *q2;
@@ -256,6 +342,19 @@ template <int L, bool INSTR> struct TrackView {
 
   // registers -> only the words that differ from `old` (sparse single buffer: in-place update)
   __device__ __forceinline__ void store_changed(uint32_t slot, const Trk &t, const Trk &old) const {
+    if constexpr (L == L_HC16 && !INSTR) {
+      using V = Mapping<L_SOA16>;
+      uint4 a, b, c, oa, ob, oc;
+      uint2 d, od;
+      hc16_pack(kind == 2, t, a, b, c, d);
+      hc16_pack(kind == 2, old, oa, ob, oc, od);
+      auto ne = [](const uint4 &x, const uint4 &y) { return x.x != y.x || x.y != y.y || x.z != y.z || x.w != y.w; };
+      if (ne(a, oa)) *reinterpret_cast<uint4 *>(base + V::index(cap, slot, 0)) = a;
+      if (ne(b, ob)) *reinterpret_cast<uint4 *>(base + V::index(cap, slot, 4)) = b;
+      if (ne(c, oc)) *reinterpret_cast<uint4 *>(base + V::index(cap, slot, 8)) = c;
+      if (d.x != od.x || d.y != od.y) *reinterpret_cast<uint2 *>(base + V::index(cap, slot, 12)) = d;
+      return;
+    }
     if constexpr ((L == L_AOS || L == L_SOA16) && !INSTR) {
       // layouts that keep a record's words in 16-byte pieces: a piece with a changed word is rewritten
       // whole (the thread owns the record; the unchanged words of the piece are written back as they

@@ -169,12 +169,12 @@ __device__ __forceinline__ void prefetch_tile(const Params &p, int kind, uint32_
             static_cast<uint32_t>(__cvta_generic_to_shared(in_buf))),
         "l"(reinterpret_cast<uint64_t>(&p.tile_map[kind][par])), "r"(0u), "r"(first), "r"(bar)
         : "memory");
-  } else if constexpr (L == L_SOA16) {  // four runs: three of 16-byte vectors, one of 8-byte vectors
+  } else if constexpr (L == L_SOA16 || L == L_HC16) {  // four runs: three of 16-byte vectors, one of 8-byte vectors
     const uint32_t n2 = (n + 1u) & ~1u;  // whole 16-byte pieces (slots are padded to whole tiles)
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(n2 * 56u) : "memory");
 #pragma unroll
     for (int gI = 0; gI < 4; ++gI)
-      bulk_g2s(in_buf + Mapping<L>::index(kGroup, 0, 4 * gI), rec + Mapping<L>::index(p.capacity, first, 4 * gI),
+      bulk_g2s(in_buf + Mapping<L_SOA16>::index(kGroup, 0, 4 * gI), rec + Mapping<L_SOA16>::index(p.capacity, first, 4 * gI),
                n2 * (gI < 3 ? 16u : 8u), mbar);
   } else {  // AoSoA-n: whole blocks, one contiguous run
     constexpr uint32_t kL = Mapping<L>::kLanes;
@@ -187,8 +187,16 @@ __device__ __forceinline__ void prefetch_tile(const Params &p, int kind, uint32_
 }
 
 // The thread's record out of the staged tile (same mapping as in global memory, capacity = kGroup).
-template <int L> __device__ __forceinline__ Trk staged_load(const uint32_t *in_buf, int gtid) {
+template <int L> __device__ __forceinline__ Trk staged_load(const uint32_t *in_buf, int gtid, int kind = 2) {
   Trk t;
+  if constexpr (L == L_HC16) {
+    using V = Mapping<L_SOA16>;
+    const uint4 a = *reinterpret_cast<const uint4 *>(in_buf + V::index(kGroup, gtid, 0));
+    const uint4 b = *reinterpret_cast<const uint4 *>(in_buf + V::index(kGroup, gtid, 4));
+    const uint4 c = *reinterpret_cast<const uint4 *>(in_buf + V::index(kGroup, gtid, 8));
+    const uint2 d = *reinterpret_cast<const uint2 *>(in_buf + V::index(kGroup, gtid, 12));
+    return hc16_unpack(kind == 2, a, b, c, d);
+  }
   if constexpr (L == L_AOS) {
     // undo the copy's 64-byte swizzle (prefetch_tile): chunk c of this thread's record is at chunk
     // c ^ s of its row, s = bits 7-8 of the row's shared-memory address
@@ -299,6 +307,7 @@ __device__ __forceinline__ TrackView<L, INSTR> make_view(const Params &p, int ki
   v.cap = p.capacity;
   v.storage_off = size_t(buf) * Mapping<L>::words(p.capacity) * 4;
   v.buf_index = uint32_t(buf);
+  v.kind = kind;
   v.sink.cta_field_rw = cta_probe + kind * (kNumFields * 2);
   v.sink.lines = p.kind[kind].instr_lines;
   v.sink.slots = p.kind[kind].instr_slots;
@@ -485,7 +494,7 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
   if (SCHEME == S_DENSE) {  // the tile was staged in shared memory by prefetch_tile
     mbar_wait(&g.mbar_in, in_phase);
     in_phase ^= 1u;
-    if (active) t = staged_load<L>(c.in_buf, gtid);
+    if (active) t = staged_load<L>(c.in_buf, gtid, KIND);
     // the warp has its records in registers; the last warp to get there refills the staging buffer
     // with the group's next tile, which then loads while this one is stepped
     __syncwarp();
@@ -528,7 +537,11 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
       if (l2_prefetch && s_next != kNoSlot) {
 #pragma unroll
         for (int f = 0; f < kNumFields; ++f)
-          asm volatile("prefetch.global.L2 [%0];" ::"l"(p.kind[KIND].rec[0] + Mapping<L>::index(p.capacity, s_next, f)));
+          if (L != L_SOA16 && L != L_HC16) {
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(p.kind[KIND].rec[0] + Mapping<L>::index(p.capacity, s_next, f)));
+          } else if (f % 4 == 0) {  // one request per 16-byte vector
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(p.kind[KIND].rec[0] + Mapping<L_SOA16>::index(p.capacity, s_next, f)));
+          }
       }
     }
     in_phase ^= 1u;
@@ -1029,6 +1042,7 @@ template <int L> __device__ __forceinline__ TrackView<L, false> plain_view(const
   v.base = p.kind[kind].rec[buf];
   v.cap = p.capacity;
   v.storage_off = 0; v.buf_index = 0;
+  v.kind = kind;
   v.sink.cta_field_rw = nullptr; v.sink.lines = nullptr; v.sink.slots = nullptr;
   return v;
 }
@@ -1206,6 +1220,6 @@ template <int L> struct OpsImpl {
   }
 };
 
-extern const LayoutOps kOpsAoS, kOpsSoA, kOpsAoSoA32, kOpsAoSoA64, kOpsSoA16, kOpsAoSoA16, kOpsAoSoA128;
+extern const LayoutOps kOpsAoS, kOpsSoA, kOpsAoSoA32, kOpsAoSoA64, kOpsSoA16, kOpsAoSoA16, kOpsAoSoA128, kOpsHC16;
 
 }  // namespace adept

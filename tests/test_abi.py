@@ -31,7 +31,7 @@ def test_library_exports_every_declared_function(L):
     lib = L.lib()
     for n in names:
         assert hasattr(lib, n), "libadept_b200.so does not export %s" % n
-    assert len(names) >= 19
+    assert len(names) >= 20
 
 
 def test_timing_variant_exports_the_same_abi(L):
@@ -61,10 +61,10 @@ def test_workspace_bytes_is_host_arithmetic(L):
     base = size()
     assert base > 3 * 2 * 4096 * 56                                  # three kinds, two dense arrays
     assert size(capacity=8192) > base and size(capacity=4097) == size(capacity=4224)   # rounded to 128 slots (one tile)
-    assert size(layout=0) > size(layout=1) == size(layout=2) == size(layout=3) == size(layout=4)   # AoS records are padded to 64 B
+    assert size(layout=0) > size(layout=1) == size(layout=2) == size(layout=3) == size(layout=4) == size(layout=7)   # AoS records are padded to 64 B
     assert size(scheme=0) < base                                     # one slot array + two slot lists
     assert size(instrument=1) > base
-    for bad in (dict(layout=7), dict(scheme=5), dict(capacity=0), dict(n_layers=0), dict(n_bins=0)):
+    for bad in (dict(layout=8), dict(scheme=5), dict(capacity=0), dict(n_layers=0), dict(n_bins=0)):
         assert size(**bad) == 0
 
 
@@ -81,6 +81,19 @@ def test_field_offset_follows_the_three_mappings(L):
             want = (f // 4) * 16 * cap + slot * 16 + (f % 4) * 4 if f < 12 else 48 * cap + slot * 8 + (f - 12) * 4
             assert L.field_offset(L.ADEPT_SOA16, cap, slot, f) == want          # 16-byte field groups
     assert L.field_offset(L.ADEPT_SOA, cap, 0, 14) == 2**64 - 1 and L.field_offset(9, cap, 0, 0) == 2**64 - 1
+    # HC16: the SoA16 geometry with the words regrouped per particle kind (hot {pos, step}, hot
+    # {nial.., vol} / {ekin, nial.0-1, vol}, read-mostly {dir, ekin} / {dir, nial.2}, cold ids)
+    order = {2: ["pos.x", "pos.y", "pos.z", "step", "nial.0", "nial.1", "nial.2", "vol", "dir.x", "dir.y", "dir.z", "ekin", "id_lo", "id_hi"],
+             0: ["pos.x", "pos.y", "pos.z", "step", "ekin", "nial.0", "nial.1", "vol", "dir.x", "dir.y", "dir.z", "nial.2", "id_lo", "id_hi"]}
+    order[1] = order[0]
+    assert L.field_offset(L.ADEPT_HC16, cap, 0, 0) == 2**64 - 1                  # needs the kind
+    for kind in range(3):
+        for slot in (0, 5, 4095):
+            for f, name in enumerate(L.FIELD_NAMES):
+                pos = order[kind].index(name)
+                assert L.field_offset(L.ADEPT_HC16, cap, slot, f, kind=kind) == L.field_offset(L.ADEPT_SOA16, cap, slot, pos)
+        assert L.field_offset(L.ADEPT_SOA, cap, 3, 2, kind=kind) == L.field_offset(L.ADEPT_SOA, cap, 3, 2)
+    assert L.field_offset(L.ADEPT_HC16, cap, 0, 0, kind=3) == 2**64 - 1
     # every (slot, field) has its own word in every layout
     for lay, words in ((L.ADEPT_AOS, 16), (L.ADEPT_SOA, 14), (L.ADEPT_AOSOA32, 14), (L.ADEPT_AOSOA64, 14),
                        (L.ADEPT_SOA16, 14)):

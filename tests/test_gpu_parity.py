@@ -11,7 +11,7 @@ from tests.helpers import make_tracks, sort_by_id
 
 pytestmark = pytest.mark.gpu
 
-LAYOUTS = ("aos", "soa", "aosoa32", "aosoa64", "soa16", "aosoa16", "aosoa128")
+LAYOUTS = ("aos", "soa", "aosoa32", "aosoa64", "soa16", "aosoa16", "aosoa128", "hc16")
 SCHEMES = ("dense", "sparse")
 INT_FIELDS = ("vol", "id_lo", "id_hi", "step")
 F32_FIELDS = ("pos", "dir", "ekin", "nial")
@@ -325,7 +325,7 @@ def test_instrumented_dense_counts_follow_the_access_rules(layout):
         assert (nxt[:counts["live"][k]] == 14).all() and (nxt[counts["live"][k]:] == 0).all()
         # heatmap rows: every 128-byte line of the used part of the current buffer was touched
         from paper_2302_08252_b200 import LAYOUTS as LAY, field_offset
-        touched = {field_offset(LAY[layout], cap, s, f) // 128 for s in (0, n_in[k] - 1) for f in range(14)}
+        touched = {field_offset(LAY[layout], cap, s, f, kind=k) // 128 for s in (0, n_in[k] - 1) for f in range(14)}
         assert all(lines[k][t] > 0 for t in touched)
     ctx.destroy()
 
@@ -383,7 +383,8 @@ def _full_size_reference(n):
                                              ("soa", "dense", 1 << 23), ("soa16", "dense", 1 << 23),
                                              ("aos", "dense", 1 << 23), ("aosoa64", "dense", 1 << 23),
                                              ("aos", "sparse", 1 << 23), ("soa", "sparse", 1 << 23),
-                                             ("aosoa32", "sparse", 1 << 23)])
+                                             ("aosoa32", "sparse", 1 << 23), ("hc16", "dense", 1 << 23),
+                                             ("hc16", "sparse", 1 << 23)])
 def test_single_step_at_full_size_counts_and_every_track(layout, scheme, n):
     """Config 3 as bench.py times it: 2^24 tracks, dense double buffer, AoSoA-32, one adept_step --
     and 2^23 tracks in seven more layout x scheme variants; all above the population at which the
@@ -693,7 +694,7 @@ def test_run_counts_real_iterations_against_the_limit():
 
 
 # ----------------------------------------------------------- slot recycling --
-@pytest.mark.parametrize("layout", ("aos", "soa", "aosoa32", "soa16"))
+@pytest.mark.parametrize("layout", ("aos", "soa", "aosoa32", "soa16", "hc16"))
 def test_sparse_slot_recycling_keeps_results_and_bounds_the_footprint(layout):
     """ADEPT_FLAG_RECYCLE_SLOTS (include/adept.h): the slot of every track that ends goes onto a ring
     and secondaries take recycled slots first.  Slots carry no physics, so every count, every tally and
@@ -804,7 +805,7 @@ def _heavy_reference():
 
 # ------------------------------------------------- extended physics ----------
 @pytest.mark.parametrize("scheme", SCHEMES)
-@pytest.mark.parametrize("layout", ("aos", "soa", "aosoa32", "soa16"))
+@pytest.mark.parametrize("layout", ("aos", "soa", "aosoa32", "soa16", "hc16"))
 def test_extended_physics_matches_oracle(layout, scheme):
     """adept_tables.physics = 1 (rules X36 delta rays on nial[1], X37 Klein-Nishina rejection sampling):
     the tiny shower track by track in every iteration, then 100 x 1 GeV showers to completion."""
@@ -913,7 +914,7 @@ def test_extended_physics_forced_interactions(scheme):
     n = 5000 + 77
     rng = np.random.default_rng(12)
     cases = ((0, (1e6, 1e-30, 1e6)), (1, (1e6, 1e-30, 1e6)), (1, (1e6, 1e6, 1e-30)), (2, (1e6, 1e-30, 1e6)))
-    for layout in ("aosoa32", "aos"):
+    for layout in ("aosoa32", "aos", "hc16"):
         for kind, nial in cases:
             t = make_tracks(n, pos=(0, 0, 25.0), ekin=1.0, nial=nial, id0=1 + 100000 * kind)
             t["ekin"] = np.exp(rng.uniform(np.log(0.25), np.log(90.0), n)).astype(np.float32)
