@@ -195,11 +195,11 @@ def bench_layout(ctx, torch, pop, steps, warmup, flush, barrier):
     for k in range(3):
         ctx.load_tracks(k, pop[k])
     torch.cuda.synchronize()
-    pristine = ctx.workspace.clone()
+    pristine = ctx.snapshot()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
 
     def one(e0, e1):
-        ctx.workspace.copy_(pristine)          # rewind (include/adept.h "Workspace"), untimed
+        ctx.rewind(pristine)                   # include/adept.h "Workspace", untimed
         flush.zero_()                          # L2 flush: 256 MiB > 126 MB L2, untimed
         if e0 is not None:
             e0.record(ctx.stream)
@@ -568,10 +568,10 @@ def sweep(args, *, layouts, steps, warmup, instr, sections, occupancies=None, sc
                         ctx.load_tracks(k, pop[k]["tracks"], pop[k]["slots"] if scheme == "sparse" else None)
                     torch.cuda.synchronize()
                     if what == "time":
-                        pristine = ctx.workspace.clone()
+                        pristine = ctx.snapshot()
                         ms = []
                         for it in range(warmup + steps):
-                            ctx.workspace.copy_(pristine)
+                            ctx.rewind(pristine)
                             flush.zero_()
                             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                             e0.record(ctx.stream)

@@ -27,9 +27,12 @@
  *    raised if an energy tally leaves its 64-bit fixed-point range (2^32 MeV in one slab).
  *
  * Workspace.  The workspace holds the complete device state of a context (control block, tables,
- * track buffers, queues, tallies).  A byte copy of it taken while no call is in flight may be
- * written back later to rewind the context (bench.py restores a pristine copy between timed
- * steps this way).
+ * track buffers, queues, tallies).  A byte copy of it taken while no call is in flight, together with
+ * adept_launch_index() at that moment, may be written back later -- followed by
+ * adept_set_launch_index() -- to rewind the context (bench.py restores a pristine copy between timed
+ * steps this way).  The launch index is the one piece of iteration state the host holds: the device keeps
+ * its per-iteration counters three deep, indexed by it, so that no thread block has to close an
+ * iteration.
  */
 #ifndef ADEPT_B200_H
 #define ADEPT_B200_H
@@ -218,7 +221,8 @@ uint64_t adept_instr_slots(const adept_ctx *);
  * warp, the cycles spent in each: cycles[0] other (prologue, table staging, tally flush),
  * [1] A1 record load, [2] A2-A7 move half, [3] A8 interact half, [4] A9 allocation (ballots, arrival
  * word, range/slot reservation, group barrier, ranks), [5] A10 stores (records, slot lists, parked
- * queue); [6], [7] unused.  Cumulative since create/reset.  adept_timing_sections() returns 1 in
+ * queue); [6] nanoseconds from the first thread block's start to the last one's end, summed over the
+ * launches; [7] unused.  Cumulative since create/reset.  adept_timing_sections() returns 1 in
  * the timing variant, 0 otherwise (all cycles then read 0).  cycles: host, ADEPT_N_SECTIONS entries. */
 #define ADEPT_N_SECTIONS 8
 int adept_timing_sections(void);
@@ -231,6 +235,11 @@ uint64_t adept_field_offset(int32_t layout, uint32_t capacity, uint32_t slot, ui
 /* The same for layouts whose placement depends on the particle kind (ADEPT_HC16; for the others `kind`
  * only has to be valid).  adept_field_offset itself returns UINT64_MAX for ADEPT_HC16. */
 uint64_t adept_field_offset_kind(int32_t layout, uint32_t kind, uint32_t capacity, uint32_t slot, uint32_t field);
+
+/* Number of step launches enqueued since create/reset (see "Workspace"); set: only together with a
+ * restored workspace copy taken at that index. */
+uint32_t adept_launch_index(const adept_ctx *);
+int adept_set_launch_index(adept_ctx *, uint32_t index);
 
 /* Drop all tracks, pending primaries and tallies; keeps geometry, tables and configuration. */
 int adept_reset(adept_ctx *);

@@ -101,6 +101,9 @@ def lib(variant: str | None = None):
         L.adept_last_error.restype = C.c_char_p
         L.adept_last_error.argtypes = [vp]
         L.adept_dev_math.argtypes = [C.c_int, vp, vp, u64, vp]
+        L.adept_launch_index.restype = u32
+        L.adept_launch_index.argtypes = [vp]
+        L.adept_set_launch_index.argtypes = [vp, u32]
         L.adept_timing_sections.restype = C.c_int
         L.adept_timing_sections.argtypes = []
         L.adept_read_sections.argtypes = [vp, vp]
@@ -255,6 +258,14 @@ class Context:
         slots = np.zeros((3, n_slots), dtype=np.uint32)
         self._check(self._L.adept_read_counters(self._h, rw.ctypes.data, lines.ctypes.data, slots.ctypes.data))
         return dict(field_rw=rw, lines=lines, slots=slots)
+
+    def snapshot(self):
+        """(workspace copy, launch index): what `rewind` needs (adept.h "Workspace").  No call may be in flight."""
+        return self.workspace.clone(), int(self._L.adept_launch_index(self._h))
+
+    def rewind(self, snap):
+        self.workspace.copy_(snap[0])
+        self._check(self._L.adept_set_launch_index(self._h, snap[1]))
 
     def read_sections(self):
         """Timing variant: warp-cycles per kernel section (adept.h adept_read_sections)."""

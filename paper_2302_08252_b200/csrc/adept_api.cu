@@ -78,7 +78,7 @@ static bool make_plan(const adept_geometry *g, const adept_tables *t, const adep
   pl.stage_records = std::min<uint32_t>(pl.capacity, kStageRecords);
   size_t off = 0;
   // control header, tallies (per slab + escaped), section clocks of the timing build
-  pl.ctl = off; off = align_up(off + kCtlHeaderBytes + (size_t(2) * g->n_layers + 1 + kNumSections + 1) * sizeof(unsigned long long));
+  pl.ctl = off; off = align_up(off + kCtlHeaderBytes + (size_t(2) * g->n_layers + 1 + kNumSections + 4) * sizeof(unsigned long long));
   pl.tables = off; off = align_up(off + pl.table_bytes);
   pl.stage = off; off = align_up(off + size_t(pl.stage_records) * kStageRecordBytes);
   pl.stage_slots = off; off = align_up(off + size_t(pl.stage_records) * 4);
@@ -123,6 +123,7 @@ struct adept_ctx {
   cudaEvent_t ev_copied[2], ev_kernel[2];
   struct Shape { int threads; unsigned grid; size_t dyn_smem; } small, large;  // CTA shapes of the step kernel
   uint64_t live_hint;     // live tracks as last seen by the host: picks the shape
+  uint32_t launch_index;  // index of the next step launch (Params::it): the device's iteration counters are kept by it
   unsigned char *ws;
   unsigned char *pinned;  // kCtlHeaderBytes + tallies
   size_t pinned_bytes;
@@ -162,9 +163,13 @@ int fail(adept_ctx *c, int code, const char *what, cudaError_t e = cudaSuccess) 
 
 Ctl *host_ctl(adept_ctx *c) { return reinterpret_cast<Ctl *>(c->pinned); }
 
-// copy control block (+ edep) to pinned memory and wait
+__global__ void close_kernel(Params p, uint32_t it, int sparse, int recycle);
+
+// close the open launches (close_kernel), copy control block (+ edep) to pinned memory and wait
 int fetch_ctl(adept_ctx *c, bool with_edep) {
   const size_t n = with_edep ? c->pinned_bytes : kCtlHeaderBytes;
+  close_kernel<<<1, 32, 0, c->stream>>>(c->params, c->launch_index, c->cfg.scheme == ADEPT_SPARSE_SINGLE ? 1 : 0, int(c->params.recycle));
+  CU(c, cudaGetLastError());
   CU(c, cudaMemcpyAsync(c->pinned, c->ws + c->plan.ctl, n, cudaMemcpyDeviceToHost, c->stream));
   CU(c, cudaStreamSynchronize(c->stream));
   c->live_hint = uint64_t(host_ctl(c)->n_cur[0]) + host_ctl(c)->n_cur[1] + host_ctl(c)->n_cur[2];
@@ -208,7 +213,23 @@ void fill_result(const adept_ctx *c, adept_result *out) {
 // write n_cur / slot_top / slots_used of one kind after a host-driven append
 __global__ void clear_bad_input_kernel(Ctl *ctl) { ctl->bad_input = 0u; }
 
-__global__ void set_counts_kernel(Ctl *ctl, int kind, uint32_t n_cur, uint32_t slot_top, unsigned long long used) {
+// Before the host reads the control block: close every launch that is still open and write the summary.
+__global__ void close_kernel(Params p, uint32_t it, int sparse, int recycle) {
+  const int lane = int(threadIdx.x);
+#ifdef ADEPT_TIMING_SECTIONS
+#define ADEPT_ROLL_ARGS p.ctl, p.capacity, it, false, lane, p.sections
+#else
+#define ADEPT_ROLL_ARGS p.ctl, p.capacity, it, false, lane
+#endif
+  if (!sparse) roll_iterations<false, false>(ADEPT_ROLL_ARGS);
+  else if (recycle) roll_iterations<true, true>(ADEPT_ROLL_ARGS);
+  else roll_iterations<true, false>(ADEPT_ROLL_ARGS);
+#undef ADEPT_ROLL_ARGS
+}
+
+// after a host-driven append: live count of `kind` for the next launch `it`, slot allocator, high-water mark
+__global__ void set_counts_kernel(Ctl *ctl, uint32_t it, int kind, uint32_t n_cur, uint32_t slot_top, unsigned long long used) {
+  ctl->n[it % 3u][kind] = n_cur;
   ctl->n_cur[kind] = n_cur;
   ctl->slot_top[kind] = slot_top;
   if (used > ctl->slots_used[kind]) ctl->slots_used[kind] = used;
@@ -258,9 +279,9 @@ static int clear_state(adept_ctx *c) {
   if (c->cfg.instrument && pl.total > pl.instr_rw)
     CU(c, cudaMemsetAsync(c->ws + pl.instr_rw, 0, pl.total - pl.instr_rw, c->stream));
 #ifdef ADEPT_TIMING_SECTIONS
-  {  // scratch word of the launch timeline: earliest CTA start of the running launch (atomicMin)
-    static const unsigned long long kNever = ~0ull;
-    CU(c, cudaMemcpyAsync(c->params.sections + kNumSections, &kNever, sizeof kNever, cudaMemcpyHostToDevice, c->stream));
+  {  // scratch of the launch timeline, by launch parity: {earliest CTA start (atomicMin), latest CTA end (atomicMax)}
+    static const unsigned long long kInit[4] = {~0ull, 0ull, ~0ull, 0ull};
+    CU(c, cudaMemcpyAsync(c->params.sections + kNumSections, kInit, sizeof kInit, cudaMemcpyHostToDevice, c->stream));
   }
 #endif
   c->pending.clear();
@@ -268,6 +289,7 @@ static int clear_state(adept_ctx *c) {
   c->next_primary = 0;
   c->e_injected = 0.0;
   c->live_hint = 0;
+  c->launch_index = 0;
   c->dead = false;
   return ADEPT_OK;
 }
@@ -304,7 +326,7 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
     return ADEPT_ECUDA;
   };
   cudaError_t e;
-  c->pinned_bytes = kCtlHeaderBytes + (size_t(2) * g->n_layers + 1 + kNumSections + 1) * sizeof(unsigned long long);
+  c->pinned_bytes = kCtlHeaderBytes + (size_t(2) * g->n_layers + 1 + kNumSections + 4) * sizeof(unsigned long long);
   if ((e = cudaMallocHost(reinterpret_cast<void **>(&c->pinned), c->pinned_bytes)) != cudaSuccess)
     return die("cudaMallocHost", e);
   if ((e = cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking)) != cudaSuccess)
@@ -506,7 +528,7 @@ static int inject_now(adept_ctx *c, const adept_primary *prim, uint64_t n) {
       if (sparse) top[k] += m;
       done += m;
     }
-    set_counts_kernel<<<1, 1, 0, c->stream>>>(c->params.ctl, k, n_cur[k], top[k], sparse ? top[k] : n_cur[k]);
+    set_counts_kernel<<<1, 1, 0, c->stream>>>(c->params.ctl, c->launch_index, k, n_cur[k], top[k], sparse ? top[k] : n_cur[k]);
     CU(c, cudaGetLastError());
   }
   for (uint64_t i = 0; i < n; ++i)
@@ -593,7 +615,7 @@ int adept_load_tracks(adept_ctx *c, uint32_t kind, const adept_track *tracks, ui
   }
   if (sparse && !slots) top = next_slot;
   c->live_hint += n;
-  set_counts_kernel<<<1, 1, 0, c->stream>>>(c->params.ctl, int(kind), n_cur, top, sparse ? top : n_cur);
+  set_counts_kernel<<<1, 1, 0, c->stream>>>(c->params.ctl, c->launch_index, int(kind), n_cur, top, sparse ? top : n_cur);
   CU(c, cudaGetLastError());
   return ADEPT_OK;
 }
@@ -633,6 +655,7 @@ int adept_read_tracks(adept_ctx *c, uint32_t kind, adept_track *out, uint64_t ca
 #endif
 static int launch_iteration(adept_ctx *c) {
   const adept_ctx::Shape &sh = (c->large.grid != 0u && c->live_hint >= ADEPT_LARGE_SHAPE_MIN_TRACKS) ? c->large : c->small;
+  c->params.it = c->launch_index++;
   CU(c, c->ops->launch_step(c->cfg.scheme, c->cfg.instrument ? 1 : 0, c->params, sh.threads, sh.grid, sh.dyn_smem,
                             c->stream));
   return ADEPT_OK;
@@ -736,6 +759,14 @@ int adept_read_sections(adept_ctx *c, uint64_t *cycles) {
                                 (size_t(2) * c->geo.n_layers + 1);
   for (int i = 0; i < kNumSections; ++i) cycles[i] = s[i];
   return rc;
+}
+
+uint32_t adept_launch_index(const adept_ctx *c) { return c ? c->launch_index : 0u; }
+
+int adept_set_launch_index(adept_ctx *c, uint32_t index) {
+  if (!c) return ADEPT_EINVAL;
+  c->launch_index = index;
+  return ADEPT_OK;
 }
 
 uint64_t adept_field_offset_kind(int32_t layout, uint32_t kind, uint32_t capacity, uint32_t slot, uint32_t field) {

@@ -72,24 +72,36 @@ __host__ __device__ constexpr size_t step_smem_bytes(int scheme, size_t table_by
 // warps and CTAs arrive.  Range 2^32 MeV (4.3e3 TeV) per slab.
 constexpr double kTallyUnit = 1.0 / 4294967296.0;
 
+// Iteration control without a "last CTA".  Every launch carries its
+// launch index `it` (Params::it, counted by the host).  The per-iteration counters are kept three
+// deep, indexed by launch index modulo 3: launch `it` reads n[it % 3] (what is alive), accumulates its
+// outputs into n[(it + 1) % 3] and its statistics into alive/esc[it % 3]; nobody touches the third
+// buffer during the launch, which is where the first warp of CTA 0 works: at the start of launch `it`
+// it closes launch it - 1 (adds its statistics to the cumulative counters, then clears its buffers for
+// launch it + 2) and opens launch `it`.  No CTA has to be the last one, so the end of an iteration is
+// not a link in the chain of round trips a small population's iteration consists of.
+// The host reads the control block only through close_kernel (adept_api.cu), which closes whatever
+// is open and writes the summary fields n_cur / parity.
 struct Ctl {
-  // dense: tracks in the current / next array.  sparse: length of the current / next slot list.
-  uint32_t n_cur[4];
-  uint32_t n_next[4];
-  uint32_t slot_top[4];  // sparse: bump allocator of never-recycled slots (rule S30)
-  uint32_t parity;       // which array / list is "current"
-  uint32_t overflow;     // sticky
-  uint32_t done_ctas;    // ticket counter: the last CTA of a step kernel ends the iteration
-  uint32_t bad_input;    // set by load_kernel when a record breaks the preconditions of adept_load_tracks
-  uint32_t it_alive[4];    // this iteration: parents that survive, per kind (reset at iteration end)
-  uint32_t it_escaped[4];  // this iteration: parents that left the calorimeter, per kind
+  uint32_t n[3][4];       // dense: tracks in the array; sparse: length of the slot list -- by launch index % 3
+  uint32_t alive[3][4];   // parents that survived the launch, per kind
+  uint32_t esc[3][4];     // parents that left the calorimeter in the launch, per kind
+  // sparse scheme with ADEPT_FLAG_RECYCLE_SLOTS: ring of freed slots per kind (KindStorage::free_ring).
+  // Monotonic counters, ring index = counter % capacity.  Slots freed in launch `it` are pushed at
+  // `free_tail` and become allocatable in launch it + 1: ring_tail[it % 3] is the tail as it was when
+  // launch `it` began (pushes of launch `it` are also counted into ring_tail[(it + 1) % 3], to which
+  // CTA 0 adds ring_tail[it % 3] itself), and pops take positions below it, so pushes and pops never
+  // meet inside a launch.  A pop that runs past it gives the excess back (free_head never passes it).
+  uint32_t ring_tail[3][4];
+  uint32_t slot_top[4];   // sparse: bump allocator of never-recycled slots (rule S30)
+  uint32_t free_head[4], free_tail[4];
+  uint32_t overflow;      // sticky
+  uint32_t bad_input;     // set by load_kernel when a record breaks the preconditions of adept_load_tracks
+  uint32_t closed;        // launches closed so far (= the index of the next launch once everything is closed)
+  uint32_t parity;        // summary (close_kernel): which array / list is "current" for the next launch
+  uint32_t n_cur[4];      // summary (close_kernel): live tracks per kind
   unsigned long long steps[3], secondaries[3], killed[3], escaped_n[3], slots_used[3];
   unsigned long long iterations;
-  // sparse scheme with ADEPT_FLAG_RECYCLE_SLOTS: ring of freed slots per kind (KindStorage::free_ring).
-  // Monotonic counters, ring index = counter % capacity.  Slots freed in iteration n are pushed at
-  // `free_tail` and become allocatable in iteration n + 1: an iteration pops only below
-  // `free_tail_start` (the tail at its start), so pushes and pops never meet inside a launch.
-  uint32_t free_head[4], free_tail[4], free_tail_start[4];
   // unsigned long long tally[n_slabs + 1] follows at byte kCtlHeaderBytes: fixed-point energy
   // deposit per slab, then the energy carried out of the calorimeter
 };
@@ -120,6 +132,7 @@ struct Params {
   uint32_t capacity;         // slots per kind (multiple of 128)
   uint32_t recycle;          // sparse scheme: 1 = freed slots are reused (ADEPT_FLAG_RECYCLE_SLOTS)
   uint32_t physics;          // adept_tables.physics: 1 = extended rules X36-X38
+  uint32_t it;               // index of this launch (counted by the host; see Ctl)
   KindStorage kind[3];
   unsigned long long *instr_field_rw;  // [3][14][2], instrumented build
   // SoA and AoS layouts, dense scheme: tensor maps of the record buffers, [kind][parity] (see

@@ -389,58 +389,76 @@ struct CtaShared {
 };
 
 // A9 + A11: the last CTA closes the iteration.
-// Run by the first warp of the last CTA: lane k < 3 closes kind k, so that the dependent global
-// accesses of the three kinds overlap (an iteration of a small population is a chain of memory round
-// trips; this is its last link).
-template <int SCHEME, int VAR> __device__ void finish_iteration(const Params &p, int lane) {
-  Ctl *c = p.ctl;
-  uint32_t n = 0u, nn = 0u;
-  constexpr bool RECYCLE = (VAR & V_RECYCLE) != 0;
-  if (lane < 3) {
-    const int k = lane;
-    n = c->n_cur[k];
-    nn = __ldcg(&c->n_next[k]);
-    const uint32_t alive = __ldcg(&c->it_alive[k]);
-    const uint32_t esc = __ldcg(&c->it_escaped[k]);
-    uint32_t top = 0u, head = 0u, start = 0u, tail = 0u;
-    if (SCHEME == S_SPARSE) top = __ldcg(&c->slot_top[k]);
-    if (SCHEME == S_SPARSE && RECYCLE) {
-      head = __ldcg(&c->free_head[k]); start = c->free_tail_start[k]; tail = __ldcg(&c->free_tail[k]);
+// A11 / A0 (see Ctl, device_state.cuh).  Run by one warp, lane k < 3 = kind k, so that the dependent
+// global accesses of the three kinds overlap: the first warp of CTA 0 at the start of launch `it`
+// (open = true), and close_kernel before the host reads the control block (open = false).
+// close: every launch below `it` that is still open gets its statistics added to the cumulative
+// counters and its buffers cleared for the launch two after it.  open: launch `it` is counted.
+template <bool SPARSE, bool RECYCLE>
+__device__ __forceinline__ void roll_iterations(Ctl *c, uint32_t capacity, uint32_t it, bool open, int lane
+#ifdef ADEPT_TIMING_SECTIONS
+                                                , unsigned long long *sections
+#endif
+) {
+  const int k = lane < 3 ? lane : 0;
+  for (uint32_t j = c->closed; j != it; ++j) {  // normally one launch (it - 1), or none
+    const uint32_t b = j % 3u, b1 = (j + 1u) % 3u;
+    if (lane < 3) {
+      const uint32_t raw = c->n[b][k], n = raw < capacity ? raw : capacity;
+      const uint32_t out = __ldcg(&c->n[b1][k]);
+      const uint32_t alive = __ldcg(&c->alive[b][k]), esc = __ldcg(&c->esc[b][k]);
+      const unsigned long long killed = c->killed[k], escaped = c->escaped_n[k], secondaries = c->secondaries[k],
+                               used = c->slots_used[k];
+      c->killed[k] = killed + (n - alive);
+      c->escaped_n[k] = escaped + esc;
+      c->secondaries[k] = secondaries + (out - alive);
+      if (out > capacity) c->overflow = 1u;
+      if (SPARSE) {
+        uint32_t top = __ldcg(&c->slot_top[k]);
+        if (top > capacity) { top = capacity; c->overflow = 1u; }
+        if (top > used) c->slots_used[k] = top;
+      } else {
+        const uint32_t live = out < capacity ? out : capacity;
+        if (live > used) c->slots_used[k] = live;
+      }
+      c->n[b][k] = 0u; c->alive[b][k] = 0u; c->esc[b][k] = 0u;
+      if (SPARSE && RECYCLE) c->ring_tail[b][k] = 0u;
     }
-    const unsigned long long steps = c->steps[k], killed = c->killed[k], escaped = c->escaped_n[k],
-                             secondaries = c->secondaries[k], used = c->slots_used[k];
-    c->steps[k] = steps + n;
-    c->killed[k] = killed + (n - alive);
-    c->escaped_n[k] = escaped + esc;
-    c->secondaries[k] = secondaries + (nn - alive);
-    if (nn > p.capacity) { nn = p.capacity; c->overflow = 1u; }
-    if (SCHEME == S_SPARSE) {
-      if (top > p.capacity) { top = p.capacity; c->slot_top[k] = top; c->overflow = 1u; }
-      if (top > used) c->slots_used[k] = top;
-    } else {
-      if (nn > used) c->slots_used[k] = nn;
+#ifdef ADEPT_TIMING_SECTIONS
+    if (lane == 0) {  // launch timeline: first CTA start -> last CTA end of launch j (ns)
+      unsigned long long *w = sections + kNumSections + 2u * (j & 1u);  // scratch of launch j: {min start, max end}
+      if (w[1] > w[0] && w[0] != ~0ull) sections[6] += w[1] - w[0];
+      w[0] = ~0ull;
+      w[1] = 0ull;
     }
-    c->n_cur[k] = nn;
-    c->n_next[k] = 0u;
-    c->it_alive[k] = 0u;
-    c->it_escaped[k] = 0u;
-    if (SCHEME == S_SPARSE && RECYCLE) {
-      // slots freed in this iteration become allocatable in the next one; pops that ran past the
-      // allocatable part of the ring took bump-allocated slots instead (interact_batch)
-      if (static_cast<int32_t>(head - start) > 0) c->free_head[k] = start;
-      c->free_tail_start[k] = tail;
-    }
+#endif
   }
-  const uint32_t live_before = __reduce_add_sync(0xFFFFFFFFu, n), live_after = __reduce_add_sync(0xFFFFFFFFu, nn);
-  if (SCHEME == S_SPARSE && live_after == 0u && lane < 3) {
-    // rule S30: slots are reused (without recycling: only) once the buffer is empty
-    const int k = lane;
-    c->slot_top[k] = 0u; c->free_head[k] = 0u; c->free_tail[k] = 0u; c->free_tail_start[k] = 0u;
+  __syncwarp();
+  const uint32_t bi = it % 3u;
+  uint32_t n_now = 0u;
+  if (lane < 3) {
+    const uint32_t raw = c->n[bi][k];
+    n_now = raw < capacity ? raw : capacity;
+  }
+  const uint32_t live = __reduce_add_sync(0xFFFFFFFFu, n_now);
+  if (lane < 3) {
+    if (SPARSE && live == 0u) {  // rule S30: slots are reused (without recycling: only) once the buffer is empty
+      c->slot_top[k] = 0u; c->free_head[k] = 0u; c->free_tail[k] = 0u;
+      c->ring_tail[0][k] = 0u; c->ring_tail[1][k] = 0u; c->ring_tail[2][k] = 0u;
+    }
+    if (open) {
+      c->steps[k] += n_now;
+      // the tail of the free ring at the start of launch it + 1 = the tail at the start of this launch
+      // + what this launch pushes (added by the pushing groups themselves)
+      if (SPARSE && RECYCLE && live != 0u) atomicAdd(&c->ring_tail[(it + 1u) % 3u][k], c->ring_tail[bi][k]);
+    } else {
+      c->n_cur[k] = n_now;  // summary for the host
+    }
   }
   if (lane == 0) {
-    c->parity ^= 1u;
-    if (live_before) c->iterations += 1ull;
-    c->done_ctas = 0u;
+    c->closed = it;
+    if (open) { if (live) c->iterations += 1ull; }
+    else c->parity = it & 1u;
   }
 }
 
@@ -602,14 +620,17 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
       g.acc[sbuf] = 0u;  // next used two tiles from now, behind a group barrier
       g.qtot[sbuf] = queued + count_of(total, 1);
       const uint32_t n_out = count_of(total, 0), n_esc = count_of(total, 2);
-      g.base[sbuf][0] = n_out ? atomicAdd(&ctl->n_next[KIND], n_out) : 0u;
+      g.base[sbuf][0] = n_out ? atomicAdd(&ctl->n[(p.it + 1u) % 3u][KIND], n_out) : 0u;
       if (n_out) atomicAdd(&c.cta->alive[KIND], n_out);
       if (n_esc) atomicAdd(&c.cta->escaped[KIND], n_esc);
       if (SCHEME == S_SPARSE && recycle) {
         const uint32_t first = tile * kGroup;
         const uint32_t n_tile = (n_kind - first < uint32_t(kGroup)) ? n_kind - first : uint32_t(kGroup);
         const uint32_t n_end = n_tile - n_out - count_of(total, 1);
-        if (n_end) g.fbase[sbuf] = atomicAdd(&ctl->free_tail[KIND], n_end);
+        if (n_end) {
+          g.fbase[sbuf] = atomicAdd(&ctl->free_tail[KIND], n_end);
+          atomicAdd(&ctl->ring_tail[(p.it + 1u) % 3u][KIND], n_end);
+        }
       }
     }
   }
@@ -715,8 +736,9 @@ __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &e
           uint32_t n_ring = 0u, h = 0u;
           if (recycle && want) {
             h = atomicAdd(&ctl->free_head[d], want);
-            const int32_t avail = static_cast<int32_t>(ctl->free_tail_start[d] - h);
+            const int32_t avail = static_cast<int32_t>(ctl->ring_tail[p.it % 3u][d] - h);
             n_ring = avail <= 0 ? 0u : (uint32_t(avail) < want ? uint32_t(avail) : want);
+            if (n_ring != want) atomicSub(&ctl->free_head[d], want - n_ring);  // the head never passes the allocatable tail
           }
           g.rbase[sbuf][q] = h;
           g.rn[sbuf][q] = n_ring;
@@ -729,11 +751,14 @@ __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &e
           got = n_ring + usable;
           g.sgot[sbuf][q] = got;
         }
-        g.base[sbuf][q] = got ? atomicAdd(&ctl->n_next[d], got) : 0u;
+        g.base[sbuf][q] = got ? atomicAdd(&ctl->n[(p.it + 1u) % 3u][d], got) : 0u;
       }
       if (SCHEME == S_SPARSE && recycle) {
         const uint32_t n_end = batch - count_of(total, KIND);
-        if (n_end) g.fbase[sbuf] = atomicAdd(&ctl->free_tail[KIND], n_end);
+        if (n_end) {
+          g.fbase[sbuf] = atomicAdd(&ctl->free_tail[KIND], n_end);
+          atomicAdd(&ctl->ring_tail[(p.it + 1u) % 3u][KIND], n_end);
+        }
       }
     }
   }
@@ -929,17 +954,28 @@ __global__ void __launch_bounds__(THREADS, (THREADS == kBlockSmall) ? ADEPT_STEP
   if (tid < kNumSections) sh.sect[tid] = 0u;
   asm volatile("griddepcontrol.wait;" ::: "memory");  // the previous launch has completed and its writes are visible
 #ifdef ADEPT_TIMING_SECTIONS
-  // launch timeline (timing build): sections[6] += first CTA start -> last CTA done (ns),
-  // sections[7] += the last CTA's end-of-iteration work (ns); sections[kNumSections] = scratch
+  // launch timeline (timing build): sections[6] += first CTA start -> last CTA end (ns), added when the
+  // launch is closed (roll_iterations); sections[kNumSections ..] = scratch {min start, max end} by launch parity
   unsigned long long t_cta_start = 0ull;
   if (tid == 0) {
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_cta_start));
-    atomicMin(&p.sections[kNumSections], t_cta_start);
+    atomicMin(&p.sections[kNumSections + 2u * (p.it & 1u)], t_cta_start);
   }
 #endif
-  // A0: what is alive (written by the previous iteration's last CTA; constant during this launch)
-  const uint32_t par = ctl->parity;
-  const uint32_t n0 = ctl->n_cur[0], n1 = ctl->n_cur[1], n2 = ctl->n_cur[2];
+  // A0: what is alive -- the outputs of the previous launch (complete: it has ended); constant during this launch
+  const uint32_t par = p.it & 1u;
+  const uint32_t bi = p.it % 3u;
+  const uint32_t r0 = ctl->n[bi][0], r1 = ctl->n[bi][1], r2 = ctl->n[bi][2];
+  const uint32_t n0 = r0 < p.capacity ? r0 : p.capacity, n1 = r1 < p.capacity ? r1 : p.capacity,
+                 n2 = r2 < p.capacity ? r2 : p.capacity;
+  // A11 of the previous launch and A0 of this one, off everybody's critical path: first warp of CTA 0
+  if (blockIdx.x == 0 && tid < 32) {
+#ifdef ADEPT_TIMING_SECTIONS
+    roll_iterations<SCHEME == S_SPARSE, (VAR & V_RECYCLE) != 0>(ctl, p.capacity, p.it, true, tid, p.sections);
+#else
+    roll_iterations<SCHEME == S_SPARSE, (VAR & V_RECYCLE) != 0>(ctl, p.capacity, p.it, true, tid);
+#endif
+  }
   const uint32_t t0 = (n0 + kGroup - 1) / kGroup, t1 = (n1 + kGroup - 1) / kGroup, t2 = (n2 + kGroup - 1) / kGroup;
   const uint32_t tiles = t0 + t1 + t2;
   __syncthreads();
@@ -971,8 +1007,8 @@ __global__ void __launch_bounds__(THREADS, (THREADS == kBlockSmall) ? ADEPT_STEP
       if (v != 0ull && atomicAdd(&p.tally[s], v) + v < v) ctl->overflow = 1u;  // 2^32 MeV in one bin: reported, not wrapped silently
     }
     if (tid < 3) {
-      if (sh.alive[tid]) atomicAdd(&ctl->it_alive[tid], sh.alive[tid]);
-      if (sh.escaped[tid]) atomicAdd(&ctl->it_escaped[tid], sh.escaped[tid]);
+      if (sh.alive[tid]) atomicAdd(&ctl->alive[bi][tid], sh.alive[tid]);
+      if (sh.escaped[tid]) atomicAdd(&ctl->esc[bi][tid], sh.escaped[tid]);
     }
     if (INSTR) {
       for (int s = tid; s < 3 * kNumFields * 2; s += kBlock)
@@ -980,33 +1016,13 @@ __global__ void __launch_bounds__(THREADS, (THREADS == kBlockSmall) ? ADEPT_STEP
     }
   }
 
-  // A11: the last CTA to arrive ends the iteration
-  __syncthreads();
-  if (tid < 32) {
-    uint32_t ticket = 0u;
-    if (tid == 0) {
-      __threadfence();
-      ticket = atomicAdd(&ctl->done_ctas, 1u);
-    }
-    ticket = __shfl_sync(0xFFFFFFFFu, ticket, 0);
-    if (ticket == gridDim.x - 1) {
-      __threadfence();
 #ifdef ADEPT_TIMING_SECTIONS
-      unsigned long long t0 = 0ull, t1 = 0ull;
-      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
-      finish_iteration<SCHEME, VAR>(p, tid);
-      __threadfence();
-      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
-      if (tid == 0) {
-        p.sections[6] += t0 - p.sections[kNumSections];
-        p.sections[7] += t1 - t0;
-        p.sections[kNumSections] = ~0ull;
-      }
-#else
-      finish_iteration<SCHEME, VAR>(p, tid);
-#endif
-    }
+  if (tid == 0) {
+    unsigned long long t_end;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_end));
+    atomicMax(&p.sections[kNumSections + 2u * (p.it & 1u) + 1u], t_end);
   }
+#endif
 }
 
 // ------------------------------------------------------------- host <-> buffer helper kernels --

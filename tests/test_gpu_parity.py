@@ -900,7 +900,7 @@ def test_timing_variant_computes_the_same_and_fills_its_section_clocks():
         assert res[0][3].sum() == 0                                   # the plain library keeps no clocks
         s = res[1][3]
         assert (s[1:6] > 0).all() and s[4] + s[5] < s[:6].sum()       # load, move, interact, alloc, store all ran
-        assert s[6] > 0 and s[7] > 0                                  # launch timeline (ns)
+        assert s[6] > 0                                               # launch timeline (ns)
 
 
 @pytest.mark.parametrize("scheme", SCHEMES)
