@@ -259,6 +259,12 @@ class Context:
         self._check(self._L.adept_read_counters(self._h, rw.ctypes.data, lines.ctypes.data, slots.ctypes.data))
         return dict(field_rw=rw, lines=lines, slots=slots)
 
+    def launch_index(self) -> int:
+        return int(self._L.adept_launch_index(self._h))
+
+    def set_launch_index(self, index: int):
+        self._check(self._L.adept_set_launch_index(self._h, index))
+
     def snapshot(self):
         """(workspace copy, launch index): what `rewind` needs (adept.h "Workspace").  No call may be in flight."""
         return self.workspace.clone(), int(self._L.adept_launch_index(self._h))

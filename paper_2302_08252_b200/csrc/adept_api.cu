@@ -655,7 +655,8 @@ int adept_read_tracks(adept_ctx *c, uint32_t kind, adept_track *out, uint64_t ca
 #endif
 static int launch_iteration(adept_ctx *c) {
   const adept_ctx::Shape &sh = (c->large.grid != 0u && c->live_hint >= ADEPT_LARGE_SHAPE_MIN_TRACKS) ? c->large : c->small;
-  c->params.it = c->launch_index++;
+  c->params.it = c->launch_index;
+  c->launch_index = next_launch(c->launch_index);
   CU(c, c->ops->launch_step(c->cfg.scheme, c->cfg.instrument ? 1 : 0, c->params, sh.threads, sh.grid, sh.dyn_smem,
                             c->stream));
   return ADEPT_OK;
@@ -764,7 +765,7 @@ int adept_read_sections(adept_ctx *c, uint64_t *cycles) {
 uint32_t adept_launch_index(const adept_ctx *c) { return c ? c->launch_index : 0u; }
 
 int adept_set_launch_index(adept_ctx *c, uint32_t index) {
-  if (!c) return ADEPT_EINVAL;
+  if (!c || index >= kLaunchWrap) return ADEPT_EINVAL;
   c->launch_index = index;
   return ADEPT_OK;
 }

@@ -82,6 +82,12 @@ constexpr double kTallyUnit = 1.0 / 4294967296.0;
 // not a link in the chain of round trips a small population's iteration consists of.
 // The host reads the control block only through close_kernel (adept_api.cu), which closes whatever
 // is open and writes the summary fields n_cur / parity.
+// Launch indices count modulo kLaunchWrap, a multiple of 6 just below 2^32, so that `it % 3` and
+// `it & 1` stay continuous when the counter wraps (after 4e9 launches).
+constexpr uint32_t kLaunchWrap = 4294967292u;
+static_assert(kLaunchWrap % 6u == 0u, "parity and buffer index must survive the wrap");
+__host__ __device__ constexpr uint32_t next_launch(uint32_t it) { return it + 1u == kLaunchWrap ? 0u : it + 1u; }
+
 struct Ctl {
   uint32_t n[3][4];       // dense: tracks in the array; sparse: length of the slot list -- by launch index % 3
   uint32_t alive[3][4];   // parents that survived the launch, per kind

@@ -401,7 +401,7 @@ __device__ __forceinline__ void roll_iterations(Ctl *c, uint32_t capacity, uint3
 #endif
 ) {
   const int k = lane < 3 ? lane : 0;
-  for (uint32_t j = c->closed; j != it; ++j) {  // normally one launch (it - 1), or none
+  for (uint32_t j = c->closed; j != it; j = next_launch(j)) {  // normally one launch (it - 1), or none
     const uint32_t b = j % 3u, b1 = (j + 1u) % 3u;
     if (lane < 3) {
       const uint32_t raw = c->n[b][k], n = raw < capacity ? raw : capacity;

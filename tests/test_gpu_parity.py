@@ -935,3 +935,49 @@ def test_extended_physics_forced_interactions(scheme):
             g = ctx.result()
             assert np.allclose(g["edep_slab"], r["edep_slab"], rtol=1e-9, atol=1e-9)
             ctx.destroy()
+
+
+# ------------------------------------------------------------------ iteration control --------------
+def test_snapshot_rewind_and_launch_index_wrap():
+    """include/adept.h "Workspace": a workspace copy + launch index rewinds a context; and the launch
+    index, by which the device keeps its per-iteration counters three deep, wraps at a multiple of 6
+    just below 2^32 without a seam (the context is started a few launches before the wrap by setting
+    the index and the control block's `closed` word, byte 248, to the same value)."""
+    import torch
+    c = CONFIGS["tiny"]
+    geo, tab = geometry_for("tiny"), tables_for("tiny")
+    prim = gen_primaries(c["n_primaries"], c["e_primary"])
+    o = Oracle(geo, tab, seed=c["seed"])
+    o.inject(prim)
+    o.run()
+    r = o.result()
+    for scheme, flags in (("dense", 0), ("sparse", 0), ("sparse", 1)):
+        ctx = _ctx(geo, tab, layout="aosoa32", scheme=scheme, capacity=c["capacity"], seed=c["seed"], flags=flags)
+        ctx.inject(prim)
+        for _ in range(5):
+            ctx.step(sync=False)
+        snap = ctx.snapshot()
+        assert snap[1] == 5 == ctx.launch_index()
+        a = ctx.run()
+        ctx.rewind(snap)
+        b = ctx.run()
+        for res in (a, b):
+            compare_counts(res, r, what=scheme)
+            assert res["iterations"] == r["iterations"]
+        assert (a["edep_slab"] == b["edep_slab"]).all()
+        ctx.destroy()
+        # the same run across the wrap of the launch index
+        wrap = 4294967292
+        ctx = _ctx(geo, tab, layout="aosoa32", scheme=scheme, capacity=c["capacity"], seed=c["seed"], flags=flags)
+        start = wrap - 7
+        ctx.workspace[248:252] = torch.tensor(list(int(start).to_bytes(4, "little")), dtype=torch.uint8, device=ctx.workspace.device)
+        torch.cuda.synchronize()
+        ctx.set_launch_index(start)
+        ctx.inject(prim)
+        g = ctx.run()
+        compare_counts(g, r, what=scheme + " across the wrap")
+        assert g["iterations"] == r["iterations"] and ctx.launch_index() < 100
+        assert (g["edep_slab"] == a["edep_slab"]).all()
+        with pytest.raises(Exception):
+            ctx.set_launch_index(wrap)
+        ctx.destroy()
