@@ -353,8 +353,8 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
         "clocks": clocks,
         "gpu_launches": args.steps,
         "e2e": {"value": e2e_value, "unit": "track-steps/s", "h2d_bytes_per_step": 56 * n_tracks,
-                "d2h_bytes_per_step": d2h + 256, "steps": e2e_steps,
-                "counts_only": {"value": e2e_counts_only, "unit": "track-steps/s", "d2h_bytes_per_step": 256,
+                "d2h_bytes_per_step": d2h + 512, "steps": e2e_steps,
+                "counts_only": {"value": e2e_counts_only, "unit": "track-steps/s", "d2h_bytes_per_step": 512,
                                 "what": "adept_load_tracks x3 + adept_step with its adept_counts read back"},
                 "what": "adept_load_tracks x3 (pinned host) + adept_step + adept_read_tracks x3"},
         "roofline": {"bound": "hbm", "achieved": m["algorithmic_GBps"], "peak": peak, "unit": "GB/s",
@@ -459,7 +459,7 @@ def showers(args, name: str, *, layout: str, scheme: str, steps: int, warmup: in
            "secondaries": [int(x) for x in res["secondaries"]], "slots_used": [int(x) for x in res["slots_used"]],
            "edep_layer_MeV": [float(x) for x in res["edep_layer"]],
            "energy_balance_rel": float((res["edep_slab"].sum() + res["e_escaped"]) / res["e_injected"] - 1.0),
-           "h2d_bytes_per_run": 32 * c["n_primaries"], "d2h_bytes_per_run": 256 + 8 * (2 * c["n_layers"] + 1)}
+           "h2d_bytes_per_run": 32 * c["n_primaries"], "d2h_bytes_per_run": 512 + 8 * (2 * c["n_layers"] + 1 + 12)}
     if with_cpu:                                           # heavy: the oracle needs ~80 s
         from oracle import Oracle
         o = Oracle(geo, tab, seed=c["seed"])

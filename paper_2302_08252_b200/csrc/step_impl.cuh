@@ -5,8 +5,9 @@
 // particle type are processed by a dedicated kernel"; here the three passes share one persistent
 // grid so that an iteration costs one launch, and a tile always holds one type, so divergence
 // between types never occurs inside a warp).  SURVEY.md §8(a) rows:
-//   A0/A11  iteration control: counts live on the device; the last CTA to finish ends the
-//           iteration (swap current/next, reset counters) -- no host round trip;
+//   A0/A11  iteration control: counts live on the device, three deep by launch index; the first warp
+//           of CTA 0 closes the previous launch and opens this one at kernel start (roll_iterations)
+//           -- no host round trip, and no CTA that has to be the last;
 //   A1      track load through the layout accessor (layout.cuh); dense scheme: the next tile is
 //           fetched into shared memory by TMA while the current one is stepped;
 //   A2-A8   the physics/geometry step (physics.cuh), tables staged in shared memory by one TMA
@@ -388,7 +389,6 @@ struct CtaShared {
   GroupShared grp[kMaxGroupsPerCta];
 };
 
-// A9 + A11: the last CTA closes the iteration.
 // A11 / A0 (see Ctl, device_state.cuh).  Run by one warp, lane k < 3 = kind k, so that the dependent
 // global accesses of the three kinds overlap: the first warp of CTA 0 at the start of launch `it`
 // (open = true), and close_kernel before the host reads the control block (open = false).
@@ -1191,7 +1191,7 @@ template <int L> struct OpsImpl {
       if (e != cudaSuccess) return e;
       // Programmatic dependent launch: the CTAs of this launch may become resident, and run their
       // prologue up to griddepcontrol.wait, while the previous kernel of the stream is still finishing
-      // (its last CTA closes the iteration alone) -- iterations of small populations are a chain of
+      // (its slowest CTA alone) -- iterations of small populations are a chain of
       // latencies, and this takes the launch latency out of it.
       cudaLaunchConfig_t cfg = {};
       cfg.gridDim = dim3(grid);
