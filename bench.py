@@ -229,10 +229,20 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
     from paper_2302_08252_b200 import Context
     from paper_2302_08252_b200.binding import TRACK_DTYPE
     dist = None
+    # Test hook (tests/test_bench_contract.py): ADEPT_BENCH_ONE_DEVICE=1 runs every rank on cuda:0 with
+    # the gloo backend, to exercise the N > 1 plumbing on a one-GPU box.  The ranks' kernels never wait
+    # on one another (the only exchanges are host-side barriers and all-reduces), so this is a test of
+    # the code path, not a measurement.
+    one_device = os.environ.get("ADEPT_BENCH_ONE_DEVICE") == "1"
+    if one_device:
+        local_rank = 0
     if world > 1:
         import torch.distributed as dist
         torch.cuda.set_device(local_rank)
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        if one_device:
+            dist.init_process_group("gloo")
+        else:
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
 
@@ -243,7 +253,7 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
     def max_over_ranks(x: float) -> float:
         if dist is None:
             return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        t = torch.tensor([x], dtype=torch.float64, device="cpu" if one_device else dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         return float(t.item())
 
@@ -329,7 +339,8 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
     # ---- N > 1: the event-sharded heavy showers beside the weak-scaled step ----
     sharded = None
     if world > 1 and "showers" in args.extras:
-        sharded = sharded_showers(args, "heavy", rank, world, local_rank, dist, max_over_ranks)
+        sharded = sharded_showers(args, "heavy" if "heavy" in args.extras else "full", rank, world, local_rank, dist,
+                                  max_over_ranks, reduce_on_cpu=one_device)
 
     if rank != 0:
         if dist is not None:
@@ -366,7 +377,7 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
         "layouts": per_layout,
     }
     if sharded is not None:
-        out["showers"] = {"heavy_sharded": sharded}
+        out["showers"] = {("heavy" if "heavy" in args.extras else "full") + "_sharded": sharded}
     if world == 1 and not args.no_cpu:
         n, dt, r = oracle_single_step(pop, n_tracks, want_tracks=True)
         out["cpu_baseline"] = {"value": n / dt, "unit": "track-steps/s", "cores": 1, "host_cores": host_cores(),
@@ -480,7 +491,7 @@ def showers(args, name: str, *, layout: str, scheme: str, steps: int, warmup: in
     return out
 
 
-def sharded_showers(args, name, rank, world, local_rank, dist, max_over_ranks) -> dict:
+def sharded_showers(args, name, rank, world, local_rank, dist, max_over_ranks, reduce_on_cpu=False) -> dict:
     """N > 1: the primaries of `name` split over the ranks, one context per GPU, one
     all-reduce of the tallies at the end (paper_2302_08252_b200/sharding.py).  Strong scaling: the
     total work is fixed."""
@@ -498,7 +509,7 @@ def sharded_showers(args, name, rank, world, local_rank, dist, max_over_ranks) -
         torch.cuda.synchronize()
         dist.barrier()
         t0 = time.perf_counter()
-        res = run_sharded(ctx, prim, rank, world)
+        res = run_sharded(ctx, prim, rank, world, device="cpu" if reduce_on_cpu else None)
         torch.cuda.synchronize()
         dt = max_over_ranks(time.perf_counter() - t0)
         if it > 0:

@@ -48,10 +48,11 @@ def reduce_results(res: dict, device=None, group=None) -> dict:
     return out
 
 
-def run_sharded(ctx, primaries: np.ndarray, rank: int, world: int, group=None) -> dict:
-    """Inject this rank's slice of `primaries` with their global indices, run to completion, reduce."""
+def run_sharded(ctx, primaries: np.ndarray, rank: int, world: int, group=None, device=None) -> dict:
+    """Inject this rank's slice of `primaries` with their global indices, run to completion, reduce
+    (on `device`, default the context's: NCCL reduces device tensors, gloo host tensors)."""
     lo, hi = shard_range(primaries.shape[0], rank, world)
     ctx.set_primary_index(lo)
     ctx.inject(primaries[lo:hi])
     res = ctx.run()
-    return reduce_results(res, device=getattr(ctx, "device", None), group=group)
+    return reduce_results(res, device=device if device is not None else getattr(ctx, "device", None), group=group)

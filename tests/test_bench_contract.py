@@ -74,3 +74,23 @@ def test_gpu_arm_prints_one_contract_line():
     p = d["parity_full_size"]
     assert p["counts_bit_exact"] and p["tracks_with_another_fate"] == 0 and p["tracks_with_any_word_differing"] == 0
     assert set(d["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
+
+
+@pytest.mark.gpu
+def test_gpu_arm_two_ranks_plumbing_on_one_device():
+    """`bench.py --gpus 2` launches its two ranks, shards the single-step population by rank (weak
+    scaling, max over ranks) and the showers by primaries (one all-reduce of the tallies).  On this
+    one-GPU box both ranks run on cuda:0 over gloo (ADEPT_BENCH_ONE_DEVICE: plumbing test, not a timing)."""
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK")}
+    env["ADEPT_BENCH_ONE_DEVICE"] = "1"
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "3", "--warmup", "3",
+                          "--tracks", "262144", "--layout", "aosoa32", "--extras", "showers"],
+                         capture_output=True, text=True, timeout=900, env=env)
+    assert out.returncode == 0, out.stderr[-3000:]
+    lines = [l for l in out.stdout.split("\n") if l.strip().startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["scaling"] == "weak" and "cpu_baseline" not in d
+    assert d["config"]["parallelism"].startswith("independent track shards")
+    sh = d["showers"]["full_sharded"]
+    assert sh["scaling"] == "strong" and sh["iterations"] == 172 and sh["track_steps"] == 6999724   # config 2, summed over the ranks
