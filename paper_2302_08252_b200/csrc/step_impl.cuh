@@ -401,7 +401,11 @@ __device__ __forceinline__ void roll_iterations(Ctl *c, uint32_t capacity, uint3
 #endif
 ) {
   const int k = lane < 3 ? lane : 0;
-  for (uint32_t j = c->closed; j != it; j = next_launch(j)) {  // normally one launch (it - 1), or none
+  // normally one launch (it - 1) is open, or none; more than two can only mean that the launch index was
+  // set without the workspace copy that belongs to it (adept.h "Workspace"): then nothing is closed
+  uint32_t first = c->closed;
+  if ((it >= first ? it - first : it + (kLaunchWrap - first)) > 2u) first = it;
+  for (uint32_t j = first; j != it; j = next_launch(j)) {
     const uint32_t b = j % 3u, b1 = (j + 1u) % 3u;
     if (lane < 3) {
       const uint32_t raw = c->n[b][k], n = raw < capacity ? raw : capacity;
