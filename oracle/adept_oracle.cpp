@@ -56,7 +56,9 @@
 #include <cmath>
 #include <cstdint>
 #include <cstring>
+#include <array>
 #include <limits>
+#include <unordered_map>
 #include <vector>
 
 namespace {
@@ -86,8 +88,9 @@ struct TablesIn {          // as passed over the C interface
   uint32_t n_bins, n_materials;
   float e_min, e_max, ln_e_min, inv_dln, e_cut;
   const float *data;       // [mat][group][qty][n_bins+1]
-  uint32_t physics;        // rule X35: 0 = rules S16-S32, 1 = with the extended rules X36, X37
-  const float *data_x;     // physics 1: [mat][2][n_bins+1]: Sigma_delta of e+- (X36), Sigma_annihilation of e+ (X38) [1/mm]
+  uint32_t physics;        // rule X35: 0 = rules S16-S32, 1 = with the extended rules X36-X38, 2 = also X39
+  const float *data_x;     // physics >= 1: [mat][3][n_bins+1]: Sigma_delta of e+- (X36), Sigma_annihilation of e+ (X38),
+                           // transport cross-section Sigma_tr of e+- (X39) [1/mm]
 };
 
 struct Result {
@@ -106,7 +109,7 @@ struct TraceRec {          // one per processed track when tracing is on
 
 enum { KIND_EM = 0, KIND_EP = 1, KIND_GAMMA = 2 };
 enum { GROUP_GAMMA = 0, GROUP_ELEC = 1 };
-enum { W_ANNIH = -2, W_GEOM = -1, W_ELOSS = 3 };
+enum { W_ANNIH = -2, W_GEOM = -1, W_ELOSS = 3, W_MSC = 5 };
 enum { FACE_ZP = 0, FACE_ZM = 1, FACE_XY = 2 };
 
 const float INF = std::numeric_limits<float>::infinity();
@@ -218,7 +221,7 @@ struct Tables {
   const float *q(uint32_t mat, int group, int qty) const {
     return data.data() + ((size_t)(mat * 2 + group) * 3 + qty) * (n_bins + 1);
   }
-  const float *qx(uint32_t mat, int which) const { return data_x.data() + ((size_t)mat * 2 + which) * (n_bins + 1); }
+  const float *qx(uint32_t mat, int which) const { return data_x.data() + ((size_t)mat * 3 + which) * (n_bins + 1); }
 };
 
 struct Bin { int j; float f; };
@@ -274,6 +277,10 @@ struct Oracle {
   bool tracing = false;
   std::vector<TraceRec> trace;
   std::vector<Primary> pending;
+  // X39: the three multiple-scattering words of an e+- track (the paper's InitialRange,
+  // DynamicRangeFactor, TlimitMin), by track id; a track without an entry has
+  // InitialRange = -1 (not initialised).  They are not part of the 14-word record.
+  std::unordered_map<uint64_t, std::array<float, 3>> msc;
 
   float zlo(uint32_t i) const {   // S21 / DESIGN §4 geometry
     return fmaf((float)(i >> 1), pitch, (i & 1u) ? geo.abs_mm : 0.0f);
@@ -357,7 +364,15 @@ bool step_track(Oracle &o, int kind, Track &t, Child children[2], int &n_childre
     return finish(false);
   }
 
-  const bool extended = tab.physics == 1u;                       // X35
+  const bool extended = tab.physics >= 1u;                       // X35
+  const bool with_msc = tab.physics == 2u && kind != KIND_GAMMA;  // X39
+  const uint64_t track_key = ((uint64_t)t.id_hi << 32) | t.id_lo;
+  float m[3] = {-1.0f, 0.0f, 0.0f};
+  if (with_msc) {
+    auto it = o.msc.find(track_key);
+    if (it != o.msc.end()) { m[0] = it->second[0]; m[1] = it->second[1]; m[2] = it->second[2]; o.msc.erase(it); }
+  }
+  auto keep_msc = [&]() { if (with_msc) o.msc[track_key] = {m[0], m[1], m[2]}; };
   // X36: e+- process 1 = delta-ray production; X38: e+ process 2 = annihilation in flight
   const int NP = (kind == KIND_GAMMA) ? 3 : (extended ? (kind == KIND_EP ? 3 : 2) : 1);
   const int group = (kind == KIND_GAMMA) ? GROUP_GAMMA : GROUP_ELEC;
@@ -395,6 +410,22 @@ bool step_track(Oracle &o, int kind, Track &t, Child children[2], int &n_childre
 
   // S21: distance to the slab faces and to the transverse box.
   const float z_lo = o.zlo(vol0), z_hi = o.zlo(vol0 + 1u);
+  // X39a, X39b: multiple-scattering step limit max(DynamicRangeFactor * InitialRange, TlimitMin),
+  // (re-)initialised at the start of a track and after every slab crossing
+  float sig_tr = 0.0f, s_m = INF;
+  if (with_msc) {
+    sig_tr = interp(tab.qx(mat, 2), bin);
+    if (sig_tr > 0.0f) {
+      if (m[0] < 0.0f) {
+        float safety = fminf(t.pos[2] - z_lo, z_hi - t.pos[2]);
+        if (!(safety > 0.0f)) safety = 0.0f;
+        m[0] = R;
+        m[1] = fmaxf(0.04f, (0.6f * safety) / R);
+        m[2] = fmaxf(1e-3f, 0.01f / sig_tr);
+      }
+      s_m = fmaxf(m[1] * m[0], m[2]);
+    }
+  }
   const float H = o.geo.half_xy_mm;
   const float dx = t.dir[0], dy = t.dir[1], dz = t.dir[2];
   const float s_z = (dz > 0.0f) ? (z_hi - t.pos[2]) / dz : (dz < 0.0f) ? (z_lo - t.pos[2]) / dz : INF;
@@ -414,6 +445,10 @@ bool step_track(Oracle &o, int kind, Track &t, Child children[2], int &n_childre
   if (kind != KIND_GAMMA) {
     note_margin(margin, s_e, s);
     if (s_e < s) { s = s_e; w = W_ELOSS; }
+    if (with_msc) {
+      note_margin(margin, s_m, s);
+      if (s_m < s) { s = s_m; w = W_MSC; }
+    }
   }
   for (int j = 0; j < NP; ++j) {
     note_margin(margin, sj[j], s);
@@ -445,9 +480,22 @@ bool step_track(Oracle &o, int kind, Track &t, Child children[2], int &n_childre
     if (E_post < e_cut) {
       if (kind == KIND_EM) { deposit(vol0, E_post); return finish(false); }
       t.ekin = E_post;                // e+: kept alive for S17 at its next step
+      keep_msc();
       return finish(true);
     }
     t.ekin = E_post;
+    // X39c: deflection by multiple scattering along the step, 1 - cos(theta) exponential with mean s Sigma_tr
+    if (with_msc && sig_tr > 0.0f && s > 0.0f) {
+      const float tau = s * sig_tr;
+      float c = fmaf(tau, lg(rng.u(3, 0)), 1.0f);
+      if (c < -1.0f) c = -1.0f;
+      const float sn = sqrtf(fmaf(-c, c, 1.0f));
+      float sphi, cphi;
+      sincos2pi(rng.u(3, 1), &sphi, &cphi);
+      float d1[3];
+      rotate(t.dir, sn, c, sphi, cphi, d1);
+      for (int i = 0; i < 3; ++i) t.dir[i] = d1[i];
+    }
   }
 
   // S25: boundary crossing / escape.
@@ -455,10 +503,10 @@ bool step_track(Oracle &o, int kind, Track &t, Child children[2], int &n_childre
     bool escape = false;
     if (face == FACE_ZP) {
       t.pos[2] = z_hi;
-      if (vol0 + 1u >= 2u * o.geo.n_layers) escape = true; else t.vol = vol0 + 1u;
+      if (vol0 + 1u >= 2u * o.geo.n_layers) escape = true; else { t.vol = vol0 + 1u; m[0] = -1.0f; }  // X39d
     } else if (face == FACE_ZM) {
       t.pos[2] = z_lo;
-      if (vol0 == 0u) escape = true; else t.vol = vol0 - 1u;
+      if (vol0 == 0u) escape = true; else { t.vol = vol0 - 1u; m[0] = -1.0f; }  // X39d
     } else {
       escape = true;
     }
@@ -469,7 +517,7 @@ bool step_track(Oracle &o, int kind, Track &t, Child children[2], int &n_childre
       o.res.escaped_n[kind] += 1;
       return finish(false);
     }
-  } else if (w != W_ELOSS) {
+  } else if (w != W_ELOSS && w != W_MSC) {
     // S26: discrete interaction of process w.
     t.nial[w] = -1.0f;
     if (kind == KIND_EP && w == 2) {
@@ -632,6 +680,7 @@ bool step_track(Oracle &o, int kind, Track &t, Child children[2], int &n_childre
     if (kind == KIND_EP) deposit(t.vol, o.two_mc2);
     return finish(false);
   }
+  keep_msc();
   return finish(true);
 }
 
@@ -760,8 +809,8 @@ orc_ctx *orc_create(const Geometry *g, const TablesIn *tin, uint64_t seed) {
   o->tab.inv_dln = tin->inv_dln; o->tab.e_cut = tin->e_cut;
   o->tab.data.assign(tin->data, tin->data + (size_t)tin->n_materials * 6 * (tin->n_bins + 1));
   o->tab.physics = tin->physics;
-  if (tin->physics > 1u || (tin->physics == 1u && !tin->data_x)) { delete o; return nullptr; }
-  if (tin->physics == 1u) o->tab.data_x.assign(tin->data_x, tin->data_x + (size_t)tin->n_materials * 2 * (tin->n_bins + 1));
+  if (tin->physics > 2u || (tin->physics >= 1u && !tin->data_x)) { delete o; return nullptr; }
+  if (tin->physics >= 1u) o->tab.data_x.assign(tin->data_x, tin->data_x + (size_t)tin->n_materials * 3 * (tin->n_bins + 1));
   o->seed = seed;
   o->pitch = g->abs_mm + g->gap_mm;
   o->two_mc2 = 2.0f * o->mc2;

@@ -109,6 +109,18 @@ def sigma_annihilation(mat: Material, T):
     return mat.n_atoms * mat.Z * per_e
 
 
+E_SCATTER = 21.2            # Rossi-Greisen scattering energy [MeV]
+
+
+def sigma_transport(mat: Material, T):
+    """Rule X39: transport cross-section of multiple scattering [1/mm], <1 - cos(theta)> per unit path =
+    theta_0^2 / 2 with the Rossi-Greisen width theta_0^2 = (E_s / (beta p c))^2 / X0."""
+    T = np.asarray(T, dtype=np.float64)
+    pc = np.sqrt(T * (T + 2.0 * MC2))
+    beta = pc / (T + MC2)
+    return (E_SCATTER / (beta * pc)) ** 2 / (2.0 * mat.X0)
+
+
 def stopping_power(mat: Material, T, e_cut: float, physics: int = 0):
     """Restricted stopping power [MeV/mm]: Bethe-Bloch collision term (no
     density correction) plus the radiative loss to photons below the cut.
@@ -165,8 +177,8 @@ class TableSet:
     inv_dln: np.float32
     nodes: np.ndarray           # float64 [n_bins+1]
     data: np.ndarray            # float32 [mat][group][qty][n_bins+1], C-contiguous
-    physics: int = 0            # rule X35: 0 = basic rules; 1 = delta rays (X36), Klein-Nishina sampling (X37), annihilation in flight (X38)
-    data_x: np.ndarray | None = None    # physics 1: float32 [mat][2][n_bins+1]: Sigma_delta (e+-), Sigma_annihilation (e+)
+    physics: int = 0            # rule X35: 0 = basic rules; 1 = delta rays (X36), Klein-Nishina sampling (X37), annihilation in flight (X38); 2 = also multiple scattering (X39)
+    data_x: np.ndarray | None = None    # physics >= 1: float32 [mat][3][n_bins+1]: Sigma_delta (e+-), Sigma_annihilation (e+), Sigma_transport (e+-)
 
     def q(self, mat: int, group: int, qty: int) -> np.ndarray:
         return self.data[mat, group, qty]
@@ -187,7 +199,8 @@ def build_tables(n_bins: int, e_min: float, e_max: float, e_cut: float,
         data[m, GROUP_ELEC, Q_RANGE] = csda_range(mat, nodes, e_cut, physics=physics)
     data_x = None
     if physics:
-        data_x = np.ascontiguousarray(np.stack([np.stack([sigma_delta(mat, nodes, e_cut), sigma_annihilation(mat, nodes)])
+        data_x = np.ascontiguousarray(np.stack([np.stack([sigma_delta(mat, nodes, e_cut), sigma_annihilation(mat, nodes),
+                                                          sigma_transport(mat, nodes)])
                                                 for mat in materials]).astype(np.float32))
     return TableSet(physics=physics, data_x=data_x,
         n_bins=n_bins, n_materials=len(materials), e_min=e_min, e_max=e_max, e_cut=e_cut,
@@ -198,7 +211,7 @@ def build_tables(n_bins: int, e_min: float, e_max: float, e_cut: float,
 
 def constant_tables(n_bins: int, e_min: float, e_max: float, e_cut: float, *,
                     pair=0.0, compt=0.0, photo=0.0, brems=0.0, stop=0.0, rng=1e30,
-                    n_materials: int = 2, physics: int = 0, delta=0.0, annih=0.0) -> TableSet:
+                    n_materials: int = 2, physics: int = 0, delta=0.0, annih=0.0, transport=0.0) -> TableSet:
     """Energy-independent tables for closed-form checks (pure absorber,
     vacuum-like geometry tests, brems-only slabs)."""
     j = np.arange(n_bins + 1, dtype=np.float64)
@@ -212,8 +225,8 @@ def constant_tables(n_bins: int, e_min: float, e_max: float, e_cut: float, *,
     data[:, GROUP_ELEC, Q_RANGE] = rng
     data_x = None
     if physics:
-        data_x = np.zeros((n_materials, 2, n_bins + 1), dtype=np.float32)
-        data_x[:, 0], data_x[:, 1] = delta, annih
+        data_x = np.zeros((n_materials, 3, n_bins + 1), dtype=np.float32)
+        data_x[:, 0], data_x[:, 1], data_x[:, 2] = delta, annih, transport
     return TableSet(n_bins, n_materials, e_min, e_max, e_cut,
                     np.float32(math.log(e_min)), np.float32(n_bins / math.log(e_max / e_min)),
                     nodes, data, physics, data_x)
