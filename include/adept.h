@@ -87,13 +87,17 @@ typedef struct {
   float ln_e_min, inv_dln; /* fl32(ln e_min), fl32(n_bins / ln(e_max/e_min)) */
   float e_cut;             /* production = tracking cut [MeV] */
   const float *data;       /* host */
-  /* Extended physics (DESIGN.md rules X35-X38).  physics = 0: the rules
+  /* Extended physics (DESIGN.md rules X35-X39).  physics = 0: the rules
    * S16-S32 only (data_x ignored).  physics = 1: e+- also produce delta rays (the 1/T^2 term common to
    * Moller and Bhabha scattering, on nial[1]), e+ also annihilate in flight (on nial[2]), and the
-   * Compton energy fraction is sampled from the full Klein-Nishina distribution; data_x is then a HOST
-   * array [n_materials][2][n_bins+1] of {Sigma_delta, Sigma_annihilation} [1/mm], and the stopping
-   * power / range in `data` must be the ones restricted to losses below the cut.  Not available in
-   * instrumented contexts or with ADEPT_FLAG_RECYCLE_SLOTS (EINVAL). */
+   * Compton energy fraction is sampled from the full Klein-Nishina distribution.  physics = 2: e+- are
+   * also deflected by multiple scattering, which limits their step by max(DynamicRangeFactor *
+   * InitialRange, TlimitMin) -- the paper's three cold track fields, kept per track
+   * in a side array of the workspace, not in the 14-word record (a track handed in through the ABI
+   * starts uninitialised, like a new one).  data_x is a HOST array [n_materials][3][n_bins+1] of
+   * {Sigma_delta, Sigma_annihilation, Sigma_transport} [1/mm], and the stopping power / range in `data`
+   * must be the ones restricted to losses below the cut.  physics >= 1 is not available in instrumented
+   * contexts or with ADEPT_FLAG_RECYCLE_SLOTS (EINVAL). */
   uint32_t physics;
   const float *data_x;     /* host */
 } adept_tables;

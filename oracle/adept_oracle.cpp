@@ -25,7 +25,7 @@
 // the next slab boundary, applies continuous energy loss and discrete
 // interactions, emits secondaries"; Philox-4x32 keyed by (track id, step, draw
 // index)).  Every point on which those two sources are silent is a numbered
-// reading in DESIGN.md §3 (rules R1-R6, M7-M11, T12-T14, S16-S31, X35-X38); the code
+// reading in DESIGN.md §3 (rules R1-R6, M7-M11, T12-T14, S16-S31, X35-X39); the code
 // below follows those rules one by one, in their order and notation, with no
 // blocking, fusion or reordering.
 //
@@ -37,14 +37,17 @@
 // per-event energy conservation; <T(x)> = T0 exp(-x/X0) for brems; Compton
 // energy-momentum conservation and Compton edge; CSDA range; pair/photo
 // branch energies; lockstep == depth-first order independence.
-// Extended physics (tables.physics = 1; DESIGN.md rules X35-X38, SURVEY.md
+// Extended physics (tables.physics = 1; DESIGN.md rules X35-X39, SURVEY.md
 // §8(f) item 3): delta-ray production on nial[1] of e+- (X36), the Compton
 // energy fraction from the full Klein-Nishina distribution by composition and
-// rejection (X37), annihilation in flight on nial[2] of e+ (X38).  Pins (tests/test_oracle_extended.py): the eps distribution
-// against quadrature of the textbook Klein-Nishina density (KS distance, mean);
+// rejection (X37), annihilation in flight on nial[2] of e+ (X38), multiple
+// scattering with three more words per e+- track (X39, tables.physics = 2).
+// Pins (tests/test_oracle_extended.py): the eps distribution against quadrature of the textbook Klein-Nishina density (KS distance, mean);
 // the delta-ray energy against the closed-form 1/T^2 CDF; exact two-body
 // energy-momentum closure; S_restricted + int T dSigma_delta = S; per-event
-// energy conservation; lockstep == depth-first.
+// energy conservation; lockstep == depth-first; X38: two-photon energy and
+// momentum closure, uniform k1, Heitler's limits; X39: the closed-form step
+// limit on constant tables, exponential 1 - cos(theta), re-initialisation at a face.
 // Parity unpinned (no external closed form exists): the full-shower
 // longitudinal profile — only sanity checks (P-table).
 //

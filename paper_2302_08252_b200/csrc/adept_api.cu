@@ -33,7 +33,7 @@ inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 struct Plan {  // carve-up of the workspace
   size_t ctl, tables, stage, stage_slots;
-  size_t rec[3], queue[3][2], ring[3];
+  size_t rec[3], queue[3][2], ring[3], msc[3];
   size_t instr_rw, instr_lines[3], instr_slots[3];
   size_t total;
   uint32_t capacity;       // rounded up to a multiple of 128 (one tile)
@@ -68,7 +68,7 @@ static bool make_plan(const adept_geometry *g, const adept_tables *t, const adep
   if (c->flags & ~uint32_t(ADEPT_FLAG_RECYCLE_SLOTS)) return false;
   if (g->n_layers == 0 || g->n_layers > 2048) return false;
   if (t->n_bins == 0 || t->n_bins > 4096 || t->n_materials == 0 || t->n_materials > 8) return false;
-  if (t->physics > 1u || (t->physics == 1u && (c->instrument || (c->flags & ADEPT_FLAG_RECYCLE_SLOTS)))) return false;
+  if (t->physics > 2u || (t->physics >= 1u && (c->instrument || (c->flags & ADEPT_FLAG_RECYCLE_SLOTS)))) return false;
   if (c->capacity_per_kind == 0 || c->capacity_per_kind > (1u << 30)) return false;
   pl.capacity = (c->capacity_per_kind + 127u) / 128u * 128u;
   pl.nbuf = (c->scheme == ADEPT_DENSE_DOUBLE) ? 2 : 1;
@@ -88,6 +88,8 @@ static bool make_plan(const adept_geometry *g, const adept_tables *t, const adep
       pl.queue[k][q] = off;
       if (c->scheme == ADEPT_SPARSE_SINGLE) off = align_up(off + size_t(pl.capacity) * 4);
     }
+    pl.msc[k] = off;    // rule X39: the three multiple-scattering words of e- / e+ tracks, [buffer][3][capacity]
+    if (t->physics == 2u && k != K_GAMMA) off = align_up(off + size_t(pl.capacity) * 3 * sizeof(float) * pl.nbuf);
     pl.ring[k] = off;   // freed slots (ADEPT_FLAG_RECYCLE_SLOTS)
     if (c->scheme == ADEPT_SPARSE_SINGLE && (c->flags & ADEPT_FLAG_RECYCLE_SLOTS)) off = align_up(off + size_t(pl.capacity) * 4);
   }
@@ -302,7 +304,7 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
   Plan pl;
   if (!make_plan(g, t, cfg, pl)) return bad("invalid geometry, tables or configuration");
   if (!t->data) return bad("tables.data is NULL");
-  if (t->physics == 1u && !t->data_x) return bad("tables.physics = 1 needs tables.data_x");
+  if (t->physics >= 1u && !t->data_x) return bad("tables.physics >= 1 needs tables.data_x");
   if (!(g->abs_mm > 0.0f) || !(g->gap_mm > 0.0f) || !(g->half_xy_mm > 0.0f)) return bad("non-positive geometry");
   if (g->mat_abs >= t->n_materials || g->mat_gap >= t->n_materials) return bad("material index out of range");
   if (!(t->e_cut > 0.0f) || !(t->e_max > t->e_min) || !(t->e_min > 0.0f)) return bad("invalid energy grid");
@@ -347,12 +349,14 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
       for (uint32_t q = 0; q < 3; ++q)
         for (uint32_t j = 0; j < nodes; ++j)
           packed[((size_t(grp) * t->n_materials + m) * nodes + j) * 4 + q] = t->data[((size_t(m) * 2 + grp) * 3 + q) * nodes + j];
-  if (t->physics == 1u)  // X36: Sigma_delta in the fourth lane of the e+- group
+  if (t->physics >= 1u)  // X36: Sigma_delta in the fourth lane of the e+- group
     for (uint32_t m = 0; m < t->n_materials; ++m)
       for (uint32_t j = 0; j < nodes; ++j)
-      {  // data_x[mat][2][node]: Sigma_delta -> fourth lane of the e+- group, Sigma_annihilation -> first lane of group 2
-        packed[((size_t(1) * t->n_materials + m) * nodes + j) * 4 + 3] = t->data_x[(size_t(m) * 2 + 0) * nodes + j];
-        packed[((size_t(2) * t->n_materials + m) * nodes + j) * 4 + 0] = t->data_x[(size_t(m) * 2 + 1) * nodes + j];
+      {  // data_x[mat][3][node]: Sigma_delta -> fourth lane of the e+- group; Sigma_annihilation, Sigma_transport ->
+         // first and second lane of group 2
+        packed[((size_t(1) * t->n_materials + m) * nodes + j) * 4 + 3] = t->data_x[(size_t(m) * 3 + 0) * nodes + j];
+        packed[((size_t(2) * t->n_materials + m) * nodes + j) * 4 + 0] = t->data_x[(size_t(m) * 3 + 1) * nodes + j];
+        packed[((size_t(2) * t->n_materials + m) * nodes + j) * 4 + 1] = t->data_x[(size_t(m) * 3 + 2) * nodes + j];
       }
   if ((e = cudaMemcpyAsync(c->ws + pl.tables, packed.data(), pl.table_bytes, cudaMemcpyHostToDevice, c->stream)) != cudaSuccess)
     return die("cudaMemcpyAsync(tables)", e);
@@ -373,7 +377,7 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
   p.capacity = pl.capacity;
   p.recycle = (cfg->scheme == ADEPT_SPARSE_SINGLE && (cfg->flags & ADEPT_FLAG_RECYCLE_SLOTS)) ? 1u : 0u;
   p.physics = t->physics;
-  const int variant = (p.recycle ? V_RECYCLE : 0) | (p.physics ? V_PHYS : 0);
+  const int variant = (p.recycle ? V_RECYCLE : 0) | (p.physics ? V_PHYS : 0) | (p.physics == 2u ? V_MSC : 0);
   for (int k = 0; k < 3; ++k) {
     uint32_t *r = reinterpret_cast<uint32_t *>(c->ws + pl.rec[k]);
     p.kind[k].rec[0] = r;
@@ -381,6 +385,8 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
     p.kind[k].queue[0] = reinterpret_cast<uint32_t *>(c->ws + pl.queue[k][0]);
     p.kind[k].queue[1] = reinterpret_cast<uint32_t *>(c->ws + pl.queue[k][1]);
     p.kind[k].free_ring = reinterpret_cast<uint32_t *>(c->ws + pl.ring[k]);
+    p.kind[k].msc[0] = reinterpret_cast<float *>(c->ws + pl.msc[k]);
+    p.kind[k].msc[1] = (pl.nbuf == 2) ? p.kind[k].msc[0] + size_t(pl.capacity) * 3 : p.kind[k].msc[0];
     p.kind[k].instr_lines = reinterpret_cast<uint32_t *>(c->ws + pl.instr_lines[k]);
     p.kind[k].instr_slots = reinterpret_cast<uint32_t *>(c->ws + pl.instr_slots[k]);
   }
@@ -421,7 +427,7 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
   const int instr = cfg->instrument ? 1 : 0;
   const size_t tile_words = c->ops->record_words(kGroup);
   c->small.threads = kBlockSmall;
-  c->small.dyn_smem = step_smem_bytes(cfg->scheme, p.table_area, p.n_slabs, tile_words, kBlockSmall, c->ops->sparse_gather);
+  c->small.dyn_smem = step_smem_bytes(cfg->scheme, p.table_area, p.n_slabs, tile_words, kBlockSmall, c->ops->sparse_gather, p.physics == 2u);
   const int per_sm = c->ops->step_ctas_per_sm(cfg->scheme, instr, variant, kBlockSmall, c->small.dyn_smem);
   if (per_sm <= 0) {
     g_create_error = "step kernel does not fit on an SM with these tables (shared memory)";
@@ -430,7 +436,7 @@ int adept_create(const adept_geometry *g, const adept_tables *t, const adept_con
   }
   c->small.grid = static_cast<unsigned>(sms * per_sm);
   c->large.threads = kBlockLarge;
-  c->large.dyn_smem = step_smem_bytes(cfg->scheme, p.table_area, p.n_slabs, tile_words, kBlockLarge, c->ops->sparse_gather);
+  c->large.dyn_smem = step_smem_bytes(cfg->scheme, p.table_area, p.n_slabs, tile_words, kBlockLarge, c->ops->sparse_gather, p.physics == 2u);
   const int per_sm_large = c->ops->step_ctas_per_sm(cfg->scheme, instr, variant, kBlockLarge, c->large.dyn_smem);
   cudaGetLastError();  // a failed attribute query of the optional shape is not an error of the context
   c->large.grid = per_sm_large > 0 ? static_cast<unsigned>(sms * per_sm_large) : 0u;

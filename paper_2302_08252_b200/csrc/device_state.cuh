@@ -38,8 +38,10 @@ constexpr int kQueueCap = 2 * kGroup;
 // An entry is the 14 record words, the pending interaction packed into the three top bits of the step
 // word (steps stay below 2^21, rule S31), and for the sparse scheme the slot (+ one pad word): 56 or
 // 64 bytes, written and read as 64-bit words (7 or 8 shared-memory instructions, conflict-free).
-__host__ __device__ constexpr int queue_words(int scheme) { return scheme == S_DENSE ? 14 : 16; }
-__host__ __device__ constexpr size_t queue_bytes(int scheme) { return size_t(kQueueCap) * queue_words(scheme) * 4; }
+// With multiple scattering (rule X39) a parked track of the dense scheme also carries its three cold
+// words (in the sparse scheme they stay in place, in the side array): 18 words.
+__host__ __device__ constexpr int queue_words(int scheme, bool msc = false) { return scheme == S_DENSE ? (msc ? 18 : 14) : 16; }
+__host__ __device__ constexpr size_t queue_bytes(int scheme, bool msc = false) { return size_t(kQueueCap) * queue_words(scheme, msc) * 4; }
 // One tile of records staged in shared memory per group (record_words(kGroup) words of the layout):
 // dense scheme, by TMA bulk / tiled copies of the contiguous tile; sparse scheme, by per-thread
 // asynchronous copies (cp.async) of the records the group's list entries name, followed by two words
@@ -62,8 +64,8 @@ __host__ __device__ constexpr size_t units_offset(size_t table_bytes, uint32_t n
   return (table_bytes + bins_bytes(n_slabs) + 127) / 128 * 128;
 }
 __host__ __device__ constexpr size_t step_smem_bytes(int scheme, size_t table_bytes, uint32_t n_slabs, size_t tile_words,
-                                                     int threads, bool gather) {
-  return units_offset(table_bytes, n_slabs) + size_t(threads / kGroup) * (in_buf_bytes(scheme, tile_words, gather) + queue_bytes(scheme));
+                                                     int threads, bool gather, bool msc = false) {
+  return units_offset(table_bytes, n_slabs) + size_t(threads / kGroup) * (in_buf_bytes(scheme, tile_words, gather) + queue_bytes(scheme, msc));
 }
 
 // Energy tallies (rule M7: sums of fp32 terms) are accumulated in 64-bit fixed point, unit
@@ -118,6 +120,10 @@ struct KindStorage {
   uint32_t *rec[2];    // dense: current/next arrays by parity; sparse: rec[0] only
   uint32_t *queue[2];  // sparse: slot lists by parity
   uint32_t *free_ring;    // sparse + slot recycling: [capacity] freed slots (Ctl::free_head / free_tail)
+  // physics 2 (rule X39), e- and e+ only: the three multiple-scattering words of a track -- the paper's
+  // cold fields InitialRange, DynamicRangeFactor, TlimitMin -- as a side array
+  // [3][capacity] next to the records, addressed like them (dense: by parity; sparse: msc[0], by slot)
+  float *msc[2];
   uint32_t *instr_lines;  // instrumented build: per 128-B line of this kind's record storage
   uint32_t *instr_slots;  // instrumented build: per slot (dense: 2 * capacity)
 };
@@ -137,7 +143,7 @@ struct Params {
   uint32_t mat_abs, mat_gap;
   uint32_t capacity;         // slots per kind (multiple of 128)
   uint32_t recycle;          // sparse scheme: 1 = freed slots are reused (ADEPT_FLAG_RECYCLE_SLOTS)
-  uint32_t physics;          // adept_tables.physics: 1 = extended rules X36-X38
+  uint32_t physics;          // adept_tables.physics: 1 = extended rules X36-X38, 2 = also X39 (multiple scattering)
   uint32_t it;               // index of this launch (counted by the host; see Ctl)
   KindStorage kind[3];
   unsigned long long *instr_field_rw;  // [3][14][2], instrumented build

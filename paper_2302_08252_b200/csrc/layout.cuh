@@ -27,6 +27,9 @@ enum LayoutId : int { L_AOS = 0, L_SOA = 1, L_AOSOA32 = 2, L_AOSOA64 = 3, L_SOA1
 struct Trk {
   float px, py, pz, dx, dy, dz, ekin, n0, n1, n2;
   uint32_t vol, id_lo, id_hi, step;
+  // rule X39 (physics 2, e+- only): InitialRange (< 0 = not initialised), DynamicRangeFactor, TlimitMin.
+  // Not part of the 14-word record: they live in the kind's side array (KindStorage::msc).
+  float m0, m1, m2;
 };
 
 __device__ __forceinline__ uint32_t trk_word(const Trk &t, int f) {
@@ -292,8 +295,9 @@ template <int L, bool INSTR> struct TrackView {
   // for e+-, vol when the step crossed into another slab.  dir never changes in the move half, ids
   // never.  A word assigned the value it already had (a zero-length step) is written again; the
   // counting build uses store_changed below instead and counts only real changes.
-  // N1: e+- also assign nial[1] (extended physics, rule X36); N2: e+ also nial[2] (rule X38).
-  template <bool GAMMA, bool N1 = false, bool N2 = false> __device__ __forceinline__ void store_moved(uint32_t slot, const Trk &t, bool vol_changed) const {
+  // N1: e+- also assign nial[1] (extended physics, rule X36); N2: e+ also nial[2] (rule X38); DIR: e+-
+  // also the direction (multiple scattering, rule X39).
+  template <bool GAMMA, bool N1 = false, bool N2 = false, bool DIR = false> __device__ __forceinline__ void store_moved(uint32_t slot, const Trk &t, bool vol_changed) const {
     if constexpr (L == L_HC16) {
       // the two hot vectors; e+ under the extended physics also assigns nial[2], which lives in vector C
       using V = Mapping<L_SOA16>;
@@ -302,7 +306,7 @@ template <int L, bool INSTR> struct TrackView {
       hc16_pack(GAMMA, t, a, b, c, d);
       *reinterpret_cast<uint4 *>(base + V::index(cap, slot, 0)) = a;
       *reinterpret_cast<uint4 *>(base + V::index(cap, slot, 4)) = b;
-      if constexpr (N2) *reinterpret_cast<uint4 *>(base + V::index(cap, slot, 8)) = c;
+      if constexpr (N2 || DIR) *reinterpret_cast<uint4 *>(base + V::index(cap, slot, 8)) = c;
       (void)vol_changed; (void)d;
     } else if constexpr (L == L_AOS || L == L_SOA16) {
       // 16-byte pieces {pos, dir.x} {dir.yz, ekin, nial0} {nial12, vol, id_lo} {id_hi, step}: a photon
@@ -334,6 +338,11 @@ template <int L, bool INSTR> struct TrackView {
         base[Map::index(cap, slot, F_EKIN)] = __float_as_uint(t.ekin);
         if constexpr (N1) base[Map::index(cap, slot, F_N1)] = __float_as_uint(t.n1);
         if constexpr (N2) base[Map::index(cap, slot, F_N2)] = __float_as_uint(t.n2);
+        if constexpr (DIR) {
+          base[Map::index(cap, slot, F_DX)] = __float_as_uint(t.dx);
+          base[Map::index(cap, slot, F_DY)] = __float_as_uint(t.dy);
+          base[Map::index(cap, slot, F_DZ)] = __float_as_uint(t.dz);
+        }
       }
       if (vol_changed) base[Map::index(cap, slot, F_VOL)] = t.vol;
       base[Map::index(cap, slot, F_STEP)] = t.step;

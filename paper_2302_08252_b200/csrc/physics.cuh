@@ -320,7 +320,9 @@ template <int PHYS> __device__ __forceinline__ void interact_gamma(Trk &t, int w
 
 // --------------------------------------------------------------------- electron / positron ---
 // PHYS = 1: delta-ray production is a second discrete process, on nial[1] (rule X36).
+// PHYS = 2: also multiple scattering (rule X39): a third step limiter and a deflection after the move.
 template <int KIND, int PHYS> __device__ __forceinline__ void move_elec(Trk &t, const Env &g, MoveOut &o) {
+  constexpr bool MSC = PHYS == 2;
   static_assert(KIND == K_EM || KIND == K_EP, "e- or e+");
   move_out_init(o);
   const Stream rs{t.id_lo, t.id_hi, t.step};
@@ -379,9 +381,28 @@ template <int KIND, int PHYS> __device__ __forceinline__ void move_elec(Trk &t, 
   int face;
   float s = geometry_step(t, g, z_lo, z_hi, face);
 
-  // S22: GEOM (-1), ELOSS (3), brems (0)
+  // X39a, X39b: multiple-scattering limit max(DynamicRangeFactor * InitialRange, TlimitMin); the three
+  // words are (re-)initialised at the start of a track and after a slab crossing (InitialRange < 0)
+  float sig_tr = 0.0f, s_m = kInf;
+  if constexpr (MSC) {
+    const float4 *tx = tab + g.group_nodes;
+    sig_tr = lerp_node(b.f, tx[b.j].y, tx[b.j + 1].y);
+    if (sig_tr > 0.0f) {
+      if (t.m0 < 0.0f) {
+        float safety = fminf(t.pz - z_lo, z_hi - t.pz);
+        if (!(safety > 0.0f)) safety = 0.0f;
+        t.m0 = R;
+        t.m1 = fmaxf(0.04f, (0.6f * safety) / R);
+        t.m2 = fmaxf(1e-3f, 0.01f / sig_tr);
+      }
+      s_m = fmaxf(t.m1 * t.m0, t.m2);
+    }
+  }
+
+  // S22: GEOM (-1), ELOSS (3), multiple scattering (5), brems (0), delta (1), annihilation in flight (2)
   int w = -1;
   if (s_e < s) { s = s_e; w = 3; }
+  if (MSC && s_m < s) { s = s_m; w = 5; }
   if (s0 < s) { s = s0; w = 0; }
   if (PHYS != 0 && s1 < s) { s = s1; w = 1; }
   if (PHYS != 0 && KIND == K_EP && s2 < s) { s = s2; w = 2; }
@@ -411,11 +432,27 @@ template <int KIND, int PHYS> __device__ __forceinline__ void move_elec(Trk &t, 
   t.ekin = E_post;
   // what the step ends in, as flags (no early exits: the outcomes of a warp's lanes differ)
   const bool below = E_post < e_cut;            // S24: e- deposits the rest and dies; e+ is kept for S17
+  if constexpr (MSC) {
+    // X39c: deflection along the step, 1 - cos(theta) exponential with mean s Sigma_tr (draws of call 3)
+    if (!below && sig_tr > 0.0f && s > 0.0f) {
+      const uint4 r = rs.call(3);
+      const float tau = s * sig_tr;
+      float c = fmaf(tau, lg(u01(r.x)), 1.0f);
+      if (c < -1.0f) c = -1.0f;
+      const float sn = sqrtf(fmaf(-c, c, 1.0f));
+      float sphi, cphi;
+      sincos2pi(u01(r.y), sphi, cphi);
+      float nx, ny, nz;
+      rotate_dir(t.dx, t.dy, t.dz, sn, c, sphi, cphi, nx, ny, nz);
+      t.dx = nx; t.dy = ny; t.dz = nz;
+    }
+  }
   const bool brems = !below && (w == 0 || w == 1 || w == 2);  // S26 (X36: w == 1, X38: w == 2) follows in interact_elec
   const bool geom = !below && w < 0;
   o.dep_b = (below && KIND == K_EM) ? E_post : 0.0f;
   o.pending = brems ? w : int(P_NONE);
   o.escaped = cross_boundary(geom, t, g, vol0, face, z_lo, z_hi);  // S25
+  if (MSC && t.vol != vol0) t.m0 = -1.0f;                          // X39d: a new slab, a new InitialRange
   o.guard = !below && !brems && !o.escaped && t.step >= (1u << 20);  // S31
   o.alive = !((below && KIND == K_EM) || o.escaped || o.guard);
 }

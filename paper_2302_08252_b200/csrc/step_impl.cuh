@@ -48,7 +48,8 @@ __device__ __forceinline__ void group_sync(int group) {
 
 // Variant bits of the step kernel (template parameter VAR): slot recycling of the sparse scheme
 // (ADEPT_FLAG_RECYCLE_SLOTS) and the extended physics rules X36-X38 (adept_tables.physics = 1).
-enum Variant : int { V_RECYCLE = 1, V_PHYS = 2 };
+enum Variant : int { V_RECYCLE = 1, V_PHYS = 2, V_MSC = 4 };  // V_MSC (rule X39) comes with V_PHYS
+__host__ __device__ constexpr int phys_of(int var) { return (var & V_MSC) ? 2 : ((var & V_PHYS) ? 1 : 0); }
 
 // ---- section clocks (timing build only) ------------------------------------------------------------
 // BASELINE.json configs[3]: "each scheme reports step plus slot-allocation/compaction time".  Allocation
@@ -327,19 +328,42 @@ __device__ __forceinline__ Trk kid_track(const Trk &parent, const Kid &k) {
   return c;
 }
 
+// ---- rule X39: the side array of the three multiple-scattering words (e- and e+ only) --------------
+__device__ __forceinline__ void msc_store(const Params &p, int kind, int buf, uint32_t idx, float m0, float m1, float m2) {
+  float *a = p.kind[kind].msc[buf];
+  a[idx] = m0;
+  a[size_t(p.capacity) + idx] = m1;
+  a[2 * size_t(p.capacity) + idx] = m2;
+}
+__device__ __forceinline__ void msc_load(const Params &p, int kind, int buf, uint32_t idx, Trk &t) {
+  const float *a = p.kind[kind].msc[buf];
+  t.m0 = a[idx];
+  t.m1 = a[size_t(p.capacity) + idx];
+  t.m2 = a[2 * size_t(p.capacity) + idx];
+}
+
 // ---- parked tracks (the queue between the two halves of the step) ----------------------------------
 // Entry q = 7 (sparse: 8) 64-bit words; the pending interaction rides in the top bits of the step word.
-template <int SCHEME>
+// (dense scheme with multiple scattering: two more 64-bit words carry the track's three cold words)
+template <int SCHEME, bool MSC = false>
 __device__ __forceinline__ void park_store(uint32_t *queue, uint32_t q, const Trk &t, int pending, uint32_t slot) {
-  uint2 *e = reinterpret_cast<uint2 *>(queue + size_t(q) * queue_words(SCHEME));
+  uint2 *e = reinterpret_cast<uint2 *>(queue + size_t(q) * queue_words(SCHEME, MSC));
+  if (SCHEME == S_DENSE && MSC) {
+    e[7] = make_uint2(__float_as_uint(t.m0), __float_as_uint(t.m1));
+    e[8] = make_uint2(__float_as_uint(t.m2), 0u);
+  }
 #pragma unroll
   for (int f = 0; f < 12; f += 2) e[f / 2] = make_uint2(trk_word(t, f), trk_word(t, f + 1));
   e[6] = make_uint2(t.id_hi, t.step | (uint32_t(pending) << 29));
   if (SCHEME == S_SPARSE) e[7] = make_uint2(slot, 0u);
 }
-template <int SCHEME>
+template <int SCHEME, bool MSC = false>
 __device__ __forceinline__ void park_load(const uint32_t *queue, uint32_t q, Trk &t, int &pending, uint32_t &slot) {
-  const uint2 *e = reinterpret_cast<const uint2 *>(queue + size_t(q) * queue_words(SCHEME));
+  const uint2 *e = reinterpret_cast<const uint2 *>(queue + size_t(q) * queue_words(SCHEME, MSC));
+  if (SCHEME == S_DENSE && MSC) {
+    const uint2 a = e[7], b = e[8];
+    t.m0 = __uint_as_float(a.x); t.m1 = __uint_as_float(a.y); t.m2 = __uint_as_float(b.x);
+  }
 #pragma unroll
   for (int f = 0; f < 12; f += 2) {
     const uint2 w = e[f / 2];
@@ -569,6 +593,8 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
     in_phase ^= 1u;
     if (active) t = cur.load(slot);
   }
+  constexpr bool kMsc = (VAR & V_MSC) != 0 && KIND != K_GAMMA;
+  if (kMsc && active) msc_load(p, KIND, (SCHEME == S_DENSE) ? int(par) : 0, slot, t);
   if (active) {
     if (INSTR && (SCHEME == S_DENSE || kGather)) {
 #pragma unroll
@@ -578,7 +604,7 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
     vol_before = t.vol;
     c.clk->mark(SEC_LOAD);
     if constexpr (KIND == K_GAMMA) move_gamma(t, env, o);
-    else move_elec<KIND, (VAR & V_PHYS) ? 1 : 0>(t, env, o);
+    else move_elec<KIND, phys_of(VAR)>(t, env, o);
     // A6: scoring into the CTA's bins (pre-step slab; the S31 guard uses the post-step slab).  A
     // photon deposits nothing in this half; the rare terms share one branch.
     if (KIND != K_GAMMA && o.dep != 0.0f) bin_add(c.bins, vol_before, o.dep);
@@ -597,7 +623,8 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
   if (SCHEME == S_SPARSE) {
     if (survives || parked) {
       if constexpr (INSTR) cur.store_changed(slot, t, old);  // counts exactly the words that changed
-      else cur.template store_moved<KIND == K_GAMMA, (VAR & V_PHYS) != 0, (VAR & V_PHYS) != 0 && KIND == K_EP>(slot, t, t.vol != vol_before);
+      else cur.template store_moved<KIND == K_GAMMA, (VAR & V_PHYS) != 0, (VAR & V_PHYS) != 0 && KIND == K_EP, kMsc>(slot, t, t.vol != vol_before);
+      if (kMsc) msc_store(p, KIND, 0, slot, t.m0, t.m1, t.m2);
     }
     c.clk->mark(SEC_STORE);
   }
@@ -644,7 +671,7 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
   // park the tracks that still owe an interaction
   if (parked) {
     const uint32_t q = queued + count_of(word, 1) + __popc(m_park & lt_mask);
-    park_store<SCHEME>(c.queue, q, t, o.pending, slot);
+    park_store<SCHEME, kMsc>(c.queue, q, t, o.pending, slot);
   }
   c.clk->mark(SEC_STORE);
   group_sync(c.group);
@@ -652,8 +679,12 @@ __device__ __forceinline__ uint32_t move_tile(const Params &p, const Env &env, c
   if (survives) {
     const uint32_t dst = g.base[sbuf][0] + count_of(word, 0) + __popc(m_surv & lt_mask);
     if (dst < p.capacity) {
-      if (SCHEME == S_DENSE) make_view<L, INSTR>(p, KIND, int(par ^ 1u), c.cta->probe).store(dst, t);  // A10
-      else p.kind[KIND].queue[par ^ 1u][dst] = slot;  // slot pushed onto the next list
+      if (SCHEME == S_DENSE) {
+        make_view<L, INSTR>(p, KIND, int(par ^ 1u), c.cta->probe).store(dst, t);  // A10
+        if (kMsc) msc_store(p, KIND, int(par ^ 1u), dst, t.m0, t.m1, t.m2);
+      } else {
+        p.kind[KIND].queue[par ^ 1u][dst] = slot;  // slot pushed onto the next list
+      }
     } else {
       ctl->overflow = 1u;
     }
@@ -689,10 +720,10 @@ __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &e
   if (have) {
     const uint32_t q = first + gtid;
     int pending;
-    park_load<SCHEME>(c.queue, q, t, pending, slot);
+    park_load<SCHEME, (VAR & V_MSC) != 0 && KIND != K_GAMMA>(c.queue, q, t, pending, slot);
     before_interaction = t;
-    if constexpr (KIND == K_GAMMA) interact_gamma<(VAR & V_PHYS) ? 1 : 0>(t, pending, env, o);
-    else interact_elec<KIND, (VAR & V_PHYS) ? 1 : 0>(t, pending, env, o);
+    if constexpr (KIND == K_GAMMA) interact_gamma<phys_of(VAR)>(t, pending, env, o);
+    else interact_elec<KIND, phys_of(VAR)>(t, pending, env, o);
     if (o.dep != 0.0f) bin_add(c.bins, t.vol, o.dep);
     if (o.dep_b != 0.0f) bin_add(c.bins, t.vol, o.dep_b);
     if (o.guard) bin_add_track_energy<KIND>(c.bins, t.vol, t.ekin);
@@ -777,24 +808,31 @@ __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &e
   const uint32_t r_k0 = count_of(word, f0) + __popc((k0d ? m_kd : m_k0) & lt_mask);
   const uint32_t r_k1 = count_of(word, Q1) + ((Q0 == Q1) ? uint32_t(__popc(m_k0)) : 0u) + __popc(m_k1 & lt_mask);
   const int nbuf = int(par ^ 1u);
+  constexpr bool kMscVar = (VAR & V_MSC) != 0;
   bool dropped = false;
   c.clk->mark(SEC_ALLOC);
   if (SCHEME == S_DENSE) {
     // A10: whole records into the next arrays
     if (o.alive) {
       const uint32_t dst = g.base[sbuf][KIND] + r_alive;
-      if (dst < p.capacity) make_view<L, INSTR>(p, KIND, nbuf, c.cta->probe).store(dst, t);
-      else dropped = true;
+      if (dst < p.capacity) {
+        make_view<L, INSTR>(p, KIND, nbuf, c.cta->probe).store(dst, t);
+        if (kMscVar && KIND != K_GAMMA) msc_store(p, KIND, nbuf, dst, t.m0, t.m1, t.m2);
+      } else dropped = true;
     }
     if (o.kid[0].kind >= 0) {
       const uint32_t dst = g.base[sbuf][f0] + r_k0;
-      if (dst < p.capacity) make_view<L, INSTR>(p, d0, nbuf, c.cta->probe).store(dst, kid_track(t, o.kid[0]));
-      else dropped = true;
+      if (dst < p.capacity) {
+        make_view<L, INSTR>(p, d0, nbuf, c.cta->probe).store(dst, kid_track(t, o.kid[0]));
+        if (kMscVar && d0 != K_GAMMA) msc_store(p, d0, nbuf, dst, -1.0f, 0.0f, 0.0f);  // X39: a new track is not initialised
+      } else dropped = true;
     }
     if (o.kid[1].kind >= 0) {
       const uint32_t dst = g.base[sbuf][Q1] + r_k1;
-      if (dst < p.capacity) make_view<L, INSTR>(p, Q1, nbuf, c.cta->probe).store(dst, kid_track(t, o.kid[1]));
-      else dropped = true;
+      if (dst < p.capacity) {
+        make_view<L, INSTR>(p, Q1, nbuf, c.cta->probe).store(dst, kid_track(t, o.kid[1]));
+        if (kMscVar && Q1 != K_GAMMA) msc_store(p, Q1, nbuf, dst, -1.0f, 0.0f, 0.0f);
+      } else dropped = true;
     }
   } else {
     // A10 sparse: the words the interaction changed, slot pushed onto the next list
@@ -820,6 +858,7 @@ __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &e
       if (r_k0 < g.sgot[sbuf][f0] && qpos < p.capacity) {
         const uint32_t s_new = child_slot(f0, r_k0);
         make_view<L, INSTR>(p, d0, 0, c.cta->probe).store(s_new, kid_track(t, o.kid[0]));
+        if (kMscVar && d0 != K_GAMMA) msc_store(p, d0, 0, s_new, -1.0f, 0.0f, 0.0f);
         p.kind[d0].queue[nbuf][qpos] = s_new;
       } else dropped = true;
     }
@@ -828,6 +867,7 @@ __device__ __forceinline__ uint32_t interact_batch(const Params &p, const Env &e
       if (r_k1 < g.sgot[sbuf][Q1] && qpos < p.capacity) {
         const uint32_t s_new = child_slot(Q1, r_k1);
         make_view<L, INSTR>(p, Q1, 0, c.cta->probe).store(s_new, kid_track(t, o.kid[1]));
+        if (kMscVar && Q1 != K_GAMMA) msc_store(p, Q1, 0, s_new, -1.0f, 0.0f, 0.0f);
         p.kind[Q1].queue[nbuf][qpos] = s_new;
       } else dropped = true;
     }
@@ -929,7 +969,7 @@ __global__ void __launch_bounds__(THREADS, (THREADS == kBlockSmall) ? ADEPT_STEP
   const int tid = threadIdx.x;
   Ctl *ctl = p.ctl;
   constexpr size_t kInBuf = in_buf_bytes(SCHEME, Mapping<L>::words(kGroup), Mapping<L>::kSparseGather);
-  constexpr size_t kPerGroup = kInBuf + queue_bytes(SCHEME);
+  constexpr size_t kPerGroup = kInBuf + queue_bytes(SCHEME, (VAR & V_MSC) != 0);
   GroupRefs c;
   c.cta = &sh;
   c.group = tid / kGroup;
@@ -1098,6 +1138,7 @@ __global__ void inject_kernel(const __grid_constant__ Params p, const StagedPrim
   int buf; uint32_t where;
   place<SCHEME>(p, kind, par, entry_base + i, slot_base + i, buf, where);
   plain_view<L>(p, kind, buf).store(where, t);
+  if (p.physics == 2u && kind != K_GAMMA) msc_store(p, kind, buf, where, -1.0f, 0.0f, 0.0f);  // X39: not initialised
 }
 
 template <int L, int SCHEME>
@@ -1121,6 +1162,7 @@ __global__ void load_kernel(const __grid_constant__ Params p, const PackedTrack 
   int buf; uint32_t where;
   place<SCHEME>(p, kind, par, entry_base + i, slots ? slots[i] : slot_base + i, buf, where);
   plain_view<L>(p, kind, buf).store(where, unpack(a));
+  if (p.physics == 2u && kind != K_GAMMA) msc_store(p, kind, buf, where, -1.0f, 0.0f, 0.0f);  // X39: not initialised
 }
 
 template <int L, int SCHEME>
@@ -1170,6 +1212,8 @@ inline cudaError_t ensure_dynamic_smem(const void *kernel, size_t bytes) {
 template <int L> struct OpsImpl {
   // The extended physics is instantiated for the plain (non-counting) kernels without slot recycling.
   template <int T, typename F> static auto pick_t(int scheme, int instr, int var, F f) {
+    if (var & V_MSC)
+      return scheme == S_DENSE ? f(step_kernel<L, S_DENSE, false, T, V_PHYS | V_MSC>) : f(step_kernel<L, S_SPARSE, false, T, V_PHYS | V_MSC>);
     if (var & V_PHYS)
       return scheme == S_DENSE ? f(step_kernel<L, S_DENSE, false, T, V_PHYS>) : f(step_kernel<L, S_SPARSE, false, T, V_PHYS>);
     if (scheme == S_DENSE) return instr ? f(step_kernel<L, S_DENSE, true, T>) : f(step_kernel<L, S_DENSE, false, T>);
@@ -1190,7 +1234,7 @@ template <int L> struct OpsImpl {
   }
   static cudaError_t launch_step(int scheme, int instr, const Params &p, int threads, unsigned grid, size_t dyn,
                                  cudaStream_t s) {
-    return pick(scheme, instr, (p.recycle ? V_RECYCLE : 0) | (p.physics ? V_PHYS : 0), threads, [&](auto *k) {
+    return pick(scheme, instr, (p.recycle ? V_RECYCLE : 0) | (p.physics ? V_PHYS : 0) | (p.physics == 2u ? V_MSC : 0), threads, [&](auto *k) {
       const cudaError_t e = ensure_dynamic_smem(reinterpret_cast<const void *>(k), dyn);
       if (e != cudaSuccess) return e;
       // Programmatic dependent launch: the CTAs of this launch may become resident, and run their

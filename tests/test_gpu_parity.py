@@ -981,3 +981,75 @@ def test_snapshot_rewind_and_launch_index_wrap():
         with pytest.raises(Exception):
             ctx.set_launch_index(wrap)
         ctx.destroy()
+
+
+# ------------------------------------------------- multiple scattering (rule X39, physics = 2) -----
+@pytest.mark.parametrize("scheme", SCHEMES)
+@pytest.mark.parametrize("layout", ("aos", "soa", "aosoa32", "hc16"))
+def test_multiple_scattering_matches_oracle(layout, scheme):
+    """adept_tables.physics = 2: the step limit from the three cold words (InitialRange,
+    DynamicRangeFactor, TlimitMin -- a side array on the device), the deflection, the re-initialisation at
+    slab crossings.  The words themselves do not cross the ABI; every step they decide does: the tiny
+    shower track by track in every iteration, 100 x 1 GeV showers to completion, and constant-table
+    steps in which the multiple-scattering limit is the one that ends the step."""
+    c = CONFIGS["tiny"]
+    geo, tab = geometry_for("tiny"), tables_for("tiny", physics=2)
+    prim = gen_primaries(c["n_primaries"], c["e_primary"])
+    o = Oracle(geo, tab, seed=c["seed"])
+    o.inject(prim)
+    ctx = _ctx(geo, tab, layout=layout, scheme=scheme, capacity=c["capacity"], seed=c["seed"])
+    ctx.inject(prim)
+    it = 0
+    while sum(o.live(k) for k in range(3)):
+        o.step()
+        compare_counts(ctx.step(), o.result(), what="iteration %d" % it)
+        for k in range(3):
+            assert compare_tracks(ctx.read_tracks(k), o.read_tracks(k, make_tracks(1).dtype), "iteration %d kind %d" % (it, k)) == 0
+        it += 1
+    r, g = o.result(), ctx.result()
+    assert np.allclose(g["edep_layer"], r["edep_layer"], rtol=1e-4, atol=1e-12)
+    ctx.destroy()
+
+    c = CONFIGS["full"]
+    geo, tab = geometry_for("full"), tables_for("full", physics=2)
+    prim = gen_primaries(100, c["e_primary"])
+    o = Oracle(geo, tab, seed=c["seed"])
+    o.inject(prim)
+    o.run()
+    r = o.result()
+    ctx = _ctx(geo, tab, layout=layout, scheme=scheme, capacity=1 << 19, seed=c["seed"])
+    ctx.inject(prim)
+    g = ctx.run()
+    compare_counts(g, r)
+    assert g["iterations"] == r["iterations"]
+    assert np.allclose(g["edep_layer"], r["edep_layer"], rtol=1e-4, atol=1e-9)
+    assert abs(g["edep_slab"].sum() + g["e_escaped"] - g["e_injected"]) < 1e-6 * g["e_injected"]
+    ctx.destroy()
+
+    # constant tables: near a face the limit 0.04 * R0 ends the step; three steps, so that kept and
+    # re-initialised words are both exercised (loaded tracks start uninitialised on both sides)
+    from workloads.tables import constant_tables
+    from workloads import Geometry
+    geo = Geometry(n_layers=3, abs_mm=3.0, gap_mm=2.0, half_xy_mm=1e4)
+    tab = constant_tables(16, 0.1, 100.0, 0.1, physics=2, transport=0.5, stop=0.0, rng=10.0)
+    n = 3000 + 17
+    rng = np.random.default_rng(5)
+    for kind in (0, 1):
+        t = make_tracks(n, pos=(0, 0, 0.0), ekin=5.0, nial=(1e6, 1e6, 1e6), id0=1 + 10000 * kind)
+        t["pos"][:, 2] = rng.uniform(0.0, 15.0, n).astype(np.float32)
+        z = t["pos"][:, 2].astype(np.float64)
+        layer = np.minimum((z / 5.0).astype(int), 2)
+        t["vol"] = (2 * layer + ((z - 5.0 * layer) >= 3.0)).astype(np.uint32)
+        ct = rng.uniform(-1, 1, n)
+        ph = rng.uniform(0, 2 * np.pi, n)
+        d = np.stack([np.sqrt(1 - ct * ct) * np.cos(ph), np.sqrt(1 - ct * ct) * np.sin(ph), ct], 1)
+        t["dir"] = (d / np.linalg.norm(d, axis=1, keepdims=True)).astype(np.float32)
+        o = Oracle(geo, tab, seed=0)
+        o.load_tracks(kind, t)
+        ctx = _ctx(geo, tab, layout=layout, scheme=scheme, capacity=1 << 13, seed=0)
+        ctx.load_tracks(kind, t)
+        for it in range(3):
+            o.step()
+            compare_counts(ctx.step(), o.result(), what="msc kind %d step %d" % (kind, it))
+            assert compare_tracks(ctx.read_tracks(kind), o.read_tracks(kind, t.dtype), "msc kind %d step %d" % (kind, it)) == 0
+        ctx.destroy()

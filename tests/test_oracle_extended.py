@@ -1,4 +1,4 @@
-"""Pins of the oracle's extended physics (DESIGN.md rules X35-X38), against
+"""Pins of the oracle's extended physics (DESIGN.md rules X35-X39), against
 what the mathematics fixes: the Klein-Nishina energy distribution by quadrature of the textbook
 differential cross-section, the 1/T^2 delta-ray spectrum by its closed-form CDF, exact two-body
 energy-momentum conservation, and the table identities of the restricted stopping power.  CPU only."""

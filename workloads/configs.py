@@ -49,7 +49,7 @@ _TABLE_CACHE: dict = {}
 
 
 def tables_for(name: str, physics: int = 0) -> TableSet:
-    """Tables of a config; physics = 1: the extended rule set (DESIGN.md rules X35-X38)."""
+    """Tables of a config; physics = 1: the extended rule set (DESIGN.md rules X35-X39)."""
     c = CONFIGS[name]
     key = (c["n_bins"], c["e_max"], physics)
     if key not in _TABLE_CACHE:
