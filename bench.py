@@ -411,6 +411,10 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
             for name in ("full", "heavy") if "heavy" in args.extras else ("full",):
                 out["showers"][name] = showers(args, name, layout=main, scheme="dense", steps=3, warmup=1,
                                                with_cpu=not args.no_cpu)
+            # config 2 under the extended rule set (DESIGN.md rules X36-X39: delta rays, Klein-Nishina sampling,
+            # annihilation in flight, multiple scattering), against the oracle under the same rules
+            out["showers"]["full_physics2"] = showers(args, "full", layout=main, scheme="dense", steps=3, warmup=1,
+                                                      with_cpu=not args.no_cpu, physics=2)
             # the paper's default container on the same workloads: sparse single buffer, AoS, with slot
             # recycling (without it config 5 needs ~5.7e7 e- slots, SURVEY.md:583); parity against the
             # oracle result already computed above
@@ -430,7 +434,7 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
 
 
 def showers(args, name: str, *, layout: str, scheme: str, steps: int, warmup: int, with_cpu: bool, batch: int = 0,
-            flags: int = 0) -> dict:
+            flags: int = 0, physics: int = 0) -> dict:
     """BASELINE.json configs[0], [1], [4] (tiny / full / heavy): adept_inject + adept_run to completion,
     wall clock around the two calls (host primaries in, tallies out: this IS the end-to-end number).
     These runs are launch-latency bound for most of their iterations, so no roofline
@@ -439,7 +443,7 @@ def showers(args, name: str, *, layout: str, scheme: str, steps: int, warmup: in
     from paper_2302_08252_b200 import Context
     from workloads import gen_primaries
     c = CONFIGS[name]
-    geo, tab = geometry_for(name), tables_for(name)
+    geo, tab = geometry_for(name), tables_for(name, physics)
     prim = gen_primaries(c["n_primaries"], c["e_primary"])
     ctx = Context(geo, tab, layout=layout, scheme=scheme, capacity=c["capacity"], seed=c["seed"],
                   batch_primaries=batch, flags=flags)
@@ -463,7 +467,7 @@ def showers(args, name: str, *, layout: str, scheme: str, steps: int, warmup: in
            "workload": "%s showers (BASELINE.json): %d x %g MeV e-, %d layers, adept_inject + adept_run to "
                        "completion, wall clock around the two calls" % (name, c["n_primaries"], c["e_primary"], c["n_layers"]),
            "layout": layout, "scheme": scheme, "capacity_per_kind": c["capacity"], "batch_primaries": batch,
-           "slot_recycling": bool(flags & 1),
+           "slot_recycling": bool(flags & 1), "physics": physics,
            "showers_per_s": c["n_primaries"] / t, "track_steps": n_steps, "iterations": int(res["iterations"]),
            "us_per_iteration": 1e6 * t / max(1, int(res["iterations"])),
            "gpu_launches_per_run": int(res["iterations"]),
@@ -646,7 +650,7 @@ def run_showers_cli(args, name: str):
     sampler = ClockSampler(0)
     sampler.start()
     b = showers(args, name, layout=layout, scheme=args.scheme, steps=args.steps, warmup=args.warmup,
-                with_cpu=not args.no_cpu, batch=args.batch, flags=1 if args.recycle else 0)
+                with_cpu=not args.no_cpu, batch=args.batch, flags=1 if args.recycle else 0, physics=args.physics)
     clocks = sampler.stop()
     out = {"metric": "track-steps/sec", "value": b["value"], "unit": "track-steps/s", "n_gpus": 1,
            "steps": args.steps, "warmup": args.warmup, "ms_per_step": b["ms_per_run"], "higher_is_better": True,
@@ -711,6 +715,7 @@ def main():
     ap.add_argument("--no-sections", action="store_true", help="sweep: skip the section-clock contexts")
     ap.add_argument("--batch", type=int, default=0, help="shower workloads: batch_primaries (0 = all at once)")
     ap.add_argument("--recycle", action="store_true", help="shower workloads, sparse scheme: recycle freed slots")
+    ap.add_argument("--physics", type=int, default=0, choices=[0, 1, 2], help="shower workloads: adept_tables.physics")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
     if "WORLD_SIZE" not in os.environ and args.gpus > 1:
