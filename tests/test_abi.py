@@ -68,6 +68,28 @@ def test_workspace_bytes_is_host_arithmetic(L):
         assert size(**bad) == 0
 
 
+def test_workspace_bytes_with_extended_physics_and_flags(L):
+    """physics 2 adds the side arrays of the three multiple-scattering words (e-, e+; per buffer), slot
+    recycling the free rings; the extended physics is refused with instrumentation or recycling."""
+    lib = L.lib()
+
+    def size(physics=0, flags=0, instrument=0, scheme=1, capacity=4096):
+        g, t, c = _args(L, scheme=scheme, capacity=capacity, instrument=instrument)
+        t.physics = physics
+        c.flags = flags
+        return lib.adept_workspace_bytes(C.byref(g), C.byref(t), C.byref(c))
+
+    base_d, base_s = size(), size(scheme=0)
+    nodes = 257
+    assert abs((size(physics=1) - base_d) - 2 * nodes * 16) < 256          # a third table group (e+ extras), blocks are 256-byte aligned
+    assert size(physics=2) - size(physics=1) == 2 * 2 * 3 * 4096 * 4       # 2 kinds x 2 buffers x 3 words
+    assert size(physics=2, scheme=0) - size(physics=1, scheme=0) == 2 * 1 * 3 * 4096 * 4
+    assert size(scheme=0, flags=1) - base_s == 3 * 4096 * 4                # one ring per kind
+    assert size(flags=1) == base_d                                          # the dense scheme ignores the flag
+    for bad in (dict(physics=3), dict(physics=1, instrument=1), dict(physics=2, scheme=0, flags=1), dict(flags=2)):
+        assert size(**bad) == 0
+
+
 def test_field_offset_follows_the_three_mappings(L):
     cap = 4096
     for slot in (0, 1, 31, 32, 33, 1000, 4095):
