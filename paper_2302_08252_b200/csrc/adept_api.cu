@@ -693,10 +693,16 @@ int adept_run(adept_ctx *c, uint64_t max_iterations, adept_result *out) {
   // iteration with nothing alive is a no-op on the device and is not counted (Ctl::iterations), so
   // over-shooting the end of a batch by a few launches is harmless; progress against
   // max_iterations is what the device counted, not what the host enqueued.
+  // A burst boundary costs a stream synchronisation and a host round trip (~ 20 us, measured: config 2
+  // 1.84 ms with bursts of 16, 1.72 ms with bursts of 64), an over-shot launch ~ 2.5 us: bursts start at
+  // 16 launches and double up to 64 while a batch is alive.
 #ifndef ADEPT_RUN_BURST
 #define ADEPT_RUN_BURST 16
 #endif
-  const uint64_t kBurst = ADEPT_RUN_BURST;
+#ifndef ADEPT_RUN_BURST_MAX
+#define ADEPT_RUN_BURST_MAX 64
+#endif
+  uint64_t next_burst = ADEPT_RUN_BURST;
   uint64_t first_iteration = 0;
   for (bool first = true;; first = false) {
     rc = fetch_ctl(c, false);
@@ -714,8 +720,10 @@ int adept_run(adept_ctx *c, uint64_t max_iterations, adept_result *out) {
       if (rc != ADEPT_OK) break;
       c->pending_done += batch;
       if (c->pending_done >= c->pending.size()) { c->pending.clear(); c->pending_done = 0; }
+      next_burst = ADEPT_RUN_BURST;
     }
-    uint64_t burst = kBurst;
+    uint64_t burst = next_burst;
+    next_burst = std::min<uint64_t>(2 * next_burst, ADEPT_RUN_BURST_MAX);
     if (max_iterations) burst = std::min<uint64_t>(burst, max_iterations - done);
     for (uint64_t i = 0; i < burst && rc == ADEPT_OK; ++i) rc = launch_iteration(c);
     if (rc != ADEPT_OK) break;
