@@ -1053,3 +1053,33 @@ def test_multiple_scattering_matches_oracle(layout, scheme):
             compare_counts(ctx.step(), o.result(), what="msc kind %d step %d" % (kind, it))
             assert compare_tracks(ctx.read_tracks(kind), o.read_tracks(kind, t.dtype), "msc kind %d step %d" % (kind, it)) == 0
         ctx.destroy()
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("physics", (1, 2))
+def test_extended_physics_in_the_large_cta_shape(physics):
+    """Two steps of 5 M tracks (the 1024-thread shape runs from 4 Mi live tracks) under the extended rule
+    sets, dense AoSoA-32 and sparse HC16: counts and every track word against the oracle."""
+    n = 5_000_000
+    geo, tab = geometry_for("single_step"), tables_for("single_step", physics)
+    pop = gen_tracks(n, 7, geo, CONFIGS["single_step"]["e_max"])
+    for p in pop:
+        p["nial"][::4] = -1.0
+    o = Oracle(geo, tab, seed=3)
+    for k in range(3):
+        o.load_tracks(k, pop[k])
+    o.step()
+    o.step()
+    r = o.result()
+    ref = [sort_by_id(o.read_tracks(k, pop[k].dtype)) for k in range(3)]
+    o.close()
+    for layout, scheme in (("aosoa32", "dense"), ("hc16", "sparse")):
+        ctx = _ctx(geo, tab, layout=layout, scheme=scheme, capacity=8 * 1024 * 1024, seed=3)
+        for k in range(3):
+            ctx.load_tracks(k, pop[k])
+        ctx.step(sync=False)
+        compare_counts(ctx.step(), r, what="%s %s" % (layout, scheme))
+        for k in range(3):
+            a = sort_by_id(ctx.read_tracks(k))
+            assert a.shape == ref[k].shape and (a.view(np.uint8) == ref[k].view(np.uint8)).all()
+        ctx.destroy()
