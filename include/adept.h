@@ -251,6 +251,52 @@ int adept_destroy(adept_ctx *);
 /* Text of the last error of this context ("" if none).  ctx may be NULL: last create error. */
 const char *adept_last_error(const adept_ctx *);
 
+/* The step for callers that cannot allocate (csrc/step_static.cu).
+ *
+ * Every call above needs a workspace from cudaMalloc (or a framework allocator), and adept_create also
+ * pins host memory and creates a stream and events.  Some callers cannot do that when they need a step:
+ * hosts that reserve all device memory at start-up and forbid allocation afterwards, plugin hooks that
+ * receive only existing buffers and a stream, and code on a latency budget that cannot afford
+ * cudaMalloc / cudaFree (either may synchronise the whole device).  adept_step_static runs the same
+ * step kernel (AoSoA-32 records, dense double buffer: PAPER.md:31, 121; rules S16-S32) and keeps
+ * everything the workspace would hold -- control block, tallies, device tables, both record arrays of
+ * each kind -- in one fixed __device__ array inside the library.  It calls no cudaMalloc, cudaMallocHost,
+ * cudaFree, stream/event constructor or allocating library routine.
+ *
+ * Limits (the price of the fixed array, which occupies adept_step_static_bytes() ~ 2.7 MiB on every GPU
+ * that loads the library, from load to process exit): at most ADEPT_STATIC_MAX_TRACKS tracks per kind,
+ * before and after every iteration; ADEPT_STATIC_MAX_LAYERS layers; ADEPT_STATIC_MAX_BINS table bins;
+ * ADEPT_STATIC_MAX_MATERIALS materials; tables.physics = 0 only.  Anything larger returns ADEPT_EINVAL
+ * before any work is enqueued (a population that outgrows the array while stepping: ADEPT_ECAPACITY,
+ * counts filled in, no tracks copied).
+ *
+ * Arguments.  geometry, tables: host, as for adept_create (tables.data is copied during the call).
+ * tracks_in[k]: DEVICE array of n_in[k] records of kind k (may be NULL when n_in[k] = 0); the
+ * preconditions of adept_load_tracks apply (EINVAL otherwise, nothing stepped).  tracks_out[k]: DEVICE
+ * array with room for out_capacity records; on return its first out->total.live[k] records are the
+ * kind-k tracks alive after `iterations` (>= 1) iterations, in unspecified order (rule S29).  If a kind
+ * has more than out_capacity live tracks: EINVAL, counts filled in, no track copied.  *out: counts and
+ * tallies of these iterations alone (e_injected is 0: the call does not know what was injected);
+ * edep_slab / edep_layer as in adept_result.  n_in, tracks_in, tracks_out: host arrays of 3 entries.
+ * cuda_stream: all work is enqueued there; the call returns after it has completed.
+ *
+ * Sharing.  All calls on a device use the one array.  It keeps the last call's contents; the call
+ * clears what must start at zero (counters, tallies) itself.  Two calls overlapping on one GPU would
+ * race on it, so the entry point holds a process-wide lock and waits for its own work: it cannot run
+ * concurrently on several streams.  The first call on each device looks up the array's device address
+ * (one-time set-up); make that first call outside any stream capture.
+ * adept_step_static_error(): text of the calling thread's last failure ("" if none). */
+#define ADEPT_STATIC_MAX_TRACKS 8192u
+#define ADEPT_STATIC_MAX_LAYERS 64u
+#define ADEPT_STATIC_MAX_BINS 256u
+#define ADEPT_STATIC_MAX_MATERIALS 2u
+int adept_step_static(const adept_geometry *geometry, const adept_tables *tables,
+                      const adept_track *const tracks_in[3], const uint32_t n_in[3],
+                      adept_track *const tracks_out[3], uint32_t out_capacity, uint32_t iterations,
+                      void *cuda_stream, adept_result *out);
+size_t adept_step_static_bytes(void);
+const char *adept_step_static_error(void);
+
 /* Elementary functions of the step, evaluated on the device for bit-equality tests against the
  * oracle (DESIGN.md rules R1, R3, M8-M10, T13).  in/out are DEVICE arrays; n = element count.
  *  fn 0: Philox-4x32-10; in = n x {ctr[4], key[2]} u32, out = n x 4 u32

@@ -107,6 +107,12 @@ def lib(variant: str | None = None):
         L.adept_timing_sections.restype = C.c_int
         L.adept_timing_sections.argtypes = []
         L.adept_read_sections.argtypes = [vp, vp]
+        L.adept_step_static.argtypes = [C.POINTER(_Geometry), C.POINTER(_Tables), C.POINTER(vp), C.POINTER(u32),
+                                        C.POINTER(vp), u32, u32, vp, C.POINTER(_Result)]
+        L.adept_step_static_bytes.restype = C.c_size_t
+        L.adept_step_static_bytes.argtypes = []
+        L.adept_step_static_error.restype = C.c_char_p
+        L.adept_step_static_error.argtypes = []
         _LIBS[so] = L
     return _LIBS[so]
 
@@ -135,6 +141,42 @@ def dev_math(fn: int, inp, out_dtype, out_shape):
         raise AdeptError(rc, "adept_dev_math")
     torch.cuda.synchronize()
     return out
+
+
+STATIC_MAX_TRACKS, STATIC_MAX_LAYERS, STATIC_MAX_BINS, STATIC_MAX_MATERIALS = 8192, 64, 256, 2
+
+
+def step_static(geometry, tables, tracks_in, tracks_out, n_in, iterations: int = 1, stream=None):
+    """adept_step_static: the transport step for callers that may not allocate device memory (a host that
+    froze its memory plan, a hook that only gets buffers and a stream).  This wrapper allocates nothing on
+    the device either: `tracks_in` / `tracks_out` are three existing torch CUDA uint8 tensors each (56-byte
+    adept_track records; an input may be None when its count is 0), `n_in` the three input counts.
+    Returns the counts / tallies dict of these iterations; `live[k]` records of tracks_out[k] are valid.
+    Problems beyond the STATIC_MAX_* limits are refused by the library (AdeptError, ADEPT_EINVAL)."""
+    import torch
+    L = lib()
+    g = _Geometry(geometry.n_layers, geometry.abs_mm, geometry.gap_mm, geometry.half_xy_mm,
+                  geometry.mat_abs, geometry.mat_gap)
+    data = np.ascontiguousarray(tables.data, dtype=np.float32)
+    t = _Tables(tables.n_bins, tables.n_materials, tables.e_min, tables.e_max, float(tables.ln_e_min),
+                float(tables.inv_dln), tables.e_cut, data.ctypes.data_as(C.POINTER(C.c_float)),
+                int(getattr(tables, "physics", 0)), None)
+    ins = (C.c_void_p * 3)(*[x.data_ptr() if x is not None else None for x in tracks_in])
+    outs = (C.c_void_p * 3)(*[x.data_ptr() for x in tracks_out])
+    out_cap = min(x.numel() * x.element_size() for x in tracks_out) // 56
+    n = (C.c_uint32 * 3)(*[int(v) for v in n_in])
+    r = _Result()
+    slab = np.zeros(2 * geometry.n_layers, dtype=np.float64)
+    layer = np.zeros(geometry.n_layers, dtype=np.float64)
+    r.edep_slab = slab.ctypes.data_as(C.POINTER(C.c_double))
+    r.edep_layer = layer.ctypes.data_as(C.POINTER(C.c_double))
+    s = stream if stream is not None else torch.cuda.current_stream(tracks_out[0].device)
+    rc = L.adept_step_static(C.byref(g), C.byref(t), ins, n, outs, out_cap, iterations, s.cuda_stream, C.byref(r))
+    if rc != 0:
+        raise AdeptError(rc, L.adept_step_static_error().decode())
+    d = _counts_dict(r.total)
+    d.update(e_escaped=float(r.e_escaped), edep_slab=slab, edep_layer=layer)
+    return d
 
 
 class Context:
