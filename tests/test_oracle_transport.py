@@ -609,3 +609,98 @@ def test_shower_profile_sanity():
     assert 0.1 < r["edep_slab"][1::2].sum() / r["edep_slab"].sum() < 0.4
     assert r["e_escaped"] / r["e_injected"] < 0.1
     assert 4e3 < r["steps"].sum() / 20 / 1.0 < 1.2e4          # track-steps per GeV
+
+
+# ------------------------------------- S21 / S22 / S25: faces, snap, ties -----
+def _one_step(kind, track, geo, tab):
+    o = Oracle(geo, tab, seed=0)
+    o.set_trace(True)
+    o.load_tracks(kind, track)
+    o.step()
+    out = [o.read_tracks(k, track.dtype) for k in range(3)]
+    return o.result(), o.trace(), out
+
+
+@pytest.mark.parametrize("dir_xy,dist", [((0.8, 0.0), 8.75), ((-0.8, 0.0), 16.25), ((0.0, 0.8), 17.5), ((0.0, -0.8), 7.5)])
+def test_distance_to_each_transverse_face(dir_xy, dist):
+    """Rule S21, box |x|,|y| <= H ("box-shaped layers"): from the off-centre point (3, -4) with
+    H = 10 the four faces are at (10 - 3)/0.8 = 8.75, (-10 - 3)/(-0.8) = 16.25, (10 + 4)/0.8 = 17.5 and
+    (-10 + 4)/(-0.8) = 7.5 -- four different numbers, so an axis or a sign taken from the wrong component
+    shows.  The distance is bracketed by a competing photoabsorption (Sigma = 1, so its step is nial[2]
+    itself): 1e-4 short of the face the photon is absorbed, 1e-4 beyond it escapes.  The decision
+    margin the trace reports (north_star: "allowed only where the oracle's decision margin is below
+    1e-6") is that 1e-4."""
+    geo = Geometry(n_layers=1, abs_mm=1000.0, gap_mm=1.0, half_xy_mm=10.0)
+    tab = constant_tables(16, E_CUT, 100.0, E_CUT, photo=1.0)
+    d = (dir_xy[0], dir_xy[1], 0.6)                      # dz != 0: the +z face is 500 / 0.6 = 833 away
+    for factor, escapes in ((1.0 - 1e-4, False), (1.0 + 1e-4, True)):
+        t = make_tracks(1, pos=(3.0, -4.0, 500.0), dir=d, ekin=2.0, nial=(1.0, 1.0, dist * factor))
+        r, tr, out = _one_step(2, t, geo, tab)
+        assert int(r["escaped_n"][2]) == (1 if escapes else 0), (dir_xy, factor)
+        assert int(r["killed"][2]) == 1 and tr["winner"][0] == (W_GEOM if escapes else 2)
+        assert r["e_escaped"] == (2.0 if escapes else 0.0)
+        assert out[0].shape[0] == (0 if escapes else 1)      # the photo-electron, made where the photon stopped
+        if not escapes:
+            assert np.allclose(out[0]["pos"][0], np.array([3.0, -4.0, 500.0]) + dist * factor * np.array(d), rtol=0, atol=1e-4)
+        assert abs(float(tr["margin"][0]) - 1e-4) < 2e-6
+
+
+def test_backward_crossing_lands_exactly_on_the_lower_face():
+    """Rule S25: a track that crosses a slab face is put ON the face (pos.z = z_lo of the slab it leaves going
+    -z, = z_hi going +z), whatever pos.z + s * dir.z rounded to, and changes slab.  Thicknesses 2.5 / 125.5
+    make every face an exact fp32 number: slab 1 is [2.5, 128].  Starting 50-120 mm above a face at 2.5 the
+    rounded s * dir.z + pos.z misses the plane by several ulps for most directions, so the snap shows."""
+    geo = Geometry(n_layers=2, abs_mm=2.5, gap_mm=125.5, half_xy_mm=1e6)
+    tab = constant_tables(16, E_CUT, 100.0, E_CUT)
+    rng = np.random.default_rng(7)
+    n = 64
+    ct = rng.uniform(0.05, 1.0, n)
+    ph = rng.uniform(0, 2 * math.pi, n)
+    z0 = rng.uniform(50.0, 120.0, n)
+    for sign, face, vol in ((-1.0, 2.5, 0), (1.0, 128.0, 2)):
+        t = make_tracks(n, ekin=1.0, vol=1)
+        t["pos"][:, 2] = z0.astype(np.float32)
+        t["dir"] = np.stack([np.sqrt(1 - ct * ct) * np.cos(ph), np.sqrt(1 - ct * ct) * np.sin(ph), sign * ct], 1).astype(np.float32)
+        r, tr, out = _one_step(2, t, geo, tab)
+        g = sort_by_id(out[2])
+        t = sort_by_id(t)
+        assert g.shape[0] == n and (tr["winner"] == W_GEOM).all()
+        assert (g["pos"][:, 2] == np.float32(face)).all() and (g["vol"] == vol).all()
+        s = (np.float32(face) - t["pos"][:, 2]) / t["dir"][:, 2]
+        s64 = s.astype(np.float64)
+        if sign < 0:   # what the move alone (rule S23) leaves in pos.z: not the plane
+            unsnapped = (s64 * t["dir"][:, 2].astype(np.float64) + t["pos"][:, 2].astype(np.float64)).astype(np.float32)
+            assert (unsnapped != np.float32(face)).sum() > n // 4
+        # x and y moved by the same step length
+        for c in (0, 1):
+            want = t["pos"][:, c].astype(np.float64) + s64 * t["dir"][:, c].astype(np.float64)
+            assert np.allclose(g["pos"][:, c], want, rtol=1e-6, atol=1e-5)
+
+
+def test_ties_go_to_the_earlier_candidate():
+    """Rule S22: the winner is found with a strict '<' in the order geometry, continuous loss, processes
+    0, 1, 2 -- so of two equal step lengths the earlier candidate wins.  All numbers are exact in fp32:
+    range 10 gives s_e = max(0.2 * 10, 0.1) = 2, Sigma = 0.5 with nial = 1 gives 1 / 0.5 = 2, and the +z face
+    is put 2 away."""
+    geo = Geometry(n_layers=2, abs_mm=4.0, gap_mm=4.0, half_xy_mm=1e6)
+    far = Geometry(n_layers=1, abs_mm=1000.0, gap_mm=1.0, half_xy_mm=1e6)
+    # geometry = continuous loss: geometry wins, the electron crosses into slab 1
+    r, tr, out = _one_step(0, make_tracks(1, pos=(0, 0, 2.0), ekin=5.0), geo, constant_tables(16, E_CUT, 100.0, E_CUT, rng=10.0))
+    assert tr["winner"][0] == W_GEOM and out[0]["vol"][0] == 1 and out[0]["pos"][0, 2] == 4.0 and tr["margin"][0] == 0.0
+    # geometry = a process: geometry wins, the photon is not absorbed
+    r, tr, out = _one_step(2, make_tracks(1, pos=(0, 0, 2.0), ekin=5.0, nial=(1.0, 1.0, 1.0)), geo,
+                           constant_tables(16, E_CUT, 100.0, E_CUT, photo=0.5))
+    assert tr["winner"][0] == W_GEOM and out[2].shape[0] == 1 and out[2]["vol"][0] == 1 and tr["margin"][0] == 0.0
+    # continuous loss = bremsstrahlung: continuous loss wins, no photon is made
+    r, tr, out = _one_step(0, make_tracks(1, pos=(0, 0, 2.0), ekin=5.0, nial=(1.0, 1.0, 1.0)), far,
+                           constant_tables(16, E_CUT, 100.0, E_CUT, rng=10.0, brems=0.5))
+    assert tr["winner"][0] == W_ELOSS and int(r["secondaries"].sum()) == 0 and out[0]["pos"][0, 2] == 4.0
+    assert out[0]["nial"][0, 0] == 0.0 and tr["margin"][0] == 0.0
+    # pair = Compton: process 0 wins, the photon converts
+    r, tr, out = _one_step(2, make_tracks(1, pos=(0, 0, 2.0), ekin=5.0, nial=(1.0, 1.0, 1e6)), far,
+                           constant_tables(16, E_CUT, 100.0, E_CUT, pair=0.5, compt=0.5))
+    assert tr["winner"][0] == 0 and out[2].shape[0] == 0 and out[1].shape[0] == 1 and tr["margin"][0] == 0.0
+    # and a strictly shorter later candidate does win
+    r, tr, out = _one_step(2, make_tracks(1, pos=(0, 0, 2.0), ekin=5.0, nial=(1.0, 0.75, 1e6)), far,
+                           constant_tables(16, E_CUT, 100.0, E_CUT, pair=0.5, compt=0.5))
+    assert tr["winner"][0] == 1 and out[2].shape[0] == 1 and abs(float(tr["margin"][0]) - 0.25) < 1e-6
