@@ -49,6 +49,100 @@ RECORD_BYTES = {"aos": 64, "soa": 56, "aosoa32": 56, "aosoa64": 56, "soa16": 56,
 TRAFFIC_CSV = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
 
 
+EXTRAS_FILE = os.path.join(ROOT, "bench_extras.json")
+LINE_LIMIT = 8192          # bytes: the driver keeps a bounded tail of stdout and parses its last JSON line
+
+
+def _r(x, digits=5):
+    """Floats of the compact line to `digits` significant digits (the full values are in the extras file)."""
+    if isinstance(x, float):
+        return float("%.*g" % (digits, x))
+    if isinstance(x, (list, tuple)):
+        return [_r(v, digits) for v in x]
+    if isinstance(x, dict):
+        return {k: _r(v, digits) for k, v in x.items()}
+    return x
+
+
+def contract_line(out: dict) -> dict:
+    """The one JSON line the driver parses, from the full result `out`: the contract keys unchanged, and of
+    the bulky extras (per-layout detail, shower blocks with their 50-bin deposits, the sweep's 40 cells with
+    per-field counts) only scalar summaries and short arrays.  Everything else goes to EXTRAS_FILE."""
+    keep = ("impl", "metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+            "vs_baseline", "dtype", "data", "config", "clocks", "gpu_launches", "e2e", "roofline", "cpu_baseline",
+            "parity_full_size")
+    line = {k: out[k] for k in keep if k in out}
+    if "layouts" in out:
+        line["layouts_ms_per_step"] = {l: _r(v["ms_per_step"]) for l, v in out["layouts"].items()}
+    if "single_step_physics" in out:
+        line["single_step_physics"] = _r(out["single_step_physics"])
+    if "showers" in out:
+        sh = {}
+        for name, b in out["showers"].items():
+            e = {k: b[k] for k in ("value", "ms_per_run", "ms_min", "iterations", "track_steps", "us_per_iteration",
+                                   "showers_per_s", "layout", "scheme", "same_counts_as_dense", "scaling") if k in b}
+            if "parity_full_size" in b:
+                e["counts_bit_exact"] = b["parity_full_size"]["counts_bit_exact"]
+                e["edep_layer_rel_err"] = b["parity_full_size"]["edep_layer_rel_err"]
+            if "cpu_baseline" in b:
+                e["cpu_value"] = b["cpu_baseline"]["value"]
+            sh[name] = _r(e)
+        line["showers"] = sh
+    if "sweep" in out:
+        sw = out["sweep"]
+        cells = sw["cells"]
+        occs = sorted({c["occupancy"] for c in cells})
+        lays = []
+        for c in cells:
+            if c["layout"] not in lays:
+                lays.append(c["layout"])
+        summ = {"workload": "BASELINE.json configs[3]", "best": _r(sw["best"]), "occupancies": occs, "layouts": lays}
+        for scheme in ("dense", "sparse"):
+            sc = [c for c in cells if c["scheme"] == scheme]
+            if not sc:
+                continue
+            at = {(c["layout"], c["occupancy"]): c for c in sc}
+            grid = lambda f: [[_r(f(at[(l, o)]), 4) if (l, o) in at else None for o in occs] for l in lays]
+            blk = {"ms_per_step": grid(lambda c: c["ms_per_step"]),
+                   "roofline_frac": grid(lambda c: c["roofline"]["frac"])}
+            if any("alloc_compaction_ms" in c for c in sc):
+                blk["alloc_compaction_ms"] = grid(lambda c: c.get("alloc_compaction_ms"))
+            counted = [c for c in sc if "field_reads" in c]
+            if counted:
+                # BASELINE.json configs[3] "per-field read/write counts" (PAPER.md:115, Fig. 5): one instrumented
+                # cell per layout of this scheme, fields in the order of `field_names`
+                # cell per scheme in the line (the other layouts' counts are in the extras file), fields in the order
+                # of `field_names`; and per counted layout the 128-byte lines touched over the method's own bytes
+                c0 = ([c for c in counted if c["layout"] == "aosoa32"] or counted)[0]
+                blk["field_counts"] = {"layout": c0["layout"], "occupancy": c0["occupancy"],
+                                       "reads": list(c0["field_reads"].values()), "writes": list(c0["field_writes"].values())}
+                blk["line_bytes_over_algorithmic"] = {c["layout"]: _r(c.get("line_bytes_over_algorithmic"), 4) for c in counted}
+                summ["field_names"] = list(c0["field_reads"].keys())
+            summ[scheme] = blk
+        line["sweep"] = summ
+    if "extras_file" in out:
+        line["extras_file"] = out["extras_file"]
+    return line
+
+
+def emit(out: dict) -> None:
+    """Write the full result to EXTRAS_FILE and print the compact contract line as the LAST line of stdout."""
+    try:
+        with open(EXTRAS_FILE, "w") as f:
+            json.dump(out, f)
+        out["extras_file"] = os.path.basename(EXTRAS_FILE)
+    except OSError as e:   # a read-only checkout: the line still goes out
+        sys.stderr.write("bench.py: could not write %s (%s)\n" % (EXTRAS_FILE, e))
+    text = json.dumps(contract_line(out), separators=(",", ":"))
+    if len(text) > LINE_LIMIT:   # never let an extra push the contract keys out of the driver's view
+        slim = contract_line({k: v for k, v in out.items() if k not in ("sweep", "showers", "layouts")})
+        slim["note"] = "extras dropped from the line (over %d bytes); see extras_file" % LINE_LIMIT
+        text = json.dumps(slim, separators=(",", ":"))
+    sys.stderr.flush()
+    sys.stdout.write(text + "\n")
+    sys.stdout.flush()
+
+
 def ncu_traffic(workload: str, layout: str, scheme: str):
     """dram__bytes_read.sum + dram__bytes_write.sum of one step_kernel launch, from the committed table
     of `ncu --set full` captures (profiles/ncu_traffic.csv; the .md beside it names the commands).
@@ -300,8 +394,8 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
     host_in = [t.numpy().view(TRACK_DTYPE) for t in pinned_in]
     pinned_out = [torch.empty(capacity * 56, dtype=torch.uint8).pin_memory() for _ in range(3)]
     host_out = [t.numpy().view(TRACK_DTYPE) for t in pinned_out]
-    e2e_steps = max(1, min(args.steps, 3))
-    e2e_t, d2h = 0.0, 0
+    e2e_steps = max(1, min(args.steps, 10))
+    e2e_t, d2h, e2e_each = 0.0, 0, []
     for it in range(1 + e2e_steps):                        # first pass is a warm-up
         ctx.reset()
         torch.cuda.synchronize()
@@ -317,6 +411,7 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
         dt = max_over_ranks(time.perf_counter() - t0)
         if it > 0:
             e2e_t += dt
+            e2e_each.append(dt)
     # the same with only the step's counts read back (tracks stay on the device for the next
     # iteration, as they do inside adept_run): reported beside the full round trip
     e2e_c = 0.0
@@ -365,6 +460,7 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
         "gpu_launches": args.steps,
         "e2e": {"value": e2e_value, "unit": "track-steps/s", "h2d_bytes_per_step": 56 * n_tracks,
                 "d2h_bytes_per_step": d2h + 512, "steps": e2e_steps,
+                "ms_min": 1e3 * float(np.min(e2e_each)), "ms_median": 1e3 * float(np.median(e2e_each)),
                 "counts_only": {"value": e2e_counts_only, "unit": "track-steps/s", "d2h_bytes_per_step": 512,
                                 "what": "adept_load_tracks x3 + adept_step with its adept_counts read back"},
                 "what": "adept_load_tracks x3 (pinned host) + adept_step + adept_read_tracks x3"},
@@ -409,8 +505,10 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
         if "showers" in args.extras:
             out["showers"] = {}
             for name in ("full", "heavy") if "heavy" in args.extras else ("full",):
+                # the oracle needs ~80 s for config 5: timed (and its counts compared) only under --extras heavy_cpu;
+                # tests/test_gpu_parity.py test_heavy_showers_at_full_size_match_the_oracle holds that parity
                 out["showers"][name] = showers(args, name, layout=main, scheme="dense", steps=3, warmup=1,
-                                               with_cpu=not args.no_cpu)
+                                               with_cpu=not args.no_cpu and (name != "heavy" or "heavy_cpu" in args.extras))
             # config 2 under the extended rule set (DESIGN.md rules X36-X39: delta rays, Klein-Nishina sampling,
             # annihilation in flight, multiple scattering), against the oracle under the same rules
             out["showers"]["full_physics2"] = showers(args, "full", layout=main, scheme="dense", steps=3, warmup=1,
@@ -427,8 +525,10 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
                                                                  / np.maximum(np.array(ref["edep_layer_MeV"]), 1e-30)))
                 out["showers"][name + "_sparse_recycle"] = b
         if "sweep" in args.extras:
-            out["sweep"] = sweep(args, layouts=("aos", "soa", "aosoa32", "hc16"), steps=5, warmup=3, instr=False, sections=True)
-    print(json.dumps(out))
+            # per-field read / write counts (configs[3]): instrumented contexts at 50 % occupancy
+            out["sweep"] = sweep(args, layouts=("aos", "soa", "aosoa32", "hc16"), steps=5, warmup=3, instr=True, sections=True,
+                                 instr_occupancies=(0.5,))
+    emit(out)
     if dist is not None:
         dist.destroy_process_group()
 
@@ -548,7 +648,8 @@ def sweep_bytes(scheme: str, layout: str, n_in: int, n_surv: int, n_sec: int) ->
 SECTION_NAMES = ("other", "load", "move", "interact", "alloc", "store")
 
 
-def sweep(args, *, layouts, steps, warmup, instr, sections, occupancies=None, schemes=("dense", "sparse")) -> dict:
+def sweep(args, *, layouts, steps, warmup, instr, sections, occupancies=None, schemes=("dense", "sparse"),
+          instr_occupancies=None) -> dict:
     """BASELINE.json configs[3]: 4 Mi slots per kind, occupancy 10..90 %, both schemes x layouts.  Per
     cell: time of one adept_step (CUDA events, state restored and L2 flushed between repetitions) with
     its roofline fraction; the share of that time spent in slot allocation / compaction (rows A9, A10;
@@ -574,7 +675,7 @@ def sweep(args, *, layouts, steps, warmup, instr, sections, occupancies=None, sc
                 variants = [("time", False, None)]
                 if sections:
                     variants.append(("sections", False, "timing"))
-                if instr:
+                if instr and (instr_occupancies is None or occ in instr_occupancies):
                     variants.append(("instr", True, None))
                 for what, instrument, variant in variants:
                     ctx = Context(geo, tab, layout=layout, scheme=scheme, capacity=cap, seed=c["seed"],
@@ -626,12 +727,19 @@ def sweep(args, *, layouts, steps, warmup, instr, sections, occupancies=None, sc
                                     lines_touched=int((cnt["lines"] > 0).sum()),
                                     slots_touched=int((cnt["slots"] > 0).sum()),
                                     bytes_touched_per_track_step=128.0 * float((cnt["lines"] > 0).sum()) / n_live)
+                        # the same step's traffic counted in 128-byte lines touched (SURVEY.md §8(d) states the sparse
+                        # SoA figure this way) beside the method's own bytes: what sector amplification adds
+                        cell["line_bytes"] = 128 * int((cnt["lines"] > 0).sum())
+                        cell["line_bytes_over_algorithmic"] = cell["line_bytes"] / max(1, cell["algorithmic_bytes"])
+                        cell["roofline"]["frac_line_bytes"] = cell["line_bytes"] / (cell["ms_per_step"] * 1e-3) / 1e9 / peak
                     ctx.destroy()
                     del ctx
                     torch.cuda.empty_cache()
                 cells.append(cell)
-                sys.stderr.write("%s\n" % json.dumps({k: cell.get(k) for k in ("occupancy", "scheme", "layout", "ms_per_step",
-                                                                                "alloc_compaction_ms", "bytes_touched_per_track_step")}))
+                # progress, as plain text: the driver takes the LAST JSON-parsable line of the run for the result line
+                sys.stderr.write("sweep cell: occupancy %g %s %s  %.4f ms/step  alloc+compaction %s ms  touched %s B/track-step\n"
+                                 % (occ, scheme, layout, cell["ms_per_step"], cell.get("alloc_compaction_ms"),
+                                    cell.get("bytes_touched_per_track_step")))
         del pop
     best = max(cells, key=lambda x: x["track_steps_per_s"])
     return {"workload": "buffer-scheme sweep (BASELINE.json configs[3]): %d slots per kind, 5 %% of live tracks "
