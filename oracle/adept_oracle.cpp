@@ -563,28 +563,35 @@ bool step_track(Oracle &o, int kind, Track &t, Child children[2], int &n_childre
     } else if (kind != KIND_GAMMA && w == 1) {
       // X36: delta-ray production (the 1/T^2 term common to Moller and Bhabha scattering) on
       // [e_cut, E/2], two-body kinematics on a free electron at rest
+      // X36 guard: the interaction happens at the POST-step energy, which continuous loss may have taken
+      // to or below 2 e_cut although Sigma_delta (looked up at the pre-step energy, and interpolated across
+      // the bin that holds 2 e_cut) was positive.  The spectrum's interval [e_cut, E/2] is then empty: no
+      // delta ray is made and the track goes on unchanged (nial[1] is spent and re-sampled at its next step).
       const float E = t.ekin;
       const float a = e_cut, b = 0.5f * E;
-      float T = (a * b) / (b - rng.u(1, 0) * (b - a));
-      if (!(T > a)) T = a;
-      if (!(T < b)) T = b;
-      const float E1 = E - T;
-      const float tau = E + o.two_mc2;
-      float cd = sqrtf((T * tau) / (E * (T + o.two_mc2)));
-      float cp = sqrtf((E1 * tau) / (E * (E1 + o.two_mc2)));
-      if (cd > 1.0f) cd = 1.0f;
-      if (cp > 1.0f) cp = 1.0f;
-      const float sd = sqrtf(fmaf(-cd, cd, 1.0f));
-      const float sp = sqrtf(fmaf(-cp, cp, 1.0f));
-      float sphi, cphi;
-      sincos2pi(rng.u(1, 1), &sphi, &cphi);
-      float dd[3], dp[3];
-      rotate(t.dir, sd, cd, sphi, cphi, dd);
-      rotate(t.dir, sp, cp, -sphi, -cphi, dp);
-      children[0].kind = KIND_EM; children[0].t = make_child(t, rng, 0, dd, T);
-      n_children = 1;
-      t.ekin = E1;
-      for (int c = 0; c < 3; ++c) t.dir[c] = dp[c];
+      note_margin(margin, b, a);
+      if (b > a) {
+        float T = (a * b) / (b - rng.u(1, 0) * (b - a));
+        if (!(T > a)) T = a;
+        if (!(T < b)) T = b;
+        const float E1 = E - T;
+        const float tau = E + o.two_mc2;
+        float cd = sqrtf((T * tau) / (E * (T + o.two_mc2)));
+        float cp = sqrtf((E1 * tau) / (E * (E1 + o.two_mc2)));
+        if (cd > 1.0f) cd = 1.0f;
+        if (cp > 1.0f) cp = 1.0f;
+        const float sd = sqrtf(fmaf(-cd, cd, 1.0f));
+        const float sp = sqrtf(fmaf(-cp, cp, 1.0f));
+        float sphi, cphi;
+        sincos2pi(rng.u(1, 1), &sphi, &cphi);
+        float dd[3], dp[3];
+        rotate(t.dir, sd, cd, sphi, cphi, dd);
+        rotate(t.dir, sp, cp, -sphi, -cphi, dp);
+        children[0].kind = KIND_EM; children[0].t = make_child(t, rng, 0, dd, T);
+        n_children = 1;
+        t.ekin = E1;
+        for (int c = 0; c < 3; ++c) t.dir[c] = dp[c];
+      }
     } else if (kind != KIND_GAMMA) {
       // bremsstrahlung, 1/k spectrum on [e_cut, E]
       const float E = t.ekin;

@@ -365,3 +365,46 @@ def test_msc_showers_conserve_energy_and_do_not_depend_on_order():
     basic = Oracle(geo, tables_for("tiny", physics=1), seed=c["seed"])
     basic.inject(prim); basic.run()
     assert ra["steps"][0] > basic.result()["steps"][0]      # scattered electrons take more, shorter steps
+
+
+def test_delta_ray_guard_at_twice_the_cut():
+    """Rule X36 guard: a forced delta-ray step of a track whose energy is at or below 2 e_cut makes no
+    secondary and leaves energy and direction alone (only nial[1] is spent); just above 2 e_cut the
+    delta ray is made, with T in [e_cut, E/2].  (Before the guard both came out at E/2 < e_cut.)"""
+    n = 2000
+    for kind in (0, 1):
+        for E0, made in ((0.15, False), (0.2, False), (0.2001, True), (0.25, True)):
+            t, o = _delta_step(kind, E0, n, 5)
+            r = o.result()
+            assert int(r["secondaries"].sum()) == (n if made else 0), (kind, E0)
+            assert r["killed"].sum() == 0 and r["edep_slab"].sum() == 0.0
+            live = o.read_tracks(0, t.dtype) if kind == 0 else np.concatenate([o.read_tracks(0, t.dtype), o.read_tracks(1, t.dtype)])
+            assert (live["ekin"] >= np.float32(E_CUT)).all(), (kind, E0, float(live["ekin"].min()))
+            if not made:
+                g, ts = sort_by_id(o.read_tracks(kind, t.dtype)), sort_by_id(t)
+                assert (g["ekin"] == ts["ekin"]).all() and (g["dir"] == ts["dir"]).all()
+                assert (g["nial"][:, 1] == -1.0).all() and (g["step"] == 1).all()
+            else:
+                kids = live[live["step"] == 0]
+                assert kids.shape[0] == n and kids["ekin"].max() <= np.float32(0.5 * E0) * (1 + 1e-6)
+
+
+def test_no_electron_or_photon_lives_below_the_cut():
+    """Invariant of the tracking cut under the extended rules (what adept_load_tracks demands of a record):
+    after every iteration of a shower every live e- and photon has ekin >= e_cut (an e+ may sit below it
+    for one step, rule S17)."""
+    c = CONFIGS["tiny"]
+    geo, tab = geometry_for("tiny"), tables_for("tiny", physics=1)
+    o = Oracle(geo, tab, seed=c["seed"])
+    o.inject(gen_primaries(64, c["e_primary"]))
+    dt = make_tracks(1).dtype
+    seen = 0
+    for _ in range(400):
+        o.step()
+        for k in (0, 2):
+            g = o.read_tracks(k, dt)
+            seen += g.shape[0]
+            assert (g["ekin"] >= np.float32(E_CUT)).all(), (k, float(g["ekin"].min()))
+        if sum(o.live(k) for k in range(3)) == 0:
+            break
+    assert seen > 2000 and o.result()["secondaries"][0] > 100
