@@ -200,7 +200,8 @@ int adept_get_result(adept_ctx *, adept_result *out);
  * e_cut <= ekin <= e_max (an e+ may also have 0 <= ekin < e_cut: it annihilates at its next step,
  * rule S17); pos and dir finite, dir not the zero vector; nial not NaN.
  * EINVAL if a slot or a record breaks these (records are checked on the device while they are
- * unpacked); nothing is changed then. */
+ * unpacked, i.e. after the transfer): the live set and its counts are unchanged then, but storage beyond
+ * the live set (free slots, the tail of the dense array) may hold the records that were valid. */
 int adept_load_tracks(adept_ctx *, uint32_t kind, const adept_track *tracks, uint64_t n,
                       const uint32_t *slots);
 
@@ -244,6 +245,9 @@ uint64_t adept_field_offset_kind(int32_t layout, uint32_t kind, uint32_t capacit
  * restored workspace copy taken at that index. */
 uint32_t adept_launch_index(const adept_ctx *);
 int adept_set_launch_index(adept_ctx *, uint32_t index);
+/* Only device state is rewound by writing a workspace copy back: primaries queued for adept_run,
+ * e_injected and the primary index are host state and stay as they are.  The live count the host uses to
+ * pick the CTA shape is refreshed from the device at the next call that synchronises. */
 
 /* Drop all tracks, pending primaries and tallies; keeps geometry, tables and configuration. */
 int adept_reset(adept_ctx *);

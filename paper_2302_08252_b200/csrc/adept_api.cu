@@ -51,11 +51,9 @@ static const LayoutOps *ops_for(int layout) {
     case ADEPT_AOSOA32: return &kOpsAoSoA32;
     case ADEPT_SOA16: return &kOpsSoA16;
     case ADEPT_HC16: return &kOpsHC16;
-#ifndef ADEPT_FEW_LAYOUTS   // experiment builds instantiate four layouts only
     case ADEPT_AOSOA64: return &kOpsAoSoA64;
     case ADEPT_AOSOA16: return &kOpsAoSoA16;
     case ADEPT_AOSOA128: return &kOpsAoSoA128;
-#endif
     default: return nullptr;
   }
 }
@@ -781,7 +779,10 @@ uint32_t adept_launch_index(const adept_ctx *c) { return c ? c->launch_index : 0
 int adept_set_launch_index(adept_ctx *c, uint32_t index) {
   if (!c || index >= kLaunchWrap) return ADEPT_EINVAL;
   c->launch_index = index;
-  return ADEPT_OK;
+  // the restored workspace may hold another population than the one last seen: re-read the live count
+  // (it picks the CTA shape of the next launches)
+  const int rc = fetch_ctl(c, false);
+  return rc == ADEPT_ECAPACITY ? ADEPT_OK : rc;
 }
 
 uint64_t adept_field_offset_kind(int32_t layout, uint32_t kind, uint32_t capacity, uint32_t slot, uint32_t field) {

@@ -509,6 +509,10 @@ template <int KIND, int PHYS> __device__ __forceinline__ void interact_elec(Trk 
     t.n1 = -1.0f;
     const float E = t.ekin;
     const float a = e_cut, b = 0.5f * E;
+    if (!(b > a)) {   // guard of rule X36: post-step energy at or below 2 e_cut, no delta ray can be made
+      runaway_guard<KIND>(t, o);
+      return;
+    }
     float T = (a * b) / (b - u01(r1.x) * (b - a));
     if (!(T > a)) T = a;
     if (!(T < b)) T = b;

@@ -443,7 +443,10 @@ __device__ __forceinline__ void roll_iterations(Ctl *c, uint32_t capacity, uint3
       if (out > capacity) c->overflow = 1u;
       if (SPARSE) {
         uint32_t top = __ldcg(&c->slot_top[k]);
-        if (top > capacity) { top = capacity; c->overflow = 1u; }
+        // after an overflow the clamped top is written back: the host may enqueue up to a burst of further
+        // launches before it sees the flag, and an allocator that kept counting could wrap past 2^32 and
+        // hand out live slots again
+        if (top > capacity) { top = capacity; c->overflow = 1u; c->slot_top[k] = capacity; }
         if (top > used) c->slots_used[k] = top;
       } else {
         const uint32_t live = out < capacity ? out : capacity;
@@ -1249,9 +1252,12 @@ template <int L> struct OpsImpl {
       cudaLaunchAttribute attr[1];
       attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
       attr[0].val.programmaticStreamSerializationAllowed = 1;
-      static const bool no_pdl = std::getenv("ADEPT_NO_PDL") != nullptr;
       cfg.attrs = attr;
-      cfg.numAttrs = no_pdl ? 0u : 1u;
+#ifdef ADEPT_NO_PDL   // experiment builds only (build.py extra_flags): plain stream-ordered launches
+      cfg.numAttrs = 0u;
+#else
+      cfg.numAttrs = 1u;
+#endif
       return cudaLaunchKernelEx(&cfg, k, p);
     });
   }
