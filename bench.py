@@ -159,8 +159,24 @@ def ncu_traffic(workload: str, layout: str, scheme: str):
             best = d                                   # later rows are later captures
     if best is None:
         return None, None
+    # the capture is of the kernels as they were then: say so when csrc/ has changed since (rows older than
+    # round 3 carry no source hash and count as stale)
+    fresh = best.get("csrc_sha") and best["csrc_sha"] == csrc_sha()
     return float(best["dram_bytes_read"]) + float(best["dram_bytes_write"]), \
-        "profiles/ncu_traffic.csv (%s, commit %s)" % (best["capture"], best["commit"])
+        "profiles/ncu_traffic.csv (%s, commit %s%s)" % (best["capture"], best["commit"],
+                                                        "" if fresh else "; STALE: csrc/ changed since the capture")
+
+
+def csrc_sha() -> str:
+    """Hash of the kernel sources, as recorded beside each ncu capture in profiles/ncu_traffic.csv."""
+    import glob
+    import hashlib
+    h = hashlib.sha1()
+    for f in sorted(glob.glob(os.path.join(ROOT, "paper_2302_08252_b200", "csrc", "*"))):
+        h.update(os.path.basename(f).encode())
+        with open(f, "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:12]
 
 
 def measured_peak():
