@@ -45,7 +45,7 @@ if ROOT not in sys.path:
 from workloads import CONFIGS, gen_tracks, geometry_for, tables_for  # noqa: E402
 
 WORKLOAD = "single_step"
-RECORD_BYTES = {"aos": 64, "soa": 56, "aosoa32": 56, "aosoa64": 56, "soa16": 56, "aosoa16": 56, "aosoa128": 56, "hc16": 56}     # bytes per record per layout
+RECORD_BYTES = {"aos": 64, "soa": 56, "aosoa32": 56, "aosoa64": 56, "soa16": 56, "aosoa16": 56, "aosoa128": 56, "hc16": 56, "aosoa8": 56}     # bytes per record per layout
 TRAFFIC_CSV = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
 
 
@@ -241,13 +241,13 @@ def population(n_tracks: int, rank: int):
     return gen_tracks(n_tracks, c["seed"] + 1000 * rank, geometry_for(WORKLOAD), c["e_max"], c["fractions"])
 
 
-def oracle_single_step(pop, sample_tracks: int, want_tracks: bool = False):
+def oracle_single_step(pop, sample_tracks: int, want_tracks: bool = False, physics: int = 0):
     """Time the oracle, as it stands, on the first `sample_tracks` tracks of each kind's share."""
     from oracle import Oracle
     c = CONFIGS[WORKLOAD]
     total = sum(p.shape[0] for p in pop)
     frac = min(1.0, sample_tracks / total)
-    o = Oracle(geometry_for(WORKLOAD), tables_for(WORKLOAD), seed=c["seed"])
+    o = Oracle(geometry_for(WORKLOAD), tables_for(WORKLOAD, physics), seed=c["seed"])
     n = 0
     for k in range(3):
         m = int(round(pop[k].shape[0] * frac))
@@ -267,6 +267,29 @@ def by_id(tracks):
     """All tracks in id order: the full-size parity check compares every one of them word for word."""
     key = tracks["id_hi"].astype(np.uint64) << np.uint64(32) | tracks["id_lo"].astype(np.uint64)
     return tracks[np.argsort(key, kind="stable")]
+
+
+def full_size_parity(gpu: dict, ref: dict) -> dict:
+    """Every output track of the GPU step against the oracle's (both in id order), word for word.
+    Discrete-branch disagreements (north_star: to be reported): a track that took another branch on the GPU
+    has another fate -- it is missing, extra, or of another kind in the output.  north_star allows them only
+    where the oracle's decision margin is below 1e-6; with none at all, none has a larger margin."""
+    keys = ("steps", "secondaries", "killed", "escaped_n", "live")
+    n_cmp = n_missing = n_diff = 0
+    for a, b in zip(gpu["tracks"], ref["tracks"]):
+        ka = a["id_hi"].astype(np.uint64) << np.uint64(32) | a["id_lo"].astype(np.uint64)
+        kb = b["id_hi"].astype(np.uint64) << np.uint64(32) | b["id_lo"].astype(np.uint64)
+        common = np.intersect1d(ka, kb)
+        n_missing += int(ka.shape[0] + kb.shape[0] - 2 * common.shape[0])
+        aa, bb = a[np.isin(ka, common)], b[np.isin(kb, common)]
+        n_cmp += int(common.shape[0])
+        n_diff += int((aa.view(np.uint8).reshape(-1, 56) != bb.view(np.uint8).reshape(-1, 56)).any(axis=1).sum())
+    return {"counts_bit_exact": bool(all((gpu[k] == ref[k]).all() for k in keys)),
+            "tracks_compared": n_cmp, "tracks_with_another_fate": n_missing,
+            "tracks_with_any_word_differing": n_diff,
+            "branch_disagreement_rate": (n_missing / max(1, n_cmp)),
+            "disagreements_with_margin_ge_1e-6": 0 if n_missing == 0 else None,   # None: would need the oracle's trace
+            "edep_rel_err": float(np.max(np.abs(gpu["edep_layer"] - ref["edep_layer"]) / np.maximum(ref["edep_layer"], 1e-30)))}
 
 
 def host_cores() -> int:
@@ -496,26 +519,39 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
                                "kind": "oracle",
                                "sample": "one oracle iteration over all %d tracks of the same population" % n,
                                "seconds": dt}
-        keys = ("steps", "secondaries", "killed", "escaped_n", "live")
-        # discrete-branch disagreements (north_star: to be reported): a track that took another branch
-        # on the GPU has another fate -- it is missing, extra, or of another kind in the output
-        n_cmp = n_missing = n_diff = 0
-        for a, b in zip(main_res["tracks"], r["tracks"]):
-            ka = a["id_hi"].astype(np.uint64) << np.uint64(32) | a["id_lo"].astype(np.uint64)
-            kb = b["id_hi"].astype(np.uint64) << np.uint64(32) | b["id_lo"].astype(np.uint64)
-            common = np.intersect1d(ka, kb)
-            n_missing += int(ka.shape[0] + kb.shape[0] - 2 * common.shape[0])
-            aa, bb = a[np.isin(ka, common)], b[np.isin(kb, common)]
-            n_cmp += int(common.shape[0])
-            n_diff += int((aa.view(np.uint8).reshape(-1, 56) != bb.view(np.uint8).reshape(-1, 56)).any(axis=1).sum())
-        out["parity_full_size"] = {"counts_bit_exact": bool(all((main_res[k] == r[k]).all() for k in keys)),
-                                   "tracks_compared": n_cmp, "tracks_with_another_fate": n_missing,
-                                   "tracks_with_any_word_differing": n_diff,
-                                   "branch_disagreement_rate": (n_missing / max(1, n_cmp)),
-                                   "edep_rel_err": float(np.max(np.abs(main_res["edep_layer"] - r["edep_layer"])
-                                                                / np.maximum(r["edep_layer"], 1e-30)))}
+        out["parity_full_size"] = full_size_parity(main_res, r)
         del r
-    del main_res, results, pop
+    del main_res, results
+    torch.cuda.empty_cache()
+    if world == 1 and "physics" in args.extras:
+        # the same step under the extended rule sets (DESIGN.md rules X36-X39): physics 2
+        # reads and writes the paper's three cold fields of every e+- in a side array, 12 B
+        out["single_step_physics"] = {}
+        n_epm = pop[0].shape[0] + pop[1].shape[0]
+        for physics in (1, 2):
+            ctx = Context(geo, tables_for(WORKLOAD, physics), layout=main, scheme="dense", capacity=capacity,
+                          seed=CONFIGS[WORKLOAD]["seed"], device="cuda:%d" % local_rank)
+            ms, res, _ = bench_layout(ctx, torch, pop, min(args.steps, 10), 3, flush, barrier)
+            ctx.destroy()
+            del ctx
+            torch.cuda.empty_cache()
+            n_out = int(res["live"].sum())
+            nbytes = RECORD_BYTES[main] * (n_tracks + n_out)
+            if physics == 2:
+                nbytes += 12 * (n_epm + int(res["live"][0]) + int(res["live"][1]))
+            t = float(np.mean(ms))
+            blk = {"ms_per_step": t, "ms_min": float(np.min(ms)), "track_steps_per_s": n_tracks / (t * 1e-3),
+                   "algorithmic_bytes_per_launch": nbytes, "roofline_frac": nbytes / (t * 1e-3) / 1e9 / peak,
+                   "vs_physics0_time": t / m["ms_per_step"]}
+            if not args.no_cpu:
+                _, dt, r = oracle_single_step(pop, n_tracks, want_tracks=True, physics=physics)
+                par = full_size_parity(res, r)
+                blk.update(counts_bit_exact=par["counts_bit_exact"], tracks_with_another_fate=par["tracks_with_another_fate"],
+                           tracks_with_any_word_differing=par["tracks_with_any_word_differing"], cpu_seconds=dt)
+                del r
+            out["single_step_physics"]["physics%d" % physics] = blk
+            del res
+    del pop
     torch.cuda.empty_cache()
     if world == 1:
         if "showers" in args.extras:
@@ -824,12 +860,13 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--layout", default="all", choices=["soa", "aosoa32", "aosoa64", "soa16", "aos", "aosoa16", "aosoa128", "hc16", "all"])
+    ap.add_argument("--layout", default="all", choices=["soa", "aosoa32", "aosoa64", "soa16", "aos", "aosoa16", "aosoa128", "hc16", "aosoa8", "all"])
     ap.add_argument("--tracks", type=int, default=CONFIGS[WORKLOAD]["n_tracks"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline legs")
     ap.add_argument("--extras", default=None,
-                    help="comma list of what the default line carries beside the headline: showers, heavy, sweep "
-                         "(default: all three at the full population, none otherwise); 'none' = headline only")
+                    help="comma list of what the default line carries beside the headline: showers, heavy, sweep, physics "
+                         "(default: all four at the full population, none otherwise); heavy_cpu = also time the oracle on "
+                         "config 5 (~80 s); 'none' = headline only")
     ap.add_argument("--workload", default="single_step", choices=["single_step", "tiny", "full", "heavy", "sweep"],
                     help="single_step = the headline (BASELINE.json configs[2]); the others as a line of their own")
     ap.add_argument("--scheme", default=None, choices=["dense", "sparse"],
@@ -850,7 +887,7 @@ def main():
     if world != args.gpus and rank == 0:
         sys.stderr.write("bench.py: --gpus %d but %d rank(s) were launched; reporting n_gpus = %d\n" % (args.gpus, world, world))
     if args.extras is None:
-        args.extras = "showers,heavy,sweep" if args.tracks == CONFIGS[WORKLOAD]["n_tracks"] else "none"
+        args.extras = "showers,heavy,sweep,physics" if args.tracks == CONFIGS[WORKLOAD]["n_tracks"] else "none"
     args.extras = set(x for x in args.extras.split(",") if x and x != "none")
     if args.impl == "reference":
         run_reference(args, rank, world)

@@ -54,12 +54,12 @@ typedef enum {
   ADEPT_ESTATE = -4     /* call not allowed in the context's current state */
 } adept_status;
 
-/* Record layout in device memory ("AoS", "SoA", "AoSoA-n" with n = 16, 32, 64 or 128
+/* Record layout in device memory ("AoS", "SoA", "AoSoA-n" with n = 8, 16, 32, 64 or 128
  * lanes; AoSoA64 on the dense double buffer was the paper's fastest variant), and "SoA16": SoA of
  * 16-byte field groups {pos.xyz, dir.x} {dir.y, dir.z, ekin, nial.0} {nial.1, nial.2, vol, id_lo}
  * {id_hi, step} -- the hot/cold grouping the paper's conclusion points to. */
 typedef enum { ADEPT_AOS = 0, ADEPT_SOA = 1, ADEPT_AOSOA32 = 2, ADEPT_AOSOA64 = 3, ADEPT_SOA16 = 4,
-               ADEPT_AOSOA16 = 5, ADEPT_AOSOA128 = 6, ADEPT_HC16 = 7 } adept_layout;
+               ADEPT_AOSOA16 = 5, ADEPT_AOSOA128 = 6, ADEPT_HC16 = 7, ADEPT_AOSOA8 = 8 } adept_layout;
 /* ADEPT_HC16: hot/cold split with per-kind grouping ("a separation of hot and cold data
  * would be a first step", "different layouts per particle type"): the SoA16 geometry with the words of a
  * record regrouped, per particle kind, into two vectors the step rewrites every time ({pos, step} and

@@ -14,10 +14,10 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.environ.get("ADEPT_B200_LIB") or os.path.join(_HERE, "libadept_b200.so")
 
-ADEPT_AOS, ADEPT_SOA, ADEPT_AOSOA32, ADEPT_AOSOA64, ADEPT_SOA16, ADEPT_AOSOA16, ADEPT_AOSOA128, ADEPT_HC16 = 0, 1, 2, 3, 4, 5, 6, 7
+ADEPT_AOS, ADEPT_SOA, ADEPT_AOSOA32, ADEPT_AOSOA64, ADEPT_SOA16, ADEPT_AOSOA16, ADEPT_AOSOA128, ADEPT_HC16, ADEPT_AOSOA8 = 0, 1, 2, 3, 4, 5, 6, 7, 8
 ADEPT_SPARSE_SINGLE, ADEPT_DENSE_DOUBLE = 0, 1
 LAYOUTS = {"aos": ADEPT_AOS, "soa": ADEPT_SOA, "aosoa32": ADEPT_AOSOA32, "aosoa64": ADEPT_AOSOA64,
-           "soa16": ADEPT_SOA16, "aosoa16": ADEPT_AOSOA16, "aosoa128": ADEPT_AOSOA128, "hc16": ADEPT_HC16}
+           "soa16": ADEPT_SOA16, "aosoa16": ADEPT_AOSOA16, "aosoa128": ADEPT_AOSOA128, "hc16": ADEPT_HC16, "aosoa8": ADEPT_AOSOA8}
 SCHEMES = {"sparse": ADEPT_SPARSE_SINGLE, "dense": ADEPT_DENSE_DOUBLE}
 FIELD_NAMES = ("pos.x", "pos.y", "pos.z", "dir.x", "dir.y", "dir.z", "ekin", "nial.0", "nial.1", "nial.2",
                "vol", "id_lo", "id_hi", "step")

@@ -15,7 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libadept_b200.so")
 LIB_TIMING = os.path.join(HERE, "libadept_b200_timing.so")   # same sources, -DADEPT_TIMING_SECTIONS (include/adept.h)
-SOURCES = ["layout_aos.cu", "layout_soa.cu", "layout_aosoa32.cu", "layout_aosoa64.cu", "layout_soa16.cu", "layout_aosoa16.cu", "layout_aosoa128.cu", "layout_hc16.cu",
+SOURCES = ["layout_aos.cu", "layout_soa.cu", "layout_aosoa32.cu", "layout_aosoa64.cu", "layout_soa16.cu", "layout_aosoa16.cu", "layout_aosoa128.cu", "layout_hc16.cu", "layout_aosoa8.cu",
            "adept_api.cu", "step_static.cu"]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "--fmad=false", "--prec-div=true", "--prec-sqrt=true", "--ftz=false",

@@ -54,6 +54,7 @@ static const LayoutOps *ops_for(int layout) {
     case ADEPT_AOSOA64: return &kOpsAoSoA64;
     case ADEPT_AOSOA16: return &kOpsAoSoA16;
     case ADEPT_AOSOA128: return &kOpsAoSoA128;
+    case ADEPT_AOSOA8: return &kOpsAoSoA8;
     default: return nullptr;
   }
 }
@@ -806,6 +807,7 @@ uint64_t adept_field_offset(int32_t layout, uint32_t capacity, uint32_t slot, ui
     case ADEPT_SOA16: return 4 * Mapping<L_SOA16>::index(cap, slot, int(field));
     case ADEPT_AOSOA16: return 4 * Mapping<L_AOSOA16>::index(cap, slot, int(field));
     case ADEPT_AOSOA128: return 4 * Mapping<L_AOSOA128>::index(cap, slot, int(field));
+    case ADEPT_AOSOA8: return 4 * Mapping<L_AOSOA8>::index(cap, slot, int(field));
     default: return UINT64_MAX;
   }
 }

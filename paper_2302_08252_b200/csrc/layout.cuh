@@ -21,7 +21,7 @@ enum Field : int {
   kNumFields = 14
 };
 enum LayoutId : int { L_AOS = 0, L_SOA = 1, L_AOSOA32 = 2, L_AOSOA64 = 3, L_SOA16 = 4, L_AOSOA16 = 5, L_AOSOA128 = 6,
-                      L_HC16 = 7 };
+                      L_HC16 = 7, L_AOSOA8 = 8 };
 
 // A track in registers.
 struct Trk {
@@ -100,6 +100,7 @@ template <> struct Mapping<L_AOSOA32> : AoSoAMapping<32> {};  // "AoSoA-n", PAPE
 template <> struct Mapping<L_AOSOA64> : AoSoAMapping<64> {};  // the paper's fastest
 template <> struct Mapping<L_AOSOA16> : AoSoAMapping<16> {};  // "several lane counts"
 template <> struct Mapping<L_AOSOA128> : AoSoAMapping<128> {};  // one block per tile
+template <> struct Mapping<L_AOSOA8> : AoSoAMapping<8> {};  // the shortest lane count of SURVEY.md §8(f) item 2: a block is 448 B, a field run one sector
 // SoA of 16-byte field groups (SURVEY.md §8(f) item 1 "grouped-SoA of 16-byte vectors"; BASELINE.json
 // north_star "coalesced, vectorised 16-byte loads of SoA fields"): four arrays of `cap` vectors --
 // {pos.xyz, dir.x}, {dir.y, dir.z, ekin, nial.0}, {nial.1, nial.2, vol, id_lo} (16 B each) and

@@ -1290,6 +1290,6 @@ template <int L> struct OpsImpl {
   }
 };
 
-extern const LayoutOps kOpsAoS, kOpsSoA, kOpsAoSoA32, kOpsAoSoA64, kOpsSoA16, kOpsAoSoA16, kOpsAoSoA128, kOpsHC16;
+extern const LayoutOps kOpsAoS, kOpsSoA, kOpsAoSoA32, kOpsAoSoA64, kOpsSoA16, kOpsAoSoA16, kOpsAoSoA128, kOpsHC16, kOpsAoSoA8;
 
 }  // namespace adept

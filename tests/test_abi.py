@@ -61,10 +61,10 @@ def test_workspace_bytes_is_host_arithmetic(L):
     base = size()
     assert base > 3 * 2 * 4096 * 56                                  # three kinds, two dense arrays
     assert size(capacity=8192) > base and size(capacity=4097) == size(capacity=4224)   # rounded to 128 slots (one tile)
-    assert size(layout=0) > size(layout=1) == size(layout=2) == size(layout=3) == size(layout=4) == size(layout=7)   # AoS records are padded to 64 B
+    assert size(layout=0) > size(layout=1) == size(layout=2) == size(layout=3) == size(layout=4) == size(layout=7) == size(layout=8)   # AoS records are padded to 64 B
     assert size(scheme=0) < base                                     # one slot array + two slot lists
     assert size(instrument=1) > base
-    for bad in (dict(layout=8), dict(scheme=5), dict(capacity=0), dict(n_layers=0), dict(n_bins=0)):
+    for bad in (dict(layout=9), dict(scheme=5), dict(capacity=0), dict(n_layers=0), dict(n_bins=0)):
         assert size(**bad) == 0
 
 
@@ -98,7 +98,7 @@ def test_field_offset_follows_the_three_mappings(L):
             assert L.field_offset(L.ADEPT_SOA, cap, slot, f) == 4 * (f * cap + slot)       # 14 arrays
             assert L.field_offset(L.ADEPT_AOSOA32, cap, slot, f) == 4 * ((slot // 32) * 448 + f * 32 + slot % 32)
             assert L.field_offset(L.ADEPT_AOSOA64, cap, slot, f) == 4 * ((slot // 64) * 896 + f * 64 + slot % 64)
-            for lay, n in ((5, 16), (6, 128)):                                      # more AoSoA lane counts
+            for lay, n in ((5, 16), (6, 128), (8, 8)):                                    # more AoSoA lane counts
                 assert L.field_offset(lay, cap, slot, f) == 4 * ((slot // n) * 14 * n + f * n + slot % n)
             want = (f // 4) * 16 * cap + slot * 16 + (f % 4) * 4 if f < 12 else 48 * cap + slot * 8 + (f - 12) * 4
             assert L.field_offset(L.ADEPT_SOA16, cap, slot, f) == want          # 16-byte field groups

@@ -213,5 +213,8 @@ def test_the_drivers_exact_command_ends_with_the_contract_line():
     for scheme in ("dense", "sparse"):
         fc = d["sweep"][scheme]["field_counts"]
         assert sum(fc["reads"]) > 0 and sum(fc["writes"]) > 0
+    for ph in ("physics1", "physics2"):   # the same step under the extended rule sets, timed and compared at full size
+        b = d["single_step_physics"][ph]
+        assert b["counts_bit_exact"] and b["tracks_with_any_word_differing"] == 0 and 0.2 < b["roofline_frac"] < 1.0
     extras = json.load(open(os.path.join(ROOT, d["extras_file"])))
     assert len(extras["sweep"]["cells"]) == 40

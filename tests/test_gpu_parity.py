@@ -11,7 +11,7 @@ from tests.helpers import make_tracks, sort_by_id
 
 pytestmark = pytest.mark.gpu
 
-LAYOUTS = ("aos", "soa", "aosoa32", "aosoa64", "soa16", "aosoa16", "aosoa128", "hc16")
+LAYOUTS = ("aos", "soa", "aosoa32", "aosoa64", "soa16", "aosoa16", "aosoa128", "hc16", "aosoa8")
 SCHEMES = ("dense", "sparse")
 INT_FIELDS = ("vol", "id_lo", "id_hi", "step")
 F32_FIELDS = ("pos", "dir", "ekin", "nial")
